@@ -1,0 +1,458 @@
+"""Pins for the fp64 CPU oracle (oracle/): everything here is `-m "not gpu"`.
+
+Each oracle function is checked against something other than itself:
+  * hand-worked closed forms (tests/golden/*.json, with citations),
+  * an independent dense numpy brute force (adjacency COUNT matrix, dense softmax),
+  * library SDPA on the complete graph (textbook special case),
+  * torch.autograd through a dense formulation (gradients never typed by hand),
+  * central finite differences through the double-input build of the oracle,
+  * invariants the mathematics fixes (north_star list) and conservation identities,
+  * brute-force python loops / scipy for the integer plan metadata.
+"""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import plan_ref
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+_NS = {"ln2": math.log(2.0), "ln3": math.log(3.0), "ln4": math.log(4.0), "ln34": math.log(34.0)}
+
+
+def _val(x):
+    return float(eval(x, {"__builtins__": {}}, _NS)) if isinstance(x, str) else float(x)
+
+
+def _arr(x):
+    if isinstance(x, list):
+        return np.array([_arr(y) for y in x], dtype=np.float64)
+    return _val(x)
+
+
+def _rand_graph(rng, n, avg, multigraph=False, empty_rows=False):
+    """Random directed (multi)graph as CSR (row = dst), unsorted neighbour order."""
+    deg = rng.poisson(avg, size=n) + (0 if empty_rows else 1)
+    if empty_rows:
+        deg[rng.integers(0, n, size=max(1, n // 5))] = 0
+    rowptr = np.zeros(n + 1, np.int32)
+    rowptr[1:] = np.cumsum(deg)
+    if multigraph:
+        colidx = rng.integers(0, n, size=rowptr[-1]).astype(np.int32)
+    else:
+        colidx = np.concatenate([rng.choice(n, size=min(d, n), replace=False) if d else np.zeros(0, int)
+                                 for d in np.minimum(deg, n)]).astype(np.int32)
+        rowptr[1:] = np.cumsum(np.minimum(deg, n))
+    return rowptr, colidx
+
+
+def _count_matrix(rowptr, colidx):
+    n = rowptr.size - 1
+    C = np.zeros((n, n))
+    for i in range(n):
+        for e in range(rowptr[i], rowptr[i + 1]):
+            C[i, colidx[e]] += 1.0
+    return C
+
+
+# --------------------------------------------------------------------------- dense brute force
+def dense_gt(C, q, k, v):
+    """Dense masked attention: S = QK^T/sqrt(d); alpha_ij = C_ij e^{S_ij} / sum_j C_ij e^{S_ij}."""
+    n, H, d = q.shape
+    O = np.zeros((n, H, d))
+    L = np.full((n, H), -np.inf)
+    for h in range(H):
+        S = q[:, h, :] @ k[:, h, :].T / math.sqrt(d)
+        with np.errstate(divide="ignore"):
+            W = np.log(C) + S
+        m = W.max(axis=1, keepdims=True)
+        ok = np.isfinite(m[:, 0])
+        E = np.exp(W[ok] - m[ok])
+        Z = E.sum(axis=1, keepdims=True)
+        O[ok, h, :] = (E / Z) @ v[:, h, :]
+        L[ok, h] = (m[ok] + np.log(Z))[:, 0]
+    return O, L
+
+
+def dense_gatv2(C, xl, xr, a, slope):
+    n, H, d = xl.shape
+    O = np.zeros((n, H, d))
+    L = np.full((n, H), -np.inf)
+    for h in range(H):
+        Z3 = xl[:, None, h, :] + xr[None, :, h, :]            # [i, j, c]
+        S = (np.where(Z3 > 0, Z3, slope * Z3) * a[h][None, None, :]).sum(-1)
+        with np.errstate(divide="ignore"):
+            W = np.log(C) + S
+        m = W.max(axis=1, keepdims=True)
+        ok = np.isfinite(m[:, 0])
+        E = np.exp(W[ok] - m[ok])
+        Zs = E.sum(axis=1, keepdims=True)
+        O[ok, h, :] = (E / Zs) @ xr[:, h, :]
+        L[ok, h] = (m[ok] + np.log(Zs))[:, 0]
+    return O, L
+
+
+def _feat(rng, n, H, d, scale=1.0):
+    return (rng.standard_normal((n, H, d)) * scale).astype(np.float32)
+
+
+# --------------------------------------------------------------------------- golden fixtures
+def test_golden_gt_two_node():
+    g = json.load(open(os.path.join(GOLD, "gt_two_node.json")))
+    rp, ci = np.array(g["rowptr"], np.int32), np.array(g["colidx"], np.int32)
+    q, k, v = (_arr(g[x]) for x in "qkv")
+    O, L = oracle.gt_forward(rp, ci, q, k, v)
+    np.testing.assert_allclose(O, _arr(g["O"]), rtol=0, atol=1e-14)
+    np.testing.assert_allclose(L, _arr(g["L"]), rtol=0, atol=1e-14)
+    for case in ("case_a", "case_b"):
+        r = oracle.gt_backward(rp, ci, q, k, v, _arr(g[case]["dO"]))
+        for name in ("dQ", "dK", "dV"):
+            np.testing.assert_allclose(r[name], _arr(g[case][name]), rtol=0, atol=1e-14, err_msg=f"{case} {name}")
+
+
+def test_golden_gatv2_two_node():
+    g = json.load(open(os.path.join(GOLD, "gatv2_two_node.json")))
+    rp, ci = np.array(g["rowptr"], np.int32), np.array(g["colidx"], np.int32)
+    xl, xr, a, dO = _arr(g["xl"]), _arr(g["xr"]), _arr(g["a"]), _arr(g["dO"])
+    r = oracle.gatv2_backward(rp, ci, xl, xr, a, g["slope"], dO)
+    for name in ("O", "L", "G", "da", "dxl", "dxr"):
+        np.testing.assert_allclose(r[name], _arr(g[name]), rtol=0, atol=1e-14, err_msg=name)
+
+
+# --------------------------------------------------------------------------- forward vs dense brute force
+@pytest.mark.parametrize("seed,n,H,d,multi,empty", [(0, 9, 1, 4, False, False), (1, 23, 3, 8, True, False),
+                                                     (2, 40, 2, 16, True, True), (3, 64, 4, 5, False, True)])
+def test_gt_forward_vs_dense(seed, n, H, d, multi, empty):
+    rng = np.random.default_rng(seed)
+    rp, ci = _rand_graph(rng, n, 4.0, multi, empty)
+    q, k, v = (_feat(rng, n, H, d) for _ in range(3))
+    O, L = oracle.gt_forward(rp, ci, q, k, v)
+    Od, Ld = dense_gt(_count_matrix(rp, ci), q.astype(np.float64), k.astype(np.float64), v.astype(np.float64))
+    np.testing.assert_allclose(O, Od, rtol=0, atol=1e-12)
+    np.testing.assert_array_equal(np.isinf(L), np.isinf(Ld))
+    np.testing.assert_allclose(L[np.isfinite(L)], Ld[np.isfinite(Ld)], rtol=0, atol=1e-12)
+    if empty:   # reading A5: empty row -> O = 0, L = -inf
+        z = np.diff(rp) == 0
+        assert z.any() and np.all(O[z] == 0) and np.all(np.isneginf(L[z]))
+
+
+@pytest.mark.parametrize("seed,n,H,d,multi,slope", [(0, 9, 1, 4, False, 0.2), (1, 23, 3, 8, True, 0.2),
+                                                     (2, 33, 2, 16, True, 0.01), (3, 20, 4, 5, False, 1.7)])
+def test_gatv2_forward_vs_dense(seed, n, H, d, multi, slope):
+    rng = np.random.default_rng(100 + seed)
+    rp, ci = _rand_graph(rng, n, 4.0, multi, seed == 2)
+    xl, xr = _feat(rng, n, H, d), _feat(rng, n, H, d)
+    a = rng.standard_normal((H, d)).astype(np.float32)
+    O, L = oracle.gatv2_forward(rp, ci, xl, xr, a, slope)
+    Od, Ld = dense_gatv2(_count_matrix(rp, ci), xl.astype(np.float64), xr.astype(np.float64), a.astype(np.float64), slope)
+    np.testing.assert_allclose(O, Od, rtol=0, atol=1e-12)
+    fin = np.isfinite(Ld)
+    np.testing.assert_array_equal(np.isfinite(L), fin)
+    np.testing.assert_allclose(L[fin], Ld[fin], rtol=0, atol=1e-12)
+
+
+def test_gt_complete_graph_is_library_sdpa():
+    """Textbook special case: the complete graph with self-loops is plain dense softmax attention."""
+    rng = np.random.default_rng(7)
+    n, H, d = 17, 3, 8
+    rp = (np.arange(n + 1) * n).astype(np.int32)
+    ci = np.tile(np.arange(n, dtype=np.int32), n)
+    q, k, v = (_feat(rng, n, H, d) for _ in range(3))
+    O, L = oracle.gt_forward(rp, ci, q, k, v)
+    tq, tk, tv = (torch.from_numpy(x.astype(np.float64)).permute(1, 0, 2) for x in (q, k, v))   # [H, n, d]
+    ref = torch.nn.functional.scaled_dot_product_attention(tq, tk, tv)                        # scale 1/sqrt(d)
+    np.testing.assert_allclose(O, ref.permute(1, 0, 2).numpy(), rtol=0, atol=1e-12)
+    lse = torch.logsumexp(tq @ tk.transpose(1, 2) / math.sqrt(d), dim=-1)                     # [H, n]
+    np.testing.assert_allclose(L, lse.T.numpy(), rtol=0, atol=1e-12)
+
+
+# --------------------------------------------------------------------------- backward vs autograd (dense)
+def _torch_dense_gt(C, q, k, v):
+    d = q.shape[-1]
+    S = torch.einsum("ihc,jhc->hij", q, k) / math.sqrt(d)
+    W = S + torch.log(C)[None]
+    A = torch.softmax(W, dim=-1)
+    return torch.einsum("hij,jhc->ihc", A, v)
+
+
+def _torch_dense_gatv2(C, xl, xr, a, slope):
+    Z = xl[:, None] + xr[None, :]                        # [i, j, h, c]
+    S = (torch.nn.functional.leaky_relu(Z, slope) * a[None, None]).sum(-1).permute(2, 0, 1)   # [h, i, j]
+    A = torch.softmax(S + torch.log(C)[None], dim=-1)
+    return torch.einsum("hij,jhc->ihc", A, xr)
+
+
+@pytest.mark.parametrize("seed,multi", [(0, False), (1, True)])
+def test_gt_backward_vs_autograd(seed, multi):
+    rng = np.random.default_rng(200 + seed)
+    n, H, d = 21, 2, 8
+    rp, ci = _rand_graph(rng, n, 3.0, multi)
+    q, k, v, dO = (_feat(rng, n, H, d) for _ in range(4))
+    r = oracle.gt_backward(rp, ci, q, k, v, dO)
+    C = torch.from_numpy(_count_matrix(rp, ci))
+    tq, tk, tv = (torch.from_numpy(x.astype(np.float64)).requires_grad_() for x in (q, k, v))
+    out = _torch_dense_gt(C, tq, tk, tv)
+    out.backward(torch.from_numpy(dO.astype(np.float64)))
+    np.testing.assert_allclose(r["O"], out.detach().numpy(), rtol=0, atol=1e-12)
+    for name, t in (("dQ", tq), ("dK", tk), ("dV", tv)):
+        np.testing.assert_allclose(r[name], t.grad.numpy(), rtol=0, atol=1e-11, err_msg=name)
+    # Delta = <O, dO> equals sum_j alpha_ij dP_ij (PAPER.md:494 / :539)
+    np.testing.assert_allclose(r["Delta"], (r["O"] * dO).sum(-1), rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("seed,multi,slope", [(0, False, 0.2), (1, True, 0.2), (2, True, 1.5)])
+def test_gatv2_backward_vs_autograd(seed, multi, slope):
+    rng = np.random.default_rng(300 + seed)
+    n, H, d = 19, 3, 4
+    rp, ci = _rand_graph(rng, n, 3.0, multi)
+    xl, xr, dO = (_feat(rng, n, H, d) for _ in range(3))
+    a = rng.standard_normal((H, d)).astype(np.float32)
+    r = oracle.gatv2_backward(rp, ci, xl, xr, a, slope, dO)
+    C = torch.from_numpy(_count_matrix(rp, ci))
+    txl, txr, ta = (torch.from_numpy(x.astype(np.float64)).requires_grad_() for x in (xl, xr, a))
+    out = _torch_dense_gatv2(C, txl, txr, ta, slope)
+    out.backward(torch.from_numpy(dO.astype(np.float64)))
+    np.testing.assert_allclose(r["O"], out.detach().numpy(), rtol=0, atol=1e-12)
+    for name, t in (("dxl", txl), ("dxr", txr), ("da", ta)):
+        np.testing.assert_allclose(r[name], t.grad.numpy(), rtol=0, atol=1e-11, err_msg=name)
+
+
+# --------------------------------------------------------------------------- backward vs finite differences
+def _fd(fun, x, eps=1e-6):
+    g = np.zeros_like(x)
+    it = np.nditer(x, flags=["multi_index"])
+    for _ in it:
+        ix = it.multi_index
+        old = x[ix]
+        x[ix] = old + eps
+        fp = fun()
+        x[ix] = old - eps
+        fm = fun()
+        x[ix] = old
+        g[ix] = (fp - fm) / (2 * eps)
+    return g
+
+
+def test_gt_backward_vs_finite_differences():
+    """north_star: backward matches central finite differences to 1e-6 relative."""
+    rng = np.random.default_rng(11)
+    n, H, d = 7, 2, 4
+    rp, ci = _rand_graph(rng, n, 2.5, multigraph=True)
+    q, k, v, dO = (rng.standard_normal((n, H, d)) for _ in range(4))      # float64 -> double-input build
+    r = oracle.gt_backward(rp, ci, q, k, v, dO)
+    loss = lambda: float((oracle.gt_forward(rp, ci, q, k, v)[0] * dO).sum())
+    for name, x in (("dQ", q), ("dK", k), ("dV", v)):
+        g = _fd(loss, x)
+        assert np.abs(r[name] - g).max() <= 1e-6 * max(1.0, np.abs(g).max()), name
+
+
+def test_gatv2_backward_vs_finite_differences():
+    rng = np.random.default_rng(12)
+    n, H, d = 7, 2, 3
+    rp, ci = _rand_graph(rng, n, 2.5, multigraph=True)
+    xl, xr, dO = (rng.standard_normal((n, H, d)) for _ in range(3))
+    a = rng.standard_normal((H, d))
+    r = oracle.gatv2_backward(rp, ci, xl, xr, a, 0.2, dO)
+    loss = lambda: float((oracle.gatv2_forward(rp, ci, xl, xr, a, 0.2)[0] * dO).sum())
+    for name, x in (("dxl", xl), ("dxr", xr), ("da", a)):
+        g = _fd(loss, x)
+        assert np.abs(r[name] - g).max() <= 1e-6 * max(1.0, np.abs(g).max()), name
+
+
+# --------------------------------------------------------------------------- invariants (north_star list)
+def test_invariants_gt():
+    rng = np.random.default_rng(21)
+    n, H, d = 50, 2, 8
+    rp, ci = _rand_graph(rng, n, 5.0)
+    q, k, v = (_feat(rng, n, H, d) for _ in range(3))
+    O, L = oracle.gt_forward(rp, ci, q, k, v)
+    # alpha sums to 1: V = const vector -> O = that vector
+    ones = np.ones_like(v)
+    np.testing.assert_allclose(oracle.gt_forward(rp, ci, q, k, ones)[0], 1.0, rtol=0, atol=1e-14)
+    # degree-1 row returns its neighbour's value exactly, and L = the single score
+    rp1 = np.arange(n + 1, dtype=np.int32)
+    ci1 = rng.permutation(n).astype(np.int32)
+    O1, L1 = oracle.gt_forward(rp1, ci1, q, k, v)
+    np.testing.assert_array_equal(O1, v[ci1].astype(np.float64))
+    s = (q.astype(np.float64) * k[ci1].astype(np.float64)).sum(-1) / math.sqrt(d)
+    np.testing.assert_allclose(L1, s, rtol=0, atol=1e-14)
+    # constant scores (Q = 0) -> neighbour mean, L = ln deg
+    O0, L0 = oracle.gt_forward(rp, ci, np.zeros_like(q), k, v)
+    deg = np.diff(rp)
+    mean = np.stack([v[ci[rp[i]:rp[i + 1]]].astype(np.float64).mean(0) for i in range(n)])
+    np.testing.assert_allclose(O0, mean, rtol=0, atol=1e-13)
+    np.testing.assert_allclose(L0, np.log(deg)[:, None].repeat(H, 1), rtol=0, atol=1e-13)
+    # neighbour-order invariance
+    ci_p = ci.copy()
+    for i in range(n):
+        ci_p[rp[i]:rp[i + 1]] = rng.permutation(ci[rp[i]:rp[i + 1]])
+    Op, Lp = oracle.gt_forward(rp, ci_p, q, k, v)
+    np.testing.assert_allclose(Op, O, rtol=0, atol=1e-13)
+    np.testing.assert_allclose(Lp, L, rtol=0, atol=1e-13)
+    # key shift: k_j + c leaves O unchanged and shifts L by <q_i, c>/sqrt(d)
+    c = rng.standard_normal((1, H, d))
+    Os, Ls = oracle.gt_forward(rp, ci, q.astype(np.float64), k.astype(np.float64) + c, v.astype(np.float64))
+    np.testing.assert_allclose(Os, O, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(Ls - L, (q.astype(np.float64) * c).sum(-1) / math.sqrt(d), rtol=0, atol=1e-12)
+
+
+def test_invariants_gatv2():
+    rng = np.random.default_rng(22)
+    n, H, d = 40, 3, 4
+    rp, ci = _rand_graph(rng, n, 4.0)
+    xl, xr, dO = (_feat(rng, n, H, d) for _ in range(3))
+    a = rng.standard_normal((H, d)).astype(np.float32)
+    # a = 0 -> constant scores -> neighbour mean of xr, L = ln deg
+    O0, L0 = oracle.gatv2_forward(rp, ci, xl, xr, np.zeros_like(a), 0.2)
+    mean = np.stack([xr[ci[rp[i]:rp[i + 1]]].astype(np.float64).mean(0) for i in range(n)])
+    np.testing.assert_allclose(O0, mean, rtol=0, atol=1e-13)
+    np.testing.assert_allclose(L0, np.log(np.diff(rp))[:, None].repeat(H, 1), rtol=0, atol=1e-13)
+    # slope = 1: e_ij = a.xl_i + a.xr_j, alpha independent of xl -> dxl == 0 (up to cancellation) and
+    # O does not depend on xl at all
+    r = oracle.gatv2_backward(rp, ci, xl, xr, a, 1.0, dO)
+    assert np.abs(r["dxl"]).max() < 1e-13
+    O2, _ = oracle.gatv2_forward(rp, ci, _feat(rng, n, H, d), xr, a, 1.0)
+    np.testing.assert_allclose(O2, r["O"], rtol=0, atol=1e-12)
+    # sigma'(0) = slope (reading A8): xl = -xr on a self-loop-only graph makes z = 0 exactly
+    rp1, ci1 = np.arange(n + 1, dtype=np.int32), np.arange(n, dtype=np.int32)
+    r1 = oracle.gatv2_backward(rp1, ci1, -xr, xr, a, 0.2, dO)
+    np.testing.assert_array_equal(r1["O"], xr.astype(np.float64))          # degree 1
+    np.testing.assert_allclose(r1["dxl"], 0.0, atol=1e-15)                 # de = alpha (dP - G) = 0 at degree 1
+    np.testing.assert_allclose(r1["dxr"], dO.astype(np.float64), atol=1e-15)
+
+
+def test_conservation_identities():
+    """Identities usable at full scale: sum_j dV_j = sum_i dO_i;
+    sum_i <q_i,dQ_i> = sum_j <k_j,dK_j>; sum_j dxr_j - sum_i dxl_i = sum_i dO_i."""
+    rng = np.random.default_rng(23)
+    n, H, d = 60, 2, 8
+    rp, ci = _rand_graph(rng, n, 6.0, multigraph=True)
+    q, k, v, dO = (_feat(rng, n, H, d) for _ in range(4))
+    r = oracle.gt_backward(rp, ci, q, k, v, dO)
+    np.testing.assert_allclose(r["dV"].sum(0), dO.astype(np.float64).sum(0), rtol=0, atol=1e-12)
+    np.testing.assert_allclose((q * r["dQ"]).sum((0, 2)), (k * r["dK"]).sum((0, 2)), rtol=0, atol=1e-11)
+    a = rng.standard_normal((H, d)).astype(np.float32)
+    g = oracle.gatv2_backward(rp, ci, q, k, a, 0.2, dO)
+    np.testing.assert_allclose(g["dxr"].sum(0) - g["dxl"].sum(0), dO.astype(np.float64).sum(0), rtol=0, atol=1e-12)
+
+
+def test_row_subsets_match_full():
+    rng = np.random.default_rng(24)
+    n, H, d = 80, 2, 8
+    rp, ci = _rand_graph(rng, n, 5.0)
+    q, k, v, dO = (_feat(rng, n, H, d) for _ in range(4))
+    full = oracle.gt_backward(rp, ci, q, k, v, dO)
+    rows = rng.choice(n, size=13, replace=False).astype(np.int32)
+    O, L = oracle.gt_forward(rp, ci, q, k, v, rows=rows)
+    np.testing.assert_array_equal(O, full["O"][rows])
+    np.testing.assert_array_equal(L, full["L"][rows])
+    dQ = oracle.gt_backward_dst(rp, ci, q, k, v, dO, full["L"], full["Delta"], rows=rows)
+    np.testing.assert_array_equal(dQ, full["dQ"][rows])
+    rpt, cit = plan_ref.transpose_csr(rp, ci)
+    dK, dV = oracle.gt_backward_src(rpt, cit, q, k, v, dO, full["L"], full["Delta"], srcs=rows)
+    np.testing.assert_array_equal(dK, full["dK"][rows])
+    np.testing.assert_array_equal(dV, full["dV"][rows])
+
+
+# --------------------------------------------------------------------------- integer plan metadata
+def test_transpose_csr_vs_bruteforce_and_scipy():
+    import scipy.sparse as sp
+    rng = np.random.default_rng(31)
+    for multi in (False, True):
+        n = 37
+        rp, ci = _rand_graph(rng, n, 4.0, multi, empty_rows=True)
+        rpt, cit = plan_ref.transpose_csr(rp, ci)
+        # brute force: scan edges in CSR order, append dst to the source's list (stable by construction)
+        lists = [[] for _ in range(n)]
+        for i in range(n):
+            for e in range(rp[i], rp[i + 1]):
+                lists[ci[e]].append(i)
+        np.testing.assert_array_equal(rpt, np.concatenate([[0], np.cumsum([len(x) for x in lists])]))
+        np.testing.assert_array_equal(cit, np.concatenate([np.array(x, np.int32) for x in lists]))
+        if not multi:
+            A = sp.csr_matrix((np.ones(ci.size), ci, rp), shape=(n, n)).T.tocsr()
+            A.sort_indices()
+            np.testing.assert_array_equal(rpt, A.indptr)
+            np.testing.assert_array_equal(cit, A.indices)
+    # symmetric graph with sorted rows: CSR^T == CSR bit for bit
+    m = rng.random((30, 30)) < 0.2
+    m = m | m.T | np.eye(30, dtype=bool)
+    A = sp.csr_matrix(m.astype(np.float64))
+    A.sort_indices()
+    rpt, cit = plan_ref.transpose_csr(A.indptr.astype(np.int32), A.indices.astype(np.int32))
+    np.testing.assert_array_equal(rpt, A.indptr)
+    np.testing.assert_array_equal(cit, A.indices)
+
+
+def test_build_bins_vs_bruteforce():
+    rng = np.random.default_rng(32)
+    deg = np.concatenate([rng.integers(0, 6, 200), rng.integers(30, 300, 40), [1000, 2500, 4097, 9000, 0, 1, 64, 65]])
+    rng.shuffle(deg)
+    rp = np.concatenate([[0], np.cumsum(deg)]).astype(np.int32)
+    wmax, cmax, sc = 64, 1024, 1000
+    b = plan_ref.build_bins(rp, wmax, cmax, sc)
+
+    def key(g):
+        bl = int(g).bit_length()
+        if g > cmax:
+            return 0
+        if g > wmax:
+            return 1 + (32 - bl)
+        return 34 + (32 - bl)
+
+    order = sorted(range(deg.size), key=lambda r: (key(deg[r]), r))
+    np.testing.assert_array_equal(b["perm"], np.array(order, np.int32))
+    assert b["n_hub"] == int((deg > cmax).sum()) and b["n_cta"] == int(((deg > wmax) & (deg <= cmax)).sum())
+    assert b["n_hub"] + b["n_cta"] + b["n_group"] == deg.size
+    # chunk table: covers each hub row exactly once, contiguous, each chunk <= split_chunk, balanced to +-1
+    ch = b["chunks"]
+    for slot in range(b["n_hub"]):
+        r = order[slot]
+        mine = ch[b["hub_chunk_ptr"][slot]:b["hub_chunk_ptr"][slot + 1]]
+        assert np.all(mine[:, 0] == r) and np.all(mine[:, 3] == slot)
+        assert mine[0, 1] == rp[r] and mine[-1, 2] == rp[r + 1]
+        np.testing.assert_array_equal(mine[1:, 1], mine[:-1, 2])
+        sizes = mine[:, 2] - mine[:, 1]
+        assert sizes.max() <= sc and sizes.max() - sizes.min() <= 1 and len(mine) == -(-deg[r] // sc)
+    # heaviest first inside each class (bit-length buckets)
+    dperm = deg[b["perm"]]
+    bl = np.array([int(x).bit_length() for x in dperm])
+    assert np.all(np.diff(bl[b["n_hub"]:b["n_hub"] + b["n_cta"]]) <= 0)
+    assert np.all(np.diff(bl[b["n_hub"] + b["n_cta"]:]) <= 0)
+
+
+def test_build_blocks_vs_bruteforce():
+    rng = np.random.default_rng(33)
+    n = 70                                   # ragged last window (70 = 4*16 + 6)
+    rp, ci = _rand_graph(rng, n, 3.0, multigraph=True, empty_rows=True)
+    # add many in-window edges
+    extra_d = rng.integers(0, n, 300)
+    extra_s = np.minimum((extra_d // 16) * 16 + rng.integers(0, 16, 300), n - 1)
+    d_all = np.concatenate([np.repeat(np.arange(n), np.diff(rp)), extra_d])
+    s_all = np.concatenate([ci, extra_s])
+    o = np.argsort(d_all, kind="stable")
+    d_all, s_all = d_all[o], s_all[o]
+    rp = np.concatenate([[0], np.cumsum(np.bincount(d_all, minlength=n))]).astype(np.int32)
+    ci = s_all.astype(np.int32)
+    b = plan_ref.build_blocks(rp, ci)
+    nw = (n + 15) // 16
+    bm = np.zeros((nw, 16), np.uint16)
+    rem_rows = [[] for _ in range(n)]
+    for i in range(n):
+        seen = set()
+        for e in range(rp[i], rp[i + 1]):
+            j = int(ci[e])
+            if j // 16 == i // 16 and j not in seen:
+                seen.add(j)
+                bm[i // 16, i % 16] |= np.uint16(1 << (j % 16))
+            else:
+                rem_rows[i].append(j)
+    np.testing.assert_array_equal(b["bitmap"], bm)
+    np.testing.assert_array_equal(b["rem_rowptr"], np.concatenate([[0], np.cumsum([len(x) for x in rem_rows])]))
+    np.testing.assert_array_equal(b["rem_colidx"], np.concatenate([np.array(x, np.int32) for x in rem_rows]))
+    # every CSR entry is accounted for exactly once
+    assert int(sum(bin(int(x)).count("1") for x in bm.ravel())) + b["rem_colidx"].size == ci.size
