@@ -1,0 +1,177 @@
+/*
+ * gnn_attn.h - C ABI of libgnn_attn.so: fused CSR graph attention for sm_100a (B200).
+ *
+ * The operations are the attention-family layers of arxiv/paper_2605_31500 (section 2.2,
+ * lines 68-76), computed without ever writing an edge-wise E x H score / softmax / message tensor
+ * to HBM:
+ *
+ *   h_i = sum_{j in N(i)} alpha_ij v_j,   alpha_ij = softmax_{j in N(i)} (e_ij)
+ *   Graph Transformer:  e_ij = <q_i, k_j> / sqrt(head_dim),        v_j = v_j
+ *   GATv2:              e_ij = a^T LeakyReLU(xl_i + xr_j),         v_j = xr_j
+ *                       (xl = W_l h, xr = W_r h are projected by the caller)
+ *   saved statistic:    L[i,h] = ln sum_j exp(e_ij)   (natural log)
+ *
+ * CONVENTIONS (all entry points)
+ *   - Every data pointer is a DEVICE pointer owned by the caller; the library never allocates or
+ *     frees device memory.  Feature pointers and workspace must be 16-byte aligned.
+ *   - Graph: int32 CSR; ROW i = DESTINATION node, colidx[rowptr[i] .. rowptr[i+1]) = its sources j
+ *     (in-neighbours).  The library processes exactly the stored entries: the caller stores the
+ *     self-loop of N(i) u {i}; duplicate entries are separate softmax terms; a row with no
+ *     entries yields O = 0, L = -inf and contributes no gradient.  nnz < 2^31.  colidx values are
+ *     not range-checked.
+ *   - Features: [n, heads, head_dim] row-major (node-major), dtype GNN_F32 or GNN_BF16.
+ *     a: [heads, head_dim] fp32.  L, Delta, G: [n, heads] fp32.  ALL GRADIENT OUTPUTS ARE fp32
+ *     [n, heads, head_dim] regardless of the feature dtype (reading A9); the forward
+ *     output O has the feature dtype (bf16: round-to-nearest-even of the fp32 accumulator).
+ *     All arithmetic is fp32.
+ *   - Supported shapes: head_dim a power of two with head_dim*sizeof(elt) in [16, 512] bytes and
+ *     heads*head_dim*sizeof(elt) <= 1024 bytes.  Anything else returns GNN_EUNSUPPORTED.
+ *   - Every compute call is asynchronous on `stream` and never synchronises.  gnn_plan_build
+ *     synchronises `stream` (it reads a few counters back to the host).
+ *   - Return value: GNN_OK or an error code; nothing is launched when an error is returned for
+ *     argument validation.  gnn_last_error() returns a thread-local message for the last error.
+ *   - Determinism: no floating-point atomics anywhere; results are bit-reproducible run to run
+ *     for the same plan options and device.
+ */
+#ifndef GNN_ATTN_H_
+#define GNN_ATTN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Opaque stream handle: pass a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream). */
+typedef void* gnn_stream_t;
+
+typedef enum { GNN_OK = 0, GNN_EINVAL = 1, GNN_EUNSUPPORTED = 2, GNN_EWORKSPACE = 3, GNN_ECUDA = 4 } gnn_status_t;
+typedef enum { GNN_F32 = 0, GNN_BF16 = 1 } gnn_dtype_t;
+
+/* Degree-aware row binning (PAPER.md:326, :456-460, :472 describe a light/heavy split with its own
+ * launch shape per bucket; the thresholds and the chunking rule below are this library's own).
+ *   deg <= warp_max_deg            : "group rows"  - one lane group (row_bytes/16 lanes) per row
+ *   warp_max_deg < deg <= cta_max  : "CTA rows"    - one CTA per row, merged in shared memory
+ *   deg > cta_max_deg              : "hub rows"    - cut into ceil(deg/split_chunk) near-equal chunks,
+ *                                    one CTA per chunk, partial states merged by a second pass
+ * Zero in any threshold selects the default (256 / 8192 / 4096).
+ * build_transpose != 0 also builds CSR^T and its bins (needed by the backward calls).
+ * build_blocks != 0 also builds the 16-row block layout (gnn_gt_attn_fwd_block).              */
+typedef struct {
+    int32_t warp_max_deg;
+    int32_t cta_max_deg;
+    int32_t split_chunk;
+    int32_t build_transpose;
+    int32_t build_blocks;
+} gnn_plan_opts_t;
+
+typedef struct gnn_plan gnn_plan_t; /* host handle; views caller-provided device storage */
+
+/* Bytes of device storage a plan for (n, nnz, opts) needs: `dev_bytes` must stay allocated for the
+ * life of the plan, `scratch_bytes` only during gnn_plan_build.  Needs a CUDA device.            */
+gnn_status_t gnn_plan_bytes(int32_t n, int64_t nnz, const gnn_plan_opts_t* opts, size_t* dev_bytes,
+                            size_t* scratch_bytes);
+
+/* Build the integer metadata, a pure function of (rowptr, colidx, opts) (bit-exact against
+ * oracle/plan_ref.py):
+ *   bins   : perm[n] = row ids sorted by (key, row id), key = 0 for hub rows, 1 + (32 - bitlen(deg))
+ *            for CTA rows, 34 + (32 - bitlen(deg)) for group rows  (heaviest first)
+ *   chunks : (row, e_begin, e_end, hub_slot) int32 x4 per chunk, in (hub_slot, chunk) order,
+ *            chunk t of a hub row with degree g and c chunks = [b + floor(t g / c), b + floor((t+1) g / c))
+ *   CSR^T  : rowptr_t[n+1], colidx_t[nnz] by a STABLE sort on the source id,
+ *            plus the same bins / chunks for CSR^T (out-degrees)
+ *   blocks : see gnn_gt_attn_fwd_block
+ * rowptr/colidx: device, must outlive the plan (the plan keeps the pointers, not a copy).
+ * On success *plan is a host handle to free with gnn_plan_destroy (device storage stays the caller's). */
+gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t dev_bytes, void* scratch, size_t scratch_bytes,
+                            int32_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx,
+                            const gnn_plan_opts_t* opts, gnn_stream_t stream);
+void gnn_plan_destroy(gnn_plan_t* plan);
+
+/* Plan introspection for the bit-exact metadata check.  `what`:                                    */
+enum {
+    GNN_PLAN_COUNTS = 0,    /* int32[8]: n_hub, n_cta, n_group, n_chunks, then the same 4 for CSR^T  */
+    GNN_PLAN_PERM = 1,      /* int32[n]                                                             */
+    GNN_PLAN_CHUNKS = 2,    /* int32[n_chunks][4]                                                   */
+    GNN_PLAN_CHUNK_PTR = 3, /* int32[n_hub + 1]                                                     */
+    GNN_PLAN_ROWPTR_T = 4,  /* int32[n + 1]                                                         */
+    GNN_PLAN_COLIDX_T = 5,  /* int32[nnz]                                                           */
+    GNN_PLAN_PERM_T = 6,
+    GNN_PLAN_CHUNKS_T = 7,
+    GNN_PLAN_CHUNK_PTR_T = 8,
+    GNN_PLAN_BLOCK_BITMAP = 9,      /* uint16[n_windows][16]                                         */
+    GNN_PLAN_BLOCK_REM_ROWPTR = 10, /* int32[n + 1]                                                  */
+    GNN_PLAN_BLOCK_REM_COLIDX = 11  /* int32[rem_nnz]                                                */
+};
+/* Copies the item to HOST memory `host_dst` (synchronous).  *bytes in = capacity, out = size needed;
+ * with host_dst == NULL only the size is returned.                                                 */
+gnn_status_t gnn_plan_export(const gnn_plan_t* plan, int what, void* host_dst, size_t* bytes);
+/* Device pointers to CSR^T held by the plan (NULL if build_transpose was 0).                        */
+const int32_t* gnn_plan_rowptr_t(const gnn_plan_t* plan);
+const int32_t* gnn_plan_colidx_t(const gnn_plan_t* plan);
+
+/* Workspace (device bytes) a compute call needs: hub-chunk partial states
+ * [n_chunks][(n_acc * heads*head_dim + n_scalar * heads)] fp32 and, for gnn_gatv2_bwd, the per-CTA
+ * `da` partials.  O(#chunks * H * d), never O(E * H).  `op`:                                         */
+enum { GNN_OP_GT_FWD = 0, GNN_OP_GT_BWD = 1, GNN_OP_GATV2_FWD = 2, GNN_OP_GATV2_BWD = 3, GNN_OP_GT_FWD_BLOCK = 4 };
+gnn_status_t gnn_workspace_bytes(const gnn_plan_t* plan, int op, int32_t heads, int32_t head_dim, gnn_dtype_t dtype,
+                                 size_t* bytes);
+
+/* ---------------------------------------------------------------------------------------------
+ * Graph Transformer attention, forward (fused CSR kernel PAPER.md:484-492).
+ *   s_ij = <q[i,h,:], k[j,h,:]> / sqrt(head_dim);  L[i,h] = ln sum_j exp(s_ij);
+ *   out[i,h,:] = sum_j exp(s_ij - L[i,h]) v[j,h,:]        (online softmax)
+ * q, k, v: [n,H,d] `dtype`, in.  out: [n,H,d] `dtype`, out.  lse: [n,H] fp32, out.
+ * rowptr/colidx must be the arrays the plan was built from.  ws: >= gnn_workspace_bytes(GT_FWD).  */
+gnn_status_t gnn_gt_attn_fwd(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                             const void* q, const void* k, const void* v, int32_t heads, int32_t head_dim,
+                             gnn_dtype_t dtype, void* out, float* lse, void* ws, size_t ws_bytes,
+                             gnn_stream_t stream);
+
+/* Graph Transformer attention, backward, recomputing alpha from lse:
+ *   alpha_ij = exp(s_ij - L_i);  dP_ij = <dout_i, v_j>;  Delta_i = sum_j alpha_ij dP_ij (= <O_i, dO_i>)
+ *   dS_ij = alpha_ij (dP_ij - Delta_i)
+ *   dq_i = sum_j dS_ij k_j / sqrt(d)      (dst pass over CSR, row-local, no atomics)
+ *   dk_j = sum_i dS_ij q_i / sqrt(d);  dv_j = sum_i alpha_ij dout_i
+ *                                         (src pass over CSR^T in CSR^T order: deterministic, no atomics)
+ * q, k, v, dout: [n,H,d] `dtype`, in.  lse: [n,H] fp32, in (from the forward).
+ * delta: [n,H] fp32, OUT (scratch the caller provides; holds Delta on return).
+ * dq, dk, dv: [n,H,d] fp32, out.  The plan must have been built with build_transpose.
+ * The forward output O is not needed (Delta is formed in fp32 inside the dst pass).              */
+gnn_status_t gnn_gt_attn_bwd(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                             const void* q, const void* k, const void* v, const float* lse, const void* dout,
+                             int32_t heads, int32_t head_dim, gnn_dtype_t dtype, float* delta, float* dq,
+                             float* dk, float* dv, void* ws, size_t ws_bytes, gnn_stream_t stream);
+
+/* GATv2 attention, forward:
+ *   s_ij = sum_c a[h,c] LeakyReLU_slope(xl[i,h,c] + xr[j,h,c]);  softmax / lse / out as above with
+ *   value xr[j,h,:].  xl, xr: [n,H,d] `dtype`, in.  a: [H,d] fp32, in.  out, lse: as gnn_gt_attn_fwd. */
+gnn_status_t gnn_gatv2_fwd(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                           const void* xl, const void* xr, const float* a, int32_t heads, int32_t head_dim,
+                           gnn_dtype_t dtype, float slope, void* out, float* lse, void* ws, size_t ws_bytes,
+                           gnn_stream_t stream);
+
+/* GATv2 attention, backward:
+ *   z_ij = xl_i + xr_j;  alpha_ij = exp(s_ij - L_i);  dP_ij = <dout_i, xr_j>;  G_i = sum_j alpha_ij dP_ij
+ *   de_ij = alpha_ij (dP_ij - G_i);  LeakyReLU'(z) = 1 if z > 0 else slope
+ *   dxl_i = sum_j de_ij a . LeakyReLU'(z_ij)                              (dst pass, "AL" kernel)
+ *   da    = sum_ij de_ij LeakyReLU(z_ij)    (per-CTA fp32 partials, fixed-order fp64 final reduction)
+ *   dxr_j = sum_i ( alpha_ij dout_i + de_ij a . LeakyReLU'(z_ij) )        (src pass over CSR^T, "R" kernel)
+ * g: [n,H] fp32, OUT (holds G on return).  dxl, dxr: [n,H,d] fp32, out.  da: [H,d] fp32, out.     */
+gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                           const void* xl, const void* xr, const float* a, const float* lse, const void* dout,
+                           int32_t heads, int32_t head_dim, gnn_dtype_t dtype, float slope, float* g, float* dxl,
+                           float* dxr, float* da, void* ws, size_t ws_bytes, gnn_stream_t stream);
+
+/* Thread-local message describing the last error returned on this thread ("" if none).           */
+const char* gnn_last_error(void);
+/* Library version string, e.g. "gnn_attn 0.1 sm_100a".                                            */
+const char* gnn_version(void);
+/* Number of kernel launches the library has issued in this process (all threads).               */
+int64_t gnn_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GNN_ATTN_H_ */

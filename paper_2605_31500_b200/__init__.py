@@ -1,0 +1,15 @@
+"""paper_2605_31500_b200 - fused CSR graph attention (Graph Transformer + GATv2, fwd + bwd) for B200.
+
+Thin Python binding over the C-ABI library ``libgnn_attn.so`` (``include/gnn_attn.h``): argument
+marshalling only; every step of the path runs in the library's sm_100a kernels.  PyTorch is used
+for device memory and streams.  There is no CPU fallback: importing works without a GPU (the
+library loads and exports its symbols), but any compute call without a CUDA device raises.
+"""
+from .binding import (  # noqa: F401
+    GnnError, lib, Plan, PlanOpts,
+    gnn_plan_bytes, gnn_plan_build, gnn_plan_destroy, gnn_plan_export, gnn_workspace_bytes,
+    gnn_gt_attn_fwd, gnn_gt_attn_bwd, gnn_gatv2_fwd, gnn_gatv2_bwd,
+    gnn_last_error, gnn_version, gnn_launch_count,
+    GNN_F32, GNN_BF16, GNN_OP_GT_FWD, GNN_OP_GT_BWD, GNN_OP_GATV2_FWD, GNN_OP_GATV2_BWD,
+    EXPORTED_SYMBOLS,
+)

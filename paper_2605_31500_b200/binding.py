@@ -1,0 +1,223 @@
+"""ctypes binding of include/gnn_attn.h.  Same names as the C ABI; tensors are marshalled to raw
+device pointers, nothing is computed here."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libgnn_attn.so")
+
+GNN_OK, GNN_EINVAL, GNN_EUNSUPPORTED, GNN_EWORKSPACE, GNN_ECUDA = range(5)
+GNN_F32, GNN_BF16 = 0, 1
+GNN_OP_GT_FWD, GNN_OP_GT_BWD, GNN_OP_GATV2_FWD, GNN_OP_GATV2_BWD = 0, 1, 2, 3
+(GNN_PLAN_COUNTS, GNN_PLAN_PERM, GNN_PLAN_CHUNKS, GNN_PLAN_CHUNK_PTR, GNN_PLAN_ROWPTR_T, GNN_PLAN_COLIDX_T,
+ GNN_PLAN_PERM_T, GNN_PLAN_CHUNKS_T, GNN_PLAN_CHUNK_PTR_T, GNN_PLAN_BLOCK_BITMAP, GNN_PLAN_BLOCK_REM_ROWPTR,
+ GNN_PLAN_BLOCK_REM_COLIDX) = range(12)
+
+EXPORTED_SYMBOLS = [
+    "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
+    "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
+    "gnn_gatv2_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count",
+]
+
+
+class GnnError(RuntimeError):
+    pass
+
+
+class PlanOpts(C.Structure):
+    _fields_ = [("warp_max_deg", C.c_int32), ("cta_max_deg", C.c_int32), ("split_chunk", C.c_int32),
+                ("build_transpose", C.c_int32), ("build_blocks", C.c_int32)]
+
+
+_lib = None
+_vp, _i32, _i64, _sz, _f = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t, C.c_float
+
+
+def lib() -> C.CDLL:
+    """Load libgnn_attn.so (built in-tree by paper_2605_31500_b200.build).  Fails loudly if missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise GnnError(f"{_LIB_PATH} is missing: run `python -m paper_2605_31500_b200.build` "
+                           "(there is no CPU fallback)")
+        L = C.CDLL(_LIB_PATH)
+        L.gnn_plan_bytes.argtypes = [_i32, _i64, C.POINTER(PlanOpts), C.POINTER(_sz), C.POINTER(_sz)]
+        L.gnn_plan_build.argtypes = [C.POINTER(_vp), _vp, _sz, _vp, _sz, _i32, _i64, _vp, _vp, C.POINTER(PlanOpts), _vp]
+        L.gnn_plan_destroy.argtypes = [_vp]
+        L.gnn_plan_destroy.restype = None
+        L.gnn_plan_export.argtypes = [_vp, C.c_int, _vp, C.POINTER(_sz)]
+        L.gnn_plan_rowptr_t.argtypes = [_vp]
+        L.gnn_plan_rowptr_t.restype = _vp
+        L.gnn_plan_colidx_t.argtypes = [_vp]
+        L.gnn_plan_colidx_t.restype = _vp
+        L.gnn_workspace_bytes.argtypes = [_vp, C.c_int, _i32, _i32, C.c_int, C.POINTER(_sz)]
+        L.gnn_gt_attn_fwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _vp, _vp, _vp, _sz, _vp]
+        L.gnn_gt_attn_bwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _vp, _vp, _i32, _i32, C.c_int,
+                                      _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+        L.gnn_gatv2_fwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _f, _vp, _vp, _vp, _sz, _vp]
+        L.gnn_gatv2_bwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _vp, _vp, _i32, _i32, C.c_int, _f,
+                                    _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+        L.gnn_last_error.restype = C.c_char_p
+        L.gnn_version.restype = C.c_char_p
+        L.gnn_launch_count.restype = _i64
+        for s in EXPORTED_SYMBOLS:
+            getattr(L, s)
+        _lib = L
+    return _lib
+
+
+def gnn_last_error() -> str:
+    return lib().gnn_last_error().decode()
+
+
+def gnn_version() -> str:
+    return lib().gnn_version().decode()
+
+
+def gnn_launch_count() -> int:
+    return int(lib().gnn_launch_count())
+
+
+def _check(rc: int):
+    if rc != GNN_OK:
+        raise GnnError(f"gnn status {rc}: {gnn_last_error()}")
+
+
+def _require_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        raise GnnError("no CUDA device: paper_2605_31500_b200 has no CPU fallback")
+    return torch
+
+
+def _ptr(t):
+    """Raw device pointer of a contiguous CUDA tensor (None -> NULL)."""
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise GnnError("expected a contiguous CUDA tensor")
+    return t.data_ptr()
+
+
+def _stream(stream=None):
+    torch = _require_cuda()
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream
+
+
+def _dtype_code(t) -> int:
+    import torch
+    if t.dtype == torch.float32:
+        return GNN_F32
+    if t.dtype == torch.bfloat16:
+        return GNN_BF16
+    raise GnnError(f"unsupported feature dtype {t.dtype}")
+
+
+# ------------------------------------------------------------------------------------ plan
+def gnn_plan_bytes(n: int, nnz: int, opts: PlanOpts):
+    _require_cuda()
+    d, s = _sz(0), _sz(0)
+    _check(lib().gnn_plan_bytes(n, nnz, C.byref(opts), C.byref(d), C.byref(s)))
+    return d.value, s.value
+
+
+def gnn_plan_build(dev_mem, scratch, n: int, nnz: int, rowptr, colidx, opts: PlanOpts, stream=None):
+    h = _vp(None)
+    _check(lib().gnn_plan_build(C.byref(h), _ptr(dev_mem), dev_mem.numel(), _ptr(scratch), scratch.numel(), n, nnz,
+                                _ptr(rowptr), _ptr(colidx), C.byref(opts), _stream(stream)))
+    return h
+
+
+def gnn_plan_destroy(handle):
+    lib().gnn_plan_destroy(handle)
+
+
+def gnn_plan_export(handle, what: int, dtype=np.int32) -> np.ndarray:
+    need = _sz(0)
+    _check(lib().gnn_plan_export(handle, what, None, C.byref(need)))
+    out = np.empty(need.value // np.dtype(dtype).itemsize, dtype=dtype)
+    cap = _sz(out.nbytes)
+    _check(lib().gnn_plan_export(handle, what, out.ctypes.data_as(_vp), C.byref(cap)))
+    return out
+
+
+def gnn_workspace_bytes(handle, op: int, heads: int, head_dim: int, dtype_code: int) -> int:
+    b = _sz(0)
+    _check(lib().gnn_workspace_bytes(handle, op, heads, head_dim, dtype_code, C.byref(b)))
+    return b.value
+
+
+class Plan:
+    """Owns the torch allocations behind a gnn_plan_t (plan storage, workspace) for one CSR graph."""
+
+    def __init__(self, rowptr, colidx, warp_max_deg=0, cta_max_deg=0, split_chunk=0, transpose=True, stream=None):
+        torch = _require_cuda()
+        if rowptr.dtype != torch.int32 or colidx.dtype != torch.int32:
+            raise GnnError("rowptr / colidx must be int32")
+        self.rowptr, self.colidx = rowptr.contiguous(), colidx.contiguous()
+        self.n, self.nnz = int(rowptr.numel()) - 1, int(colidx.numel())
+        self.opts = PlanOpts(warp_max_deg, cta_max_deg, split_chunk, 1 if transpose else 0, 0)
+        dev_bytes, scratch_bytes = gnn_plan_bytes(self.n, self.nnz, self.opts)
+        self.dev_mem = torch.empty(dev_bytes, dtype=torch.uint8, device=rowptr.device)
+        scratch = torch.empty(scratch_bytes, dtype=torch.uint8, device=rowptr.device)
+        self.handle = gnn_plan_build(self.dev_mem, scratch, self.n, self.nnz, self.rowptr, self.colidx, self.opts, stream)
+        del scratch
+        self._ws = None
+        self.plan_bytes = dev_bytes
+
+    def export(self, what: int, dtype=np.int32) -> np.ndarray:
+        return gnn_plan_export(self.handle, what, dtype)
+
+    def counts(self) -> dict:
+        c = self.export(GNN_PLAN_COUNTS)
+        keys = ["n_hub", "n_cta", "n_group", "n_chunks"]
+        return {**{k: int(v) for k, v in zip(keys, c[:4])}, **{k + "_t": int(v) for k, v in zip(keys, c[4:])}}
+
+    def workspace(self, op: int, heads: int, head_dim: int, dtype_code: int):
+        import torch
+        need = gnn_workspace_bytes(self.handle, op, heads, head_dim, dtype_code)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = torch.empty(need, dtype=torch.uint8, device=self.rowptr.device)
+        return self._ws
+
+    def __del__(self):
+        h = getattr(self, "handle", None)
+        if h is not None and _lib is not None:
+            _lib.gnn_plan_destroy(h)
+            self.handle = None
+
+
+# ------------------------------------------------------------------------------------ compute
+def gnn_gt_attn_fwd(plan: Plan, q, k, v, out, lse, stream=None):
+    n, H, d = q.shape
+    ws = plan.workspace(GNN_OP_GT_FWD, H, d, _dtype_code(q))
+    _check(lib().gnn_gt_attn_fwd(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v), H, d,
+                                 _dtype_code(q), _ptr(out), _ptr(lse), _ptr(ws), ws.numel(), _stream(stream)))
+
+
+def gnn_gt_attn_bwd(plan: Plan, q, k, v, lse, dout, delta, dq, dk, dv, stream=None):
+    n, H, d = q.shape
+    ws = plan.workspace(GNN_OP_GT_BWD, H, d, _dtype_code(q))
+    _check(lib().gnn_gt_attn_bwd(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v),
+                                 _ptr(lse), _ptr(dout), H, d, _dtype_code(q), _ptr(delta), _ptr(dq), _ptr(dk), _ptr(dv),
+                                 _ptr(ws), ws.numel(), _stream(stream)))
+
+
+def gnn_gatv2_fwd(plan: Plan, xl, xr, a, slope, out, lse, stream=None):
+    n, H, d = xl.shape
+    ws = plan.workspace(GNN_OP_GATV2_FWD, H, d, _dtype_code(xl))
+    _check(lib().gnn_gatv2_fwd(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(xl), _ptr(xr), _ptr(a), H, d,
+                               _dtype_code(xl), float(slope), _ptr(out), _ptr(lse), _ptr(ws), ws.numel(), _stream(stream)))
+
+
+def gnn_gatv2_bwd(plan: Plan, xl, xr, a, lse, dout, slope, g, dxl, dxr, da, stream=None):
+    n, H, d = xl.shape
+    ws = plan.workspace(GNN_OP_GATV2_BWD, H, d, _dtype_code(xl))
+    _check(lib().gnn_gatv2_bwd(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(xl), _ptr(xr), _ptr(a),
+                               _ptr(lse), _ptr(dout), H, d, _dtype_code(xl), float(slope), _ptr(g), _ptr(dxl), _ptr(dxr),
+                               _ptr(da), _ptr(ws), ws.numel(), _stream(stream)))

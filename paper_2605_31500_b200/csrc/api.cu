@@ -1,0 +1,219 @@
+// api.cu - the C-ABI entry points of include/gnn_attn.h: argument validation and pass sequencing.
+// Every step of the path runs in this library's kernels; nothing here computes on the host.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "internal.h"
+#include "kernels.cuh"
+
+namespace gnn {
+
+unsigned long long g_launches = 0;
+static thread_local char t_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_err, sizeof(t_err), fmt, ap);
+    va_end(ap);
+}
+
+namespace {
+
+bool make_shape(int32_t n, int32_t heads, int32_t head_dim, int dtype, Shape& sh, const char* who) {
+    if (dtype != GNN_F32 && dtype != GNN_BF16) { set_error("%s: unknown dtype %d", who, dtype); return false; }
+    const int esz = dtype == GNN_F32 ? 4 : 2, vec = 16 / esz;
+    if (heads < 1 || head_dim < 1 || (head_dim & (head_dim - 1)) || head_dim * esz < 16 || head_dim * esz > 512 ||
+        (long long)heads * head_dim * esz > 1024) {
+        set_error("%s: unsupported shape heads=%d head_dim=%d dtype=%d (head_dim must be a power of two with "
+                  "16 <= head_dim*sizeof <= 512 and heads*head_dim*sizeof <= 1024)", who, heads, head_dim, dtype);
+        return false;
+    }
+    sh.n = n; sh.H = heads; sh.d = head_dim; sh.rowe = heads * head_dim; sh.rowv = sh.rowe / vec;
+    sh.lph = head_dim / vec;
+    sh.lph_log2 = 0;
+    while ((1 << sh.lph_log2) < sh.lph) ++sh.lph_log2;
+    return true;
+}
+
+bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
+
+struct WsLayout { size_t partials, da_part, total; int da_slots; };
+
+// workspace of one API call = max over its passes of the chunk partials (+ da partials for GATv2 bwd)
+WsLayout ws_layout(const gnn_plan* P, int op, const Shape& sh) {
+    WsLayout w = {0, 0, 0, 0};
+    size_t part = 0;
+    auto need = [&](Pass ps, const BinView& b) {
+        const size_t x = (size_t)b.n_chunks * pass_state_floats(ps, sh) * sizeof(float);
+        if (x > part) part = x;
+    };
+    switch (op) {
+        case GNN_OP_GT_FWD: need(kGtFwd, P->fwd); break;
+        case GNN_OP_GT_BWD: need(kGtBwdDst, P->fwd); need(kGtBwdSrc, P->tr); break;
+        case GNN_OP_GATV2_FWD: need(kGatFwd, P->fwd); break;
+        case GNN_OP_GATV2_BWD: need(kGatBwdDst, P->fwd); need(kGatBwdSrc, P->tr); break;
+        default: break;
+    }
+    w.partials = 0;
+    w.da_part = (part + 255) / 256 * 256;
+    size_t da = 0;
+    if (op == GNN_OP_GATV2_BWD) {
+        w.da_slots = grid_plan(P->fwd, P->sm_count, group_width(sh.rowv)).da_slots();
+        da = (size_t)w.da_slots * sh.rowe * sizeof(float);
+    }
+    w.total = w.da_part + da + 256;
+    return w;
+}
+
+bool check_common(const gnn_plan* P, const int32_t* rowptr, const int32_t* colidx, int32_t n, const char* who) {
+    if (!P) { set_error("%s: NULL plan", who); return false; }
+    if (rowptr != P->rowptr || colidx != P->colidx || n != P->n) {
+        set_error("%s: rowptr/colidx/n differ from the arrays the plan was built from", who);
+        return false;
+    }
+    return true;
+}
+
+LaunchCtx make_ctx(const gnn_plan* P, bool transposed, void* ws, const WsLayout& w, gnn_stream_t stream) {
+    LaunchCtx c;
+    c.stream = (cudaStream_t)stream;
+    c.sm_count = P->sm_count;
+    c.rowptr = transposed ? P->rowptr_t : P->rowptr;
+    c.colidx = transposed ? P->colidx_t : P->colidx;
+    c.bins = transposed ? P->tr : P->fwd;
+    c.partials = (float*)((char*)ws + w.partials);
+    c.da_part = (float*)((char*)ws + w.da_part);
+    c.da_slot_base = 0;
+    return c;
+}
+
+gnn_status_t cuda_status(cudaError_t e, const char* who) {
+    if (e == cudaSuccess) return GNN_OK;
+    set_error("%s: CUDA error: %s", who, cudaGetErrorString(e));
+    return GNN_ECUDA;
+}
+
+}  // namespace
+}  // namespace gnn
+
+using namespace gnn;
+
+extern "C" const char* gnn_last_error(void) { return t_err; }
+extern "C" const char* gnn_version(void) { return "gnn_attn 0.1 sm_100a"; }
+extern "C" int64_t gnn_launch_count(void) { return (int64_t)g_launches; }
+
+extern "C" gnn_status_t gnn_workspace_bytes(const gnn_plan_t* P, int op, int32_t heads, int32_t head_dim,
+                                            gnn_dtype_t dtype, size_t* bytes) {
+    if (!P || !bytes) { set_error("gnn_workspace_bytes: NULL plan or bytes"); return GNN_EINVAL; }
+    if (op < GNN_OP_GT_FWD || op > GNN_OP_GATV2_BWD) { set_error("gnn_workspace_bytes: unknown op %d", op); return GNN_EINVAL; }
+    Shape sh;
+    if (!make_shape(P->n, heads, head_dim, dtype, sh, "gnn_workspace_bytes")) return GNN_EUNSUPPORTED;
+    if ((op == GNN_OP_GT_BWD || op == GNN_OP_GATV2_BWD) && !P->opts.build_transpose) {
+        set_error("gnn_workspace_bytes: backward needs a plan built with build_transpose");
+        return GNN_EINVAL;
+    }
+    *bytes = ws_layout(P, op, sh).total;
+    return GNN_OK;
+}
+
+extern "C" gnn_status_t gnn_gt_attn_fwd(const gnn_plan_t* P, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                        const void* q, const void* k, const void* v, int32_t heads, int32_t head_dim,
+                                        gnn_dtype_t dtype, void* out, float* lse, void* ws, size_t ws_bytes,
+                                        gnn_stream_t stream) {
+    const char* who = "gnn_gt_attn_fwd";
+    if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
+    if (!q || !k || !v || !out || !lse || !ws) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
+    if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !aligned16(ws)) {
+        set_error("%s: feature pointers and workspace must be 16-byte aligned", who);
+        return GNN_EINVAL;
+    }
+    Shape sh;
+    if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
+    const WsLayout w = ws_layout(P, GNN_OP_GT_FWD, sh);
+    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
+    GtArgs a = {};
+    a.q = q; a.k = k; a.v = v; a.out = out; a.lse = lse;
+    return cuda_status(launch_gt_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a), who);
+}
+
+extern "C" gnn_status_t gnn_gt_attn_bwd(const gnn_plan_t* P, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                        const void* q, const void* k, const void* v, const float* lse,
+                                        const void* dout, int32_t heads, int32_t head_dim, gnn_dtype_t dtype,
+                                        float* delta, float* dq, float* dk, float* dv, void* ws, size_t ws_bytes,
+                                        gnn_stream_t stream) {
+    const char* who = "gnn_gt_attn_bwd";
+    if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
+    if (!P->opts.build_transpose) { set_error("%s: plan was built without build_transpose", who); return GNN_EINVAL; }
+    if (!q || !k || !v || !lse || !dout || !delta || !dq || !dk || !dv || !ws) {
+        set_error("%s: NULL pointer argument", who);
+        return GNN_EINVAL;
+    }
+    if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(dout) || !aligned16(dq) || !aligned16(dk) ||
+        !aligned16(dv) || !aligned16(ws)) {
+        set_error("%s: feature/gradient pointers and workspace must be 16-byte aligned", who);
+        return GNN_EINVAL;
+    }
+    Shape sh;
+    if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
+    const WsLayout w = ws_layout(P, GNN_OP_GT_BWD, sh);
+    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
+    GtArgs a = {};
+    a.q = q; a.k = k; a.v = v; a.dout = dout; a.lse = const_cast<float*>(lse); a.delta = delta;
+    a.dq = dq; a.dk = dk; a.dv = dv;
+    cudaError_t e = launch_gt_bwd_dst(dtype, sh, make_ctx(P, false, ws, w, stream), a);   // dQ, Delta
+    if (e == cudaSuccess) e = launch_gt_bwd_src(dtype, sh, make_ctx(P, true, ws, w, stream), a);  // dK, dV
+    return cuda_status(e, who);
+}
+
+extern "C" gnn_status_t gnn_gatv2_fwd(const gnn_plan_t* P, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                      const void* xl, const void* xr, const float* a_, int32_t heads, int32_t head_dim,
+                                      gnn_dtype_t dtype, float slope, void* out, float* lse, void* ws, size_t ws_bytes,
+                                      gnn_stream_t stream) {
+    const char* who = "gnn_gatv2_fwd";
+    if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
+    if (!xl || !xr || !a_ || !out || !lse || !ws) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
+    if (!aligned16(xl) || !aligned16(xr) || !aligned16(a_) || !aligned16(out) || !aligned16(ws)) {
+        set_error("%s: feature pointers, a and workspace must be 16-byte aligned", who);
+        return GNN_EINVAL;
+    }
+    Shape sh;
+    if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
+    const WsLayout w = ws_layout(P, GNN_OP_GATV2_FWD, sh);
+    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
+    GatArgs a = {};
+    a.xl = xl; a.xr = xr; a.a = a_; a.out = out; a.lse = lse; a.slope = slope;
+    return cuda_status(launch_gat_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a), who);
+}
+
+extern "C" gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* P, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                      const void* xl, const void* xr, const float* a_, const float* lse,
+                                      const void* dout, int32_t heads, int32_t head_dim, gnn_dtype_t dtype,
+                                      float slope, float* g, float* dxl, float* dxr, float* da, void* ws,
+                                      size_t ws_bytes, gnn_stream_t stream) {
+    const char* who = "gnn_gatv2_bwd";
+    if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
+    if (!P->opts.build_transpose) { set_error("%s: plan was built without build_transpose", who); return GNN_EINVAL; }
+    if (!xl || !xr || !a_ || !lse || !dout || !g || !dxl || !dxr || !da || !ws) {
+        set_error("%s: NULL pointer argument", who);
+        return GNN_EINVAL;
+    }
+    if (!aligned16(xl) || !aligned16(xr) || !aligned16(a_) || !aligned16(dout) || !aligned16(dxl) || !aligned16(dxr) ||
+        !aligned16(ws)) {
+        set_error("%s: feature/gradient pointers, a and workspace must be 16-byte aligned", who);
+        return GNN_EINVAL;
+    }
+    Shape sh;
+    if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
+    const WsLayout w = ws_layout(P, GNN_OP_GATV2_BWD, sh);
+    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
+    GatArgs a = {};
+    a.xl = xl; a.xr = xr; a.a = a_; a.dout = dout; a.lse = const_cast<float*>(lse); a.g = g; a.dxl = dxl; a.dxr = dxr;
+    a.slope = slope;
+    const LaunchCtx c = make_ctx(P, false, ws, w, stream);
+    cudaError_t e = launch_gat_bwd_dst(dtype, sh, c, a);                                   // dxl, G, da partials
+    if (e == cudaSuccess) e = launch_da_reduce(c.da_part, w.da_slots, sh.rowe, da, c.stream);  // da
+    if (e == cudaSuccess) e = launch_gat_bwd_src(dtype, sh, make_ctx(P, true, ws, w, stream), a);  // dxr
+    return cuda_status(e, who);
+}

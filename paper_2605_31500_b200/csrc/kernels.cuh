@@ -1,0 +1,347 @@
+// kernels.cuh - the three traversal kernels + launcher, generic over an Op (see ops.cuh).
+#pragma once
+#include "engine.cuh"
+
+namespace gnn {
+
+extern unsigned long long g_launches;  // host-side launch counter (api.cu)
+
+// ------------------------------------------------------------------------------------------------
+// state <-> shared memory (serialised layout of state_floats<Op>)
+template <class Op> __device__ __forceinline__ void state_to_smem(const typename Op::St& st, float* dst,
+                                                                  const typename Op::GeoT& g, const Shape& sh) {
+    constexpr int NV = Op::kNV, VEC = Op::kVEC;
+#pragma unroll
+    for (int a = 0; a < Op::NA; ++a)
+#pragma unroll
+        for (int t = 0; t < NV; ++t)
+            if (g.act[t]) {
+#pragma unroll
+                for (int c = 0; c < VEC; c += 4)
+                    *reinterpret_cast<float4*>(dst + a * sh.rowe + g.eoff[t] + c) =
+                        make_float4(st.acc[a][t][c], st.acc[a][t][c + 1], st.acc[a][t][c + 2], st.acc[a][t][c + 3]);
+            }
+#pragma unroll
+    for (int s = 0; s < Op::NS; ++s)
+#pragma unroll
+        for (int t = 0; t < NV; ++t)
+            if (g.lead[t]) dst[Op::NA * sh.rowe + s * sh.H + g.hd[t]] = st.sc[s][t];
+}
+
+template <class Op> __device__ __forceinline__ void state_from_smem(typename Op::St& st, const float* src,
+                                                                    const typename Op::GeoT& g, const Shape& sh) {
+    constexpr int NV = Op::kNV, VEC = Op::kVEC;
+#pragma unroll
+    for (int a = 0; a < Op::NA; ++a)
+#pragma unroll
+        for (int t = 0; t < NV; ++t)
+#pragma unroll
+            for (int c = 0; c < VEC; ++c) st.acc[a][t][c] = g.act[t] ? src[a * sh.rowe + g.eoff[t] + c] : 0.f;
+#pragma unroll
+    for (int s = 0; s < Op::NS; ++s)
+#pragma unroll
+        for (int t = 0; t < NV; ++t) st.sc[s][t] = g.act[t] ? src[Op::NA * sh.rowe + s * sh.H + g.hd[t]] : 0.f;
+    if (Op::SOFTMAX) {
+#pragma unroll
+        for (int t = 0; t < NV; ++t)
+            st.m[t] = g.act[t] ? src[Op::NA * sh.rowe + Op::NS * sh.H + g.hd[t]] : -INFINITY;
+    }
+}
+
+// per-CTA reduction of the per-thread `da` accumulators (GATv2 dst pass) -> da_part[slot][rowe],
+// fixed order over groups.  smem: NG * rowe floats.
+template <class Op>
+__device__ __forceinline__ void cta_write_da(const float (&da)[Op::kNV][Op::kVEC], float* smem, float* da_part,
+                                             int slot, const typename Op::GeoT& g, const Shape& sh, int gi, int ng) {
+    constexpr int NV = Op::kNV, VEC = Op::kVEC;
+    __syncthreads();
+#pragma unroll
+    for (int t = 0; t < NV; ++t)
+        if (g.act[t]) {
+#pragma unroll
+            for (int c = 0; c < VEC; ++c) smem[gi * sh.rowe + g.eoff[t] + c] = da[t][c];
+        }
+    __syncthreads();
+    for (int e = threadIdx.x; e < sh.rowe; e += blockDim.x) {
+        float s = 0.f;
+        for (int k = 0; k < ng; ++k) s += smem[k * sh.rowe + e];
+        da_part[(size_t)slot * sh.rowe + e] = s;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// group rows: one lane group per row, rows perm[first .. first+count), static round-robin over warps
+template <class Op>
+__global__ void __launch_bounds__(kCtaThreads)
+group_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
+             const int32_t* __restrict__ perm, int first, int count, float* da_part, int da_slot) {
+    constexpr int G = Op::kG, NV = Op::kNV, VEC = Op::kVEC;
+    constexpr int GPW = 32 / G;
+    extern __shared__ float4 smem4[];
+    float* smem = reinterpret_cast<float*>(smem4);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    typename Op::GeoT g;
+    g.init(sh, lane);
+    const int gl = lane & (G - 1);
+    float da[NV][VEC];
+#pragma unroll
+    for (int t = 0; t < NV; ++t)
+#pragma unroll
+        for (int c = 0; c < VEC; ++c) da[t][c] = 0.f;
+
+    const int ntiles = (count + GPW - 1) / GPW;
+    const int total_warps = gridDim.x * kWarpsPerCta;
+    for (int tile = blockIdx.x * kWarpsPerCta + warp; tile < ntiles; tile += total_warps) {
+        const int idx = tile * GPW + lane / G;
+        const bool valid = idx < count;
+        int row = 0, e0 = 0, len = 0;
+        if (valid) {
+            row = __ldg(perm + first + idx);
+            e0 = __ldg(rowptr + row);
+            len = __ldg(rowptr + row + 1) - e0;
+        }
+        typename Op::Own own;
+        Op::load_own(own, p, sh, row, valid, g);
+        typename Op::St st;
+        st.reset();
+        int maxlen = len;
+#pragma unroll
+        for (int o = G; o < 32; o <<= 1) maxlen = max(maxlen, __shfl_xor_sync(0xffffffffu, maxlen, o));
+        for (int base = 0; base < maxlen; base += G) {
+            const int my = (base + gl < len) ? __ldg(colidx + e0 + base + gl) : -1;
+            const int cnt = min(G, maxlen - base);
+            for (int u0 = 0; u0 < cnt; u0 += kU) {
+                int nbr[kU];
+#pragma unroll
+                for (int u = 0; u < kU; ++u) nbr[u] = __shfl_sync(0xffffffffu, my, u0 + u, G);
+                Op::batch(st, own, p, sh, nbr, g);
+            }
+        }
+        if (valid) Op::finalize(st, p, sh, row, g, da);
+    }
+    if (Op::HAS_DA)
+        cta_write_da<Op>(da, smem, da_part, da_slot + blockIdx.x, g, sh, warp * GPW + lane / G, kWarpsPerCta * GPW);
+}
+
+// ------------------------------------------------------------------------------------------------
+// CTA rows + hub chunks: one CTA per segment; seg < n_chunks is hub chunk `seg` (partial state ->
+// partials[seg]), otherwise the full row perm[n_hub + seg - n_chunks] (finalised in place).
+// smem: NG * (NA*rowe + NS*H) + state_floats + NG * H floats.
+template <class Op>
+__global__ void __launch_bounds__(kCtaThreads)
+segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
+               BinView bins, float* __restrict__ partials, float* da_part, int da_slot) {
+    constexpr int G = Op::kG, NV = Op::kNV, VEC = Op::kVEC;
+    constexpr int GPW = 32 / G, NG = kWarpsPerCta * GPW;
+    extern __shared__ float4 smem4[];
+    float* smem = reinterpret_cast<float*>(smem4);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int gi = warp * GPW + lane / G, gl = lane & (G - 1);
+    typename Op::GeoT g;
+    g.init(sh, lane);
+    const int TEp = Op::NA * sh.rowe + Op::NS * sh.H;  // floats per group partial (without max)
+    const int TE = state_floats<Op>(sh);
+    const int TEs = (TEp + 3) & ~3;     // group stride in smem, keeps float4 stores aligned
+    float* s_part = smem;               // [NG][TEs]
+    float* s_merged = smem + NG * TEs;  // [TE]
+    float* s_max = s_merged + TE;       // [NG][H]
+    float da[NV][VEC];
+#pragma unroll
+    for (int t = 0; t < NV; ++t)
+#pragma unroll
+        for (int c = 0; c < VEC; ++c) da[t][c] = 0.f;
+
+    const int nseg = bins.n_chunks + bins.n_cta;
+    for (int seg = blockIdx.x; seg < nseg; seg += gridDim.x) {
+        int row, e0, e1;
+        const bool partial = seg < bins.n_chunks;
+        if (partial) {
+            const int4 ch = __ldg(reinterpret_cast<const int4*>(bins.chunks) + seg);
+            row = ch.x; e0 = ch.y; e1 = ch.z;
+        } else {
+            row = __ldg(bins.perm + bins.n_hub + (seg - bins.n_chunks));
+            e0 = __ldg(rowptr + row);
+            e1 = __ldg(rowptr + row + 1);
+        }
+        typename Op::Own own;
+        Op::load_own(own, p, sh, row, true, g);
+        typename Op::St st;
+        st.reset();
+        const int nblk = (e1 - e0 + G - 1) / G;
+        for (int b0 = warp * GPW; b0 < nblk; b0 += NG) {
+            const int eb = e0 + (b0 + lane / G) * G;
+            const int my = (eb + gl < e1) ? __ldg(colidx + eb + gl) : -1;
+#pragma unroll 1
+            for (int u0 = 0; u0 < G; u0 += kU) {
+                int nbr[kU];
+#pragma unroll
+                for (int u = 0; u < kU; ++u) nbr[u] = __shfl_sync(0xffffffffu, my, u0 + u, G);
+                if (__all_sync(0xffffffffu, nbr[0] < 0)) break;  // warp-uniform tail exit
+                Op::batch(st, own, p, sh, nbr, g);
+            }
+        }
+        // ---- cross-group merge: global max, rescale, fixed-order sum
+        if (Op::SOFTMAX) {
+#pragma unroll
+            for (int t = 0; t < NV; ++t)
+                if (g.lead[t]) s_max[gi * sh.H + g.hd[t]] = st.m[t];
+            __syncthreads();
+#pragma unroll
+            for (int t = 0; t < NV; ++t) {
+                float mg = -INFINITY;
+                if (g.act[t])
+                    for (int k = 0; k < NG; ++k) mg = fmaxf(mg, s_max[k * sh.H + g.hd[t]]);
+                const float f = (st.m[t] == -INFINITY) ? 0.f : ex2(st.m[t] - mg);
+#pragma unroll
+                for (int a = 0; a < Op::NA; ++a)
+#pragma unroll
+                    for (int c = 0; c < VEC; ++c) st.acc[a][t][c] *= f;
+#pragma unroll
+                for (int s = 0; s < Op::NS; ++s) st.sc[s][t] *= f;
+                st.m[t] = mg;
+            }
+        }
+        state_to_smem<Op>(st, s_part + gi * TEs, g, sh);
+        __syncthreads();
+        for (int e = threadIdx.x; e < TEp; e += kCtaThreads) {
+            float s = 0.f;
+            for (int k = 0; k < NG; ++k) s += s_part[k * TEs + e];
+            s_merged[e] = s;
+        }
+        if (Op::SOFTMAX && gi == 0) {
+#pragma unroll
+            for (int t = 0; t < NV; ++t)
+                if (g.lead[t]) s_merged[TEp + g.hd[t]] = st.m[t];
+        }
+        __syncthreads();
+        if (partial) {
+            for (int e = threadIdx.x; e < TE; e += kCtaThreads) partials[(size_t)seg * TE + e] = s_merged[e];
+        } else if (gi == 0) {
+            state_from_smem<Op>(st, s_merged, g, sh);
+            Op::finalize(st, p, sh, row, g, da);
+        }
+        __syncthreads();
+    }
+    if (Op::HAS_DA) cta_write_da<Op>(da, smem, da_part, da_slot + blockIdx.x, g, sh, gi, NG);
+}
+
+// ------------------------------------------------------------------------------------------------
+// hub rows: merge the chunk partials of hub slot blockIdx.x in ascending chunk order, finalise.
+// smem: state_floats + rowe (da) floats.
+template <class Op>
+__global__ void __launch_bounds__(kCtaThreads)
+hub_merge_kernel(typename Op::Params p, Shape sh, BinView bins, const float* __restrict__ partials, float* da_part,
+                 int da_slot) {
+    constexpr int G = Op::kG, NV = Op::kNV, VEC = Op::kVEC;
+    extern __shared__ float4 smem4[];
+    float* s_merged = reinterpret_cast<float*>(smem4);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    typename Op::GeoT g;
+    g.init(sh, lane);
+    const int TEp = Op::NA * sh.rowe + Op::NS * sh.H;
+    const int TE = state_floats<Op>(sh);
+    const int slot = blockIdx.x;
+    const int c0 = __ldg(bins.chunk_ptr + slot), c1 = __ldg(bins.chunk_ptr + slot + 1);
+    const int row = __ldg(bins.chunks + 4 * c0);
+    if (Op::SOFTMAX) {
+        for (int h = threadIdx.x; h < sh.H; h += kCtaThreads) {
+            float mg = -INFINITY;
+            for (int c = c0; c < c1; ++c) mg = fmaxf(mg, partials[(size_t)c * TE + TEp + h]);
+            s_merged[TEp + h] = mg;
+        }
+        __syncthreads();
+    }
+    for (int e = threadIdx.x; e < TEp; e += kCtaThreads) {
+        const int h = e < Op::NA * sh.rowe ? (e % sh.rowe) / sh.d : (e - Op::NA * sh.rowe) % sh.H;
+        float s = 0.f;
+        if (Op::SOFTMAX) {
+            const float mg = s_merged[TEp + h];
+            for (int c = c0; c < c1; ++c) {
+                const float mc = partials[(size_t)c * TE + TEp + h];
+                const float f = (mc == -INFINITY) ? 0.f : ex2(mc - mg);
+                s += partials[(size_t)c * TE + e] * f;
+            }
+        } else {
+            for (int c = c0; c < c1; ++c) s += partials[(size_t)c * TE + e];
+        }
+        s_merged[e] = s;
+    }
+    __syncthreads();
+    float da[NV][VEC];
+#pragma unroll
+    for (int t = 0; t < NV; ++t)
+#pragma unroll
+        for (int c = 0; c < VEC; ++c) da[t][c] = 0.f;
+    if (warp == 0 && lane < G) {
+        typename Op::St st;
+        state_from_smem<Op>(st, s_merged, g, sh);
+        Op::finalize(st, p, sh, row, g, da);
+        if (Op::HAS_DA) {
+#pragma unroll
+            for (int t = 0; t < NV; ++t)
+                if (g.act[t]) {
+#pragma unroll
+                    for (int c = 0; c < VEC; ++c) da_part[(size_t)(da_slot + slot) * sh.rowe + g.eoff[t] + c] = da[t][c];
+                }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+struct GridPlan {
+    int seg_grid, grp_grid, hub_grid;
+    int da_slots() const { return seg_grid + grp_grid + hub_grid; }
+};
+
+inline GridPlan grid_plan(const BinView& b, int sm_count, int G) {
+    const int GPW = 32 / G;
+    GridPlan gp;
+    const int nseg = b.n_chunks + b.n_cta;
+    gp.seg_grid = nseg < sm_count * 8 ? nseg : sm_count * 8;
+    const int ntiles = (b.n_group + GPW - 1) / GPW;
+    const int nblk = (ntiles + kWarpsPerCta - 1) / kWarpsPerCta;
+    gp.grp_grid = nblk < sm_count * 16 ? nblk : sm_count * 16;
+    gp.hub_grid = b.n_hub;
+    return gp;
+}
+
+template <class Op> inline size_t seg_smem_bytes(const Shape& sh) {
+    constexpr int NG = kWarpsPerCta * (32 / Op::kG);
+    const int TEp = Op::NA * sh.rowe + Op::NS * sh.H;
+    size_t f = (size_t)NG * ((TEp + 3) & ~3) + state_floats<Op>(sh) + (size_t)NG * sh.H;
+    size_t da = Op::HAS_DA ? (size_t)NG * sh.rowe : 0;
+    return 4 * (f > da ? f : da) + 16;
+}
+
+template <class Op> inline cudaError_t run_op(const typename Op::Params& p, const Shape& sh, const LaunchCtx& c) {
+    const BinView& b = c.bins;
+    const GridPlan gp = grid_plan(b, c.sm_count, Op::kG);
+    constexpr int NG = kWarpsPerCta * (32 / Op::kG);
+    int slot = c.da_slot_base;
+    if (gp.seg_grid > 0) {
+        const size_t smem = seg_smem_bytes<Op>(sh);
+        if (smem > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(segment_kernel<Op>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
+        segment_kernel<Op><<<gp.seg_grid, kCtaThreads, smem, c.stream>>>(p, sh, c.rowptr, c.colidx, b, c.partials,
+                                                                         c.da_part, slot);
+        ++g_launches;
+    }
+    slot += gp.seg_grid;
+    if (gp.grp_grid > 0) {
+        const size_t smem = Op::HAS_DA ? 4 * (size_t)NG * sh.rowe + 16 : 16;
+        group_kernel<Op><<<gp.grp_grid, kCtaThreads, smem, c.stream>>>(p, sh, c.rowptr, c.colidx, b.perm,
+                                                                       b.n_hub + b.n_cta, b.n_group, c.da_part, slot);
+        ++g_launches;
+    }
+    slot += gp.grp_grid;
+    if (gp.hub_grid > 0) {
+        const size_t smem = 4 * (size_t)state_floats<Op>(sh) + 16;
+        hub_merge_kernel<Op><<<gp.hub_grid, kCtaThreads, smem, c.stream>>>(p, sh, b, c.partials, c.da_part, slot);
+        ++g_launches;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace gnn

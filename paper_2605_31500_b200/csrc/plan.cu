@@ -1,0 +1,339 @@
+// plan.cu - integer metadata of the hot path, built on the device (rows a1, a2 of the scope table):
+// degree bins + hub chunk table and the transposed CSR by a stable
+// sort on the source id.  Pure functions of (rowptr, colidx, opts); the numpy
+// reference in oracle/plan_ref.py states the same definitions independently and the tests compare
+// bit for bit.  Sorting / scanning uses CUB's stable LSD radix sort (a library primitive, one-time
+// preprocessing outside the timed layer, like the paper's format construction).
+#include <cub/device/device_radix_sort.cuh>
+
+#include <new>
+
+#include "internal.h"
+
+namespace gnn {
+extern unsigned long long g_launches;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+__device__ __forceinline__ int bit_length(int x) { return 32 - __clz(x); }
+
+// key(i): 0 hub; 1 + (32 - bl(deg)) CTA rows; 34 + (32 - bl(deg)) group rows
+__global__ void key_kernel(const int32_t* __restrict__ rowptr, int n, int warp_max, int cta_max,
+                           uint32_t* __restrict__ key, int32_t* __restrict__ rowid) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int deg = rowptr[i + 1] - rowptr[i];
+    const int bl = bit_length(deg);
+    uint32_t k = 34 + (32 - bl);
+    if (deg > warp_max) k = 1 + (32 - bl);
+    if (deg > cta_max) k = 0;
+    key[i] = k;
+    rowid[i] = i;
+}
+
+__device__ int lower_bound_u32(const uint32_t* a, int n, uint32_t v) {
+    int lo = 0, hi = n;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (a[mid] < v) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+// counts[0..3] = n_hub, n_cta, n_group, n_chunks; chunk_ptr[0..n_hub]  (single thread: n_hub is small)
+__global__ void count_kernel(const uint32_t* __restrict__ key_sorted, const int32_t* __restrict__ perm,
+                             const int32_t* __restrict__ rowptr, int n, int split, int32_t* __restrict__ counts,
+                             int32_t* __restrict__ chunk_ptr, int max_hub) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int n_hub = lower_bound_u32(key_sorted, n, 1u);
+    const int n_heavy = lower_bound_u32(key_sorted, n, 34u);
+    int acc = 0;
+    chunk_ptr[0] = 0;
+    for (int s = 0; s < n_hub && s < max_hub; ++s) {
+        const int r = perm[s];
+        const int g = rowptr[r + 1] - rowptr[r];
+        acc += (g + split - 1) / split;
+        chunk_ptr[s + 1] = acc;
+    }
+    counts[0] = n_hub;
+    counts[1] = n_heavy - n_hub;
+    counts[2] = n - n_heavy;
+    counts[3] = acc;
+}
+
+// one CTA per hub slot: chunk t = [b + floor(t g / c), b + floor((t+1) g / c))
+__global__ void chunk_kernel(const int32_t* __restrict__ perm, const int32_t* __restrict__ rowptr,
+                             const int32_t* __restrict__ chunk_ptr, int32_t* __restrict__ chunks) {
+    const int slot = blockIdx.x;
+    const int r = perm[slot];
+    const int b = rowptr[r];
+    const long long g = rowptr[r + 1] - b;
+    const int c0 = chunk_ptr[slot];
+    const long long c = chunk_ptr[slot + 1] - c0;
+    for (int t = threadIdx.x; t < c; t += blockDim.x) {
+        int4 v;
+        v.x = r;
+        v.y = b + (int)((t * g) / c);
+        v.z = b + (int)(((t + 1) * g) / c);
+        v.w = slot;
+        reinterpret_cast<int4*>(chunks)[c0 + t] = v;
+    }
+}
+
+__global__ void row_of_edge_kernel(const int32_t* __restrict__ rowptr, int n, long long nnz,
+                                   int32_t* __restrict__ row_of_edge) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= nnz) return;
+    int lo = 0, hi = n;  // last row with rowptr[row] <= e
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if ((long long)rowptr[mid] <= e) lo = mid; else hi = mid;
+    }
+    row_of_edge[e] = lo;
+}
+
+// rowptr_t[j] = number of entries with source id < j = lower_bound(sorted source ids, j)
+__global__ void rowptr_t_kernel(const uint32_t* __restrict__ src_sorted, long long nnz, int n,
+                                int32_t* __restrict__ rowptr_t) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j > n) return;
+    long long lo = 0, hi = nnz;
+    while (lo < hi) {
+        const long long mid = (lo + hi) >> 1;
+        if (src_sorted[mid] < (uint32_t)j) lo = mid + 1; else hi = mid;
+    }
+    rowptr_t[j] = (int32_t)lo;
+}
+
+struct Layout {
+    // persistent
+    size_t perm, chunks, chunk_ptr, counts, rowptr_t, colidx_t, perm_t, chunks_t, chunk_ptr_t, dev_total;
+    // scratch
+    size_t key, key_sorted, rowid, ekey_sorted, erow, cub, scratch_total;
+    size_t cub_bytes;
+    long long max_chunks, max_hub;
+};
+
+gnn_plan_opts_t resolve(const gnn_plan_opts_t* o) {
+    gnn_plan_opts_t r = {256, 8192, 4096, 0, 0};
+    if (o) {
+        if (o->warp_max_deg > 0) r.warp_max_deg = o->warp_max_deg;
+        if (o->cta_max_deg > 0) r.cta_max_deg = o->cta_max_deg;
+        if (o->split_chunk > 0) r.split_chunk = o->split_chunk;
+        r.build_transpose = o->build_transpose;
+        r.build_blocks = o->build_blocks;
+    }
+    if (r.cta_max_deg < r.warp_max_deg) r.cta_max_deg = r.warp_max_deg;
+    return r;
+}
+
+int n_bits(int n) {
+    int b = 1;
+    while (b < 32 && (1ll << b) < (long long)n) ++b;
+    return b;
+}
+
+cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout& L) {
+    L.max_hub = nnz / (o.cta_max_deg + 1) + 1;
+    L.max_chunks = nnz / o.split_chunk + L.max_hub + 1;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t at = off; off += up(bytes); return at; };
+    L.perm = take(sizeof(int32_t) * (size_t)n);
+    L.chunks = take(sizeof(int32_t) * 4 * (size_t)L.max_chunks);
+    L.chunk_ptr = take(sizeof(int32_t) * (size_t)(L.max_hub + 1));
+    L.counts = take(sizeof(int32_t) * 8);
+    L.rowptr_t = L.colidx_t = L.perm_t = L.chunks_t = L.chunk_ptr_t = 0;
+    if (o.build_transpose) {
+        L.rowptr_t = take(sizeof(int32_t) * ((size_t)n + 1));
+        L.colidx_t = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
+        L.perm_t = take(sizeof(int32_t) * (size_t)n);
+        L.chunks_t = take(sizeof(int32_t) * 4 * (size_t)L.max_chunks);
+        L.chunk_ptr_t = take(sizeof(int32_t) * (size_t)(L.max_hub + 1));
+    }
+    L.dev_total = off;
+    size_t t1 = 0, t2 = 0;
+    cudaError_t e = cub::DeviceRadixSort::SortPairs(nullptr, t1, (const uint32_t*)nullptr, (uint32_t*)nullptr,
+                                                    (const int32_t*)nullptr, (int32_t*)nullptr, (long long)n, 0, 7);
+    if (e != cudaSuccess) return e;
+    if (o.build_transpose) {
+        e = cub::DeviceRadixSort::SortPairs(nullptr, t2, (const uint32_t*)nullptr, (uint32_t*)nullptr,
+                                            (const int32_t*)nullptr, (int32_t*)nullptr, (long long)nnz, 0, n_bits(n));
+        if (e != cudaSuccess) return e;
+    }
+    L.cub_bytes = t1 > t2 ? t1 : t2;
+    off = 0;
+    L.key = take(sizeof(uint32_t) * (size_t)n);
+    L.key_sorted = take(sizeof(uint32_t) * (size_t)n);
+    L.rowid = take(sizeof(int32_t) * (size_t)n);
+    L.ekey_sorted = L.erow = 0;
+    if (o.build_transpose) {
+        L.ekey_sorted = take(sizeof(uint32_t) * (size_t)(nnz > 0 ? nnz : 1));
+        L.erow = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
+    }
+    L.cub = take(L.cub_bytes + 16);
+    L.scratch_total = off;
+    return cudaSuccess;
+}
+
+// bins + chunk table of one CSR (rowptr); synchronises to read the counts back
+cudaError_t build_bins(const int32_t* rowptr, int n, const gnn_plan_opts_t& o, const Layout& L, char* scratch,
+                       int32_t* perm, int32_t* chunks, int32_t* chunk_ptr, int32_t* counts_dev, int32_t* counts_host,
+                       cudaStream_t st) {
+    uint32_t* key = (uint32_t*)(scratch + L.key);
+    uint32_t* key_sorted = (uint32_t*)(scratch + L.key_sorted);
+    int32_t* rowid = (int32_t*)(scratch + L.rowid);
+    const int tb = 256;
+    key_kernel<<<(n + tb - 1) / tb, tb, 0, st>>>(rowptr, n, o.warp_max_deg, o.cta_max_deg, key, rowid);
+    size_t cb = L.cub_bytes;
+    cudaError_t e = cub::DeviceRadixSort::SortPairs(scratch + L.cub, cb, (const uint32_t*)key, key_sorted,
+                                                    (const int32_t*)rowid, perm, (long long)n, 0, 7, st);
+    if (e != cudaSuccess) return e;
+    count_kernel<<<1, 32, 0, st>>>(key_sorted, perm, rowptr, n, o.split_chunk, counts_dev, chunk_ptr, (int)L.max_hub);
+    g_launches += 3;
+    e = cudaMemcpyAsync(counts_host, counts_dev, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return e;
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return e;
+    if (counts_host[0] > 0) {
+        chunk_kernel<<<counts_host[0], 128, 0, st>>>(perm, rowptr, chunk_ptr, chunks);
+        ++g_launches;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace
+}  // namespace gnn
+
+using namespace gnn;
+
+extern "C" gnn_status_t gnn_plan_bytes(int32_t n, int64_t nnz, const gnn_plan_opts_t* opts, size_t* dev_bytes,
+                                       size_t* scratch_bytes) {
+    if (n < 1 || nnz < 0 || nnz >= (1ll << 31) || !dev_bytes || !scratch_bytes) {
+        set_error("gnn_plan_bytes: need n >= 1, 0 <= nnz < 2^31 and non-NULL outputs");
+        return GNN_EINVAL;
+    }
+    const gnn_plan_opts_t o = resolve(opts);
+    Layout L;
+    cudaError_t e = make_layout(n, nnz, o, L);
+    if (e != cudaSuccess) {
+        set_error("gnn_plan_bytes: CUDA error: %s", cudaGetErrorString(e));
+        return GNN_ECUDA;
+    }
+    *dev_bytes = L.dev_total;
+    *scratch_bytes = L.scratch_total;
+    return GNN_OK;
+}
+
+extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t dev_bytes, void* scratch,
+                                       size_t scratch_bytes, int32_t n, int64_t nnz, const int32_t* rowptr,
+                                       const int32_t* colidx, const gnn_plan_opts_t* opts, gnn_stream_t stream) {
+    if (!plan || !dev_mem || !scratch || !rowptr || (!colidx && nnz > 0) || n < 1 || nnz < 0 || nnz >= (1ll << 31)) {
+        set_error("gnn_plan_build: NULL pointer or bad sizes (n=%d nnz=%lld)", n, (long long)nnz);
+        return GNN_EINVAL;
+    }
+    if (((uintptr_t)dev_mem | (uintptr_t)scratch) & 255) {
+        set_error("gnn_plan_build: dev_mem and scratch must be 256-byte aligned");
+        return GNN_EINVAL;
+    }
+    const gnn_plan_opts_t o = resolve(opts);
+    if (o.build_blocks) {
+        set_error("gnn_plan_build: build_blocks is not available in this build");
+        return GNN_EUNSUPPORTED;
+    }
+    Layout L;
+    cudaError_t e = make_layout(n, nnz, o, L);
+    if (e != cudaSuccess) {
+        set_error("gnn_plan_build: CUDA error: %s", cudaGetErrorString(e));
+        return GNN_ECUDA;
+    }
+    if (dev_bytes < L.dev_total || scratch_bytes < L.scratch_total) {
+        set_error("gnn_plan_build: storage too small (dev %zu < %zu or scratch %zu < %zu)", dev_bytes, L.dev_total,
+                  scratch_bytes, L.scratch_total);
+        return GNN_EWORKSPACE;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    char* dm = (char*)dev_mem;
+    char* sc = (char*)scratch;
+    gnn_plan* P = new (std::nothrow) gnn_plan();
+    if (!P) { set_error("gnn_plan_build: out of host memory"); return GNN_EINVAL; }
+    P->n = n; P->nnz = nnz; P->opts = o; P->rowptr = rowptr; P->colidx = colidx;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&P->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    int32_t* counts_dev = (int32_t*)(dm + L.counts);
+    int32_t hc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    e = build_bins(rowptr, n, o, L, sc, (int32_t*)(dm + L.perm), (int32_t*)(dm + L.chunks),
+                   (int32_t*)(dm + L.chunk_ptr), counts_dev, hc, st);
+    if (e == cudaSuccess && o.build_transpose) {
+        P->rowptr_t = (int32_t*)(dm + L.rowptr_t);
+        P->colidx_t = (int32_t*)(dm + L.colidx_t);
+        uint32_t* ekey_sorted = (uint32_t*)(sc + L.ekey_sorted);
+        int32_t* erow = (int32_t*)(sc + L.erow);
+        if (nnz > 0) {
+            row_of_edge_kernel<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(rowptr, n, nnz, erow);
+            ++g_launches;
+            size_t cb = L.cub_bytes;
+            e = cub::DeviceRadixSort::SortPairs(sc + L.cub, cb, (const uint32_t*)colidx, ekey_sorted,
+                                                (const int32_t*)erow, P->colidx_t, (long long)nnz, 0, n_bits(n), st);
+        }
+        if (e == cudaSuccess) {
+            rowptr_t_kernel<<<(n + 1 + 255) / 256, 256, 0, st>>>(ekey_sorted, nnz, n, P->rowptr_t);
+            ++g_launches;
+            e = build_bins(P->rowptr_t, n, o, L, sc, (int32_t*)(dm + L.perm_t), (int32_t*)(dm + L.chunks_t),
+                           (int32_t*)(dm + L.chunk_ptr_t), counts_dev + 4, hc + 4, st);
+        }
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+        set_error("gnn_plan_build: CUDA error: %s", cudaGetErrorString(e));
+        delete P;
+        return GNN_ECUDA;
+    }
+    P->fwd = BinView{(int32_t*)(dm + L.perm), (int32_t*)(dm + L.chunks), (int32_t*)(dm + L.chunk_ptr), hc[0], hc[1], hc[2], hc[3]};
+    if (o.build_transpose)
+        P->tr = BinView{(int32_t*)(dm + L.perm_t), (int32_t*)(dm + L.chunks_t), (int32_t*)(dm + L.chunk_ptr_t), hc[4], hc[5], hc[6], hc[7]};
+    *plan = P;
+    return GNN_OK;
+}
+
+extern "C" void gnn_plan_destroy(gnn_plan_t* plan) { delete plan; }
+
+extern "C" const int32_t* gnn_plan_rowptr_t(const gnn_plan_t* plan) { return plan ? plan->rowptr_t : nullptr; }
+extern "C" const int32_t* gnn_plan_colidx_t(const gnn_plan_t* plan) { return plan ? plan->colidx_t : nullptr; }
+
+extern "C" gnn_status_t gnn_plan_export(const gnn_plan_t* P, int what, void* host_dst, size_t* bytes) {
+    if (!P || !bytes) { set_error("gnn_plan_export: NULL plan or bytes"); return GNN_EINVAL; }
+    const void* src = nullptr;
+    size_t need = 0;
+    int32_t counts[8] = {P->fwd.n_hub, P->fwd.n_cta, P->fwd.n_group, P->fwd.n_chunks,
+                         P->tr.n_hub, P->tr.n_cta, P->tr.n_group, P->tr.n_chunks};
+    const bool T = P->opts.build_transpose != 0;
+    switch (what) {
+        case GNN_PLAN_COUNTS: need = sizeof(counts); break;
+        case GNN_PLAN_PERM: src = P->fwd.perm; need = 4 * (size_t)P->n; break;
+        case GNN_PLAN_CHUNKS: src = P->fwd.chunks; need = 16 * (size_t)P->fwd.n_chunks; break;
+        case GNN_PLAN_CHUNK_PTR: src = P->fwd.chunk_ptr; need = 4 * ((size_t)P->fwd.n_hub + 1); break;
+        case GNN_PLAN_ROWPTR_T: if (T) { src = P->rowptr_t; need = 4 * ((size_t)P->n + 1); } break;
+        case GNN_PLAN_COLIDX_T: if (T) { src = P->colidx_t; need = 4 * (size_t)P->nnz; } break;
+        case GNN_PLAN_PERM_T: if (T) { src = P->tr.perm; need = 4 * (size_t)P->n; } break;
+        case GNN_PLAN_CHUNKS_T: if (T) { src = P->tr.chunks; need = 16 * (size_t)P->tr.n_chunks; } break;
+        case GNN_PLAN_CHUNK_PTR_T: if (T) { src = P->tr.chunk_ptr; need = 4 * ((size_t)P->tr.n_hub + 1); } break;
+        default: break;
+    }
+    if (what != GNN_PLAN_COUNTS && !src) {
+        set_error("gnn_plan_export: item %d is not part of this plan", what);
+        return GNN_EINVAL;
+    }
+    const size_t cap = *bytes;
+    *bytes = need;
+    if (!host_dst) return GNN_OK;
+    if (cap < need) { set_error("gnn_plan_export: buffer too small (%zu < %zu)", cap, need); return GNN_EWORKSPACE; }
+    if (what == GNN_PLAN_COUNTS) { memcpy(host_dst, counts, need); return GNN_OK; }
+    if (need == 0) return GNN_OK;
+    cudaError_t e = cudaMemcpy(host_dst, src, need, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) { set_error("gnn_plan_export: CUDA error: %s", cudaGetErrorString(e)); return GNN_ECUDA; }
+    return GNN_OK;
+}
