@@ -1,0 +1,457 @@
+#!/usr/bin/env python
+"""bench.py - fused GT / GATv2 attention forward+backward GEdges/s on one BASELINE.json workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--cfg C] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (plan resident; forward + backward = dst pass + src pass)
+over the config's synthetic graph.  Prints ONE JSON line (see DESIGN.md section 8 for every key).
+`value` = edges * ranks / max-over-ranks device time, inputs resident in HBM.  `e2e` = the same metric with
+the host->device copies of every input and the device->host copies of every output inside the timed region.
+`--impl reference` times the fp64 CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import gnn_inputs as GI  # noqa: E402
+
+METRIC = "fused GT/GATv2 attn GEdges/s (fwd+bwd)"
+UNIT = "GEdges/s"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--cfg", type=int, default=3, help="BASELINE.json config 1..5 (default 3: the large power-law GT graph)")
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink the workload (debug only; < 1 is not a bench value)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--warp-max-deg", type=int, default=0)
+    ap.add_argument("--cta-max-deg", type=int, default=0)
+    ap.add_argument("--split-chunk", type=int, default=0)
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------ byte model
+def byte_model(c, plan_counts, deg_in, deg_out, perm, perm_t):
+    """Algorithmic bytes per kernel launch (SURVEY.md section 8(d) per-edge / per-node figures x units) and
+    compulsory bytes per pass (every array read or written once)."""
+    n, e, H, d = c["n"], c["e"], c["heads"], c["head_dim"]
+    b = 4 if c["dtype"] == "f32" else 2
+    R = H * d
+    if c["layer"] == "gt":
+        per = {  # pass: (bytes per edge, bytes per row)
+            "gt_fwd": (4 + 2 * R * b, 8 + 2 * R * b + 4 * H),
+            "gt_bwd_dst": (4 + 2 * R * b, 8 + 2 * R * b + 4 * H + 4 * R + 4 * H),
+            "gt_bwd_src": (4 + 2 * R * b + 8 * H, 8 + 2 * R * b + 8 * R),
+        }
+        csr = 4 * (n + 1) + 4 * e
+        comp = {"fwd": csr + 4 * n * R * b + 4 * n * H,
+                "bwd": 2 * csr + 4 * n * R * b + 4 * n * H + 12 * n * R + 8 * n * H}
+    else:
+        per = {
+            "gatv2_fwd": (4 + R * b, 8 + 2 * R * b + 4 * H),
+            "gatv2_bwd_dst": (4 + R * b, 8 + 2 * R * b + 4 * H + 4 * R + 4 * H),
+            "gatv2_bwd_src": (4 + 2 * R * b + 8 * H, 8 + R * b + 4 * R),
+        }
+        csr = 4 * (n + 1) + 4 * e
+        comp = {"fwd": csr + 3 * n * R * b + 4 * n * H + 4 * R,
+                "bwd": 2 * csr + 3 * n * R * b + 4 * n * H + 8 * n * R + 8 * n * H + 8 * R}
+    alg = {}
+    for ps, (pe, pn) in per.items():
+        t = ps.endswith("_src")
+        deg, pm = (deg_out, perm_t) if t else (deg_in, perm)
+        sfx = "_t" if t else ""
+        nh, nc = plan_counts["n_hub" + sfx], plan_counts["n_cta" + sfx]
+        ng, nch = plan_counts["n_group" + sfx], plan_counts["n_chunks" + sfx]
+        e_heavy = int(deg[pm[: nh + nc]].sum())
+        e_group = int(deg[pm[nh + nc:]].sum())
+        alg[ps + "/segment"] = e_heavy * pe + (nc + nch) * pn
+        alg[ps + "/group"] = e_group * pe + ng * pn
+    return alg, comp
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 8:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        os.unlink(self.f.name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------ oracle arm
+def oracle_sample_pass(c, f32, rows, srcs, rp_t, ci_t):
+    """One pass of the fp64 oracle over `rows` (forward + dst-side backward) and `srcs` (src-side backward).
+    Returns seconds per stage.  L / Delta for destinations outside `rows` are placeholders in the src stage
+    (timing only; these outputs are discarded)."""
+    import oracle
+    n, H = c["n"], c["heads"]
+    rp, ci = c["rowptr"], c["colidx"]
+    t = {}
+    if c["layer"] == "gt":
+        q, k, v, do = f32["q"], f32["k"], f32["v"], f32["do"]
+        t0 = time.perf_counter()
+        O, L = oracle.gt_forward(rp, ci, q, k, v, rows=rows)
+        t["fwd"] = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        Dl = oracle.rowdot(O, do, rows=rows)
+        Lf, Df = np.zeros((n, H)), np.zeros((n, H))
+        Lf[rows], Df[rows] = L, Dl
+        oracle.gt_backward_dst(rp, ci, q, k, v, do, Lf, Df, rows=rows)
+        t["bwd_dst"] = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        oracle.gt_backward_src(rp_t, ci_t, q, k, v, do, Lf, Df, srcs=srcs)
+        t["bwd_src"] = time.perf_counter() - t0
+    else:
+        xl, xr, a, do, sl = f32["xl"], f32["xr"], c["a_f32"], f32["do"], c["slope"]
+        t0 = time.perf_counter()
+        O, L = oracle.gatv2_forward(rp, ci, xl, xr, a, sl, rows=rows)
+        t["fwd"] = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        Gv = oracle.rowdot(O, do, rows=rows)
+        Lf, Gf = np.zeros((n, H)), np.zeros((n, H))
+        Lf[rows], Gf[rows] = L, Gv
+        oracle.gatv2_backward_dst(rp, ci, xl, xr, a, sl, do, Lf, Gf, rows=rows)
+        t["bwd_dst"] = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        oracle.gatv2_backward_src(rp_t, ci_t, xl, xr, a, sl, do, Lf, Gf, srcs=srcs)
+        t["bwd_src"] = time.perf_counter() - t0
+    return t
+
+
+class OracleArm:
+    """Times oracle/ (as it stands) on a bounded sample: uniformly drawn destination rows for the forward and
+    the dst-side backward, uniformly drawn source rows of the oracle's own CSR^T for the src-side backward.
+    GEdges/s = 1 / (sum over the three stages of seconds per sampled edge)."""
+
+    def __init__(self, c, target_seconds: float):
+        import oracle
+        from oracle import plan_ref
+        oracle.build()
+        self.c = c
+        self.cores = oracle.num_threads()
+        names = ("q", "k", "v", "do") if c["layer"] == "gt" else ("xl", "xr", "do")
+        self.f32 = {}
+        for nm in names:
+            x = c.get(nm + "_f32")
+            self.f32[nm] = x if x is not None else GI.bf16_bits_to_f32(c[nm + "_st"])
+        self.rp_t, self.ci_t = plan_ref.transpose_csr(c["rowptr"], c["colidx"])
+        rng = np.random.default_rng(12345)
+        n = c["n"]
+        self.order_r = rng.permutation(n).astype(np.int32)
+        self.order_s = rng.permutation(n).astype(np.int32)
+        self.deg_in = np.diff(c["rowptr"].astype(np.int64))
+        self.deg_out = np.diff(self.rp_t.astype(np.int64))
+        # calibrate the sample size on a small probe
+        k = min(n, 2000)
+        t = self.run(k, k)
+        per_row = sum(t.values()) / k
+        self.k = int(max(64, min(n, target_seconds / max(per_row, 1e-9))))
+
+    def run(self, kr=None, ks=None):
+        kr = self.k if kr is None else kr
+        ks = self.k if ks is None else ks
+        rows, srcs = np.sort(self.order_r[:kr]), np.sort(self.order_s[:ks])
+        self.er, self.es = int(self.deg_in[rows].sum()), int(self.deg_out[srcs].sum())
+        return oracle_sample_pass(self.c, self.f32, rows, srcs, self.rp_t, self.ci_t)
+
+    def gedges(self, t) -> float:
+        sec_per_edge = t["fwd"] / max(self.er, 1) + t["bwd_dst"] / max(self.er, 1) + t["bwd_src"] / max(self.es, 1)
+        return 1e-9 / sec_per_edge
+
+    def sample_text(self) -> str:
+        return (f"{self.k} uniformly drawn dst rows ({self.er} edges: fwd + dst-side bwd) and {self.k} src rows "
+                f"({self.es} edges: src-side bwd) of the full-size {self.c['name']} graph; per-edge stage times summed")
+
+
+def workload_config(c, args):
+    return {"workload": c["name"], "layer": c["layer"], "nodes": c["n"], "edges": c["e"], "heads": c["heads"],
+            "head_dim": c["head_dim"], "feature_dtype": c["dtype"], "scale": args.scale,
+            "graph": "synthetic seeded generator (gnn_inputs), stands in for the paper's datasets"}
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False)
+    arm = OracleArm(c, target_seconds=min(args.cpu_seconds, 20.0))
+    for _ in range(args.warmup):
+        arm.run()
+    t0 = time.perf_counter()
+    vals = []
+    for _ in range(args.steps):
+        vals.append(arm.gedges(arm.run()))
+    wall = time.perf_counter() - t0
+    v = float(len(vals) / sum(1.0 / x for x in vals))
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(args.steps, 1), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(c, args),
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": arm.cores, "kind": "oracle", "sample": arm.sample_text()},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------ CUDA arm
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2605_31500_b200 as G
+    import paper_2605_31500_b200.binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback (use --impl reference for the oracle arm)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False)   # replicas: every rank runs the same workload
+    n, e, H, d, dt = c["n"], c["e"], c["heads"], c["head_dim"], c["dtype"]
+    gt = c["layer"] == "gt"
+    names = ("q", "k", "v", "do") if gt else ("xl", "xr", "do")
+
+    def to_torch(a):
+        t = torch.from_numpy(np.ascontiguousarray(a))
+        return t.view(torch.bfloat16) if (dt == "bf16" and a.dtype == np.uint16) else t
+
+    host = {nm: to_torch(c[nm + "_st"]) for nm in names}
+    host["rowptr"], host["colidx"] = torch.from_numpy(c["rowptr"]), torch.from_numpy(c["colidx"])
+    if not gt:
+        host["a"] = torch.from_numpy(c["a_f32"])
+    devt = {k: v.to(dev) for k, v in host.items()}
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    plan = G.Plan(devt["rowptr"], devt["colidx"], warp_max_deg=args.warp_max_deg, cta_max_deg=args.cta_max_deg,
+                  split_chunk=args.split_chunk, transpose=True)
+    torch.cuda.synchronize()
+    plan_ms = 1e3 * (time.perf_counter() - t0)
+
+    f32 = dict(dtype=torch.float32, device=dev)
+    out = torch.empty((n, H, d), dtype=devt[names[0]].dtype, device=dev)
+    lse, stat = torch.empty((n, H), **f32), torch.empty((n, H), **f32)
+    g1, g2 = torch.empty((n, H, d), **f32), torch.empty((n, H, d), **f32)
+    g3 = torch.empty((n, H, d), **f32) if gt else torch.empty((H, d), **f32)
+
+    if gt:
+        def fwd():
+            G.gnn_gt_attn_fwd(plan, devt["q"], devt["k"], devt["v"], out, lse)
+
+        def bwd():
+            G.gnn_gt_attn_bwd(plan, devt["q"], devt["k"], devt["v"], lse, devt["do"], stat, g1, g2, g3)
+    else:
+        def fwd():
+            G.gnn_gatv2_fwd(plan, devt["xl"], devt["xr"], devt["a"], c["slope"], out, lse)
+
+        def bwd():
+            G.gnn_gatv2_bwd(plan, devt["xl"], devt["xr"], devt["a"], lse, devt["do"], c["slope"], stat, g1, g2, g3)
+
+    def step():
+        fwd()
+        bwd()
+
+    in_bytes = sum(int(v.numel()) * v.element_size() for v in host.values())
+    outs = [out, lse, stat, g1, g2, g3]
+    out_bytes = sum(int(v.numel()) * v.element_size() for v in outs)
+    l2_bytes = torch.cuda.get_device_properties(dev).L2_cache_size
+    need_flush = in_bytes < 4 * l2_bytes
+    flush = torch.empty(max(2 * l2_bytes, 1 << 28), dtype=torch.uint8, device=dev) if need_flush else None
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, k):
+        """sum of per-step CUDA-event times (ms); L2 flushed between steps (outside the events) for small inputs"""
+        evs = []
+        for _ in range(k):
+            if flush is not None:
+                flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            evs.append((a, b))
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in evs]
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    clocks = ClockSampler(local_rank)
+    l0 = G.gnn_launch_count()
+    ms_steps = timed(step, args.steps)
+    launches = G.gnn_launch_count() - l0
+    barrier()
+    ms_fwd = timed(fwd, args.steps)
+    ms_bwd = timed(bwd, args.steps)
+    clk = clocks.stop()
+    total_ms = float(sum(ms_steps))
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = world * e * args.steps / (total_ms * 1e-3) * 1e-9
+
+    # ---- per-kernel device times (library event profiler), same inputs, right after the timed region
+    G.gnn_profile_enable(True)
+    for _ in range(args.steps):
+        if flush is not None:
+            flush.zero_()
+        step()
+    G.gnn_profile_enable(False)
+    recs = G.gnn_profile_collect(64 * args.steps + 64)
+    kern = {}
+    for nm, ms in recs:
+        kern.setdefault(nm, []).append(ms)
+    kern_ms = {k: float(np.mean(v)) for k, v in kern.items()}
+
+    # ---- byte model and rooflines
+    cnt = plan.counts()
+    perm, perm_t = plan.export(B.GNN_PLAN_PERM), plan.export(B.GNN_PLAN_PERM_T)
+    deg_in = np.diff(c["rowptr"].astype(np.int64))
+    deg_out = np.diff(plan.export(B.GNN_PLAN_ROWPTR_T).astype(np.int64))
+    alg, comp = byte_model(c, cnt, deg_in, deg_out, perm, perm_t)
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    else:
+        peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+    dom = max((k for k in kern_ms if k in alg), key=lambda k: kern_ms[k])
+    achieved = alg[dom] / (kern_ms[dom] * 1e-3) * 1e-9
+    step_ms = total_ms / args.steps
+    comp_step = comp["fwd"] + comp["bwd"]
+    roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom],
+            "kernel_ms": kern_ms[dom], "kernel_share_of_step": kern_ms[dom] / sum(kern_ms.values()),
+            "kernels_ms": kern_ms,
+            "kernels_algorithmic_gbs": {k: alg[k] / (kern_ms[k] * 1e-3) * 1e-9 for k in kern_ms if k in alg and kern_ms[k] > 0},
+            "compulsory": {"bytes_fwd": comp["fwd"], "bytes_bwd": comp["bwd"],
+                           "gbs_fwd": comp["fwd"] / (np.mean(ms_fwd) * 1e-3) * 1e-9,
+                           "gbs_bwd": comp["bwd"] / (np.mean(ms_bwd) * 1e-3) * 1e-9,
+                           "gbs_step": comp_step / (step_ms * 1e-3) * 1e-9,
+                           "frac_fwd": comp["fwd"] / (np.mean(ms_fwd) * 1e-3) * 1e-9 / peak,
+                           "frac_bwd": comp["bwd"] / (np.mean(ms_bwd) * 1e-3) * 1e-9 / peak,
+                           "frac_step": comp_step / (step_ms * 1e-3) * 1e-9 / peak}}
+
+    # ---- end to end: pinned host inputs -> device, step, every output -> pinned host, all inside the events
+    e2e = None
+    if args.e2e_steps > 0:
+        pin_in = {k: v.pin_memory() for k, v in host.items()}
+        pin_out = [torch.empty(o.shape, dtype=o.dtype, pin_memory=True) for o in outs]
+
+        def e2e_step():
+            for k2, v in pin_in.items():
+                devt[k2].copy_(v, non_blocking=True)
+            step()
+            for po, o in zip(pin_out, outs):
+                po.copy_(o, non_blocking=True)
+
+        e2e_step()
+        barrier()
+        ms_e2e = timed(e2e_step, args.e2e_steps)
+        t_e2e = float(sum(ms_e2e))
+        if world > 1:
+            t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_e2e = float(t.item())
+        e2e = {"value": world * e * args.e2e_steps / (t_e2e * 1e-3) * 1e-9, "unit": UNIT,
+               "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes, "steps": args.e2e_steps,
+               "ms_per_step": t_e2e / args.e2e_steps}
+        del pin_in, pin_out
+    peak_mem = int(torch.cuda.max_memory_allocated(dev))
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        arm = OracleArm(c, args.cpu_seconds)
+        cpu = {"value": arm.gedges(arm.run()), "unit": UNIT, "cores": arm.cores, "kind": "oracle", "sample": arm.sample_text()}
+
+    if rank == 0:
+        cfgd = workload_config(c, args)
+        cfgd.update({"l2": "L2 flushed between timed steps" if need_flush else "inputs larger than L2 (no flush)",
+                     "plan": cnt, "plan_opts": {"warp_max_deg": plan.opts.warp_max_deg, "cta_max_deg": plan.opts.cta_max_deg,
+                                                "split_chunk": plan.opts.split_chunk},
+                     "plan_build_ms": plan_ms, "degree_stats": GI.degree_stats(c["rowptr"], c["colidx"])})
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfgd,
+                "ms_fwd": float(np.mean(ms_fwd)), "ms_bwd": float(np.mean(ms_bwd)),
+                "gedges_fwd": e / (np.mean(ms_fwd) * 1e-3) * 1e-9, "gedges_bwd": e / (np.mean(ms_bwd) * 1e-3) * 1e-9,
+                "peak_device_bytes": peak_mem, "device_bytes_inputs": in_bytes, "device_bytes_outputs": out_bytes,
+                "plan_bytes": plan.plan_bytes, "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
+                "roofline": roof, "cpu_baseline": cpu}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

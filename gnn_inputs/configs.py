@@ -2,10 +2,13 @@
 
 ``make_config(cfg, scale)`` returns a dict with the graph (int32 CSR, row = dst) and the
 feature tensors in storage dtype (``*_st``: fp32 array, or uint16 bf16 bit patterns) plus
-their exact fp32 up-casts (``*_f32``) for the oracle.  ``scale`` < 1 shrinks node and edge
+their exact fp32 up-casts (``*_f32``) for the oracle (``keep_f32=False`` skips the up-cast copies of
+bf16 tensors to save host memory at full size; ``gnn_inputs.bf16_bits_to_f32`` recreates them).  ``scale`` < 1 shrinks node and edge
 counts proportionally (parity tests); scale = 1 is the BASELINE.json size.
 """
 from __future__ import annotations
+
+from concurrent.futures import ThreadPoolExecutor
 
 import numpy as np
 
@@ -50,14 +53,17 @@ def _graph(cfg: int, scale: float, seed: int):
     raise ValueError(cfg)
 
 
-def make_config(cfg: int, scale: float = 1.0, seed: int = 0, with_grads: bool = True) -> dict:
+def make_config(cfg: int, scale: float = 1.0, seed: int = 0, with_grads: bool = True, keep_f32: bool = True) -> dict:
     c = dict(CONFIGS[cfg])
     n, (rowptr, colidx) = _graph(cfg, scale, seed)
     h, d, dt = c["heads"], c["head_dim"], c["dtype"]
     out = dict(c, cfg=cfg, scale=scale, seed=seed, n=n, e=int(colidx.size), rowptr=rowptr, colidx=colidx)
     if c["layer"] == "gt":
-        for name, stream in (("q", 10), ("k", 11), ("v", 12)) + ((("do", 13),) if with_grads else ()):
-            st, f32 = store(normal_tensor(rng_for(cfg, stream, seed), (n, h, d)), dt)
+        names = (("q", 10), ("k", 11), ("v", 12)) + ((("do", 13),) if with_grads else ())
+        # independent streams -> drawn in parallel threads (numpy releases the GIL); same values either way
+        with ThreadPoolExecutor(max_workers=len(names)) as ex:
+            res = list(ex.map(lambda ns: store(normal_tensor(rng_for(cfg, ns[1], seed), (n, h, d)), dt, keep_f32), names))
+        for (name, _), (st, f32) in zip(names, res):
             out[name + "_st"], out[name + "_f32"] = st, f32
     else:
         fin = c["in_dim"]
@@ -67,10 +73,10 @@ def make_config(cfg: int, scale: float = 1.0, seed: int = 0, with_grads: bool = 
         a = normal_tensor(rng_for(cfg, 23, seed), (h, d), std=d ** -0.5)            # N(0, var 1/head_dim)
         # dense input projections: outside the fused kernels
         for name, w in (("xl", w_s), ("xr", w_t)):
-            st, f32 = store((x @ w.T).reshape(n, h, d), dt)
+            st, f32 = store((x @ w.T).reshape(n, h, d), dt, keep_f32)
             out[name + "_st"], out[name + "_f32"] = st, f32
         out["a_f32"] = np.ascontiguousarray(a, dtype=np.float32)
         if with_grads:
-            st, f32 = store(normal_tensor(rng_for(cfg, 24, seed), (n, h, d)), dt)
+            st, f32 = store(normal_tensor(rng_for(cfg, 24, seed), (n, h, d)), dt, keep_f32)
             out["do_st"], out["do_f32"] = st, f32
     return out

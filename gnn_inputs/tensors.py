@@ -40,7 +40,7 @@ def normal_tensor(rng: np.random.Generator, shape, std: float = 1.0, chunk: int 
     return out.reshape(shape)
 
 
-def store(x32: np.ndarray, dtype: str):
+def store(x32: np.ndarray, dtype: str, keep_f32: bool = True):
     """Round an fp32 tensor to the storage dtype.
 
     Returns (stored, as_f32): ``stored`` is what is handed to the GPU (fp32 array, or
@@ -52,5 +52,5 @@ def store(x32: np.ndarray, dtype: str):
         return x32, x32
     if dtype == "bf16":
         bits = f32_to_bf16_bits(x32)
-        return bits, bf16_bits_to_f32(bits)
+        return bits, (bf16_bits_to_f32(bits) if keep_f32 else None)
     raise ValueError(f"unknown dtype {dtype!r}")

@@ -171,6 +171,14 @@ const char* gnn_version(void);
 /* Number of kernel launches the library has issued in this process (all threads).               */
 int64_t gnn_launch_count(void);
 
+/* Measurement aid (bench.py): when enabled, every kernel launch of the library is bracketed by two
+ * CUDA events on the launch stream.  gnn_profile_collect synchronises on them, writes up to
+ * max_records records - names[i] is a 48-byte NUL-terminated "pass/kernel" string, ms[i] its device
+ * time in milliseconds, in launch order - clears the list and returns the number written.  Not
+ * thread-safe; off by default (the timed `value` runs have it off).                                */
+void gnn_profile_enable(int on);
+int32_t gnn_profile_collect(char* names, float* ms, int32_t max_records);
+
 #ifdef __cplusplus
 }
 #endif

@@ -20,7 +20,8 @@ GNN_OP_GT_FWD, GNN_OP_GT_BWD, GNN_OP_GATV2_FWD, GNN_OP_GATV2_BWD = 0, 1, 2, 3
 EXPORTED_SYMBOLS = [
     "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
     "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
-    "gnn_gatv2_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count",
+    "gnn_gatv2_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
+    "gnn_profile_collect",
 ]
 
 
@@ -64,6 +65,10 @@ def lib() -> C.CDLL:
         L.gnn_last_error.restype = C.c_char_p
         L.gnn_version.restype = C.c_char_p
         L.gnn_launch_count.restype = _i64
+        L.gnn_profile_enable.argtypes = [C.c_int]
+        L.gnn_profile_enable.restype = None
+        L.gnn_profile_collect.argtypes = [_vp, _vp, _i32]
+        L.gnn_profile_collect.restype = _i32
         for s in EXPORTED_SYMBOLS:
             getattr(L, s)
         _lib = L
@@ -80,6 +85,18 @@ def gnn_version() -> str:
 
 def gnn_launch_count() -> int:
     return int(lib().gnn_launch_count())
+
+
+def gnn_profile_enable(on: bool) -> None:
+    lib().gnn_profile_enable(1 if on else 0)
+
+
+def gnn_profile_collect(max_records: int = 4096):
+    """[(name, ms), ...] for every launch since the last collect (synchronises)."""
+    names = C.create_string_buffer(48 * max_records)
+    ms = (C.c_float * max_records)()
+    k = lib().gnn_profile_collect(C.cast(names, _vp), C.cast(ms, _vp), max_records)
+    return [(names.raw[48 * i:48 * (i + 1)].split(b"\0", 1)[0].decode(), float(ms[i])) for i in range(k)]
 
 
 def _check(rc: int):

@@ -3,6 +3,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <vector>
 
 #include "internal.h"
 #include "kernels.cuh"
@@ -17,6 +18,24 @@ void set_error(const char* fmt, ...) {
     va_start(ap, fmt);
     vsnprintf(t_err, sizeof(t_err), fmt, ap);
     va_end(ap);
+}
+
+// ---- per-launch event profiler (measurement aid for bench.py; off by default)
+struct ProfRec { char name[48]; cudaEvent_t a, b; };
+static bool g_prof_on = false;
+static std::vector<ProfRec> g_prof;
+void prof_begin(const char* pass, const char* kernel, cudaStream_t st) {
+    if (!g_prof_on) return;
+    ProfRec r;
+    snprintf(r.name, sizeof(r.name), "%s/%s", pass, kernel);
+    cudaEventCreate(&r.a);
+    cudaEventCreate(&r.b);
+    cudaEventRecord(r.a, st);
+    g_prof.push_back(r);
+}
+void prof_end(cudaStream_t st) {
+    if (!g_prof_on || g_prof.empty()) return;
+    cudaEventRecord(g_prof.back().b, st);
 }
 
 namespace {
@@ -103,6 +122,25 @@ using namespace gnn;
 extern "C" const char* gnn_last_error(void) { return t_err; }
 extern "C" const char* gnn_version(void) { return "gnn_attn 0.1 sm_100a"; }
 extern "C" int64_t gnn_launch_count(void) { return (int64_t)g_launches; }
+
+extern "C" void gnn_profile_enable(int on) { g_prof_on = on != 0; }
+extern "C" int32_t gnn_profile_collect(char* names, float* ms, int32_t max_records) {
+    int32_t k = 0;
+    for (auto& r : g_prof) {
+        cudaEventSynchronize(r.b);
+        float t = 0.f;
+        cudaEventElapsedTime(&t, r.a, r.b);
+        if (k < max_records && names && ms) {
+            strncpy(names + (size_t)k * 48, r.name, 48);
+            ms[k] = t;
+            ++k;
+        }
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    g_prof.clear();
+    return k;
+}
 
 extern "C" gnn_status_t gnn_workspace_bytes(const gnn_plan_t* P, int op, int32_t heads, int32_t head_dim,
                                             gnn_dtype_t dtype, size_t* bytes) {

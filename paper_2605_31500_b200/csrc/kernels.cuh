@@ -5,6 +5,9 @@
 namespace gnn {
 
 extern unsigned long long g_launches;  // host-side launch counter (api.cu)
+// optional per-launch CUDA-event timing (gnn_profile_enable); no-ops when disabled
+void prof_begin(const char* pass, const char* kernel, cudaStream_t st);
+void prof_end(cudaStream_t st);
 
 // ------------------------------------------------------------------------------------------------
 // state <-> shared memory (serialised layout of state_floats<Op>)
@@ -324,21 +327,27 @@ template <class Op> inline cudaError_t run_op(const typename Op::Params& p, cons
             cudaError_t e = cudaFuncSetAttribute(segment_kernel<Op>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
         }
+        prof_begin(Op::kName, "segment", c.stream);
         segment_kernel<Op><<<gp.seg_grid, kCtaThreads, smem, c.stream>>>(p, sh, c.rowptr, c.colidx, b, c.partials,
                                                                          c.da_part, slot);
+        prof_end(c.stream);
         ++g_launches;
     }
     slot += gp.seg_grid;
     if (gp.grp_grid > 0) {
         const size_t smem = Op::HAS_DA ? 4 * (size_t)NG * sh.rowe + 16 : 16;
+        prof_begin(Op::kName, "group", c.stream);
         group_kernel<Op><<<gp.grp_grid, kCtaThreads, smem, c.stream>>>(p, sh, c.rowptr, c.colidx, b.perm,
                                                                        b.n_hub + b.n_cta, b.n_group, c.da_part, slot);
+        prof_end(c.stream);
         ++g_launches;
     }
     slot += gp.grp_grid;
     if (gp.hub_grid > 0) {
         const size_t smem = 4 * (size_t)state_floats<Op>(sh) + 16;
+        prof_begin(Op::kName, "hub_merge", c.stream);
         hub_merge_kernel<Op><<<gp.hub_grid, kCtaThreads, smem, c.stream>>>(p, sh, b, c.partials, c.da_part, slot);
+        prof_end(c.stream);
         ++g_launches;
     }
     return cudaGetLastError();

@@ -7,6 +7,7 @@ namespace gnn {
 
 // ------------------------------------------------------------------------------------ GATv2 forward
 template <typename T, int G_, int NV_> struct GatFwd : OpBase<T, G_, NV_> {
+    static constexpr const char* kName = "gatv2_fwd";
     using B = OpBase<T, G_, NV_>;
     using typename B::GeoT;
     static constexpr int NV = NV_, VEC = B::kVEC;
@@ -94,6 +95,7 @@ template <typename T, int G_, int NV_> struct GatFwd : OpBase<T, G_, NV_> {
 //   A1 = sum w as, B1 = sum alpha as, A2 = sum w sg, B2 = sum alpha sg, G = sum w
 //   dxl_i = A1 - G B1;  this row's share of da = A2 - G B2      (== sum_j de_ij ...)
 template <typename T, int G_, int NV_> struct GatBwdDst : OpBase<T, G_, NV_> {
+    static constexpr const char* kName = "gatv2_bwd_dst";
     using B = OpBase<T, G_, NV_>;
     using typename B::GeoT;
     static constexpr int NV = NV_, VEC = B::kVEC;
@@ -187,6 +189,7 @@ template <typename T, int G_, int NV_> struct GatBwdDst : OpBase<T, G_, NV_> {
 
 // ----------------------------------------------------- GATv2 backward, src pass over CSR^T ("R" kernel)
 template <typename T, int G_, int NV_> struct GatBwdSrc : OpBase<T, G_, NV_> {
+    static constexpr const char* kName = "gatv2_bwd_src";
     using B = OpBase<T, G_, NV_>;
     using typename B::GeoT;
     static constexpr int NV = NV_, VEC = B::kVEC;

@@ -46,6 +46,7 @@ __device__ __forceinline__ float softmax_step(float& m, float& l, const float (&
 
 // ------------------------------------------------------------------------------------- GT forward
 template <typename T, int G_, int NV_> struct GtFwd : OpBase<T, G_, NV_> {
+    static constexpr const char* kName = "gt_fwd";
     using B = OpBase<T, G_, NV_>;
     using typename B::GeoT;
     static constexpr int NV = NV_, VEC = B::kVEC;
@@ -130,6 +131,7 @@ template <typename T, int G_, int NV_> struct GtFwd : OpBase<T, G_, NV_> {
 // One sweep, no O needed: A = sum alpha dP k, B = sum alpha k, Delta = sum alpha dP;
 // dQ = (A - Delta B)/sqrt(d)   (== sum_j alpha (dP - Delta) k_j / sqrt(d))
 template <typename T, int G_, int NV_> struct GtBwdDst : OpBase<T, G_, NV_> {
+    static constexpr const char* kName = "gt_bwd_dst";
     using B = OpBase<T, G_, NV_>;
     using typename B::GeoT;
     static constexpr int NV = NV_, VEC = B::kVEC;
@@ -220,6 +222,7 @@ template <typename T, int G_, int NV_> struct GtBwdDst : OpBase<T, G_, NV_> {
 // rows are SOURCES j, entries the destinations i they feed; dK_j, dV_j accumulate in registers in
 // CSR^T order: deterministic, no atomics (the paper uses atomicAdd here).
 template <typename T, int G_, int NV_> struct GtBwdSrc : OpBase<T, G_, NV_> {
+    static constexpr const char* kName = "gt_bwd_src";
     using B = OpBase<T, G_, NV_>;
     using typename B::GeoT;
     static constexpr int NV = NV_, VEC = B::kVEC;

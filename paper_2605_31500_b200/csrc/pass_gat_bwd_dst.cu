@@ -17,7 +17,9 @@ __global__ void da_reduce_kernel(const float* __restrict__ part, int slots, int 
     da[e] = (float)s;
 }
 cudaError_t launch_da_reduce(const float* da_part, int slots, int rowe, float* da, cudaStream_t st) {
+    prof_begin("gatv2_bwd_dst", "da_reduce", st);
     da_reduce_kernel<<<(rowe + 63) / 64, 64, 0, st>>>(da_part, slots, rowe, da);
+    prof_end(st);
     ++g_launches;
     return cudaGetLastError();
 }
