@@ -13,7 +13,7 @@
  *
  * CONVENTIONS (all entry points)
  *   - Every data pointer is a DEVICE pointer owned by the caller; the library never allocates or
- *     frees device memory.  Feature pointers and workspace must be 16-byte aligned.
+ *     frees device memory.  Feature, gradient and workspace pointers must be 32-byte aligned (256-bit gathers).
  *   - Graph: int32 CSR; ROW i = DESTINATION node, colidx[rowptr[i] .. rowptr[i+1]) = its sources j
  *     (in-neighbours).  The library processes exactly the stored entries: the caller stores the
  *     self-loop of N(i) u {i}; duplicate entries are separate softmax terms; a row with no
@@ -24,8 +24,9 @@
  *     [n, heads, head_dim] regardless of the feature dtype (reading A9); the forward
  *     output O has the feature dtype (bf16: round-to-nearest-even of the fp32 accumulator).
  *     All arithmetic is fp32.
- *   - Supported shapes: head_dim a power of two with head_dim*sizeof(elt) in [16, 512] bytes and
- *     heads*head_dim*sizeof(elt) <= 1024 bytes.  Anything else returns GNN_EUNSUPPORTED.
+ *   - Supported shapes: head_dim a power of two with head_dim*sizeof(elt) >= 16 bytes,
+ *     heads*head_dim*sizeof(elt) <= 1024 bytes, and heads*head_dim*sizeof(elt) / min(head_dim*sizeof(elt), 32)
+ *     <= 32 (a row must fit one warp at 32 bytes per lane).  Anything else returns GNN_EUNSUPPORTED.
  *   - Every compute call is asynchronous on `stream` and never synchronises.  gnn_plan_build
  *     synchronises `stream` (it reads a few counters back to the host).
  *   - Return value: GNN_OK or an error code; nothing is launched when an error is returned for

@@ -42,26 +42,27 @@ namespace {
 
 bool make_shape(int32_t n, int32_t heads, int32_t head_dim, int dtype, Shape& sh, const char* who) {
     if (dtype != GNN_F32 && dtype != GNN_BF16) { set_error("%s: unknown dtype %d", who, dtype); return false; }
-    const int esz = dtype == GNN_F32 ? 4 : 2, vec = 16 / esz;
-    if (heads < 1 || head_dim < 1 || (head_dim & (head_dim - 1)) || head_dim * esz < 16 || head_dim * esz > 512 ||
-        (long long)heads * head_dim * esz > 1024) {
+    const int esz = dtype == GNN_F32 ? 4 : 2;
+    LaneCfg lf, lb;
+    if (heads < 1 || head_dim < 1 || (head_dim & (head_dim - 1)) || head_dim * esz < 16 ||
+        (long long)heads * head_dim * esz > 1024 || !pick_lane_cfg(kGtFwd, esz, heads, head_dim, lf) ||
+        !pick_lane_cfg(kGtBwdDst, esz, heads, head_dim, lb) || !pick_lane_cfg(kGatBwdDst, esz, heads, head_dim, lb)) {
         set_error("%s: unsupported shape heads=%d head_dim=%d dtype=%d (head_dim must be a power of two with "
-                  "16 <= head_dim*sizeof <= 512 and heads*head_dim*sizeof <= 1024)", who, heads, head_dim, dtype);
+                  "head_dim*sizeof >= 16, heads*head_dim*sizeof <= 1024, and at most 32 lanes of "
+                  "min(head_dim*sizeof, 32) bytes per row)", who, heads, head_dim, dtype);
         return false;
     }
-    sh.n = n; sh.H = heads; sh.d = head_dim; sh.rowe = heads * head_dim; sh.rowv = sh.rowe / vec;
-    sh.lph = head_dim / vec;
-    sh.lph_log2 = 0;
-    while ((1 << sh.lph_log2) < sh.lph) ++sh.lph_log2;
+    sh.n = n; sh.H = heads; sh.d = head_dim; sh.rowe = heads * head_dim;
+    sh.ch = sh.lanes = sh.lpl = sh.lpl_log2 = 0;  // filled per pass (pass_shape)
     return true;
 }
 
-bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
+bool aligned16(const void* p) { return (((uintptr_t)p) & 31) == 0; }  // 256-bit gathers need 32-byte alignment
 
 struct WsLayout { size_t partials, da_part, total; int da_slots; };
 
 // workspace of one API call = max over its passes of the chunk partials (+ da partials for GATv2 bwd)
-WsLayout ws_layout(const gnn_plan* P, int op, const Shape& sh) {
+WsLayout ws_layout(const gnn_plan* P, int op, const Shape& sh, int esz) {
     WsLayout w = {0, 0, 0, 0};
     size_t part = 0;
     auto need = [&](Pass ps, const BinView& b) {
@@ -79,7 +80,9 @@ WsLayout ws_layout(const gnn_plan* P, int op, const Shape& sh) {
     w.da_part = (part + 255) / 256 * 256;
     size_t da = 0;
     if (op == GNN_OP_GATV2_BWD) {
-        w.da_slots = grid_plan(P->fwd, P->sm_count, group_width(sh.rowv)).da_slots();
+        LaneCfg lc;
+        pick_lane_cfg(kGatBwdDst, esz, sh.H, sh.d, lc);
+        w.da_slots = grid_plan(P->fwd, P->sm_count, lc.g).da_slots();
         da = (size_t)w.da_slots * sh.rowe * sizeof(float);
     }
     w.total = w.da_part + da + 256;
@@ -152,7 +155,7 @@ extern "C" gnn_status_t gnn_workspace_bytes(const gnn_plan_t* P, int op, int32_t
         set_error("gnn_workspace_bytes: backward needs a plan built with build_transpose");
         return GNN_EINVAL;
     }
-    *bytes = ws_layout(P, op, sh).total;
+    *bytes = ws_layout(P, op, sh, dtype == GNN_F32 ? 4 : 2).total;
     return GNN_OK;
 }
 
@@ -164,12 +167,12 @@ extern "C" gnn_status_t gnn_gt_attn_fwd(const gnn_plan_t* P, const int32_t* rowp
     if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
     if (!q || !k || !v || !out || !lse || !ws) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
     if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !aligned16(ws)) {
-        set_error("%s: feature pointers and workspace must be 16-byte aligned", who);
+        set_error("%s: feature pointers and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
     Shape sh;
     if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
-    const WsLayout w = ws_layout(P, GNN_OP_GT_FWD, sh);
+    const WsLayout w = ws_layout(P, GNN_OP_GT_FWD, sh, dtype == GNN_F32 ? 4 : 2);
     if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
     GtArgs a = {};
     a.q = q; a.k = k; a.v = v; a.out = out; a.lse = lse;
@@ -190,12 +193,12 @@ extern "C" gnn_status_t gnn_gt_attn_bwd(const gnn_plan_t* P, const int32_t* rowp
     }
     if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(dout) || !aligned16(dq) || !aligned16(dk) ||
         !aligned16(dv) || !aligned16(ws)) {
-        set_error("%s: feature/gradient pointers and workspace must be 16-byte aligned", who);
+        set_error("%s: feature/gradient pointers and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
     Shape sh;
     if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
-    const WsLayout w = ws_layout(P, GNN_OP_GT_BWD, sh);
+    const WsLayout w = ws_layout(P, GNN_OP_GT_BWD, sh, dtype == GNN_F32 ? 4 : 2);
     if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
     GtArgs a = {};
     a.q = q; a.k = k; a.v = v; a.dout = dout; a.lse = const_cast<float*>(lse); a.delta = delta;
@@ -213,12 +216,12 @@ extern "C" gnn_status_t gnn_gatv2_fwd(const gnn_plan_t* P, const int32_t* rowptr
     if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
     if (!xl || !xr || !a_ || !out || !lse || !ws) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
     if (!aligned16(xl) || !aligned16(xr) || !aligned16(a_) || !aligned16(out) || !aligned16(ws)) {
-        set_error("%s: feature pointers, a and workspace must be 16-byte aligned", who);
+        set_error("%s: feature pointers, a and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
     Shape sh;
     if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
-    const WsLayout w = ws_layout(P, GNN_OP_GATV2_FWD, sh);
+    const WsLayout w = ws_layout(P, GNN_OP_GATV2_FWD, sh, dtype == GNN_F32 ? 4 : 2);
     if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
     GatArgs a = {};
     a.xl = xl; a.xr = xr; a.a = a_; a.out = out; a.lse = lse; a.slope = slope;
@@ -239,12 +242,12 @@ extern "C" gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* P, const int32_t* rowptr
     }
     if (!aligned16(xl) || !aligned16(xr) || !aligned16(a_) || !aligned16(dout) || !aligned16(dxl) || !aligned16(dxr) ||
         !aligned16(ws)) {
-        set_error("%s: feature/gradient pointers, a and workspace must be 16-byte aligned", who);
+        set_error("%s: feature/gradient pointers, a and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
     Shape sh;
     if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
-    const WsLayout w = ws_layout(P, GNN_OP_GATV2_BWD, sh);
+    const WsLayout w = ws_layout(P, GNN_OP_GATV2_BWD, sh, dtype == GNN_F32 ? 4 : 2);
     if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
     GatArgs a = {};
     a.xl = xl; a.xr = xr; a.a = a_; a.dout = dout; a.lse = const_cast<float*>(lse); a.g = g; a.dxl = dxl; a.dxr = dxr;

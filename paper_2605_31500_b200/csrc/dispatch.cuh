@@ -1,12 +1,14 @@
-// dispatch.cuh - picks the (dtype, lane-group width, vectors per lane) instantiation of a pass.
+// dispatch.cuh - picks the (dtype, bytes per lane, lane-group width) instantiation of a pass.
 #pragma once
 #include "internal.h"
 #include "kernels.cuh"
 
 namespace gnn {
 
-template <template <typename, int, int> class OpT, Pass PASS, typename Fill>
-inline cudaError_t dispatch_pass(int dtype, const Shape& sh, const LaunchCtx& c, Fill fill) {
+template <template <typename, int, int, int, int> class OpT, Pass PASS, typename Fill>
+inline cudaError_t dispatch_pass(int dtype, const Shape& sh0, const LaunchCtx& c, Fill fill) {
+    LaneCfg lc;
+    const Shape sh = pass_shape(sh0, PASS, dtype == GNN_F32 ? 4 : 2, lc);
     auto go = [&](auto* tag) -> cudaError_t {
         using Op = typename std::remove_pointer<decltype(tag)>::type;
         static_assert(Op::NA == kPassInfo[PASS].na && Op::NS == kPassInfo[PASS].ns &&
@@ -16,16 +18,24 @@ inline cudaError_t dispatch_pass(int dtype, const Shape& sh, const LaunchCtx& c,
         fill(p);
         return run_op<Op>(p, sh, c);
     };
-    const int gw = group_width(sh.rowv);
-    const int nv = sh.rowv > 32 ? 2 : 1;
-#define GNN_GO(T)                                                             \
-    if (gw == 8) return go((OpT<T, 8, 1>*)nullptr);                           \
-    if (gw == 16) return go((OpT<T, 16, 1>*)nullptr);                         \
-    if (gw == 32 && nv == 1) return go((OpT<T, 32, 1>*)nullptr);              \
-    if (gw == 32 && nv == 2) return go((OpT<T, 32, 2>*)nullptr);
+#define GNN_G(T, VB, NV)                                                                     \
+    {                                                                                        \
+        constexpr int KU = pass_ku(PASS, VB * NV);                                           \
+        if (lc.g == 4) return go((OpT<T, VB, NV, 4, KU>*)nullptr);                           \
+        if (lc.g == 8) return go((OpT<T, VB, NV, 8, KU>*)nullptr);                           \
+        if (lc.g == 16) return go((OpT<T, VB, NV, 16, KU>*)nullptr);                         \
+        if (lc.g == 32) return go((OpT<T, VB, NV, 32, KU>*)nullptr);                         \
+    }
+#define GNN_GO(T)                                                                            \
+    if (lc.cb == 16) GNN_G(T, 16, 1)                                                         \
+    if (lc.cb == 32) GNN_G(T, 32, 1)                                                         \
+    if constexpr (pass_inst_max_cb(PASS) >= 64) {                                                 \
+        if (lc.cb == 64) GNN_G(T, 32, 2)                                                     \
+    }
     if (dtype == GNN_F32) { GNN_GO(float) }
     if (dtype == GNN_BF16) { GNN_GO(__nv_bfloat16) }
 #undef GNN_GO
+#undef GNN_G
     return cudaErrorInvalidValue;
 }
 

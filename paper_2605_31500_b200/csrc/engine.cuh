@@ -1,12 +1,14 @@
 // engine.cuh - traversal engine shared by the six fused CSR attention passes (sm_100a).
 //
-// One "lane group" of G lanes covers one feature row of a node: every lane owns NV 16-byte vectors
-// (VEC = 4 fp32 or 8 bf16 channels each), so a gathered neighbour row is a single coalesced 128-bit
-// load per lane ("vectorized float4 loads"; the paper's block-per-(node, head) shape,
-// PAPER.md:484, is prior art - here all heads of a row travel together so the gather is one
-// contiguous H*d*b-byte burst).  A head's d channels sit in LPH = d/VEC adjacent lanes, so the score
-// dot product is a log2(LPH)-step xor-shuffle, and the online-softmax state (running max, sum,
-// accumulator) lives in registers.
+// One "lane group" of G lanes covers one feature row of a node.  Every lane owns CH = NV * VEC
+// CONTIGUOUS channels of ONE head, fetched with NV 128-bit or 256-bit read-only loads
+// (LDG.E.128 / LDG.E.256, the latter new on sm_100), so a gathered neighbour row is one contiguous
+// H*d*b-byte burst per group ("vectorized float4 loads"; the paper's
+// block-per-(node, head) shape, is prior art - here all heads of a row travel
+// together).  A head's d channels sit in LPL = d/CH adjacent lanes, so the score dot product ends
+// in a log2(LPL)-step xor-shuffle (none at all when a lane holds a whole head), and the
+// online-softmax state (running max, sum, accumulator) lives in registers.  Wider CH
+// means fewer lanes repeat the same per-(edge, head) scalar work and more edges per warp instruction.
 //
 // Three kernels per pass, picked by the plan's degree bins:
 //   group_kernel    rows with deg <= warp_max_deg : one lane group per row, 32/G rows per warp,
@@ -25,24 +27,20 @@
 
 namespace gnn {
 
-constexpr int kCtaThreads = 256;
+constexpr int kCtaThreads = 128;
 constexpr int kWarpsPerCta = kCtaThreads / 32;
-constexpr int kU = 4;  // edges gathered per lane group per batch (independent loads in flight)
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 
-template <typename T> struct Elt;
-template <> struct Elt<float> { static constexpr int VEC = 4; };
-template <> struct Elt<__nv_bfloat16> { static constexpr int VEC = 8; };
-
 struct Shape {
-    int n;        // nodes
-    int H;        // heads
-    int d;        // head_dim
-    int rowe;     // H * d elements per feature row
-    int rowv;     // 16-byte vectors per feature row
-    int lph;      // lanes per head = d / VEC (power of two, <= 32)
-    int lph_log2;
+    int n;          // nodes
+    int H;          // heads
+    int d;          // head_dim
+    int rowe;       // H * d elements per feature row
+    int ch;         // channels per lane (CH)
+    int lanes;      // active lanes per row = rowe / ch
+    int lpl;        // lanes per head = d / ch (power of two)
+    int lpl_log2;
 };
 
 struct BinView {
@@ -74,97 +72,127 @@ __device__ __forceinline__ float lg2(float x) {
     return y;
 }
 
-// 16-byte read-only gather of one lane's vector, converted to fp32.  pred == false -> zeros, no traffic.
-__device__ __forceinline__ void load_vec(const float* base, size_t elt, bool pred, float (&o)[4]) {
-    float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (pred) r = __ldg(reinterpret_cast<const float4*>(base + elt));
-    o[0] = r.x; o[1] = r.y; o[2] = r.z; o[3] = r.w;
+// ---- raw VB-byte gathers (VB = 16 or 32), kept unconverted until use so in-flight loads stay small
+template <int VB> struct Raw { uint32_t w[VB / 4]; };
+
+template <int VB> __device__ __forceinline__ Raw<VB> ldg_raw(const void* p, bool pred);
+template <> __device__ __forceinline__ Raw<16> ldg_raw<16>(const void* p, bool pred) {
+    Raw<16> r;
+    r.w[0] = r.w[1] = r.w[2] = r.w[3] = 0u;
+    if (pred)
+        asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];"
+                     : "=r"(r.w[0]), "=r"(r.w[1]), "=r"(r.w[2]), "=r"(r.w[3]) : "l"(p));
+    return r;
 }
-__device__ __forceinline__ void load_vec(const __nv_bfloat16* base, size_t elt, bool pred, float (&o)[8]) {
-    uint4 r = make_uint4(0u, 0u, 0u, 0u);
-    if (pred) r = __ldg(reinterpret_cast<const uint4*>(base + elt));
-    const uint32_t w[4] = {r.x, r.y, r.z, r.w};
+template <> __device__ __forceinline__ Raw<32> ldg_raw<32>(const void* p, bool pred) {
+    Raw<32> r;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        o[2 * i] = __uint_as_float(w[i] << 16);
-        o[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+    for (int i = 0; i < 8; ++i) r.w[i] = 0u;
+    if (pred)
+        asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=r"(r.w[0]), "=r"(r.w[1]), "=r"(r.w[2]), "=r"(r.w[3]), "=r"(r.w[4]), "=r"(r.w[5]),
+                       "=r"(r.w[6]), "=r"(r.w[7]) : "l"(p));
+    return r;
+}
+
+// element i of a raw vector as fp32 (exact up-cast for bf16)
+template <typename T, int VB> __device__ __forceinline__ float raw_elt(const Raw<VB>& r, int i);
+template <> __device__ __forceinline__ float raw_elt<float, 16>(const Raw<16>& r, int i) { return __uint_as_float(r.w[i]); }
+template <> __device__ __forceinline__ float raw_elt<float, 32>(const Raw<32>& r, int i) { return __uint_as_float(r.w[i]); }
+template <> __device__ __forceinline__ float raw_elt<__nv_bfloat16, 16>(const Raw<16>& r, int i) {
+    return __uint_as_float((i & 1) ? (r.w[i >> 1] & 0xffff0000u) : (r.w[i >> 1] << 16));
+}
+template <> __device__ __forceinline__ float raw_elt<__nv_bfloat16, 32>(const Raw<32>& r, int i) {
+    return __uint_as_float((i & 1) ? (r.w[i >> 1] & 0xffff0000u) : (r.w[i >> 1] << 16));
+}
+
+// A lane's CH contiguous channels of a [*, rowe] tensor of T: NV raw vectors.
+template <typename T, int VB, int NV> struct Chunk {
+    static constexpr int VEC = VB / (int)sizeof(T), CH = NV * VEC;
+    Raw<VB> v[NV];
+    __device__ __forceinline__ void load(const T* base, size_t elt, bool pred) {
+#pragma unroll
+        for (int t = 0; t < NV; ++t) v[t] = ldg_raw<VB>(base + elt + t * VEC, pred);
     }
-}
-// fp32 vector (always fp32 in memory: a, gradients)
-template <int VEC> __device__ __forceinline__ void load_f32(const float* base, size_t elt, bool pred, float (&o)[VEC]) {
+    __device__ __forceinline__ float get(int c) const { return raw_elt<T, VB>(v[c / VEC], c % VEC); }
+    __device__ __forceinline__ void to_float(float (&o)[CH]) const {
 #pragma unroll
-    for (int i = 0; i < VEC; i += 4) {
+        for (int c = 0; c < CH; ++c) o[c] = get(c);
+    }
+};
+
+// CH contiguous fp32 values (a, gradients): plain 128-bit accesses
+template <int CH> __device__ __forceinline__ void load_f32(const float* base, size_t elt, bool pred, float (&o)[CH]) {
+#pragma unroll
+    for (int i = 0; i < CH; i += 4) {
         float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
         if (pred) r = __ldg(reinterpret_cast<const float4*>(base + elt + i));
         o[i] = r.x; o[i + 1] = r.y; o[i + 2] = r.z; o[i + 3] = r.w;
     }
 }
-template <int VEC> __device__ __forceinline__ void store_f32(float* base, size_t elt, const float (&v)[VEC]) {
+template <int CH> __device__ __forceinline__ void store_f32(float* base, size_t elt, const float (&v)[CH]) {
 #pragma unroll
-    for (int i = 0; i < VEC; i += 4)
+    for (int i = 0; i < CH; i += 4)
         *reinterpret_cast<float4*>(base + elt + i) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
 }
-// store in the feature dtype (bf16: round-to-nearest-even)
-__device__ __forceinline__ void store_vec(float* base, size_t elt, const float (&v)[4]) {
-    *reinterpret_cast<float4*>(base + elt) = make_float4(v[0], v[1], v[2], v[3]);
+// store CH values in the feature dtype (bf16: round-to-nearest-even)
+template <int CH> __device__ __forceinline__ void store_feat(float* base, size_t elt, const float (&v)[CH]) {
+    store_f32<CH>(base, elt, v);
 }
-__device__ __forceinline__ void store_vec(__nv_bfloat16* base, size_t elt, const float (&v)[8]) {
-    uint4 r;
-    uint32_t* w = reinterpret_cast<uint32_t*>(&r);
+template <int CH> __device__ __forceinline__ void store_feat(__nv_bfloat16* base, size_t elt, const float (&v)[CH]) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        __nv_bfloat162 b = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]);
-        w[i] = *reinterpret_cast<uint32_t*>(&b);
+    for (int i = 0; i < CH; i += 8) {
+        uint4 r;
+        uint32_t* w = reinterpret_cast<uint32_t*>(&r);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            __nv_bfloat162 b = __floats2bfloat162_rn(v[i + 2 * j], v[i + 2 * j + 1]);
+            w[j] = *reinterpret_cast<uint32_t*>(&b);
+        }
+        *reinterpret_cast<uint4*>(base + elt + i) = r;
     }
-    *reinterpret_cast<uint4*>(base + elt) = r;
 }
 
 // lane geometry inside a group
-template <int G, int NV, int VEC> struct Geo {
-    int eoff[NV];   // element offset of this lane's vector t inside a feature row
-    int hd[NV];     // head of vector t
-    bool act[NV];   // vector t exists (rowv need not fill the group)
-    bool lead[NV];  // first lane of its head (writes per-head scalars)
-    int lph;
+template <int G> struct Geo {
+    int eoff;    // element offset of this lane's channels inside a feature row
+    int hd;      // head of this lane
+    bool act;    // lane holds channels (the row need not fill the group)
+    bool lead;   // first lane of its head (writes per-head scalars)
+    int lpl;     // lanes per head
     __device__ __forceinline__ void init(const Shape& sh, int lane) {
         const int gl = lane & (G - 1);
-        lph = sh.lph;
-#pragma unroll
-        for (int t = 0; t < NV; ++t) {
-            const int vi = gl + t * G;
-            act[t] = vi < sh.rowv;
-            eoff[t] = vi * VEC;
-            hd[t] = vi >> sh.lph_log2;
-            lead[t] = act[t] && ((vi & (sh.lph - 1)) == 0);
-        }
+        lpl = sh.lpl;
+        act = gl < sh.lanes;
+        eoff = gl * sh.ch;
+        hd = gl >> sh.lpl_log2;
+        lead = act && ((gl & (sh.lpl - 1)) == 0);
     }
 };
 
-// sum x[i] over the LPH lanes of a head (all 32 lanes must call)
-template <int N> __device__ __forceinline__ void head_reduce(float (&x)[N], int lph) {
-    for (int o = 1; o < lph; o <<= 1) {
+// sum x[i] over the LPL lanes of a head (all 32 lanes must call; lpl is warp-uniform)
+template <int N> __device__ __forceinline__ void head_reduce(float (&x)[N], int lpl) {
 #pragma unroll
-        for (int i = 0; i < N; ++i) x[i] += __shfl_xor_sync(0xffffffffu, x[i], o);
+    for (int o = 1; o < 32; o <<= 1) {
+        if (lpl > o) {
+#pragma unroll
+            for (int i = 0; i < N; ++i) x[i] += __shfl_xor_sync(0xffffffffu, x[i], o);
+        }
     }
 }
 
-template <int NA, int NS, int NV, int VEC> struct State {
-    float acc[NA][NV][VEC];
-    float sc[NS > 0 ? NS : 1][NV];
-    float m[NV];  // running max in the log2 domain (softmax passes only)
+template <int NA, int NS, int CH> struct State {
+    float acc[NA][CH];
+    float sc[NS > 0 ? NS : 1];
+    float m;  // running max in the log2 domain (softmax passes only)
     __device__ __forceinline__ void reset() {
 #pragma unroll
         for (int a = 0; a < NA; ++a)
 #pragma unroll
-            for (int t = 0; t < NV; ++t)
+            for (int c = 0; c < CH; ++c) acc[a][c] = 0.f;
 #pragma unroll
-                for (int c = 0; c < VEC; ++c) acc[a][t][c] = 0.f;
-#pragma unroll
-        for (int s = 0; s < (NS > 0 ? NS : 1); ++s)
-#pragma unroll
-            for (int t = 0; t < NV; ++t) sc[s][t] = 0.f;
-#pragma unroll
-        for (int t = 0; t < NV; ++t) m[t] = -INFINITY;
+        for (int s = 0; s < (NS > 0 ? NS : 1); ++s) sc[s] = 0.f;
+        m = -INFINITY;
     }
 };
 

@@ -35,8 +35,44 @@ constexpr PassInfo kPassInfo[kNumPass] = {{1, 1, 1, 0}, {2, 1, 0, 0}, {2, 0, 0, 
 inline int pass_state_floats(Pass p, const Shape& sh) {
     return kPassInfo[p].na * sh.rowe + (kPassInfo[p].ns + kPassInfo[p].softmax) * sh.H;
 }
-// lane-group width for a feature row of `rowv` 16-byte vectors; 0 = unsupported
-inline int group_width(int rowv) { return rowv <= 8 ? 8 : rowv <= 16 ? 16 : rowv <= 64 ? 32 : 0; }
+// Lane layout of a pass: each lane owns `cb` contiguous bytes of one head (nv loads of vb bytes), a row
+// takes `lanes` lanes inside a group of g lanes (power of two, 4..32).  Forward passes use up to 64 bytes
+// per lane, backward passes (more live accumulators) up to 32 (16 for the 4-accumulator GATv2 dst pass).
+struct LaneCfg { int vb, nv, cb, g, lanes; };
+constexpr int pass_max_cb(Pass p) { return (p == kGtFwd || p == kGatFwd) ? 64 : (p == kGatBwdDst) ? 16 : 32; }
+// widest lane the pass is instantiated for (wide rows may exceed the preferred pass_max_cb)
+constexpr int pass_inst_max_cb(Pass p) { return (p == kGtFwd || p == kGatFwd) ? 64 : 32; }
+// edges gathered per lane group per batch (independent loads in flight), by pass and bytes per lane
+constexpr int pass_ku(Pass p, int cb) {
+    return (p == kGtFwd) ? (cb == 64 ? 2 : 4)
+         : (p == kGatFwd) ? (cb == 64 ? 2 : 4)
+         : (p == kGatBwdDst) ? (cb == 32 ? 2 : 4)
+         : (cb == 32 ? 2 : 4);
+}
+inline bool pick_lane_cfg(Pass p, int esz, int heads, int head_dim, LaneCfg& lc) {
+    const int head_bytes = head_dim * esz, row_bytes = heads * head_bytes;
+    int cb = pass_max_cb(p);
+    while (cb > head_bytes) cb >>= 1;
+    while (row_bytes / cb > 32 && cb * 2 <= head_bytes && cb * 2 <= pass_inst_max_cb(p)) cb <<= 1;  // wide rows
+    if (cb < 16 || row_bytes / cb > 32) return false;
+    lc.cb = cb;
+    lc.vb = cb >= 32 ? 32 : 16;
+    lc.nv = cb / lc.vb;
+    lc.lanes = row_bytes / cb;
+    lc.g = 4;
+    while (lc.g < lc.lanes) lc.g <<= 1;
+    return true;
+}
+// fill the lane-dependent fields of a Shape for one pass
+inline Shape pass_shape(Shape sh, Pass p, int esz, LaneCfg& lc) {
+    pick_lane_cfg(p, esz, sh.H, sh.d, lc);
+    sh.ch = lc.cb / esz;
+    sh.lanes = lc.lanes;
+    sh.lpl = sh.d / sh.ch;
+    sh.lpl_log2 = 0;
+    while ((1 << sh.lpl_log2) < sh.lpl) ++sh.lpl_log2;
+    return sh;
+}
 
 void set_error(const char* fmt, ...);
 
@@ -52,6 +88,7 @@ struct GatArgs {
     float *lse, *g, *dxl, *dxr;
     float slope;
 };
+// `Shape` passed to the launchers carries n, H, d, rowe; the lane fields are filled per pass inside.
 cudaError_t launch_gt_fwd(int dtype, const Shape&, const LaunchCtx&, const GtArgs&);
 cudaError_t launch_gt_bwd_dst(int dtype, const Shape&, const LaunchCtx&, const GtArgs&);
 cudaError_t launch_gt_bwd_src(int dtype, const Shape&, const LaunchCtx&, const GtArgs&);

@@ -13,57 +13,44 @@ void prof_end(cudaStream_t st);
 // state <-> shared memory (serialised layout of state_floats<Op>)
 template <class Op> __device__ __forceinline__ void state_to_smem(const typename Op::St& st, float* dst,
                                                                   const typename Op::GeoT& g, const Shape& sh) {
-    constexpr int NV = Op::kNV, VEC = Op::kVEC;
+    constexpr int CH = Op::kCH;
+    if (g.act) {
 #pragma unroll
-    for (int a = 0; a < Op::NA; ++a)
+        for (int a = 0; a < Op::NA; ++a)
 #pragma unroll
-        for (int t = 0; t < NV; ++t)
-            if (g.act[t]) {
+            for (int c = 0; c < CH; c += 4)
+                *reinterpret_cast<float4*>(dst + a * sh.rowe + g.eoff + c) =
+                    make_float4(st.acc[a][c], st.acc[a][c + 1], st.acc[a][c + 2], st.acc[a][c + 3]);
+    }
+    if (g.lead) {
 #pragma unroll
-                for (int c = 0; c < VEC; c += 4)
-                    *reinterpret_cast<float4*>(dst + a * sh.rowe + g.eoff[t] + c) =
-                        make_float4(st.acc[a][t][c], st.acc[a][t][c + 1], st.acc[a][t][c + 2], st.acc[a][t][c + 3]);
-            }
-#pragma unroll
-    for (int s = 0; s < Op::NS; ++s)
-#pragma unroll
-        for (int t = 0; t < NV; ++t)
-            if (g.lead[t]) dst[Op::NA * sh.rowe + s * sh.H + g.hd[t]] = st.sc[s][t];
+        for (int s = 0; s < Op::NS; ++s) dst[Op::NA * sh.rowe + s * sh.H + g.hd] = st.sc[s];
+    }
 }
 
 template <class Op> __device__ __forceinline__ void state_from_smem(typename Op::St& st, const float* src,
                                                                     const typename Op::GeoT& g, const Shape& sh) {
-    constexpr int NV = Op::kNV, VEC = Op::kVEC;
+    constexpr int CH = Op::kCH;
 #pragma unroll
     for (int a = 0; a < Op::NA; ++a)
 #pragma unroll
-        for (int t = 0; t < NV; ++t)
+        for (int c = 0; c < CH; ++c) st.acc[a][c] = g.act ? src[a * sh.rowe + g.eoff + c] : 0.f;
 #pragma unroll
-            for (int c = 0; c < VEC; ++c) st.acc[a][t][c] = g.act[t] ? src[a * sh.rowe + g.eoff[t] + c] : 0.f;
-#pragma unroll
-    for (int s = 0; s < Op::NS; ++s)
-#pragma unroll
-        for (int t = 0; t < NV; ++t) st.sc[s][t] = g.act[t] ? src[Op::NA * sh.rowe + s * sh.H + g.hd[t]] : 0.f;
-    if (Op::SOFTMAX) {
-#pragma unroll
-        for (int t = 0; t < NV; ++t)
-            st.m[t] = g.act[t] ? src[Op::NA * sh.rowe + Op::NS * sh.H + g.hd[t]] : -INFINITY;
-    }
+    for (int s = 0; s < Op::NS; ++s) st.sc[s] = g.act ? src[Op::NA * sh.rowe + s * sh.H + g.hd] : 0.f;
+    if (Op::SOFTMAX) st.m = g.act ? src[Op::NA * sh.rowe + Op::NS * sh.H + g.hd] : -INFINITY;
 }
 
 // per-CTA reduction of the per-thread `da` accumulators (GATv2 dst pass) -> da_part[slot][rowe],
 // fixed order over groups.  smem: NG * rowe floats.
 template <class Op>
-__device__ __forceinline__ void cta_write_da(const float (&da)[Op::kNV][Op::kVEC], float* smem, float* da_part,
-                                             int slot, const typename Op::GeoT& g, const Shape& sh, int gi, int ng) {
-    constexpr int NV = Op::kNV, VEC = Op::kVEC;
+__device__ __forceinline__ void cta_write_da(const float (&da)[Op::kCH], float* smem, float* da_part, int slot,
+                                             const typename Op::GeoT& g, const Shape& sh, int gi, int ng) {
+    constexpr int CH = Op::kCH;
     __syncthreads();
+    if (g.act) {
 #pragma unroll
-    for (int t = 0; t < NV; ++t)
-        if (g.act[t]) {
-#pragma unroll
-            for (int c = 0; c < VEC; ++c) smem[gi * sh.rowe + g.eoff[t] + c] = da[t][c];
-        }
+        for (int c = 0; c < CH; ++c) smem[gi * sh.rowe + g.eoff + c] = da[c];
+    }
     __syncthreads();
     for (int e = threadIdx.x; e < sh.rowe; e += blockDim.x) {
         float s = 0.f;
@@ -78,7 +65,7 @@ template <class Op>
 __global__ void __launch_bounds__(kCtaThreads)
 group_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
              const int32_t* __restrict__ perm, int first, int count, float* da_part, int da_slot) {
-    constexpr int G = Op::kG, NV = Op::kNV, VEC = Op::kVEC;
+    constexpr int G = Op::kG, CH = Op::kCH, kU = Op::kU;
     constexpr int GPW = 32 / G;
     extern __shared__ float4 smem4[];
     float* smem = reinterpret_cast<float*>(smem4);
@@ -86,11 +73,9 @@ group_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowptr
     typename Op::GeoT g;
     g.init(sh, lane);
     const int gl = lane & (G - 1);
-    float da[NV][VEC];
+    float da[CH];
 #pragma unroll
-    for (int t = 0; t < NV; ++t)
-#pragma unroll
-        for (int c = 0; c < VEC; ++c) da[t][c] = 0.f;
+    for (int c = 0; c < CH; ++c) da[c] = 0.f;
 
     const int ntiles = (count + GPW - 1) / GPW;
     const int total_warps = gridDim.x * kWarpsPerCta;
@@ -134,7 +119,7 @@ template <class Op>
 __global__ void __launch_bounds__(kCtaThreads)
 segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
                BinView bins, float* __restrict__ partials, float* da_part, int da_slot) {
-    constexpr int G = Op::kG, NV = Op::kNV, VEC = Op::kVEC;
+    constexpr int G = Op::kG, CH = Op::kCH, kU = Op::kU;
     constexpr int GPW = 32 / G, NG = kWarpsPerCta * GPW;
     extern __shared__ float4 smem4[];
     float* smem = reinterpret_cast<float*>(smem4);
@@ -148,11 +133,9 @@ segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowp
     float* s_part = smem;               // [NG][TEs]
     float* s_merged = smem + NG * TEs;  // [TE]
     float* s_max = s_merged + TE;       // [NG][H]
-    float da[NV][VEC];
+    float da[CH];
 #pragma unroll
-    for (int t = 0; t < NV; ++t)
-#pragma unroll
-        for (int c = 0; c < VEC; ++c) da[t][c] = 0.f;
+    for (int c = 0; c < CH; ++c) da[c] = 0.f;
 
     const int nseg = bins.n_chunks + bins.n_cta;
     for (int seg = blockIdx.x; seg < nseg; seg += gridDim.x) {
@@ -185,24 +168,19 @@ segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowp
         }
         // ---- cross-group merge: global max, rescale, fixed-order sum
         if (Op::SOFTMAX) {
-#pragma unroll
-            for (int t = 0; t < NV; ++t)
-                if (g.lead[t]) s_max[gi * sh.H + g.hd[t]] = st.m[t];
+            if (g.lead) s_max[gi * sh.H + g.hd] = st.m;
             __syncthreads();
+            float mg = -INFINITY;
+            if (g.act)
+                for (int k = 0; k < NG; ++k) mg = fmaxf(mg, s_max[k * sh.H + g.hd]);
+            const float f = (st.m == -INFINITY) ? 0.f : ex2(st.m - mg);
 #pragma unroll
-            for (int t = 0; t < NV; ++t) {
-                float mg = -INFINITY;
-                if (g.act[t])
-                    for (int k = 0; k < NG; ++k) mg = fmaxf(mg, s_max[k * sh.H + g.hd[t]]);
-                const float f = (st.m[t] == -INFINITY) ? 0.f : ex2(st.m[t] - mg);
+            for (int a = 0; a < Op::NA; ++a)
 #pragma unroll
-                for (int a = 0; a < Op::NA; ++a)
+                for (int c = 0; c < CH; ++c) st.acc[a][c] *= f;
 #pragma unroll
-                    for (int c = 0; c < VEC; ++c) st.acc[a][t][c] *= f;
-#pragma unroll
-                for (int s = 0; s < Op::NS; ++s) st.sc[s][t] *= f;
-                st.m[t] = mg;
-            }
+            for (int s = 0; s < Op::NS; ++s) st.sc[s] *= f;
+            st.m = mg;
         }
         state_to_smem<Op>(st, s_part + gi * TEs, g, sh);
         __syncthreads();
@@ -211,11 +189,7 @@ segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowp
             for (int k = 0; k < NG; ++k) s += s_part[k * TEs + e];
             s_merged[e] = s;
         }
-        if (Op::SOFTMAX && gi == 0) {
-#pragma unroll
-            for (int t = 0; t < NV; ++t)
-                if (g.lead[t]) s_merged[TEp + g.hd[t]] = st.m[t];
-        }
+        if (Op::SOFTMAX && gi == 0 && g.lead) s_merged[TEp + g.hd] = st.m;
         __syncthreads();
         if (partial) {
             for (int e = threadIdx.x; e < TE; e += kCtaThreads) partials[(size_t)seg * TE + e] = s_merged[e];
@@ -235,7 +209,7 @@ template <class Op>
 __global__ void __launch_bounds__(kCtaThreads)
 hub_merge_kernel(typename Op::Params p, Shape sh, BinView bins, const float* __restrict__ partials, float* da_part,
                  int da_slot) {
-    constexpr int G = Op::kG, NV = Op::kNV, VEC = Op::kVEC;
+    constexpr int G = Op::kG, CH = Op::kCH;
     extern __shared__ float4 smem4[];
     float* s_merged = reinterpret_cast<float*>(smem4);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -270,22 +244,16 @@ hub_merge_kernel(typename Op::Params p, Shape sh, BinView bins, const float* __r
         s_merged[e] = s;
     }
     __syncthreads();
-    float da[NV][VEC];
+    float da[CH];
 #pragma unroll
-    for (int t = 0; t < NV; ++t)
-#pragma unroll
-        for (int c = 0; c < VEC; ++c) da[t][c] = 0.f;
+    for (int c = 0; c < CH; ++c) da[c] = 0.f;
     if (warp == 0 && lane < G) {
         typename Op::St st;
         state_from_smem<Op>(st, s_merged, g, sh);
         Op::finalize(st, p, sh, row, g, da);
-        if (Op::HAS_DA) {
+        if (Op::HAS_DA && g.act) {
 #pragma unroll
-            for (int t = 0; t < NV; ++t)
-                if (g.act[t]) {
-#pragma unroll
-                    for (int c = 0; c < VEC; ++c) da_part[(size_t)(da_slot + slot) * sh.rowe + g.eoff[t] + c] = da[t][c];
-                }
+            for (int c = 0; c < CH; ++c) da_part[(size_t)(da_slot + slot) * sh.rowe + g.eoff + c] = da[c];
         }
     }
 }
@@ -300,10 +268,10 @@ inline GridPlan grid_plan(const BinView& b, int sm_count, int G) {
     const int GPW = 32 / G;
     GridPlan gp;
     const int nseg = b.n_chunks + b.n_cta;
-    gp.seg_grid = nseg < sm_count * 8 ? nseg : sm_count * 8;
+    gp.seg_grid = nseg < sm_count * 16 ? nseg : sm_count * 16;
     const int ntiles = (b.n_group + GPW - 1) / GPW;
     const int nblk = (ntiles + kWarpsPerCta - 1) / kWarpsPerCta;
-    gp.grp_grid = nblk < sm_count * 16 ? nblk : sm_count * 16;
+    gp.grp_grid = nblk < sm_count * 32 ? nblk : sm_count * 32;
     gp.hub_grid = b.n_hub;
     return gp;
 }
