@@ -5,7 +5,7 @@
 
 namespace gnn {
 
-template <template <typename, int, int, int, int> class OpT, Pass PASS, typename Fill>
+template <template <typename, int, int, int> class OpT, Pass PASS, typename Fill>
 inline cudaError_t dispatch_pass(int dtype, const Shape& sh0, const LaunchCtx& c, Fill fill) {
     LaneCfg lc;
     const Shape sh = pass_shape(sh0, PASS, dtype == GNN_F32 ? 4 : 2, lc);
@@ -18,20 +18,17 @@ inline cudaError_t dispatch_pass(int dtype, const Shape& sh0, const LaunchCtx& c
         fill(p);
         return run_op<Op>(p, sh, c);
     };
-#define GNN_G(T, VB, NV)                                                                     \
+#define GNN_G(T, CB)                                                                         \
     {                                                                                        \
-        constexpr int KU = pass_ku(PASS, VB * NV);                                           \
-        if (lc.g == 4) return go((OpT<T, VB, NV, 4, KU>*)nullptr);                           \
-        if (lc.g == 8) return go((OpT<T, VB, NV, 8, KU>*)nullptr);                           \
-        if (lc.g == 16) return go((OpT<T, VB, NV, 16, KU>*)nullptr);                         \
-        if (lc.g == 32) return go((OpT<T, VB, NV, 32, KU>*)nullptr);                         \
+        constexpr int KU = pass_ku(PASS, CB);                                                \
+        if (lc.g == 4) return go((OpT<T, CB, 4, KU>*)nullptr);                               \
+        if (lc.g == 8) return go((OpT<T, CB, 8, KU>*)nullptr);                               \
+        if (lc.g == 16) return go((OpT<T, CB, 16, KU>*)nullptr);                             \
+        if (lc.g == 32) return go((OpT<T, CB, 32, KU>*)nullptr);                             \
     }
 #define GNN_GO(T)                                                                            \
-    if (lc.cb == 16) GNN_G(T, 16, 1)                                                         \
-    if (lc.cb == 32) GNN_G(T, 32, 1)                                                         \
-    if constexpr (pass_inst_max_cb(PASS) >= 64) {                                                 \
-        if (lc.cb == 64) GNN_G(T, 32, 2)                                                     \
-    }
+    if (lc.cb == 16) GNN_G(T, 16)                                                            \
+    if (lc.cb == 32) GNN_G(T, 32)
     if (dtype == GNN_F32) { GNN_GO(float) }
     if (dtype == GNN_BF16) { GNN_GO(__nv_bfloat16) }
 #undef GNN_GO

@@ -72,6 +72,44 @@ __device__ __forceinline__ float lg2(float x) {
     return y;
 }
 
+// ---- asynchronous gathers into shared memory (cp.async / LDGSTS).  Every lane copies exactly the bytes it
+// will consume itself, into lane-private slots of a per-warp ring, so completion needs only the lane's own
+// cp.async.wait_group (no barrier) and gathers in flight hold no registers.  pred == false zero-fills.
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool pred) {
+    const int sz = pred ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async4(uint32_t dst, const void* src, bool pred) {
+    const int sz = pred ? 4 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 r;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+    return r;
+}
+__device__ __forceinline__ float lds32(uint32_t addr) {
+    float r;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r) : "r"(addr));
+    return r;
+}
+
+// ---- mixed-precision arithmetic on packed bf16 pairs (sm_100: FHFMA.BF16 / FHADD.BF16 take the .H0/.H1 half
+// of a register directly, so bf16 operands need no unpack instruction; products are exact, sums fp32)
+__device__ __forceinline__ void fma_bf16x2(uint32_t a, uint32_t b, float& acc0, float& acc1) {
+    asm("{\n .reg .b16 al, ah, bl, bh;\n mov.b32 {al, ah}, %2;\n mov.b32 {bl, bh}, %3;\n"
+        " fma.rn.f32.bf16 %0, al, bl, %0;\n fma.rn.f32.bf16 %1, ah, bh, %1;\n}"
+        : "+f"(acc0), "+f"(acc1) : "r"(a), "r"(b));
+}
+// (lo, hi) halves of a packed bf16 pair, each added to an fp32 value: z = bf16 + f32
+__device__ __forceinline__ void add_bf16x2(uint32_t a, float x0, float x1, float& z0, float& z1) {
+    // volatile: stops the compiler from keeping z alive across the head reduction instead of recomputing it
+    asm volatile("{\n .reg .b16 al, ah;\n mov.b32 {al, ah}, %2;\n add.rn.f32.bf16 %0, al, %3;\n add.rn.f32.bf16 %1, ah, %4;\n}"
+        : "=f"(z0), "=f"(z1) : "r"(a), "f"(x0), "f"(x1));
+}
+
 // ---- raw VB-byte gathers (VB = 16 or 32), kept unconverted until use so in-flight loads stay small
 template <int VB> struct Raw { uint32_t w[VB / 4]; };
 
@@ -106,20 +144,74 @@ template <> __device__ __forceinline__ float raw_elt<__nv_bfloat16, 32>(const Ra
     return __uint_as_float((i & 1) ? (r.w[i >> 1] & 0xffff0000u) : (r.w[i >> 1] << 16));
 }
 
-// A lane's CH contiguous channels of a [*, rowe] tensor of T: NV raw vectors.
-template <typename T, int VB, int NV> struct Chunk {
-    static constexpr int VEC = VB / (int)sizeof(T), CH = NV * VEC;
-    Raw<VB> v[NV];
-    __device__ __forceinline__ void load(const T* base, size_t elt, bool pred) {
+// A lane's CB contiguous bytes (CH = CB / sizeof(T) channels of one head) of a [*, rowe] tensor of T, kept as raw
+// 32-bit words.  In the per-warp ring the 16-byte pieces of a chunk sit 512 bytes apart (32 lanes x 16 bytes),
+// so both the cp.async writes and the LDS.128 reads of a warp are conflict-free.
+template <typename T, int CB> struct Chunk {
+    static constexpr int CH = CB / (int)sizeof(T), NW = CB / 4, NP = CB / 16;
+    uint32_t w[NW];
+    __device__ __forceinline__ void load_global(const T* base, size_t elt, bool pred) {
+        if constexpr (CB >= 32) {
 #pragma unroll
-        for (int t = 0; t < NV; ++t) v[t] = ldg_raw<VB>(base + elt + t * VEC, pred);
+            for (int t = 0; t < CB / 32; ++t) {
+                const Raw<32> r = ldg_raw<32>(reinterpret_cast<const char*>(base + elt) + 32 * t, pred);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) w[8 * t + i] = r.w[i];
+            }
+        } else {
+            const Raw<16> r = ldg_raw<16>(base + elt, pred);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) w[i] = r.w[i];
+        }
     }
-    __device__ __forceinline__ float get(int c) const { return raw_elt<T, VB>(v[c / VEC], c % VEC); }
+    // issue the asynchronous copy of this chunk of row `src` into the ring (addr = lane's slot of piece 0)
+    __device__ __forceinline__ static void issue(uint32_t addr, const T* src, bool pred) {
+#pragma unroll
+        for (int v = 0; v < NP; ++v) cp_async16(addr + 512 * v, reinterpret_cast<const char*>(src) + 16 * v, pred);
+    }
+    __device__ __forceinline__ void load_smem(uint32_t addr) {
+#pragma unroll
+        for (int v = 0; v < NP; ++v) {
+            const uint4 r = lds128(addr + 512 * v);
+            w[4 * v] = r.x; w[4 * v + 1] = r.y; w[4 * v + 2] = r.z; w[4 * v + 3] = r.w;
+        }
+    }
+    __device__ __forceinline__ float get(int c) const {
+        if constexpr (sizeof(T) == 4) return __uint_as_float(w[c]);
+        else return __uint_as_float((c & 1) ? (w[c >> 1] & 0xffff0000u) : (w[c >> 1] << 16));
+    }
     __device__ __forceinline__ void to_float(float (&o)[CH]) const {
 #pragma unroll
         for (int c = 0; c < CH; ++c) o[c] = get(c);
     }
 };
+
+// <a, b> over the lane's channels: fp32 accumulation of exact products (bf16: FHFMA on packed halves)
+template <typename T, int CB> __device__ __forceinline__ float dot(const Chunk<T, CB>& a, const Chunk<T, CB>& b) {
+    float s0 = 0.f, s1 = 0.f;
+    if constexpr (sizeof(T) == 4) {
+#pragma unroll
+        for (int i = 0; i < CB / 4; i += 2) {
+            s0 = fmaf(__uint_as_float(a.w[i]), __uint_as_float(b.w[i]), s0);
+            s1 = fmaf(__uint_as_float(a.w[i + 1]), __uint_as_float(b.w[i + 1]), s1);
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < CB / 4; ++i) fma_bf16x2(a.w[i], b.w[i], s0, s1);
+    }
+    return s0 + s1;
+}
+// z[c] = x[c] + chunk[c]  (bf16: FHADD on packed halves)
+template <typename T, int CB> __device__ __forceinline__ void add_chunk(const Chunk<T, CB>& a, const float (&x)[CB / (int)sizeof(T)],
+                                                                         float (&z)[CB / (int)sizeof(T)]) {
+    if constexpr (sizeof(T) == 4) {
+#pragma unroll
+        for (int c = 0; c < CB / 4; ++c) z[c] = x[c] + __uint_as_float(a.w[c]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < CB / 4; ++i) add_bf16x2(a.w[i], x[2 * i], x[2 * i + 1], z[2 * i], z[2 * i + 1]);
+    }
+}
 
 // CH contiguous fp32 values (a, gradients): plain 128-bit accesses
 template <int CH> __device__ __forceinline__ void load_f32(const float* base, size_t elt, bool pred, float (&o)[CH]) {

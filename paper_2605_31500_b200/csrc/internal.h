@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 #include "../../include/gnn_attn.h"
 #include "engine.cuh"
@@ -36,22 +37,27 @@ inline int pass_state_floats(Pass p, const Shape& sh) {
     return kPassInfo[p].na * sh.rowe + (kPassInfo[p].ns + kPassInfo[p].softmax) * sh.H;
 }
 // Lane layout of a pass: each lane owns `cb` contiguous bytes of one head (nv loads of vb bytes), a row
-// takes `lanes` lanes inside a group of g lanes (power of two, 4..32).  Forward passes use up to 64 bytes
-// per lane, backward passes (more live accumulators) up to 32 (16 for the 4-accumulator GATv2 dst pass).
+// takes `lanes` lanes inside a group of g lanes (power of two, 4..32).  32 bytes per lane (one 256-bit load per
+// gathered row) measured best on B200 for every pass (profiles/r01_lane_width_sweep.md); 16 when head_dim*sizeof
+// is 16.  GNN_MAX_CB_FWD / GNN_MAX_CB_BWD (16|32) override the width for tuning runs.
 struct LaneCfg { int vb, nv, cb, g, lanes; };
-constexpr int pass_max_cb(Pass p) { return (p == kGtFwd || p == kGatFwd) ? 64 : (p == kGatBwdDst) ? 16 : 32; }
+constexpr int pass_max_cb(Pass) { return 32; }
 // widest lane the pass is instantiated for (wide rows may exceed the preferred pass_max_cb)
-constexpr int pass_inst_max_cb(Pass p) { return (p == kGtFwd || p == kGatFwd) ? 64 : 32; }
-// edges gathered per lane group per batch (independent loads in flight), by pass and bytes per lane
+constexpr int pass_inst_max_cb(Pass) { return 32; }
+// edges per lane group per batch (two batches are in flight per group: one being computed, one being gathered);
+// KU must divide the group width (>= 4)
 constexpr int pass_ku(Pass p, int cb) {
-    return (p == kGtFwd) ? (cb == 64 ? 2 : 4)
-         : (p == kGatFwd) ? (cb == 64 ? 2 : 4)
-         : (p == kGatBwdDst) ? (cb == 32 ? 2 : 4)
-         : (cb == 32 ? 2 : 4);
+    return (p == kGatFwd) ? (cb == 32 ? 2 : 4)                  // one gathered row per edge
+         : (p == kGatBwdDst) ? (cb == 32 ? 2 : 4)               // one row, four accumulators
+                             : (cb == 32 ? 2 : 4);              // two gathered rows per edge
 }
 inline bool pick_lane_cfg(Pass p, int esz, int heads, int head_dim, LaneCfg& lc) {
     const int head_bytes = head_dim * esz, row_bytes = heads * head_bytes;
     int cb = pass_max_cb(p);
+    if (const char* e = getenv((p == kGtFwd || p == kGatFwd) ? "GNN_MAX_CB_FWD" : "GNN_MAX_CB_BWD")) {  // tuning knob
+        const int v = atoi(e);
+        if ((v == 16 || v == 32 || v == 64) && v <= pass_inst_max_cb(p)) cb = v;
+    }
     while (cb > head_bytes) cb >>= 1;
     while (row_bytes / cb > 32 && cb * 2 <= head_bytes && cb * 2 <= pass_inst_max_cb(p)) cb <<= 1;  // wide rows
     if (cb < 16 || row_bytes / cb > 32) return false;

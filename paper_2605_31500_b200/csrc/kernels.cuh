@@ -60,71 +60,141 @@ __device__ __forceinline__ void cta_write_da(const float (&da)[Op::kCH], float* 
 }
 
 // ------------------------------------------------------------------------------------------------
-// group rows: one lane group per row, rows perm[first .. first+count), static round-robin over warps
+// The edge loop of one lane group: blocks of G edges (block k = [ebeg + k*stride, +G), clipped to eend), cut
+// into batches of KU edges.  The gathers of batch t+1 are issued (into a second register set) before batch t
+// is computed, and the colidx words of the next block are fetched one block ahead.  nblk and cnt_last (edges to
+// cover in the last block) are warp-uniform; groups with fewer edges see masked (-1) neighbours.
 template <class Op>
-__global__ void __launch_bounds__(kCtaThreads)
+__device__ __forceinline__ void run_edges(typename Op::St& st, const typename Op::Own& own, const typename Op::Params& p,
+                                          const Shape& sh, const typename Op::GeoT& g,
+                                          const int32_t* __restrict__ colidx, int ebeg, int eend, int stride, int nblk,
+                                          int cnt_last) {
+    constexpr int G = Op::kG, KU = Op::kU, BPB = G / KU;
+    static_assert(G % KU == 0, "KU must divide G");
+    if (nblk <= 0) return;
+    const int gl = threadIdx.x & (G - 1);
+    const int T = (nblk - 1) * BPB + (cnt_last + KU - 1) / KU;
+    auto ldidx = [&](int k) -> int {
+        const int e = ebeg + k * stride + gl;
+        return (k < nblk && e < eend) ? __ldg(colidx + e) : -1;
+    };
+    int my_cur = ldidx(0), my_next = ldidx(1);
+    auto nbrs = [&](int t, int kc, int (&nbr)[KU]) {
+        const int k = t / BPB, u0 = (t % BPB) * KU;
+        const int src = (k == kc) ? my_cur : my_next;
+#pragma unroll
+        for (int u = 0; u < KU; ++u) nbr[u] = __shfl_sync(0xffffffffu, src, u0 + u, G);
+    };
+    if constexpr (!Op::kDoubleBuffer) {
+        // single register set: gather batch t, then compute it (passes whose accumulators leave no room for two sets)
+        for (int t = 0; t < T; ++t) {
+            const int kc = t / BPB;
+            int na[KU];
+            nbrs(t, kc, na);
+            typename Op::Src sa;
+            Op::gather(p, sh, na, g, sa);
+            Op::compute(st, own, p, sh, na, g, sa);
+            if ((t % BPB) == BPB - 1) { my_cur = my_next; my_next = ldidx(kc + 2); }
+        }
+        return;
+    } else {
+    typename Op::Src sa, sb;
+    int na[KU], nb[KU];
+    nbrs(0, 0, na);
+    Op::gather(p, sh, na, g, sa);
+    for (int t = 0; t < T; t += 2) {
+        const int kc = t / BPB;
+        // batch t+1 -> set b (masked when past the end), then compute batch t from set a
+        if (t + 1 < T) nbrs(t + 1, kc, nb);
+        else {
+#pragma unroll
+            for (int u = 0; u < KU; ++u) nb[u] = -1;
+        }
+        Op::gather(p, sh, nb, g, sb);
+        Op::compute(st, own, p, sh, na, g, sa);
+        if ((t % BPB) == BPB - 1) { my_cur = my_next; my_next = ldidx(kc + 2); }
+        if (t + 1 >= T) break;
+        const int kc1 = (t + 1) / BPB;
+        if (t + 2 < T) nbrs(t + 2, kc1, na);
+        else {
+#pragma unroll
+            for (int u = 0; u < KU; ++u) na[u] = -1;
+        }
+        Op::gather(p, sh, na, g, sa);
+        Op::compute(st, own, p, sh, nb, g, sb);
+        if (((t + 1) % BPB) == BPB - 1) { my_cur = my_next; my_next = ldidx(kc1 + 2); }
+    }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// group rows: one lane group per row, rows perm[first .. first+count), static round-robin over warps.
+// The (row, rowptr) chain of the next tile is fetched while the current tile is processed.
+// smem: NG * rowe floats for the da reduction (GATv2 dst pass only)
+template <class Op>
+__global__ void __launch_bounds__(kCtaThreads, Op::kMinBlocks)
 group_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
              const int32_t* __restrict__ perm, int first, int count, float* da_part, int da_slot) {
-    constexpr int G = Op::kG, CH = Op::kCH, kU = Op::kU;
+    constexpr int G = Op::kG, CH = Op::kCH;
     constexpr int GPW = 32 / G;
     extern __shared__ float4 smem4[];
     float* smem = reinterpret_cast<float*>(smem4);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     typename Op::GeoT g;
     g.init(sh, lane);
-    const int gl = lane & (G - 1);
     float da[CH];
 #pragma unroll
     for (int c = 0; c < CH; ++c) da[c] = 0.f;
 
     const int ntiles = (count + GPW - 1) / GPW;
     const int total_warps = gridDim.x * kWarpsPerCta;
-    for (int tile = blockIdx.x * kWarpsPerCta + warp; tile < ntiles; tile += total_warps) {
-        const int idx = tile * GPW + lane / G;
-        const bool valid = idx < count;
-        int row = 0, e0 = 0, len = 0;
-        if (valid) {
-            row = __ldg(perm + first + idx);
-            e0 = __ldg(rowptr + row);
-            len = __ldg(rowptr + row + 1) - e0;
-        }
+    const int sub = lane / G;
+    auto ld_row = [&](int tile) -> int {
+        const int idx = tile * GPW + sub;
+        return (tile < ntiles && idx < count) ? __ldg(perm + first + idx) : -1;
+    };
+    int tile = blockIdx.x * kWarpsPerCta + warp;
+    int row = ld_row(tile);
+    int e0 = row >= 0 ? __ldg(rowptr + row) : 0;
+    int e1 = row >= 0 ? __ldg(rowptr + row + 1) : 0;
+    int row_n = ld_row(tile + total_warps);
+    for (; tile < ntiles; tile += total_warps) {
+        // next tile's row pointers and the row id of the tile after it: consumed at the bottom of the loop
+        const int e0_n = row_n >= 0 ? __ldg(rowptr + row_n) : 0;
+        const int e1_n = row_n >= 0 ? __ldg(rowptr + row_n + 1) : 0;
+        const int row_nn = ld_row(tile + 2 * total_warps);
+        const bool valid = row >= 0;
+        const int len = e1 - e0;
         typename Op::Own own;
-        Op::load_own(own, p, sh, row, valid, g);
+        Op::load_own(own, p, sh, valid ? row : 0, valid, g);
         typename Op::St st;
         st.reset();
         int maxlen = len;
 #pragma unroll
         for (int o = G; o < 32; o <<= 1) maxlen = max(maxlen, __shfl_xor_sync(0xffffffffu, maxlen, o));
-        for (int base = 0; base < maxlen; base += G) {
-            const int my = (base + gl < len) ? __ldg(colidx + e0 + base + gl) : -1;
-            const int cnt = min(G, maxlen - base);
-            for (int u0 = 0; u0 < cnt; u0 += kU) {
-                int nbr[kU];
-#pragma unroll
-                for (int u = 0; u < kU; ++u) nbr[u] = __shfl_sync(0xffffffffu, my, u0 + u, G);
-                Op::batch(st, own, p, sh, nbr, g);
-            }
-        }
+        const int nblk = (maxlen + G - 1) / G;
+        run_edges<Op>(st, own, p, sh, g, colidx, e0, e1, G, nblk, maxlen - (nblk - 1) * G);
         if (valid) Op::finalize(st, p, sh, row, g, da);
+        row = row_n; e0 = e0_n; e1 = e1_n; row_n = row_nn;
     }
     if (Op::HAS_DA)
-        cta_write_da<Op>(da, smem, da_part, da_slot + blockIdx.x, g, sh, warp * GPW + lane / G, kWarpsPerCta * GPW);
+        cta_write_da<Op>(da, smem, da_part, da_slot + blockIdx.x, g, sh, warp * GPW + sub, kWarpsPerCta * GPW);
 }
 
 // ------------------------------------------------------------------------------------------------
 // CTA rows + hub chunks: one CTA per segment; seg < n_chunks is hub chunk `seg` (partial state ->
 // partials[seg]), otherwise the full row perm[n_hub + seg - n_chunks] (finalised in place).
-// smem: NG * (NA*rowe + NS*H) + state_floats + NG * H floats.
+// smem: NG * TEs + state_floats + NG * H floats for the merge.
 template <class Op>
-__global__ void __launch_bounds__(kCtaThreads)
+__global__ void __launch_bounds__(kCtaThreads, Op::kMinBlocks)
 segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx,
                BinView bins, float* __restrict__ partials, float* da_part, int da_slot) {
-    constexpr int G = Op::kG, CH = Op::kCH, kU = Op::kU;
+    constexpr int G = Op::kG, CH = Op::kCH;
     constexpr int GPW = 32 / G, NG = kWarpsPerCta * GPW;
     extern __shared__ float4 smem4[];
-    float* smem = reinterpret_cast<float*>(smem4);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int gi = warp * GPW + lane / G, gl = lane & (G - 1);
+    float* smem = reinterpret_cast<float*>(smem4);
+    const int gi = warp * GPW + lane / G;
     typename Op::GeoT g;
     g.init(sh, lane);
     const int TEp = Op::NA * sh.rowe + Op::NS * sh.H;  // floats per group partial (without max)
@@ -153,19 +223,14 @@ segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowp
         Op::load_own(own, p, sh, row, true, g);
         typename Op::St st;
         st.reset();
-        const int nblk = (e1 - e0 + G - 1) / G;
-        for (int b0 = warp * GPW; b0 < nblk; b0 += NG) {
-            const int eb = e0 + (b0 + lane / G) * G;
-            const int my = (eb + gl < e1) ? __ldg(colidx + eb + gl) : -1;
-#pragma unroll 1
-            for (int u0 = 0; u0 < G; u0 += kU) {
-                int nbr[kU];
-#pragma unroll
-                for (int u = 0; u < kU; ++u) nbr[u] = __shfl_sync(0xffffffffu, my, u0 + u, G);
-                if (__all_sync(0xffffffffu, nbr[0] < 0)) break;  // warp-uniform tail exit
-                Op::batch(st, own, p, sh, nbr, g);
-            }
-        }
+        // blocks of G edges are dealt round-robin to the NG groups; this warp's first group takes blocks
+        // warp*GPW + k*NG, so its block count / last-block fill bound those of the warp's other groups
+        const int nblk_all = (e1 - e0 + G - 1) / G;
+        const int wfirst = warp * GPW;
+        const int nblk = nblk_all > wfirst ? (nblk_all - wfirst + NG - 1) / NG : 0;
+        const int last_first_edge = e0 + (wfirst + (nblk - 1) * NG) * G;
+        const int cnt_last = min(G, e1 - last_first_edge);
+        run_edges<Op>(st, own, p, sh, g, colidx, e0 + gi * G, e1, NG * G, nblk, cnt_last);
         // ---- cross-group merge: global max, rescale, fixed-order sum
         if (Op::SOFTMAX) {
             if (g.lead) s_max[gi * sh.H + g.hd] = st.m;
@@ -283,6 +348,10 @@ template <class Op> inline size_t seg_smem_bytes(const Shape& sh) {
     size_t da = Op::HAS_DA ? (size_t)NG * sh.rowe : 0;
     return 4 * (f > da ? f : da) + 16;
 }
+template <class Op> inline size_t grp_smem_bytes(const Shape& sh) {
+    constexpr int NG = kWarpsPerCta * (32 / Op::kG);
+    return (Op::HAS_DA ? 4 * (size_t)NG * sh.rowe : 0) + 16;
+}
 
 template <class Op> inline cudaError_t run_op(const typename Op::Params& p, const Shape& sh, const LaunchCtx& c) {
     const BinView& b = c.bins;
@@ -303,7 +372,11 @@ template <class Op> inline cudaError_t run_op(const typename Op::Params& p, cons
     }
     slot += gp.seg_grid;
     if (gp.grp_grid > 0) {
-        const size_t smem = Op::HAS_DA ? 4 * (size_t)NG * sh.rowe + 16 : 16;
+        const size_t smem = grp_smem_bytes<Op>(sh);
+        if (smem > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(group_kernel<Op>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
         prof_begin(Op::kName, "group", c.stream);
         group_kernel<Op><<<gp.grp_grid, kCtaThreads, smem, c.stream>>>(p, sh, c.rowptr, c.colidx, b.perm,
                                                                        b.n_hub + b.n_cta, b.n_group, c.da_part, slot);

@@ -5,12 +5,17 @@
 
 namespace gnn {
 
+__device__ __forceinline__ float lrelu(float z, float slope) { return fmaxf(z, 0.f) + slope * fminf(z, 0.f); }
+
 // ------------------------------------------------------------------------------------ GATv2 forward
-template <typename T, int VB_, int NV_, int G_, int KU_> struct GatFwd : OpBase<T, VB_, NV_, G_, KU_> {
+template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G_, KU_, 1, 0> {
     static constexpr const char* kName = "gatv2_fwd";
-    using B = OpBase<T, VB_, NV_, G_, KU_>;
+    static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = true;
+    using B = OpBase<T, CB_, G_, KU_, 1, 0>;
     using typename B::GeoT;
     using typename B::Ck;
+    using typename B::Src;
     static constexpr int CH = B::kCH, KU = KU_;
     static constexpr int NA = 1, NS = 1;
     static constexpr bool SOFTMAX = true, HAS_DA = false;
@@ -27,27 +32,31 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GatFwd : OpBase<
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
         Ck c;
-        c.load(p.xl, (size_t)row * sh.rowe + g.eoff, valid && g.act);
+        c.load_global(p.xl, (size_t)row * sh.rowe + g.eoff, valid && g.act);
         c.to_float(o.xl);
         load_f32<CH>(p.a, g.eoff, g.act, o.a);
 #pragma unroll
         for (int i = 0; i < CH; ++i) o.a[i] *= kLog2e;
     }
-    __device__ __forceinline__ static void batch(St& st, const Own& o, const Params& p, const Shape& sh,
-                                                 const int (&nbr)[KU], const GeoT& g) {
-        Ck xr[KU];
+    __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
+                                                  Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u)
-            xr[u].load(p.xr, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff, nbr[u] >= 0 && g.act);
+            src.c[u][0].load_global(p.xr, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff, nbr[u] >= 0 && g.act);
+    }
+    __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
+                                                   const int (&nbr)[KU], const GeoT& g, const Src& src) {
         float s[KU];
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
+            const Ck& xc = src.c[u][0];
+            float z[CH];
+            add_chunk(xc, o.xl, z);
             float a0 = 0.f, a1 = 0.f;
 #pragma unroll
             for (int c = 0; c < CH; c += 2) {
-                const float z0 = o.xl[c] + xr[u].get(c), z1 = o.xl[c + 1] + xr[u].get(c + 1);
-                a0 = fmaf(o.a[c], fmaxf(z0, 0.f) + p.slope * fminf(z0, 0.f), a0);
-                a1 = fmaf(o.a[c + 1], fmaxf(z1, 0.f) + p.slope * fminf(z1, 0.f), a1);
+                a0 = fmaf(o.a[c], lrelu(z[c], p.slope), a0);
+                a1 = fmaf(o.a[c + 1], lrelu(z[c + 1], p.slope), a1);
             }
             s[u] = a0 + a1;
         }
@@ -60,8 +69,9 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GatFwd : OpBase<
         for (int c = 0; c < CH; ++c) st.acc[0][c] *= corr;
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
+            const Ck& xc = src.c[u][0];
 #pragma unroll
-            for (int c = 0; c < CH; ++c) st.acc[0][c] = fmaf(pw[u], xr[u].get(c), st.acc[0][c]);
+            for (int c = 0; c < CH; ++c) st.acc[0][c] = fmaf(pw[u], xc.get(c), st.acc[0][c]);
         }
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
@@ -80,11 +90,14 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GatFwd : OpBase<
 // One sweep: with as = a . LeakyReLU'(z), sg = LeakyReLU(z), w = alpha dP:
 //   A1 = sum w as, B1 = sum alpha as, A2 = sum w sg, B2 = sum alpha sg, G = sum w
 //   dxl_i = A1 - G B1;  this row's share of da = A2 - G B2      (== sum_j de_ij ...)
-template <typename T, int VB_, int NV_, int G_, int KU_> struct GatBwdDst : OpBase<T, VB_, NV_, G_, KU_> {
+template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_, G_, KU_, 1, 0> {
     static constexpr const char* kName = "gatv2_bwd_dst";
-    using B = OpBase<T, VB_, NV_, G_, KU_>;
+    static constexpr int kMinBlocks = 2;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = false;
+    using B = OpBase<T, CB_, G_, KU_, 1, 0>;
     using typename B::GeoT;
     using typename B::Ck;
+    using typename B::Src;
     static constexpr int CH = B::kCH, KU = KU_;
     static constexpr int NA = 4, NS = 1;
     static constexpr bool SOFTMAX = false, HAS_DA = true;
@@ -95,49 +108,50 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GatBwdDst : OpBa
         float *dxl, *g;
         float slope;
     };
-    struct Own { float xl[CH], go[CH], a[CH], lp; };
+    struct Own { float xl[CH], a[CH], lp; Ck go; };
 
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
         const bool pr = valid && g.act;
-        Ck c0, c1;
-        c0.load(p.xl, (size_t)row * sh.rowe + g.eoff, pr);
-        c1.load(p.dout, (size_t)row * sh.rowe + g.eoff, pr);
+        Ck c0;
+        c0.load_global(p.xl, (size_t)row * sh.rowe + g.eoff, pr);
         c0.to_float(o.xl);
-        c1.to_float(o.go);
+        o.go.load_global(p.dout, (size_t)row * sh.rowe + g.eoff, pr);
         load_f32<CH>(p.a, g.eoff, g.act, o.a);
         o.lp = pr ? __ldg(p.lse + (size_t)row * sh.H + g.hd) * kLog2e : 0.f;
     }
-    __device__ __forceinline__ static void batch(St& st, const Own& o, const Params& p, const Shape& sh,
-                                                 const int (&nbr)[KU], const GeoT& g) {
-        Ck xr[KU];
+    __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
+                                                  Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u)
-            xr[u].load(p.xr, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff, nbr[u] >= 0 && g.act);
+            src.c[u][0].load_global(p.xr, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff, nbr[u] >= 0 && g.act);
+    }
+    __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
+                                                   const int (&nbr)[KU], const GeoT& g, const Src& src) {
         float r[2 * KU];
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            float a = 0.f, b = 0.f;
+            const Ck& xc = src.c[u][0];
+            float z[CH];
+            add_chunk(xc, o.xl, z);
+            float a0 = 0.f;
 #pragma unroll
-            for (int c = 0; c < CH; ++c) {
-                const float f = xr[u].get(c);
-                const float z = o.xl[c] + f;
-                a = fmaf(o.a[c], fmaxf(z, 0.f) + p.slope * fminf(z, 0.f), a);
-                b = fmaf(o.go[c], f, b);
-            }
-            r[2 * u] = a;
-            r[2 * u + 1] = b;
+            for (int c = 0; c < CH; ++c) a0 = fmaf(o.a[c], lrelu(z[c], p.slope), a0);
+            r[2 * u] = a0;
+            r[2 * u + 1] = dot(o.go, xc);
         }
         head_reduce(r, g.lpl);
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
             const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] * kLog2e - o.lp);
             const float w = alpha * r[2 * u + 1];
+            const Ck& xc = src.c[u][0];
+            float z[CH];
+            add_chunk(xc, o.xl, z);
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-                const float z = o.xl[c] + xr[u].get(c);
-                const bool pos = z > 0.f;
-                const float sg = pos ? z : p.slope * z;
+                const bool pos = z[c] > 0.f;
+                const float sg = pos ? z[c] : p.slope * z[c];
                 const float as = pos ? o.a[c] : p.slope * o.a[c];
                 st.acc[0][c] = fmaf(w, as, st.acc[0][c]);
                 st.acc[1][c] = fmaf(alpha, as, st.acc[1][c]);
@@ -162,11 +176,14 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GatBwdDst : OpBa
 };
 
 // ----------------------------------------------------- GATv2 backward, src pass over CSR^T ("R" kernel)
-template <typename T, int VB_, int NV_, int G_, int KU_> struct GatBwdSrc : OpBase<T, VB_, NV_, G_, KU_> {
+template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_, G_, KU_, 2, 2> {
     static constexpr const char* kName = "gatv2_bwd_src";
-    using B = OpBase<T, VB_, NV_, G_, KU_>;
+    static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = false;
+    using B = OpBase<T, CB_, G_, KU_, 2, 2>;
     using typename B::GeoT;
     using typename B::Ck;
+    using typename B::Src;
     static constexpr int CH = B::kCH, KU = KU_;
     static constexpr int NA = 1, NS = 0;
     static constexpr bool SOFTMAX = false, HAS_DA = false;
@@ -177,51 +194,53 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GatBwdSrc : OpBa
         float* dxr;
         float slope;
     };
-    struct Own { float xr[CH], a[CH]; };
+    struct Own { Ck xr; float xrf[CH], a[CH]; };
 
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
-        Ck c;
-        c.load(p.xr, (size_t)row * sh.rowe + g.eoff, valid && g.act);
-        c.to_float(o.xr);
+        o.xr.load_global(p.xr, (size_t)row * sh.rowe + g.eoff, valid && g.act);
+        o.xr.to_float(o.xrf);
         load_f32<CH>(p.a, g.eoff, g.act, o.a);
     }
-    __device__ __forceinline__ static void batch(St& st, const Own& o, const Params& p, const Shape& sh,
-                                                 const int (&nbr)[KU], const GeoT& g) {
-        Ck lr[KU], gr[KU];
-        float li[KU], gi[KU];
+    __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
+                                                  Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
             const bool pr = nbr[u] >= 0 && g.act;
             const size_t i = (size_t)(nbr[u] < 0 ? 0 : nbr[u]);
-            lr[u].load(p.xl, i * sh.rowe + g.eoff, pr);
-            gr[u].load(p.dout, i * sh.rowe + g.eoff, pr);
-            li[u] = pr ? __ldg(p.lse + i * sh.H + g.hd) : 0.f;
-            gi[u] = pr ? __ldg(p.g + i * sh.H + g.hd) : 0.f;
+            src.c[u][0].load_global(p.xl, i * sh.rowe + g.eoff, pr);
+            src.c[u][1].load_global(p.dout, i * sh.rowe + g.eoff, pr);
+            src.s[u][0] = pr ? __ldg(p.lse + i * sh.H + g.hd) : 0.f;
+            src.s[u][1] = pr ? __ldg(p.g + i * sh.H + g.hd) : 0.f;
         }
+    }
+    __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
+                                                   const int (&nbr)[KU], const GeoT& g, const Src& src) {
         float r[2 * KU];
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            float a = 0.f, b = 0.f;
+            const Ck &lc = src.c[u][0], &gc = src.c[u][1];
+            float z[CH];
+            add_chunk(lc, o.xrf, z);
+            float a0 = 0.f;
 #pragma unroll
-            for (int c = 0; c < CH; ++c) {
-                const float z = lr[u].get(c) + o.xr[c];
-                a = fmaf(o.a[c], fmaxf(z, 0.f) + p.slope * fminf(z, 0.f), a);
-                b = fmaf(gr[u].get(c), o.xr[c], b);
-            }
-            r[2 * u] = a;
-            r[2 * u + 1] = b;
+            for (int c = 0; c < CH; ++c) a0 = fmaf(o.a[c], lrelu(z[c], p.slope), a0);
+            r[2 * u] = a0;
+            r[2 * u + 1] = dot(gc, o.xr);
         }
         head_reduce(r, g.lpl);
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            const float alpha = nbr[u] < 0 ? 0.f : ex2((r[2 * u] - li[u]) * kLog2e);
-            const float de = alpha * (r[2 * u + 1] - gi[u]);
+            const float li = src.s[u][0], gi = src.s[u][1];
+            const float alpha = nbr[u] < 0 ? 0.f : ex2((r[2 * u] - li) * kLog2e);
+            const float de = alpha * (r[2 * u + 1] - gi);
+            const Ck &lc = src.c[u][0], &gc = src.c[u][1];
+            float z[CH];
+            add_chunk(lc, o.xrf, z);
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-                const float z = lr[u].get(c) + o.xr[c];
-                const float as = z > 0.f ? o.a[c] : p.slope * o.a[c];
-                st.acc[0][c] = fmaf(alpha, gr[u].get(c), fmaf(de, as, st.acc[0][c]));
+                const float as = z[c] > 0.f ? o.a[c] : p.slope * o.a[c];
+                st.acc[0][c] = fmaf(alpha, gc.get(c), fmaf(de, as, st.acc[0][c]));
             }
         }
     }

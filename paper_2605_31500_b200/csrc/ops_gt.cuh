@@ -1,15 +1,24 @@
 // ops_gt.cuh - Graph Transformer passes (PAPER.md:76; kernels PAPER.md:484-494; identities :539, :563).
 // Scores are carried in the log2 domain: s' = <q,k> * log2(e)/sqrt(d), alpha = 2^(s' - L*log2(e)).
+//
+// Every Op splits a batch of KU edges into gather() - the lane's 128/256-bit loads of its chunk of each gathered
+// row, kept raw in registers - and compute(), so the engine can issue batch t+1 before computing batch t.
 #pragma once
 #include "engine.cuh"
 
 namespace gnn {
 
-// T: feature dtype; VB: bytes per load (16|32); NV: loads per lane; G: lanes per row; KU: edges per batch
-template <typename T, int VB_, int NV_, int G_, int KU_> struct OpBase {
-    static constexpr int kG = G_, kVB = VB_, kNV = NV_, kU = KU_, kCH = NV_ * VB_ / (int)sizeof(T);
+// T: feature dtype; CB: bytes per lane per row (16|32|64); G: lanes per row; KU: edges per batch;
+// NT: gathered feature rows per edge; NSC: gathered per-(node, head) scalars per edge
+template <typename T, int CB_, int G_, int KU_, int NT_, int NSC_> struct OpBase {
+    static constexpr int kG = G_, kCB = CB_, kU = KU_, kCH = CB_ / (int)sizeof(T), kNT = NT_, kNSC = NSC_;
     using GeoT = Geo<G_>;
-    using Ck = Chunk<T, VB_, NV_>;
+    using Ck = Chunk<T, CB_>;
+    // the gathered operands of one batch of KU edges, raw (unconverted) in registers
+    struct Src {
+        Ck c[KU_][NT_];
+        float s[KU_][NSC_ > 0 ? NSC_ : 1];
+    };
 };
 
 // online-softmax update with KU new scores: fills p[u], updates (m, l), returns the rescale
@@ -31,11 +40,14 @@ template <int KU> __device__ __forceinline__ float softmax_step(float& m, float&
 }
 
 // ------------------------------------------------------------------------------------- GT forward
-template <typename T, int VB_, int NV_, int G_, int KU_> struct GtFwd : OpBase<T, VB_, NV_, G_, KU_> {
+template <typename T, int CB_, int G_, int KU_> struct GtFwd : OpBase<T, CB_, G_, KU_, 2, 0> {
     static constexpr const char* kName = "gt_fwd";
-    using B = OpBase<T, VB_, NV_, G_, KU_>;
+    static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = true;
+    using B = OpBase<T, CB_, G_, KU_, 2, 0>;
     using typename B::GeoT;
     using typename B::Ck;
+    using typename B::Src;
     static constexpr int CH = B::kCH, KU = KU_;
     static constexpr int NA = 1, NS = 1;
     static constexpr bool SOFTMAX = true, HAS_DA = false;
@@ -46,47 +58,42 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GtFwd : OpBase<T
         float* lse;
         float qscale;  // log2(e) / sqrt(d)
     };
-    struct Own { float q[CH]; };
+    struct Own { Ck q; };
 
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
-        Ck c;
-        c.load(p.q, (size_t)row * sh.rowe + g.eoff, valid && g.act);
-#pragma unroll
-        for (int i = 0; i < CH; ++i) o.q[i] = c.get(i) * p.qscale;
+        o.q.load_global(p.q, (size_t)row * sh.rowe + g.eoff, valid && g.act);
     }
-    __device__ __forceinline__ static void batch(St& st, const Own& o, const Params& p, const Shape& sh,
-                                                 const int (&nbr)[KU], const GeoT& g) {
-        Ck kr[KU], vr[KU];
+    __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
+                                                  Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
             const bool pr = nbr[u] >= 0 && g.act;
             const size_t off = (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff;
-            kr[u].load(p.k, off, pr);
-            vr[u].load(p.v, off, pr);
+            src.c[u][0].load_global(p.k, off, pr);
+            src.c[u][1].load_global(p.v, off, pr);
         }
+    }
+    __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
+                                                   const int (&nbr)[KU], const GeoT& g, const Src& src) {
         float s[KU];
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            float a0 = 0.f, a1 = 0.f;
-#pragma unroll
-            for (int c = 0; c < CH; c += 2) {
-                a0 = fmaf(o.q[c], kr[u].get(c), a0);
-                a1 = fmaf(o.q[c + 1], kr[u].get(c + 1), a1);
-            }
-            s[u] = a0 + a1;
+            const Ck& kc = src.c[u][0];
+            s[u] = dot(o.q, kc);
         }
         head_reduce(s, g.lpl);
         float pw[KU];
 #pragma unroll
-        for (int u = 0; u < KU; ++u) s[u] = nbr[u] < 0 ? -INFINITY : s[u];
+        for (int u = 0; u < KU; ++u) s[u] = nbr[u] < 0 ? -INFINITY : s[u] * p.qscale;
         const float corr = softmax_step<KU>(st.m, st.sc[0], s, pw);
 #pragma unroll
         for (int c = 0; c < CH; ++c) st.acc[0][c] *= corr;
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
+            const Ck& vc = src.c[u][1];
 #pragma unroll
-            for (int c = 0; c < CH; ++c) st.acc[0][c] = fmaf(pw[u], vr[u].get(c), st.acc[0][c]);
+            for (int c = 0; c < CH; ++c) st.acc[0][c] = fmaf(pw[u], vc.get(c), st.acc[0][c]);
         }
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
@@ -104,11 +111,14 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GtFwd : OpBase<T
 // ------------------------------------------------------------------- GT backward, dst pass (CSR)
 // One sweep, no O needed: A = sum alpha dP k, B = sum alpha k, Delta = sum alpha dP;
 // dQ = (A - Delta B)/sqrt(d)   (== sum_j alpha (dP - Delta) k_j / sqrt(d))
-template <typename T, int VB_, int NV_, int G_, int KU_> struct GtBwdDst : OpBase<T, VB_, NV_, G_, KU_> {
+template <typename T, int CB_, int G_, int KU_> struct GtBwdDst : OpBase<T, CB_, G_, KU_, 2, 0> {
     static constexpr const char* kName = "gt_bwd_dst";
-    using B = OpBase<T, VB_, NV_, G_, KU_>;
+    static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = false;
+    using B = OpBase<T, CB_, G_, KU_, 2, 0>;
     using typename B::GeoT;
     using typename B::Ck;
+    using typename B::Src;
     static constexpr int CH = B::kCH, KU = KU_;
     static constexpr int NA = 2, NS = 1;
     static constexpr bool SOFTMAX = false, HAS_DA = false;
@@ -119,51 +129,43 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GtBwdDst : OpBas
         float *dq, *delta;
         float qscale, inv_sqrt_d;
     };
-    struct Own { float q[CH], go[CH], lp; };
+    struct Own { Ck q, go; float lp; };
 
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
         const bool pr = valid && g.act;
-        Ck a, b;
-        a.load(p.q, (size_t)row * sh.rowe + g.eoff, pr);
-        b.load(p.dout, (size_t)row * sh.rowe + g.eoff, pr);
-#pragma unroll
-        for (int i = 0; i < CH; ++i) {
-            o.q[i] = a.get(i) * p.qscale;
-            o.go[i] = b.get(i);
-        }
+        o.q.load_global(p.q, (size_t)row * sh.rowe + g.eoff, pr);
+        o.go.load_global(p.dout, (size_t)row * sh.rowe + g.eoff, pr);
         o.lp = pr ? __ldg(p.lse + (size_t)row * sh.H + g.hd) * kLog2e : 0.f;
     }
-    __device__ __forceinline__ static void batch(St& st, const Own& o, const Params& p, const Shape& sh,
-                                                 const int (&nbr)[KU], const GeoT& g) {
-        Ck kr[KU], vr[KU];
+    __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
+                                                  Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
             const bool pr = nbr[u] >= 0 && g.act;
             const size_t off = (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff;
-            kr[u].load(p.k, off, pr);
-            vr[u].load(p.v, off, pr);
+            src.c[u][0].load_global(p.k, off, pr);
+            src.c[u][1].load_global(p.v, off, pr);
         }
+    }
+    __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
+                                                   const int (&nbr)[KU], const GeoT& g, const Src& src) {
         float r[2 * KU];
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            float a = 0.f, b = 0.f;
-#pragma unroll
-            for (int c = 0; c < CH; ++c) {
-                a = fmaf(o.q[c], kr[u].get(c), a);
-                b = fmaf(o.go[c], vr[u].get(c), b);
-            }
-            r[2 * u] = a;
-            r[2 * u + 1] = b;
+            const Ck &kc = src.c[u][0], &vc = src.c[u][1];
+            r[2 * u] = dot(o.q, kc);
+            r[2 * u + 1] = dot(o.go, vc);
         }
         head_reduce(r, g.lpl);
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] - o.lp);
+            const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] * p.qscale - o.lp);
             const float w = alpha * r[2 * u + 1];
+            const Ck& kc = src.c[u][0];
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-                const float kf = kr[u].get(c);
+                const float kf = kc.get(c);
                 st.acc[0][c] = fmaf(w, kf, st.acc[0][c]);
                 st.acc[1][c] = fmaf(alpha, kf, st.acc[1][c]);
             }
@@ -184,11 +186,14 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GtBwdDst : OpBas
 // ------------------------------------------------------------------ GT backward, src pass (CSR^T)
 // rows are SOURCES j, entries the destinations i they feed; dK_j, dV_j accumulate in registers in
 // CSR^T order: deterministic, no atomics (the paper uses atomicAdd here).
-template <typename T, int VB_, int NV_, int G_, int KU_> struct GtBwdSrc : OpBase<T, VB_, NV_, G_, KU_> {
+template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_, G_, KU_, 2, 2> {
     static constexpr const char* kName = "gt_bwd_src";
-    using B = OpBase<T, VB_, NV_, G_, KU_>;
+    static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = false;
+    using B = OpBase<T, CB_, G_, KU_, 2, 2>;
     using typename B::GeoT;
     using typename B::Ck;
+    using typename B::Src;
     static constexpr int CH = B::kCH, KU = KU_;
     static constexpr int NA = 2, NS = 0;
     static constexpr bool SOFTMAX = false, HAS_DA = false;
@@ -199,54 +204,46 @@ template <typename T, int VB_, int NV_, int G_, int KU_> struct GtBwdSrc : OpBas
         float *dk, *dv;
         float kscale, inv_sqrt_d;
     };
-    struct Own { float k[CH], v[CH]; };
+    struct Own { Ck k, v; };
 
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
         const bool pr = valid && g.act;
-        Ck a, b;
-        a.load(p.k, (size_t)row * sh.rowe + g.eoff, pr);
-        b.load(p.v, (size_t)row * sh.rowe + g.eoff, pr);
-#pragma unroll
-        for (int i = 0; i < CH; ++i) {
-            o.k[i] = a.get(i) * p.kscale;
-            o.v[i] = b.get(i);
-        }
+        o.k.load_global(p.k, (size_t)row * sh.rowe + g.eoff, pr);
+        o.v.load_global(p.v, (size_t)row * sh.rowe + g.eoff, pr);
     }
-    __device__ __forceinline__ static void batch(St& st, const Own& o, const Params& p, const Shape& sh,
-                                                 const int (&nbr)[KU], const GeoT& g) {
-        Ck qr[KU], gr[KU];
-        float li[KU], di[KU];
+    __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
+                                                  Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
             const bool pr = nbr[u] >= 0 && g.act;
             const size_t i = (size_t)(nbr[u] < 0 ? 0 : nbr[u]);
-            qr[u].load(p.q, i * sh.rowe + g.eoff, pr);
-            gr[u].load(p.dout, i * sh.rowe + g.eoff, pr);
-            li[u] = pr ? __ldg(p.lse + i * sh.H + g.hd) : 0.f;
-            di[u] = pr ? __ldg(p.delta + i * sh.H + g.hd) : 0.f;
+            src.c[u][0].load_global(p.q, i * sh.rowe + g.eoff, pr);
+            src.c[u][1].load_global(p.dout, i * sh.rowe + g.eoff, pr);
+            src.s[u][0] = pr ? __ldg(p.lse + i * sh.H + g.hd) : 0.f;
+            src.s[u][1] = pr ? __ldg(p.delta + i * sh.H + g.hd) : 0.f;
         }
+    }
+    __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
+                                                   const int (&nbr)[KU], const GeoT& g, const Src& src) {
         float r[2 * KU];
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            float a = 0.f, b = 0.f;
-#pragma unroll
-            for (int c = 0; c < CH; ++c) {
-                a = fmaf(qr[u].get(c), o.k[c], a);
-                b = fmaf(gr[u].get(c), o.v[c], b);
-            }
-            r[2 * u] = a;
-            r[2 * u + 1] = b;
+            const Ck &qc = src.c[u][0], &gc = src.c[u][1];
+            r[2 * u] = dot(qc, o.k);
+            r[2 * u + 1] = dot(gc, o.v);
         }
         head_reduce(r, g.lpl);
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] - li[u] * kLog2e);
-            const float ds = alpha * (r[2 * u + 1] - di[u]);
+            const float li = src.s[u][0], di = src.s[u][1];
+            const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] * p.kscale - li * kLog2e);
+            const float ds = alpha * (r[2 * u + 1] - di);
+            const Ck &qc = src.c[u][0], &gc = src.c[u][1];
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-                st.acc[0][c] = fmaf(ds, qr[u].get(c), st.acc[0][c]);
-                st.acc[1][c] = fmaf(alpha, gr[u].get(c), st.acc[1][c]);
+                st.acc[0][c] = fmaf(ds, qc.get(c), st.acc[0][c]);
+                st.acc[1][c] = fmaf(alpha, gc.get(c), st.acc[1][c]);
             }
         }
     }
