@@ -217,6 +217,22 @@ class OracleArm:
                 f"({self.es} edges: src-side bwd) of the full-size {self.c['name']} graph; per-edge stage times summed")
 
 
+def max_over_ranks(x: float, world: int, device=None) -> float:
+    """MAX of a per-rank scalar over the job (device time of the slowest rank)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_gedges(edges_per_rank: int, steps: int, world: int, total_ms: float) -> float:
+    """Whole-job GEdges/s: every rank processed `edges_per_rank` edges per step (replicas, weak scaling)."""
+    return world * edges_per_rank * steps / (total_ms * 1e-3) * 1e-9
+
+
 def workload_config(c, args):
     return {"workload": c["name"], "layer": c["layer"], "nodes": c["n"], "edges": c["e"], "heads": c["heads"],
             "head_dim": c["head_dim"], "feature_dtype": c["dtype"], "scale": args.scale,
@@ -343,12 +359,8 @@ def run_ours(args, rank, world, local_rank):
     ms_fwd = timed(fwd, args.steps)
     ms_bwd = timed(bwd, args.steps)
     clk = clocks.stop()
-    total_ms = float(sum(ms_steps))
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    value = world * e * args.steps / (total_ms * 1e-3) * 1e-9
+    total_ms = max_over_ranks(float(sum(ms_steps)), world, dev)
+    value = job_gedges(e, args.steps, world, total_ms)
 
     # ---- per-kernel device times (library event profiler), same inputs, right after the timed region
     G.gnn_profile_enable(True)
@@ -374,12 +386,18 @@ def run_ours(args, rank, world, local_rank):
         peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     else:
         peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "r01_dram_traffic.json")
+    if os.path.exists(tpath) and args.scale == 1.0 and not (args.warp_max_deg or args.cta_max_deg or args.split_chunk):
+        traffic = json.load(open(tpath)).get(c["name"], {})
     dom = max((k for k in kern_ms if k in alg), key=lambda k: kern_ms[k])
     achieved = alg[dom] / (kern_ms[dom] * 1e-3) * 1e-9
     step_ms = total_ms / args.steps
     comp_step = comp["fwd"] + comp["bwd"]
     roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom],
+            "traffic": (traffic or {}).get(dom), "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch "
+            "(profiles/r01_dram_traffic.json)" if traffic else None, "kernels_traffic": traffic or None,
+            "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom],
             "kernel_ms": kern_ms[dom], "kernel_share_of_step": kern_ms[dom] / sum(kern_ms.values()),
             "kernels_ms": kern_ms,
             "kernels_algorithmic_gbs": {k: alg[k] / (kern_ms[k] * 1e-3) * 1e-9 for k in kern_ms if k in alg and kern_ms[k] > 0},
@@ -407,12 +425,8 @@ def run_ours(args, rank, world, local_rank):
         e2e_step()
         barrier()
         ms_e2e = timed(e2e_step, args.e2e_steps)
-        t_e2e = float(sum(ms_e2e))
-        if world > 1:
-            t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_e2e = float(t.item())
-        e2e = {"value": world * e * args.e2e_steps / (t_e2e * 1e-3) * 1e-9, "unit": UNIT,
+        t_e2e = max_over_ranks(float(sum(ms_e2e)), world, dev)
+        e2e = {"value": job_gedges(e, args.e2e_steps, world, t_e2e), "unit": UNIT,
                "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes, "steps": args.e2e_steps,
                "ms_per_step": t_e2e / args.e2e_steps}
         del pin_in, pin_out

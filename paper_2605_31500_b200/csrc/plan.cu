@@ -118,7 +118,7 @@ struct Layout {
 };
 
 gnn_plan_opts_t resolve(const gnn_plan_opts_t* o) {
-    gnn_plan_opts_t r = {256, 8192, 4096, 0, 0};
+    gnn_plan_opts_t r = {1024, 8192, 4096, 0, 0};
     if (o) {
         if (o->warp_max_deg > 0) r.warp_max_deg = o->warp_max_deg;
         if (o->cta_max_deg > 0) r.cta_max_deg = o->cta_max_deg;

@@ -1,0 +1,131 @@
+"""Full-size parity (BASELINE.json sizes, default plan = the launch configuration bench.py times):
+sampled outputs against the fp64 oracle evaluated row by row, plus conservation identities that hold at any
+size: sum_j dV_j = sum_i dO_i, sum_i <q_i,dQ_i> = sum_j <k_j,dK_j>,
+sum_j dxr_j - sum_i dxl_i = sum_i dO_i, and the plan metadata bit-exact on the full graph."""
+import numpy as np
+import pytest
+
+import gnn_inputs as GI
+import oracle
+from oracle import plan_ref
+from test_gpu_parity import check, _dev, DEFAULT_OPTS
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+N_DST, N_SRC = 4000, 48   # sampled destination rows / source rows per config
+
+
+def _f32(c, nm):
+    x = c.get(nm + "_f32")
+    return x if x is not None else GI.bf16_bits_to_f32(c[nm + "_st"])
+
+
+def _samples(c, rp_t, rng):
+    """uniform rows + the heaviest rows (hubs / CTA rows) of each side; sources kept light enough that the
+    oracle's forward over all their destinations stays in seconds"""
+    n = c["n"]
+    deg_in = np.diff(c["rowptr"].astype(np.int64))
+    deg_out = np.diff(rp_t.astype(np.int64))
+    rows = np.unique(np.concatenate([rng.choice(n, size=min(n, N_DST), replace=False), np.argsort(-deg_in)[:6]]))
+    srcs = np.unique(np.concatenate([rng.choice(n, size=min(n, N_SRC), replace=False),
+                                     np.argsort(-deg_out)[:2]]))
+    return rows.astype(np.int32), srcs.astype(np.int32), deg_in, deg_out
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_fullsize_sampled_parity(cfg):
+    import torch
+    import paper_2605_31500_b200 as G
+    import paper_2605_31500_b200.binding as B
+    c = GI.make_config(cfg, keep_f32=False)
+    n, H, d, dt, gt = c["n"], c["heads"], c["head_dim"], c["dtype"], c["layer"] == "gt"
+    rp, ci = torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda()
+    plan = G.Plan(rp, ci, transpose=True, **DEFAULT_OPTS)
+    names = ("q", "k", "v", "do") if gt else ("xl", "xr", "do")
+    T = {nm: _dev(c[nm + "_st"], dt) for nm in names}
+    out = torch.empty_like(T[names[0]])
+    lse = torch.empty((n, H), dtype=torch.float32, device="cuda")
+    stat = torch.empty_like(lse)
+    g1, g2 = (torch.empty((n, H, d), dtype=torch.float32, device="cuda") for _ in range(2))
+    if gt:
+        g3 = torch.empty((n, H, d), dtype=torch.float32, device="cuda")
+        G.gnn_gt_attn_fwd(plan, T["q"], T["k"], T["v"], out, lse)
+        G.gnn_gt_attn_bwd(plan, T["q"], T["k"], T["v"], lse, T["do"], stat, g1, g2, g3)
+    else:
+        a = torch.from_numpy(c["a_f32"]).cuda()
+        g3 = torch.empty((H, d), dtype=torch.float32, device="cuda")
+        G.gnn_gatv2_fwd(plan, T["xl"], T["xr"], a, c["slope"], out, lse)
+        G.gnn_gatv2_bwd(plan, T["xl"], T["xr"], a, lse, T["do"], c["slope"], stat, g1, g2, g3)
+    torch.cuda.synchronize()
+
+    # ---- metadata, bit-exact on the full graph
+    rp_t, ci_t = plan_ref.transpose_csr(c["rowptr"], c["colidx"])
+    assert np.array_equal(plan.export(B.GNN_PLAN_ROWPTR_T), rp_t)
+    assert np.array_equal(plan.export(B.GNN_PLAN_COLIDX_T), ci_t)
+    cnt = plan.counts()
+    ref = plan_ref.build_bins(c["rowptr"], *_resolved_opts())
+    assert np.array_equal(plan.export(B.GNN_PLAN_PERM), ref["perm"])
+    assert np.array_equal(plan.export(B.GNN_PLAN_CHUNKS).reshape(-1, 4), ref["chunks"])
+    ref_t = plan_ref.build_bins(rp_t, *_resolved_opts())
+    assert np.array_equal(plan.export(B.GNN_PLAN_PERM_T), ref_t["perm"])
+    assert np.array_equal(plan.export(B.GNN_PLAN_CHUNKS_T).reshape(-1, 4), ref_t["chunks"])
+    assert cnt["n_chunks"] == ref["chunks"].shape[0] and cnt["n_chunks_t"] == ref_t["chunks"].shape[0]
+
+    # ---- conservation identities on the full outputs (fp64 sums on the device)
+    do64 = T["do"].double()
+    sum_do = do64.sum(0)
+    if gt:
+        dq, dk, dv = g1.double(), g2.double(), g3.double()
+        scale = float(do64.abs().sum(0).max())
+        assert float((dv.sum(0) - sum_do).abs().max()) <= 1e-5 * scale + 1e-3
+        lhs = float((T["q"].double() * dq).sum())
+        rhs = float((T["k"].double() * dk).sum())
+        den = float((T["q"].double() * dq).abs().sum())
+        assert abs(lhs - rhs) <= 1e-5 * den
+    else:
+        dxl, dxr = g1.double(), g2.double()
+        scale = float(do64.abs().sum(0).max())
+        assert float((dxr.sum(0) - dxl.sum(0) - sum_do).abs().max()) <= 1e-5 * scale + 1e-3
+
+    # ---- sampled rows against the oracle
+    rng = np.random.default_rng(99 + cfg)
+    rows, srcs, deg_in, deg_out = _samples(c, rp_t, rng)
+    f = {nm: _f32(c, nm) for nm in names}
+    rows_t, srcs_t = torch.from_numpy(rows.astype(np.int64)).cuda(), torch.from_numpy(srcs.astype(np.int64)).cuda()
+    host = lambda t, idx: t[idx].float().cpu().numpy().astype(np.float64)
+    # destinations whose L / Delta the sampled sources need
+    need = np.unique(np.concatenate([ci_t[rp_t[j]:rp_t[j + 1]] for j in srcs] + [rows])).astype(np.int32)
+    if gt:
+        O, L = oracle.gt_forward(c["rowptr"], c["colidx"], f["q"], f["k"], f["v"], rows=need)
+        Dl = oracle.rowdot(O, f["do"], rows=need)
+        Lf, Df = np.zeros((n, H)), np.zeros((n, H))
+        Lf[need], Df[need] = L, Dl
+        pos = np.searchsorted(need, rows)
+        check(f"cfg{cfg}:O", host(out, rows_t), O[pos], dt)
+        check(f"cfg{cfg}:L", host(lse, rows_t), L[pos], dt)
+        check(f"cfg{cfg}:Delta", host(stat, rows_t), Dl[pos], dt)
+        dQ = oracle.gt_backward_dst(c["rowptr"], c["colidx"], f["q"], f["k"], f["v"], f["do"], Lf, Df, rows=rows)
+        check(f"cfg{cfg}:dQ", host(g1, rows_t), dQ, dt)
+        dK, dV = oracle.gt_backward_src(rp_t, ci_t, f["q"], f["k"], f["v"], f["do"], Lf, Df, srcs=srcs)
+        check(f"cfg{cfg}:dK", host(g2, srcs_t), dK, dt)
+        check(f"cfg{cfg}:dV", host(g3, srcs_t), dV, dt)
+    else:
+        af, sl = c["a_f32"], c["slope"]
+        O, L = oracle.gatv2_forward(c["rowptr"], c["colidx"], f["xl"], f["xr"], af, sl, rows=need)
+        Gv = oracle.rowdot(O, f["do"], rows=need)
+        Lf, Gf = np.zeros((n, H)), np.zeros((n, H))
+        Lf[need], Gf[need] = L, Gv
+        pos = np.searchsorted(need, rows)
+        check(f"cfg{cfg}:O", host(out, rows_t), O[pos], dt)
+        check(f"cfg{cfg}:L", host(lse, rows_t), L[pos], dt)
+        check(f"cfg{cfg}:G", host(stat, rows_t), Gv[pos], dt)
+        dxl, _ = oracle.gatv2_backward_dst(c["rowptr"], c["colidx"], f["xl"], f["xr"], af, sl, f["do"], Lf, Gf, rows=rows)
+        check(f"cfg{cfg}:dxl", host(g1, rows_t), dxl, dt)
+        dxr = oracle.gatv2_backward_src(rp_t, ci_t, f["xl"], f["xr"], af, sl, f["do"], Lf, Gf, srcs=srcs)
+        check(f"cfg{cfg}:dxr", host(g2, srcs_t), dxr, dt)
+        assert np.all(np.isfinite(g3.cpu().numpy()))   # da: full-size value needs the whole oracle; checked at scale in test_gpu_parity
+
+
+def _resolved_opts():
+    """the library's default thresholds (include/gnn_attn.h)"""
+    return 1024, 8192, 4096
