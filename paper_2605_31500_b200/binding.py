@@ -172,13 +172,14 @@ def gnn_workspace_bytes(handle, op: int, heads: int, head_dim: int, dtype_code: 
 class Plan:
     """Owns the torch allocations behind a gnn_plan_t (plan storage, workspace) for one CSR graph."""
 
-    def __init__(self, rowptr, colidx, warp_max_deg=0, cta_max_deg=0, split_chunk=0, transpose=True, stream=None):
+    def __init__(self, rowptr, colidx, warp_max_deg=0, cta_max_deg=0, split_chunk=0, transpose=True, blocks=False,
+                 stream=None):
         torch = _require_cuda()
         if rowptr.dtype != torch.int32 or colidx.dtype != torch.int32:
             raise GnnError("rowptr / colidx must be int32")
         self.rowptr, self.colidx = rowptr.contiguous(), colidx.contiguous()
         self.n, self.nnz = int(rowptr.numel()) - 1, int(colidx.numel())
-        self.opts = PlanOpts(warp_max_deg, cta_max_deg, split_chunk, 1 if transpose else 0, 0)
+        self.opts = PlanOpts(warp_max_deg, cta_max_deg, split_chunk, 1 if transpose else 0, 1 if blocks else 0)
         dev_bytes, scratch_bytes = gnn_plan_bytes(self.n, self.nnz, self.opts)
         self.dev_mem = torch.empty(dev_bytes, dtype=torch.uint8, device=rowptr.device)
         scratch = torch.empty(scratch_bytes, dtype=torch.uint8, device=rowptr.device)

@@ -5,6 +5,7 @@
 // bit for bit.  Sorting / scanning uses CUB's stable LSD radix sort (a library primitive, one-time
 // preprocessing outside the timed layer, like the paper's format construction).
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
 
 #include <new>
 
@@ -108,9 +109,37 @@ __global__ void rowptr_t_kernel(const uint32_t* __restrict__ src_sorted, long lo
     rowptr_t[j] = (int32_t)lo;
 }
 
+// a11 - 16-row block layout (own layout; the paper's WSB, is prior art): window w = rows
+// [16w, 16w+16); bit c of bitmap[row] is set iff the FIRST entry (row <- 16w + c) exists; every other entry
+// (sources outside the window, duplicate in-window entries) goes to the remainder CSR in original order.
+// One thread per row (rows of the locally dense graphs are short); pass 0 counts, pass 1 writes.
+__global__ void block_layout_kernel(const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx, int n,
+                                    int pass, uint16_t* __restrict__ bitmap, int32_t* __restrict__ rem_cnt,
+                                    const int32_t* __restrict__ rem_rowptr, int32_t* __restrict__ rem_colidx) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int w0 = (i >> 4) << 4;
+    uint32_t seen = 0;
+    int cnt = 0;
+    int32_t* out = pass ? rem_colidx + rem_rowptr[i] : nullptr;
+    for (int e = rowptr[i]; e < rowptr[i + 1]; ++e) {
+        const int j = colidx[e];
+        const unsigned c = (unsigned)(j - w0);
+        if (c < 16u && !((seen >> c) & 1u)) { seen |= 1u << c; continue; }
+        if (pass) out[cnt] = j;
+        ++cnt;
+    }
+    if (!pass) { bitmap[i] = (uint16_t)seen; rem_cnt[i] = cnt; }
+}
+__global__ void pad_bitmap_kernel(uint16_t* bitmap, int n, int n_pad) {
+    const int i = n + blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_pad) bitmap[i] = 0;
+}
+
 struct Layout {
     // persistent
     size_t perm, chunks, chunk_ptr, counts, rowptr_t, colidx_t, perm_t, chunks_t, chunk_ptr_t, dev_total;
+    size_t blk_bitmap, blk_rem_rowptr, blk_rem_colidx, blk_cnt;
     // scratch
     size_t key, key_sorted, rowid, ekey_sorted, erow, cub, scratch_total;
     size_t cub_bytes;
@@ -153,8 +182,14 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
         L.chunks_t = take(sizeof(int32_t) * 4 * (size_t)L.max_chunks);
         L.chunk_ptr_t = take(sizeof(int32_t) * (size_t)(L.max_hub + 1));
     }
+    L.blk_bitmap = L.blk_rem_rowptr = L.blk_rem_colidx = 0;
+    if (o.build_blocks) {
+        L.blk_bitmap = take(sizeof(uint16_t) * (((size_t)n + 15) / 16 * 16));
+        L.blk_rem_rowptr = take(sizeof(int32_t) * ((size_t)n + 1));
+        L.blk_rem_colidx = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
+    }
     L.dev_total = off;
-    size_t t1 = 0, t2 = 0;
+    size_t t1 = 0, t2 = 0, t3 = 0;
     cudaError_t e = cub::DeviceRadixSort::SortPairs(nullptr, t1, (const uint32_t*)nullptr, (uint32_t*)nullptr,
                                                     (const int32_t*)nullptr, (int32_t*)nullptr, (long long)n, 0, 7);
     if (e != cudaSuccess) return e;
@@ -163,7 +198,12 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
                                             (const int32_t*)nullptr, (int32_t*)nullptr, (long long)nnz, 0, n_bits(n));
         if (e != cudaSuccess) return e;
     }
+    if (o.build_blocks) {
+        e = cub::DeviceScan::InclusiveSum(nullptr, t3, (const int32_t*)nullptr, (int32_t*)nullptr, n);
+        if (e != cudaSuccess) return e;
+    }
     L.cub_bytes = t1 > t2 ? t1 : t2;
+    if (t3 > L.cub_bytes) L.cub_bytes = t3;
     off = 0;
     L.key = take(sizeof(uint32_t) * (size_t)n);
     L.key_sorted = take(sizeof(uint32_t) * (size_t)n);
@@ -173,6 +213,7 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
         L.ekey_sorted = take(sizeof(uint32_t) * (size_t)(nnz > 0 ? nnz : 1));
         L.erow = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
     }
+    L.blk_cnt = o.build_blocks ? take(sizeof(int32_t) * (size_t)n) : 0;
     L.cub = take(L.cub_bytes + 16);
     L.scratch_total = off;
     return cudaSuccess;
@@ -239,10 +280,6 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
         return GNN_EINVAL;
     }
     const gnn_plan_opts_t o = resolve(opts);
-    if (o.build_blocks) {
-        set_error("gnn_plan_build: build_blocks is not available in this build");
-        return GNN_EUNSUPPORTED;
-    }
     Layout L;
     cudaError_t e = make_layout(n, nnz, o, L);
     if (e != cudaSuccess) {
@@ -286,7 +323,27 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
                            (int32_t*)(dm + L.chunk_ptr_t), counts_dev + 4, hc + 4, st);
         }
     }
+    int32_t rem_nnz = 0;
+    if (e == cudaSuccess && o.build_blocks) {
+        P->n_windows = (n + 15) / 16;
+        P->blk_bitmap = (uint16_t*)(dm + L.blk_bitmap);
+        P->blk_rem_rowptr = (int32_t*)(dm + L.blk_rem_rowptr);
+        P->blk_rem_colidx = (int32_t*)(dm + L.blk_rem_colidx);
+        int32_t* cnt = (int32_t*)(sc + L.blk_cnt);
+        const int tb = 128, gb = (n + tb - 1) / tb;
+        block_layout_kernel<<<gb, tb, 0, st>>>(rowptr, colidx, n, 0, P->blk_bitmap, cnt, nullptr, nullptr);
+        if (P->n_windows * 16 > n) pad_bitmap_kernel<<<1, 32, 0, st>>>(P->blk_bitmap, n, P->n_windows * 16);
+        e = cudaMemsetAsync(P->blk_rem_rowptr, 0, sizeof(int32_t), st);
+        size_t cb = L.cub_bytes;
+        if (e == cudaSuccess) e = cub::DeviceScan::InclusiveSum(sc + L.cub, cb, (const int32_t*)cnt, P->blk_rem_rowptr + 1, n, st);
+        if (e == cudaSuccess) {
+            block_layout_kernel<<<gb, tb, 0, st>>>(rowptr, colidx, n, 1, nullptr, nullptr, P->blk_rem_rowptr, P->blk_rem_colidx);
+            g_launches += 3;
+            e = cudaMemcpyAsync(&rem_nnz, P->blk_rem_rowptr + n, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        }
+    }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    P->rem_nnz = rem_nnz;
     if (e != cudaSuccess) {
         set_error("gnn_plan_build: CUDA error: %s", cudaGetErrorString(e));
         delete P;
@@ -321,8 +378,12 @@ extern "C" gnn_status_t gnn_plan_export(const gnn_plan_t* P, int what, void* hos
         case GNN_PLAN_PERM_T: if (T) { src = P->tr.perm; need = 4 * (size_t)P->n; } break;
         case GNN_PLAN_CHUNKS_T: if (T) { src = P->tr.chunks; need = 16 * (size_t)P->tr.n_chunks; } break;
         case GNN_PLAN_CHUNK_PTR_T: if (T) { src = P->tr.chunk_ptr; need = 4 * ((size_t)P->tr.n_hub + 1); } break;
+        case GNN_PLAN_BLOCK_BITMAP: if (P->blk_bitmap) { src = P->blk_bitmap; need = 2 * 16 * (size_t)P->n_windows; } break;
+        case GNN_PLAN_BLOCK_REM_ROWPTR: if (P->blk_bitmap) { src = P->blk_rem_rowptr; need = 4 * ((size_t)P->n + 1); } break;
+        case GNN_PLAN_BLOCK_REM_COLIDX: if (P->blk_bitmap) { src = P->blk_rem_colidx; need = 4 * (size_t)P->rem_nnz; } break;
         default: break;
     }
+    if (what == GNN_PLAN_BLOCK_REM_COLIDX && P->blk_bitmap && P->rem_nnz == 0) { *bytes = 0; return GNN_OK; }
     if (what != GNN_PLAN_COUNTS && !src) {
         set_error("gnn_plan_export: item %d is not part of this plan", what);
         return GNN_EINVAL;

@@ -235,3 +235,25 @@ def test_errors_are_reported():
     q3 = torch.zeros((c["n"], 4, 12), device="cuda")
     with pytest.raises(G.GnnError, match="unsupported shape"):
         G.gnn_gt_attn_fwd(plan, q3, q3, q3, q3, lse)
+
+
+def test_block_layout_bit_exact():
+    """Row a11: per-window 16x16 bitmaps + remainder CSR, bit-exact vs oracle/plan_ref.py, on the locally dense
+    config (scaled) and on a multigraph whose size is not a multiple of 16 (duplicates go to the remainder)."""
+    import paper_2605_31500_b200 as G
+    import paper_2605_31500_b200.binding as B
+    torch = _torch()
+    rng = np.random.default_rng(3)
+    n = 1003
+    dst = rng.integers(0, n, size=20000)
+    src = np.where(rng.random(20000) < 0.7, (dst // 16) * 16 + rng.integers(0, 16, size=20000), rng.integers(0, n, size=20000))
+    src = np.minimum(src, n - 1)
+    rp_m, ci_m = GI.csr_from_pairs(n, dst, src, self_loops=False, dedupe=False)
+    c4 = GI.make_config(4, scale=0.004)
+    for rowptr, colidx in ((c4["rowptr"], c4["colidx"]), (rp_m, ci_m)):
+        plan = G.Plan(torch.from_numpy(rowptr).cuda(), torch.from_numpy(colidx).cuda(), transpose=False, blocks=True)
+        ref = plan_ref.build_blocks(rowptr, colidx)
+        assert np.array_equal(plan.export(B.GNN_PLAN_BLOCK_BITMAP, np.uint16).reshape(-1, 16), ref["bitmap"])
+        assert np.array_equal(plan.export(B.GNN_PLAN_BLOCK_REM_ROWPTR), ref["rem_rowptr"])
+        assert np.array_equal(plan.export(B.GNN_PLAN_BLOCK_REM_COLIDX), ref["rem_colidx"])
+        assert int(ref["rem_rowptr"][-1]) + int(np.unpackbits(ref["bitmap"].view(np.uint8)).sum()) == colidx.size
