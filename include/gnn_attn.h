@@ -165,6 +165,17 @@ gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* plan, const int32_t* rowptr, const 
                            int32_t heads, int32_t head_dim, gnn_dtype_t dtype, float slope, float* g, float* dxl,
                            float* dxr, float* da, void* ws, size_t ws_bytes, gnn_stream_t stream);
 
+/* Graph Transformer attention forward, block-sparse tensor-core variant for locally dense graphs (the paper's
+ * WSB / Tensor-Core forward, re-designed for tcgen05 + TMEM): tiles of 128 destination rows
+ * (8 windows of 16) compute S = Q_tile K_tile^T and O = P V_tile with tcgen05.mma, masked by the plan's per-row
+ * 16-bit bitmaps of in-window edges; every other edge (the remainder CSR of the plan) is gathered as in
+ * gnn_gt_attn_fwd and merged into the same online softmax.  Same result as gnn_gt_attn_fwd up to rounding
+ * (P is rounded to bf16 for the second product).  The plan must have been built with build_blocks;
+ * bf16 features, head_dim == 64 only (GNN_EUNSUPPORTED otherwise); feature pointers 16-byte aligned; no workspace. */
+gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                   const void* q, const void* k, const void* v, int32_t heads, int32_t head_dim,
+                                   gnn_dtype_t dtype, void* out, float* lse, gnn_stream_t stream);
+
 /* Thread-local message describing the last error returned on this thread ("" if none).           */
 const char* gnn_last_error(void);
 /* Library version string, e.g. "gnn_attn 0.1 sm_100a".                                            */

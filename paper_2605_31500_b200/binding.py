@@ -20,7 +20,7 @@ GNN_OP_GT_FWD, GNN_OP_GT_BWD, GNN_OP_GATV2_FWD, GNN_OP_GATV2_BWD = 0, 1, 2, 3
 EXPORTED_SYMBOLS = [
     "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
     "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
-    "gnn_gatv2_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
+    "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
     "gnn_profile_collect",
 ]
 
@@ -62,6 +62,7 @@ def lib() -> C.CDLL:
         L.gnn_gatv2_fwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _f, _vp, _vp, _vp, _sz, _vp]
         L.gnn_gatv2_bwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _vp, _vp, _i32, _i32, C.c_int, _f,
                                     _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+        L.gnn_gt_attn_fwd_block.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _vp, _vp, _vp]
         L.gnn_last_error.restype = C.c_char_p
         L.gnn_version.restype = C.c_char_p
         L.gnn_launch_count.restype = _i64
@@ -216,6 +217,12 @@ def gnn_gt_attn_fwd(plan: Plan, q, k, v, out, lse, stream=None):
     ws = plan.workspace(GNN_OP_GT_FWD, H, d, _dtype_code(q))
     _check(lib().gnn_gt_attn_fwd(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v), H, d,
                                  _dtype_code(q), _ptr(out), _ptr(lse), _ptr(ws), ws.numel(), _stream(stream)))
+
+
+def gnn_gt_attn_fwd_block(plan: Plan, q, k, v, out, lse, stream=None):
+    n, H, d = q.shape
+    _check(lib().gnn_gt_attn_fwd_block(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v), H, d,
+                                       _dtype_code(q), _ptr(out), _ptr(lse), _stream(stream)))
 
 
 def gnn_gt_attn_bwd(plan: Plan, q, k, v, lse, dout, delta, dq, dk, dv, stream=None):

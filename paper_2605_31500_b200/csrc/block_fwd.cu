@@ -1,0 +1,299 @@
+// block_fwd.cu - row a12: block-sparse Graph Transformer forward on the 5th-generation tensor cores
+// (tcgen05.mma, accumulators in TMEM) for locally dense graphs, merged with the CSR remainder.
+//
+// Paper's version: per 16-row window and head, WMMA 16x16x16 on A100: S = Q_win K_blk^T,
+// bitmap mask, FlashAttention-style online softmax, acc += P V_blk.  tcgen05.mma has M in {64, 128}, so here one
+// CTA owns a tile of 128 destination rows = 8 windows and, per head, issues ONE 128x128xd product
+// S = Q_tile K_tile^T (bf16 in, fp32 in TMEM); thread t owns row t (TMEM lane t), reads back only the 16 columns
+// of its own window's diagonal block, masks them with the plan's 16-bit row bitmap (row a11), forms
+// p = 2^(s - m) in registers, writes P (bf16, zero off the diagonal blocks) to shared memory and a second
+// product O = P V_tile (128x128 by 128xd) accumulates the block part in TMEM.  The off-diagonal blocks are wasted
+// tensor work (8x) - far below the HBM time of the tile.  The remainder edges (sources
+// outside the window: the long-range in-edges) are then gathered per row exactly as in the CSR path and merged
+// into the same online-softmax state, so the result equals the plain CSR forward.
+//
+// Operand staging: Q, K (K-major) and V^T (K-major over the source index) are written by the CTA's threads into
+// the canonical no-swizzle core-matrix layout (8 rows x 16 bytes per core matrix; LBO = 128 B between the two
+// K core matrices of one MMA, SBO = bytes per 8-row group), described to the tensor core by 64-bit shared-memory
+// matrix descriptors; completion is signalled with tcgen05.commit on an mbarrier.
+#include <cuda_bf16.h>
+
+#include "internal.h"
+#include "kernels.cuh"
+
+namespace gnn {
+namespace {
+
+constexpr int kTile = 128;  // destination rows per CTA = MMA M = TMEM lanes
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// 64-bit shared-memory matrix descriptor, SWIZZLE_NONE, version 1 (sm_100)
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    return (uint64_t)((saddr >> 4) & 0x3fff) | ((uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16) |
+           ((uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32) | (1ull << 46);
+}
+// instruction descriptor: kind::f16, A = B = bf16 (K-major), D = fp32, M x N
+__host__ __device__ constexpr uint32_t make_idesc(int M, int N) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void umma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n"
+                 " tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
+                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                 ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile("{\n .reg .pred p;\n W_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                 " @p bra D_%=;\n bra W_%=;\n D_%=:\n}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
+    uint32_t r[32];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                 "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+                 "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+                   "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+                   "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+                 : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+// byte offset of element (r, k) in the canonical no-swizzle K-major layout (core matrix = 8 rows x 16 bytes)
+__device__ __forceinline__ uint32_t canon(int r, int k, int sbo) {
+    return (uint32_t)((r & 7) * 16 + (r >> 3) * sbo + (k & 7) * 2 + (k >> 3) * 128);
+}
+
+template <int D>
+__global__ void __launch_bounds__(kTile, 2)
+gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ k,
+                    const __nv_bfloat16* __restrict__ v, __nv_bfloat16* __restrict__ out, float* __restrict__ lse,
+                    const uint16_t* __restrict__ bitmap, const int32_t* __restrict__ rem_rowptr,
+                    const int32_t* __restrict__ rem_colidx, int n, int H, float sscale) {
+    constexpr int SBO_QK = (D / 8) * 128, SBO_PV = (kTile / 8) * 128;
+    constexpr int kBytesQK = kTile * D * 2, kBytesP = kTile * kTile * 2;
+    constexpr int CPR = D / 8;  // 16-byte chunks per row slice
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* sQ = smem;
+    uint8_t* sK = sQ + kBytesQK;
+    uint8_t* sVt = sK + kBytesQK;
+    uint8_t* sP = sVt + kBytesQK;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(sP + kBytesP);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bar + 1);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int row0 = blockIdx.x * kTile, row = row0 + tid;
+    const bool rvalid = row < n;
+    const size_t rowe = (size_t)H * D;
+
+    // ---- one-time setup: zero P (off-diagonal blocks stay zero), barrier, TMEM (256 columns: S 128 + O D)
+    for (int i = tid; i < kBytesP / 16; i += kTile) reinterpret_cast<uint4*>(sP)[i] = make_uint4(0, 0, 0, 0);
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = *tmem_slot;
+    const uint32_t t_lane = tmem + ((uint32_t)(warp * 32) << 16);
+    uint32_t phase = 0;
+
+    const uint32_t bits = rvalid ? (uint32_t)__ldg(bitmap + row) : 0u;
+    const int rb = rvalid ? __ldg(rem_rowptr + row) : 0, re = rvalid ? __ldg(rem_rowptr + row + 1) : 0;
+    const int wl = tid >> 4;  // window of this row inside the tile
+    constexpr uint32_t kIdescS = make_idesc(kTile, kTile), kIdescO = make_idesc(kTile, D);
+
+    for (int h = 0; h < H; ++h) {
+        // ---- stage Q, K (K-major) and V^T for this head
+        for (int idx = tid; idx < kTile * CPR; idx += kTile) {
+            const int r = idx / CPR, kc = idx % CPR;
+            uint4 a = make_uint4(0, 0, 0, 0), b = a, c = a;
+            if (row0 + r < n) {
+                const size_t off = (size_t)(row0 + r) * rowe + (size_t)h * D + kc * 8;
+                a = __ldg(reinterpret_cast<const uint4*>(q + off));
+                b = __ldg(reinterpret_cast<const uint4*>(k + off));
+                c = __ldg(reinterpret_cast<const uint4*>(v + off));
+            }
+            *reinterpret_cast<uint4*>(sQ + canon(r, kc * 8, SBO_QK)) = a;
+            *reinterpret_cast<uint4*>(sK + canon(r, kc * 8, SBO_QK)) = b;
+            const uint16_t* cv = reinterpret_cast<const uint16_t*>(&c);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) *reinterpret_cast<uint16_t*>(sVt + canon(kc * 8 + i, r, SBO_PV)) = cv[i];
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        // ---- S = Q K^T on the tensor cores (one elected thread issues)
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int s = 0; s < D / 16; ++s)
+                umma(tmem, make_desc(smem_u32(sQ) + s * 256, 128, SBO_QK), make_desc(smem_u32(sK) + s * 256, 128, SBO_QK),
+                     kIdescS, s > 0);
+            umma_commit(bar);
+        }
+        mbar_wait(bar, phase);
+        phase ^= 1;
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        // ---- this row's 16 scores of its own window's diagonal block; mask; block-local softmax
+        float m = -INFINITY, l = 0.f;
+        {
+            float sv[32];
+            tmem_ld32(t_lane + warp * 32, sv);
+            float s16[16];
+#pragma unroll
+            for (int c = 0; c < 16; ++c) {
+                const float x = (lane >= 16) ? sv[16 + c] : sv[c];
+                s16[c] = ((bits >> c) & 1u) ? x * sscale : -INFINITY;
+                m = fmaxf(m, s16[c]);
+            }
+            const float ms = (m == -INFINITY) ? 0.f : m;
+            uint32_t pk[8];
+#pragma unroll
+            for (int c = 0; c < 16; c += 2) {
+                const __nv_bfloat162 pb = __floats2bfloat162_rn(ex2(s16[c] - ms), ex2(s16[c + 1] - ms));
+                l += __low2float(pb) + __high2float(pb);   // normalise with the rounded weights the MMA will use
+                pk[c >> 1] = *reinterpret_cast<const uint32_t*>(&pb);
+            }
+            uint8_t* prow = sP + canon(tid, 16 * wl, SBO_PV);
+            *reinterpret_cast<uint4*>(prow) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+            *reinterpret_cast<uint4*>(prow + 128) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        // ---- O_block = P V on the tensor cores
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int s = 0; s < kTile / 16; ++s)
+                umma(tmem + 128, make_desc(smem_u32(sP) + s * 256, 128, SBO_PV), make_desc(smem_u32(sVt) + s * 256, 128, SBO_PV),
+                     kIdescO, s > 0);
+            umma_commit(bar);
+        }
+        mbar_wait(bar, phase);
+        phase ^= 1;
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        float acc[D];
+#pragma unroll
+        for (int c0 = 0; c0 < D; c0 += 32) {
+            float t32[32];
+            tmem_ld32(t_lane + 128 + c0, t32);
+#pragma unroll
+            for (int i = 0; i < 32; ++i) acc[c0 + i] = t32[i];
+        }
+        // ---- remainder edges of this row (sources outside the window): CSR gather, same online softmax
+        if (re > rb) {
+            uint32_t qw[D / 2];
+            const uint4* qp = reinterpret_cast<const uint4*>(q + (size_t)row * rowe + (size_t)h * D);
+#pragma unroll
+            for (int i = 0; i < CPR; ++i) {
+                const uint4 t = __ldg(qp + i);
+                qw[4 * i] = t.x; qw[4 * i + 1] = t.y; qw[4 * i + 2] = t.z; qw[4 * i + 3] = t.w;
+            }
+            for (int e = rb; e < re; ++e) {
+                const size_t off = (size_t)__ldg(rem_colidx + e) * rowe + (size_t)h * D;
+                const uint4* kp = reinterpret_cast<const uint4*>(k + off);
+                const uint4* vp = reinterpret_cast<const uint4*>(v + off);
+                float s0 = 0.f, s1 = 0.f;
+                uint4 vv[CPR];
+#pragma unroll
+                for (int i = 0; i < CPR; ++i) {
+                    const uint4 t = __ldg(kp + i);
+                    vv[i] = __ldg(vp + i);
+                    fma_bf16x2(qw[4 * i], t.x, s0, s1);
+                    fma_bf16x2(qw[4 * i + 1], t.y, s0, s1);
+                    fma_bf16x2(qw[4 * i + 2], t.z, s0, s1);
+                    fma_bf16x2(qw[4 * i + 3], t.w, s0, s1);
+                }
+                const float s = (s0 + s1) * sscale;
+                const float mx = fmaxf(m, s);
+                const float corr = ex2(m - mx), p = ex2(s - mx);
+                l = l * corr + p;
+                m = mx;
+#pragma unroll
+                for (int i = 0; i < CPR; ++i) {
+                    const uint32_t w[4] = {vv[i].x, vv[i].y, vv[i].z, vv[i].w};
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        acc[8 * i + 2 * j] = fmaf(p, __uint_as_float(w[j] << 16), acc[8 * i + 2 * j] * corr);
+                        acc[8 * i + 2 * j + 1] = fmaf(p, __uint_as_float(w[j] & 0xffff0000u), acc[8 * i + 2 * j + 1] * corr);
+                    }
+                }
+            }
+        }
+        // ---- normalise and store
+        if (rvalid) {
+            const float inv = l > 0.f ? 1.f / l : 0.f;
+            uint4* op = reinterpret_cast<uint4*>(out + (size_t)row * rowe + (size_t)h * D);
+#pragma unroll
+            for (int i = 0; i < CPR; ++i) {
+                uint32_t w[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const __nv_bfloat162 b2 = __floats2bfloat162_rn(acc[8 * i + 2 * j] * inv, acc[8 * i + 2 * j + 1] * inv);
+                    w[j] = *reinterpret_cast<const uint32_t*>(&b2);
+                }
+                op[i] = make_uint4(w[0], w[1], w[2], w[3]);
+            }
+            lse[(size_t)row * H + h] = l > 0.f ? (m + lg2(l)) * kLn2 : -INFINITY;
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();   // smem operands and TMEM are reused by the next head
+    }
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(tmem) : "memory");
+}
+
+}  // namespace
+}  // namespace gnn
+
+using namespace gnn;
+
+extern "C" gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* P, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                              const void* q, const void* k, const void* v, int32_t heads, int32_t head_dim,
+                                              gnn_dtype_t dtype, void* out, float* lse, gnn_stream_t stream) {
+    const char* who = "gnn_gt_attn_fwd_block";
+    if (!P || rowptr != P->rowptr || colidx != P->colidx || n != P->n) {
+        set_error("%s: NULL plan, or rowptr/colidx/n differ from the arrays the plan was built from", who);
+        return GNN_EINVAL;
+    }
+    if (!P->blk_bitmap) { set_error("%s: plan was built without build_blocks", who); return GNN_EINVAL; }
+    if (!q || !k || !v || !out || !lse) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
+    if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) != 0) {
+        set_error("%s: feature pointers must be 16-byte aligned", who);
+        return GNN_EINVAL;
+    }
+    if (dtype != GNN_BF16 || head_dim != 64 || heads < 1) {
+        set_error("%s: unsupported shape heads=%d head_dim=%d dtype=%d (bf16, head_dim 64 only)", who, heads, head_dim, dtype);
+        return GNN_EUNSUPPORTED;
+    }
+    constexpr int D = 64;
+    const size_t smem = 3 * (size_t)kTile * D * 2 + (size_t)kTile * kTile * 2 + 64;
+    cudaError_t e = cudaFuncSetAttribute(gt_fwd_block_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) {
+        const int grid = (n + kTile - 1) / kTile;
+        prof_begin("gt_fwd_block", "tile", (cudaStream_t)stream);
+        gt_fwd_block_kernel<D><<<grid, kTile, smem, (cudaStream_t)stream>>>(
+            (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, (__nv_bfloat16*)out, lse, P->blk_bitmap,
+            P->blk_rem_rowptr, P->blk_rem_colidx, n, heads, kLog2e / sqrtf((float)D));
+        prof_end((cudaStream_t)stream);
+        ++g_launches;
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) { set_error("%s: CUDA error: %s", who, cudaGetErrorString(e)); return GNN_ECUDA; }
+    return GNN_OK;
+}

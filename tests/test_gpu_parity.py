@@ -257,3 +257,36 @@ def test_block_layout_bit_exact():
         assert np.array_equal(plan.export(B.GNN_PLAN_BLOCK_REM_ROWPTR), ref["rem_rowptr"])
         assert np.array_equal(plan.export(B.GNN_PLAN_BLOCK_REM_COLIDX), ref["rem_colidx"])
         assert int(ref["rem_rowptr"][-1]) + int(np.unpackbits(ref["bitmap"].view(np.uint8)).sum()) == colidx.size
+
+
+@pytest.mark.parametrize("heads", [1, 8])
+def test_block_tensor_core_forward(heads):
+    """Row a12: the tcgen05/TMEM block-sparse forward (+ CSR remainder merge) against the oracle, on the locally
+    dense config scaled down (ragged last tile: n is not a multiple of 128) and on a graph with empty rows,
+    rows without in-window edges and duplicate entries."""
+    import paper_2605_31500_b200 as G
+    torch = _torch()
+    c4 = GI.make_config(4, scale=0.0041)
+    rng = np.random.default_rng(5)
+    n = 1000
+    dst = rng.integers(0, n, size=9000)
+    src = np.where(rng.random(9000) < 0.6, (dst // 16) * 16 + rng.integers(0, 16, size=9000), rng.integers(0, n, size=9000))
+    src = np.minimum(src, n - 1)
+    keep = (dst % 7 != 0)                                   # rows with no entries at all
+    rp_m, ci_m = GI.csr_from_pairs(n, dst[keep], src[keep], self_loops=False, dedupe=False)
+    cm = _custom("gt", n, rp_m, ci_m, heads, 64, "bf16", seed=11)
+    c4h = _custom("gt", c4["n"], c4["rowptr"], c4["colidx"], heads, 64, "bf16", seed=12)
+    for c in (c4h, cm):
+        nn, H, d = c["n"], c["heads"], c["head_dim"]
+        plan = G.Plan(torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda(), transpose=False, blocks=True)
+        q, k, v = (_dev(c[x + "_st"], "bf16") for x in "qkv")
+        out = torch.full_like(q, float("nan"))
+        lse = torch.full((nn, H), float("nan"), dtype=torch.float32, device="cuda")
+        G.gnn_gt_attn_fwd_block(plan, q, k, v, out, lse)
+        torch.cuda.synchronize()
+        O, L = oracle.gt_forward(c["rowptr"], c["colidx"], c["q_f32"], c["k_f32"], c["v_f32"])
+        check(f"{c['name']}:block:O", _host(out), O, "bf16")
+        check(f"{c['name']}:block:L", _host(lse), L, "bf16")
+    q3 = torch.zeros((nn, 2, 32), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(G.GnnError, match="unsupported shape"):
+        G.gnn_gt_attn_fwd_block(plan, q3, q3, q3, q3, lse)
