@@ -33,9 +33,10 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes
     return (uint64_t)((saddr >> 4) & 0x3fff) | ((uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16) |
            ((uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32) | (1ull << 46);
 }
-// instruction descriptor: kind::f16, A = B = bf16 (K-major), D = fp32, M x N
-__host__ __device__ constexpr uint32_t make_idesc(int M, int N) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+// instruction descriptor: kind::f16, A = bf16 K-major, B = bf16 K-major or MN-major, D = fp32, M x N
+__host__ __device__ constexpr uint32_t make_idesc(int M, int N, bool b_mn_major) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(N >> 3) << 17) |
+           ((uint32_t)(M >> 4) << 24);
 }
 __device__ __forceinline__ void umma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
     asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n"
@@ -74,20 +75,23 @@ __device__ __forceinline__ uint32_t canon(int r, int k, int sbo) {
 }
 
 template <int D>
-__global__ void __launch_bounds__(kTile, 2)
+__global__ void __launch_bounds__(kTile, 3)
 gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ k,
                     const __nv_bfloat16* __restrict__ v, __nv_bfloat16* __restrict__ out, float* __restrict__ lse,
                     const uint16_t* __restrict__ bitmap, const int32_t* __restrict__ rem_rowptr,
                     const int32_t* __restrict__ rem_colidx, int n, int H, float sscale) {
-    constexpr int SBO_QK = (D / 8) * 128, SBO_PV = (kTile / 8) * 128;
+    constexpr int SBO_QK = (D / 8) * 128, SBO_P = (kTile / 8) * 128;
+    constexpr int LBO_V = (D / 8) * 128;   // V stays [source j][channel c] = MN-major B operand: 8x8 core matrices,
+                                           // channel groups 128 B apart (SBO), source groups LBO_V apart
     constexpr int kBytesQK = kTile * D * 2, kBytesP = kTile * kTile * 2;
+    static_assert(kBytesP <= 2 * kBytesQK, "P aliases the Q and K staging buffers");
     constexpr int CPR = D / 8;  // 16-byte chunks per row slice
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t* sQ = smem;
     uint8_t* sK = sQ + kBytesQK;
-    uint8_t* sVt = sK + kBytesQK;
-    uint8_t* sP = sVt + kBytesQK;
-    uint64_t* bar = reinterpret_cast<uint64_t*>(sP + kBytesP);
+    uint8_t* sP = smem;                      // P overwrites Q and K once S = Q K^T has completed
+    uint8_t* sV = smem + 2 * kBytesQK;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(sV + kBytesQK);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bar + 1);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -95,14 +99,13 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     const bool rvalid = row < n;
     const size_t rowe = (size_t)H * D;
 
-    // ---- one-time setup: zero P (off-diagonal blocks stay zero), barrier, TMEM (256 columns: S 128 + O D)
-    for (int i = tid; i < kBytesP / 16; i += kTile) reinterpret_cast<uint4*>(sP)[i] = make_uint4(0, 0, 0, 0);
+    // ---- one-time setup: barrier, TMEM (128 columns: S, later overwritten by O)
     if (tid == 0) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" ::"r"(smem_u32(tmem_slot)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -115,12 +118,36 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     const uint32_t bits = rvalid ? (uint32_t)__ldg(bitmap + row) : 0u;
     const int rb = rvalid ? __ldg(rem_rowptr + row) : 0, re = rvalid ? __ldg(rem_rowptr + row + 1) : 0;
     const int wl = tid >> 4;  // window of this row inside the tile
-    constexpr uint32_t kIdescS = make_idesc(kTile, kTile), kIdescO = make_idesc(kTile, D);
+    constexpr uint32_t kIdescS = make_idesc(kTile, kTile, false), kIdescO = make_idesc(kTile, D, true);
+
+    // staging map: a warp covers 8 rows x 4 chunks per step, so its 16-byte shared stores fill whole 128-byte
+    // core matrices (conflict-free) while each row still reads 64 contiguous bytes from global memory
+    auto stage_rc = [&](int idx, int& r, int& kc) {
+        r = (idx & 7) + 8 * (idx / (8 * CPR));
+        kc = (idx >> 3) % CPR;
+    };
+    auto prefetch_head = [&](int h) {   // pull the next head's tile slices and remainder rows towards L2
+        {   // the head slice of a row is one (D*2)-byte line: thread t prefetches row t's three slices
+            const int r = tid;
+            if (row0 + r < n) {
+                const size_t off = (size_t)(row0 + r) * rowe + (size_t)h * D;
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(q + off));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(k + off));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(v + off));
+            }
+        }
+        for (int e = rb; e < re; ++e) {
+            const size_t off = (size_t)__ldg(rem_colidx + e) * rowe + (size_t)h * D;
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(k + off));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(v + off));
+        }
+    };
 
     for (int h = 0; h < H; ++h) {
-        // ---- stage Q, K (K-major) and V^T for this head
+        // ---- stage Q, K (K-major) and V (MN-major) for this head
         for (int idx = tid; idx < kTile * CPR; idx += kTile) {
-            const int r = idx / CPR, kc = idx % CPR;
+            int r, kc;
+            stage_rc(idx, r, kc);
             uint4 a = make_uint4(0, 0, 0, 0), b = a, c = a;
             if (row0 + r < n) {
                 const size_t off = (size_t)(row0 + r) * rowe + (size_t)h * D + kc * 8;
@@ -130,10 +157,9 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
             }
             *reinterpret_cast<uint4*>(sQ + canon(r, kc * 8, SBO_QK)) = a;
             *reinterpret_cast<uint4*>(sK + canon(r, kc * 8, SBO_QK)) = b;
-            const uint16_t* cv = reinterpret_cast<const uint16_t*>(&c);
-#pragma unroll
-            for (int i = 0; i < 8; ++i) *reinterpret_cast<uint16_t*>(sVt + canon(kc * 8 + i, r, SBO_PV)) = cv[i];
+            *reinterpret_cast<uint4*>(sV + (r & 7) * 16 + kc * 128 + (r >> 3) * LBO_V) = c;
         }
+        if (h + 1 < H) prefetch_head(h + 1);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
@@ -150,7 +176,7 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
         phase ^= 1;
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         // ---- this row's 16 scores of its own window's diagonal block; mask; block-local softmax
-        float m = -INFINITY, l = 0.f;
+        float m = -INFINITY, l = 0.f, lx = 0.f;   // l: sum of the bf16-rounded weights (normalises O); lx: exact (for L)
         {
             float sv[32];
             tmem_ld32(t_lane + warp * 32, sv);
@@ -165,11 +191,16 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
             uint32_t pk[8];
 #pragma unroll
             for (int c = 0; c < 16; c += 2) {
-                const __nv_bfloat162 pb = __floats2bfloat162_rn(ex2(s16[c] - ms), ex2(s16[c + 1] - ms));
+                const float p0 = ex2(s16[c] - ms), p1 = ex2(s16[c + 1] - ms);
+                const __nv_bfloat162 pb = __floats2bfloat162_rn(p0, p1);
                 l += __low2float(pb) + __high2float(pb);   // normalise with the rounded weights the MMA will use
+                lx += p0 + p1;
                 pk[c >> 1] = *reinterpret_cast<const uint32_t*>(&pb);
             }
-            uint8_t* prow = sP + canon(tid, 16 * wl, SBO_PV);
+            // P aliases Q/K: clear this row (16 chunks of 16 bytes), then write its diagonal block
+#pragma unroll
+            for (int cc = 0; cc < kTile / 8; ++cc) *reinterpret_cast<uint4*>(sP + canon(tid, cc * 8, SBO_P)) = make_uint4(0, 0, 0, 0);
+            uint8_t* prow = sP + canon(tid, 16 * wl, SBO_P);
             *reinterpret_cast<uint4*>(prow) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
             *reinterpret_cast<uint4*>(prow + 128) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
         }
@@ -181,7 +212,7 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
             for (int s = 0; s < kTile / 16; ++s)
-                umma(tmem + 128, make_desc(smem_u32(sP) + s * 256, 128, SBO_PV), make_desc(smem_u32(sVt) + s * 256, 128, SBO_PV),
+                umma(tmem, make_desc(smem_u32(sP) + s * 256, 128, SBO_P), make_desc(smem_u32(sV) + s * 2 * LBO_V, LBO_V, 128),
                      kIdescO, s > 0);
             umma_commit(bar);
         }
@@ -192,7 +223,7 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
 #pragma unroll
         for (int c0 = 0; c0 < D; c0 += 32) {
             float t32[32];
-            tmem_ld32(t_lane + 128 + c0, t32);
+            tmem_ld32(t_lane + c0, t32);
 #pragma unroll
             for (int i = 0; i < 32; ++i) acc[c0 + i] = t32[i];
         }
@@ -224,6 +255,7 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
                 const float mx = fmaxf(m, s);
                 const float corr = ex2(m - mx), p = ex2(s - mx);
                 l = l * corr + p;
+                lx = lx * corr + p;
                 m = mx;
 #pragma unroll
                 for (int i = 0; i < CPR; ++i) {
@@ -250,12 +282,12 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
                 }
                 op[i] = make_uint4(w[0], w[1], w[2], w[3]);
             }
-            lse[(size_t)row * H + h] = l > 0.f ? (m + lg2(l)) * kLn2 : -INFINITY;
+            lse[(size_t)row * H + h] = lx > 0.f ? (m + lg2(lx)) * kLn2 : -INFINITY;
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();   // smem operands and TMEM are reused by the next head
     }
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(tmem) : "memory");
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" ::"r"(tmem) : "memory");
 }
 
 }  // namespace
@@ -282,7 +314,7 @@ extern "C" gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* P, const int32_t
         return GNN_EUNSUPPORTED;
     }
     constexpr int D = 64;
-    const size_t smem = 3 * (size_t)kTile * D * 2 + (size_t)kTile * kTile * 2 + 64;
+    const size_t smem = 3 * (size_t)kTile * D * 2 + 64;   // Q, K (aliased by P), V, barrier, TMEM slot
     cudaError_t e = cudaFuncSetAttribute(gt_fwd_block_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) {
         const int grid = (n + kTile - 1) / kTile;

@@ -40,7 +40,7 @@ def test_fullsize_sampled_parity(cfg):
     c = GI.make_config(cfg, keep_f32=False)
     n, H, d, dt, gt = c["n"], c["heads"], c["head_dim"], c["dtype"], c["layer"] == "gt"
     rp, ci = torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda()
-    plan = G.Plan(rp, ci, transpose=True, **DEFAULT_OPTS)
+    plan = G.Plan(rp, ci, transpose=True, blocks=(cfg == 4), **DEFAULT_OPTS)
     names = ("q", "k", "v", "do") if gt else ("xl", "xr", "do")
     T = {nm: _dev(c[nm + "_st"], dt) for nm in names}
     out = torch.empty_like(T[names[0]])
@@ -109,6 +109,14 @@ def test_fullsize_sampled_parity(cfg):
         dK, dV = oracle.gt_backward_src(rp_t, ci_t, f["q"], f["k"], f["v"], f["do"], Lf, Df, srcs=srcs)
         check(f"cfg{cfg}:dK", host(g2, srcs_t), dK, dt)
         check(f"cfg{cfg}:dV", host(g3, srcs_t), dV, dt)
+        if cfg == 4:   # row a12 at full size: the tcgen05 block path on the same sampled rows, and vs the CSR path everywhere
+            out_b, lse_b = torch.full_like(out, float("nan")), torch.full_like(lse, float("nan"))
+            G.gnn_gt_attn_fwd_block(plan, T["q"], T["k"], T["v"], out_b, lse_b)
+            torch.cuda.synchronize()
+            check(f"cfg{cfg}:block:O", host(out_b, rows_t), O[pos], dt)
+            check(f"cfg{cfg}:block:L", host(lse_b, rows_t), L[pos], dt)
+            assert float((out_b.float() - out.float()).abs().max()) <= 4e-2     # two bf16 roundings of nearby values
+            assert float((lse_b - lse).abs().max()) <= 1e-3
     else:
         af, sl = c["a_f32"], c["slope"]
         O, L = oracle.gatv2_forward(c["rowptr"], c["colidx"], f["xl"], f["xr"], af, sl, rows=need)
