@@ -37,7 +37,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_unit(u):
         src, obj = os.path.join(CSRC, u + ".cu"), os.path.join(OBJ, u + ".o")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+        extra = os.environ.get("GNN_NVCC_EXTRA", "").split()   # e.g. -DGNN_FWD_KU=1 for tuning builds
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed for {u}:\n{r.stdout}\n{r.stderr}")

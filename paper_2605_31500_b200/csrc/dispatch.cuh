@@ -20,9 +20,9 @@ inline cudaError_t dispatch_pass(int dtype, const Shape& sh0, const LaunchCtx& c
     };
 #define GNN_G(T, CB)                                                                         \
     {                                                                                        \
-        constexpr int KU = pass_ku(PASS, CB);                                                \
-        if (lc.g == 4) return go((OpT<T, CB, 4, KU>*)nullptr);                               \
-        if (lc.g == 8) return go((OpT<T, CB, 8, KU>*)nullptr);                               \
+        constexpr int KU = pass_ku(PASS, CB); /* edges per batch; never more than the group width */ \
+        if (lc.g == 4) return go((OpT<T, CB, 4, (KU < 4 ? KU : 4)>*)nullptr);                \
+        if (lc.g == 8) return go((OpT<T, CB, 8, (KU < 8 ? KU : 8)>*)nullptr);                \
         if (lc.g == 16) return go((OpT<T, CB, 16, KU>*)nullptr);                             \
         if (lc.g == 32) return go((OpT<T, CB, 32, KU>*)nullptr);                             \
     }

@@ -27,6 +27,20 @@
 
 namespace gnn {
 
+// tuning knobs (profiles/r01_lane_width_sweep.md): resident CTAs per SM the register budget is held to and
+// register double-buffering of the gathers, for the forward and the backward passes
+#ifndef GNN_FWD_MINB
+#define GNN_FWD_MINB 4
+#endif
+#ifndef GNN_FWD_DB
+#define GNN_FWD_DB 0
+#endif
+#ifndef GNN_BWD_MINB
+#define GNN_BWD_MINB 3
+#endif
+#ifndef GNN_BWD_DB
+#define GNN_BWD_DB 0
+#endif
 constexpr int kCtaThreads = 128;
 constexpr int kWarpsPerCta = kCtaThreads / 32;
 constexpr float kLog2e = 1.4426950408889634f;

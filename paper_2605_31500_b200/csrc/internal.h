@@ -44,12 +44,25 @@ struct LaneCfg { int vb, nv, cb, g, lanes; };
 constexpr int pass_max_cb(Pass) { return 32; }
 // widest lane the pass is instantiated for (wide rows may exceed the preferred pass_max_cb)
 constexpr int pass_inst_max_cb(Pass) { return 32; }
-// edges per lane group per batch (two batches are in flight per group: one being computed, one being gathered);
-// KU must divide the group width (>= 4)
+// edges gathered per lane group per batch, all in flight before the batch is computed (capped at the group
+// width); 4 measured best on cfg 3 / 5 for every pass but the 4-accumulator GATv2 dst pass (profiles/r01_lane_width_sweep.md)
+#ifndef GNN_FWD_KU
+#define GNN_FWD_KU 4
+#endif
+#ifndef GNN_GAT_DST_KU
+#define GNN_GAT_DST_KU 4
+#endif
+#ifndef GNN_GAT_SRC_KU
+#define GNN_GAT_SRC_KU 2
+#endif
+#ifndef GNN_BWD_KU
+#define GNN_BWD_KU 4
+#endif
 constexpr int pass_ku(Pass p, int cb) {
-    return (p == kGatFwd) ? (cb == 32 ? 2 : 4)                  // one gathered row per edge
-         : (p == kGatBwdDst) ? (cb == 32 ? 2 : 4)               // one row, four accumulators
-                             : (cb == 32 ? 2 : 4);              // two gathered rows per edge
+    return (p == kGatFwd || p == kGtFwd) ? (cb == 32 ? GNN_FWD_KU : 4)
+         : (p == kGatBwdDst)             ? (cb == 32 ? GNN_GAT_DST_KU : 4)   // four accumulator vectors
+         : (p == kGatBwdSrc)             ? (cb == 32 ? GNN_GAT_SRC_KU : 4)
+                                         : (cb == 32 ? GNN_BWD_KU : 4);
 }
 inline bool pick_lane_cfg(Pass p, int esz, int heads, int head_dim, LaneCfg& lc) {
     const int head_bytes = head_dim * esz, row_bytes = heads * head_bytes;

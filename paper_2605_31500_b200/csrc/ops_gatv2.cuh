@@ -10,8 +10,8 @@ __device__ __forceinline__ float lrelu(float z, float slope) { return fmaxf(z, 0
 // ------------------------------------------------------------------------------------ GATv2 forward
 template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G_, KU_, 1, 0> {
     static constexpr const char* kName = "gatv2_fwd";
-    static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
-    static constexpr bool kDoubleBuffer = true;
+    static constexpr int kMinBlocks = GNN_FWD_MINB;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = GNN_FWD_DB != 0;
     using B = OpBase<T, CB_, G_, KU_, 1, 0>;
     using typename B::GeoT;
     using typename B::Ck;
@@ -179,7 +179,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
 template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_, G_, KU_, 2, 2> {
     static constexpr const char* kName = "gatv2_bwd_src";
     static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
-    static constexpr bool kDoubleBuffer = false;
+    static constexpr bool kDoubleBuffer = GNN_BWD_DB != 0;
     using B = OpBase<T, CB_, G_, KU_, 2, 2>;
     using typename B::GeoT;
     using typename B::Ck;

@@ -42,8 +42,8 @@ template <int KU> __device__ __forceinline__ float softmax_step(float& m, float&
 // ------------------------------------------------------------------------------------- GT forward
 template <typename T, int CB_, int G_, int KU_> struct GtFwd : OpBase<T, CB_, G_, KU_, 2, 0> {
     static constexpr const char* kName = "gt_fwd";
-    static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
-    static constexpr bool kDoubleBuffer = true;
+    static constexpr int kMinBlocks = GNN_FWD_MINB;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = GNN_FWD_DB != 0;
     using B = OpBase<T, CB_, G_, KU_, 2, 0>;
     using typename B::GeoT;
     using typename B::Ck;
@@ -113,8 +113,8 @@ template <typename T, int CB_, int G_, int KU_> struct GtFwd : OpBase<T, CB_, G_
 // dQ = (A - Delta B)/sqrt(d)   (== sum_j alpha (dP - Delta) k_j / sqrt(d))
 template <typename T, int CB_, int G_, int KU_> struct GtBwdDst : OpBase<T, CB_, G_, KU_, 2, 0> {
     static constexpr const char* kName = "gt_bwd_dst";
-    static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
-    static constexpr bool kDoubleBuffer = false;
+    static constexpr int kMinBlocks = GNN_BWD_MINB;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = GNN_BWD_DB != 0;
     using B = OpBase<T, CB_, G_, KU_, 2, 0>;
     using typename B::GeoT;
     using typename B::Ck;
@@ -188,8 +188,8 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdDst : OpBase<T, CB_,
 // CSR^T order: deterministic, no atomics (the paper uses atomicAdd here).
 template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_, G_, KU_, 2, 2> {
     static constexpr const char* kName = "gt_bwd_src";
-    static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
-    static constexpr bool kDoubleBuffer = false;
+    static constexpr int kMinBlocks = GNN_BWD_MINB;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = GNN_BWD_DB != 0;
     using B = OpBase<T, CB_, G_, KU_, 2, 2>;
     using typename B::GeoT;
     using typename B::Ck;

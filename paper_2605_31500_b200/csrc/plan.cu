@@ -146,8 +146,10 @@ struct Layout {
     long long max_chunks, max_hub;
 };
 
-gnn_plan_opts_t resolve(const gnn_plan_opts_t* o) {
-    gnn_plan_opts_t r = {1024, 8192, 4096, 0, 0};
+// defaults: warp_max_deg 1024 on large graphs (nnz >= 2^24: enough rows in flight that long single-group rows
+// do not form a tail) and 256 on small ones; cta_max_deg 8192; split_chunk 4096
+gnn_plan_opts_t resolve(const gnn_plan_opts_t* o, int64_t nnz) {
+    gnn_plan_opts_t r = {nnz >= (1ll << 24) ? 1024 : 256, 8192, 4096, 0, 0};
     if (o) {
         if (o->warp_max_deg > 0) r.warp_max_deg = o->warp_max_deg;
         if (o->cta_max_deg > 0) r.cta_max_deg = o->cta_max_deg;
@@ -256,7 +258,7 @@ extern "C" gnn_status_t gnn_plan_bytes(int32_t n, int64_t nnz, const gnn_plan_op
         set_error("gnn_plan_bytes: need n >= 1, 0 <= nnz < 2^31 and non-NULL outputs");
         return GNN_EINVAL;
     }
-    const gnn_plan_opts_t o = resolve(opts);
+    const gnn_plan_opts_t o = resolve(opts, nnz);
     Layout L;
     cudaError_t e = make_layout(n, nnz, o, L);
     if (e != cudaSuccess) {
@@ -279,7 +281,7 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
         set_error("gnn_plan_build: dev_mem and scratch must be 256-byte aligned");
         return GNN_EINVAL;
     }
-    const gnn_plan_opts_t o = resolve(opts);
+    const gnn_plan_opts_t o = resolve(opts, nnz);
     Layout L;
     cudaError_t e = make_layout(n, nnz, o, L);
     if (e != cudaSuccess) {

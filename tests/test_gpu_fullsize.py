@@ -63,10 +63,10 @@ def test_fullsize_sampled_parity(cfg):
     assert np.array_equal(plan.export(B.GNN_PLAN_ROWPTR_T), rp_t)
     assert np.array_equal(plan.export(B.GNN_PLAN_COLIDX_T), ci_t)
     cnt = plan.counts()
-    ref = plan_ref.build_bins(c["rowptr"], *_resolved_opts())
+    ref = plan_ref.build_bins(c["rowptr"], *_resolved_opts(c["e"]))
     assert np.array_equal(plan.export(B.GNN_PLAN_PERM), ref["perm"])
     assert np.array_equal(plan.export(B.GNN_PLAN_CHUNKS).reshape(-1, 4), ref["chunks"])
-    ref_t = plan_ref.build_bins(rp_t, *_resolved_opts())
+    ref_t = plan_ref.build_bins(rp_t, *_resolved_opts(c["e"]))
     assert np.array_equal(plan.export(B.GNN_PLAN_PERM_T), ref_t["perm"])
     assert np.array_equal(plan.export(B.GNN_PLAN_CHUNKS_T).reshape(-1, 4), ref_t["chunks"])
     assert cnt["n_chunks"] == ref["chunks"].shape[0] and cnt["n_chunks_t"] == ref_t["chunks"].shape[0]
@@ -134,6 +134,6 @@ def test_fullsize_sampled_parity(cfg):
         assert np.all(np.isfinite(g3.cpu().numpy()))   # da: full-size value needs the whole oracle; checked at scale in test_gpu_parity
 
 
-def _resolved_opts():
+def _resolved_opts(nnz):
     """the library's default thresholds (include/gnn_attn.h)"""
-    return 1024, 8192, 4096
+    return (1024 if nnz >= (1 << 24) else 256), 8192, 4096
