@@ -25,6 +25,7 @@ namespace gnn {
 namespace {
 
 constexpr int kTile = 128;  // destination rows per CTA = MMA M = TMEM lanes
+constexpr int kTS = 68;     // floats per row slot of the transpose buffer (64 + m, l, lx + pad): 272 B
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -143,6 +144,20 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
         }
     };
 
+    // cooperative role (8 lanes per row, group g4 of the warp takes rows g4 + 4 i): the remainder sources of the
+    // group's 8 rows are head-invariant - the first two per row stay in registers
+    const int g4 = lane >> 3, gl = lane & 7;
+    int cj0[8], cj1[8], ccnt[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int rowc = row0 + warp * 32 + g4 + 4 * i;
+        const bool cv = rowc < n;
+        const int rbc = cv ? __ldg(rem_rowptr + rowc) : 0;
+        ccnt[i] = cv ? __ldg(rem_rowptr + rowc + 1) - rbc : 0;
+        cj0[i] = ccnt[i] > 0 ? __ldg(rem_colidx + rbc) : -1;
+        cj1[i] = ccnt[i] > 1 ? __ldg(rem_colidx + rbc + 1) : -1;
+    }
+
     for (int h = 0; h < H; ++h) {
         // ---- stage Q, K (K-major) and V (MN-major) for this head
         for (int idx = tid; idx < kTile * CPR; idx += kTile) {
@@ -197,9 +212,12 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
                 lx += p0 + p1;
                 pk[c >> 1] = *reinterpret_cast<const uint32_t*>(&pb);
             }
-            // P aliases Q/K: clear this row (16 chunks of 16 bytes), then write its diagonal block
+            // P aliases Q/K.  The rows of warp w occupy the contiguous 8 KB [w * 8192, +8192) of the canonical layout:
+            // the warp clears its own region with conflict-free stores, then every lane writes its diagonal block
 #pragma unroll
-            for (int cc = 0; cc < kTile / 8; ++cc) *reinterpret_cast<uint4*>(sP + canon(tid, cc * 8, SBO_P)) = make_uint4(0, 0, 0, 0);
+            for (int it = 0; it < 16; ++it)
+                *reinterpret_cast<uint4*>(sP + warp * 8192 + (it * 32 + lane) * 16) = make_uint4(0, 0, 0, 0);
+            __syncwarp();
             uint8_t* prow = sP + canon(tid, 16 * wl, SBO_P);
             *reinterpret_cast<uint4*>(prow) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
             *reinterpret_cast<uint4*>(prow + 128) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
@@ -219,70 +237,133 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
         mbar_wait(bar, phase);
         phase ^= 1;
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        float acc[D];
+        // ---- hand the block part over to the cooperative layout: thread t (owner of row t) writes its unnormalised
+        // O row and (m, l, lx) into the warp's transpose buffer (aliases the dead Q/K/P/V staging area; 272-byte row
+        // slots keep 16-byte accesses conflict-free)
+        float* sT = reinterpret_cast<float*>(smem) + warp * (32 * kTS);
+        {
+            float* slot = sT + lane * kTS;
 #pragma unroll
-        for (int c0 = 0; c0 < D; c0 += 32) {
-            float t32[32];
-            tmem_ld32(t_lane + c0, t32);
+            for (int c0 = 0; c0 < D; c0 += 32) {
+                float t32[32];
+                tmem_ld32(t_lane + c0, t32);
 #pragma unroll
-            for (int i = 0; i < 32; ++i) acc[c0 + i] = t32[i];
-        }
-        // ---- remainder edges of this row (sources outside the window): CSR gather, same online softmax
-        if (re > rb) {
-            uint32_t qw[D / 2];
-            const uint4* qp = reinterpret_cast<const uint4*>(q + (size_t)row * rowe + (size_t)h * D);
-#pragma unroll
-            for (int i = 0; i < CPR; ++i) {
-                const uint4 t = __ldg(qp + i);
-                qw[4 * i] = t.x; qw[4 * i + 1] = t.y; qw[4 * i + 2] = t.z; qw[4 * i + 3] = t.w;
+                for (int i = 0; i < 32; i += 4)
+                    *reinterpret_cast<float4*>(slot + c0 + i) = make_float4(t32[i], t32[i + 1], t32[i + 2], t32[i + 3]);
             }
-            for (int e = rb; e < re; ++e) {
-                const size_t off = (size_t)__ldg(rem_colidx + e) * rowe + (size_t)h * D;
-                const uint4* kp = reinterpret_cast<const uint4*>(k + off);
-                const uint4* vp = reinterpret_cast<const uint4*>(v + off);
-                float s0 = 0.f, s1 = 0.f;
-                uint4 vv[CPR];
+            slot[D] = m; slot[D + 1] = l; slot[D + 2] = lx;
+        }
+        __syncwarp();
+        // ---- remainder edges (sources outside the window) and the final merge, 8 lanes per row: every gather is a
+        // coalesced 128-byte row slice and the O row is stored coalesced (a lane owns 8 channels of the head).
+        // Rows are handled four at a time so that 20 independent 16-byte gathers are in flight per lane.
 #pragma unroll
-                for (int i = 0; i < CPR; ++i) {
-                    const uint4 t = __ldg(kp + i);
-                    vv[i] = __ldg(vp + i);
-                    fma_bf16x2(qw[4 * i], t.x, s0, s1);
-                    fma_bf16x2(qw[4 * i + 1], t.y, s0, s1);
-                    fma_bf16x2(qw[4 * i + 2], t.z, s0, s1);
-                    fma_bf16x2(qw[4 * i + 3], t.w, s0, s1);
+        for (int half = 0; half < 2; ++half) {
+            uint4 Lq[4], Lk0[4], Lk1[4], Lv0[4], Lv1[4];
+#pragma unroll
+            for (int ii = 0; ii < 4; ++ii) {
+                const int i = 4 * half + ii;
+                const int rowc = row0 + warp * 32 + g4 + 4 * i;
+                const uint4 z = make_uint4(0, 0, 0, 0);
+                Lq[ii] = Lk0[ii] = Lk1[ii] = Lv0[ii] = Lv1[ii] = z;
+                if (cj0[i] >= 0) {
+                    const size_t off = (size_t)cj0[i] * rowe + (size_t)h * D;
+                    Lq[ii] = __ldg(reinterpret_cast<const uint4*>(q + (size_t)rowc * rowe + (size_t)h * D) + gl);
+                    Lk0[ii] = __ldg(reinterpret_cast<const uint4*>(k + off) + gl);
+                    Lv0[ii] = __ldg(reinterpret_cast<const uint4*>(v + off) + gl);
                 }
-                const float s = (s0 + s1) * sscale;
-                const float mx = fmaxf(m, s);
-                const float corr = ex2(m - mx), p = ex2(s - mx);
-                l = l * corr + p;
-                lx = lx * corr + p;
-                m = mx;
+                if (cj1[i] >= 0) {
+                    const size_t off = (size_t)cj1[i] * rowe + (size_t)h * D;
+                    Lk1[ii] = __ldg(reinterpret_cast<const uint4*>(k + off) + gl);
+                    Lv1[ii] = __ldg(reinterpret_cast<const uint4*>(v + off) + gl);
+                }
+            }
 #pragma unroll
-                for (int i = 0; i < CPR; ++i) {
-                    const uint32_t w[4] = {vv[i].x, vv[i].y, vv[i].z, vv[i].w};
+            for (int ii = 0; ii < 4; ++ii) {
+                const int i = 4 * half + ii;
+                const int rl = g4 + 4 * i;
+                const int rowc = row0 + warp * 32 + rl;
+                const bool cv = rowc < n;
+                float mr = -INFINITY, lr = 0.f, a[8];
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        acc[8 * i + 2 * j] = fmaf(p, __uint_as_float(w[j] << 16), acc[8 * i + 2 * j] * corr);
-                        acc[8 * i + 2 * j + 1] = fmaf(p, __uint_as_float(w[j] & 0xffff0000u), acc[8 * i + 2 * j + 1] * corr);
+                for (int c = 0; c < 8; ++c) a[c] = 0.f;
+                // one step of the online softmax over two gathered sources (masked when the id is negative)
+                auto pair_step = [&](int j0, int j1, const uint4& qv, const uint4& k0, const uint4& k1, const uint4& v0,
+                                     const uint4& v1) {
+                    float d0 = 0.f, d0b = 0.f, d1 = 0.f, d1b = 0.f;
+                    fma_bf16x2(qv.x, k0.x, d0, d0b); fma_bf16x2(qv.y, k0.y, d0, d0b);
+                    fma_bf16x2(qv.z, k0.z, d0, d0b); fma_bf16x2(qv.w, k0.w, d0, d0b);
+                    fma_bf16x2(qv.x, k1.x, d1, d1b); fma_bf16x2(qv.y, k1.y, d1, d1b);
+                    fma_bf16x2(qv.z, k1.z, d1, d1b); fma_bf16x2(qv.w, k1.w, d1, d1b);
+                    d0 += d0b; d1 += d1b;
+#pragma unroll
+                    for (int o = 1; o < 8; o <<= 1) {
+                        d0 += __shfl_xor_sync(0xffffffffu, d0, o);
+                        d1 += __shfl_xor_sync(0xffffffffu, d1, o);
+                    }
+                    const float s0 = j0 < 0 ? -INFINITY : d0 * sscale, s1 = j1 < 0 ? -INFINITY : d1 * sscale;
+                    const float mx = fmaxf(mr, fmaxf(s0, s1));
+                    const float ms = (mx == -INFINITY) ? 0.f : mx;
+                    const float corr = ex2(mr - ms), p0 = ex2(s0 - ms), p1 = ex2(s1 - ms);
+                    lr = lr * corr + p0 + p1;
+                    mr = mx;
+                    const uint32_t w0[4] = {v0.x, v0.y, v0.z, v0.w}, w1[4] = {v1.x, v1.y, v1.z, v1.w};
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj) {
+                        float x = a[2 * jj] * corr, y = a[2 * jj + 1] * corr;
+                        x = fmaf(p0, __uint_as_float(w0[jj] << 16), x);
+                        y = fmaf(p0, __uint_as_float(w0[jj] & 0xffff0000u), y);
+                        a[2 * jj] = fmaf(p1, __uint_as_float(w1[jj] << 16), x);
+                        a[2 * jj + 1] = fmaf(p1, __uint_as_float(w1[jj] & 0xffff0000u), y);
+                    }
+                };
+                pair_step(cj0[i], cj1[i], Lq[ii], Lk0[ii], Lk1[ii], Lv0[ii], Lv1[ii]);
+                // rows with more than two remainder sources: further pairs, gathered directly (warp-uniform trip count)
+                int maxcnt = ccnt[i];
+                maxcnt = max(maxcnt, __shfl_xor_sync(0xffffffffu, maxcnt, 8));
+                maxcnt = max(maxcnt, __shfl_xor_sync(0xffffffffu, maxcnt, 16));
+                if (maxcnt > 2) {
+                    const int rbc = cv ? __ldg(rem_rowptr + rowc) : 0;
+                    for (int eb = 2; eb < maxcnt; eb += 2) {
+                        const int j0 = eb < ccnt[i] ? __ldg(rem_colidx + rbc + eb) : -1;
+                        const int j1 = eb + 1 < ccnt[i] ? __ldg(rem_colidx + rbc + eb + 1) : -1;
+                        uint4 k0 = make_uint4(0, 0, 0, 0), k1 = k0, v0 = k0, v1 = k0;
+                        if (j0 >= 0) {
+                            const size_t off = (size_t)j0 * rowe + (size_t)h * D;
+                            k0 = __ldg(reinterpret_cast<const uint4*>(k + off) + gl);
+                            v0 = __ldg(reinterpret_cast<const uint4*>(v + off) + gl);
+                        }
+                        if (j1 >= 0) {
+                            const size_t off = (size_t)j1 * rowe + (size_t)h * D;
+                            k1 = __ldg(reinterpret_cast<const uint4*>(k + off) + gl);
+                            v1 = __ldg(reinterpret_cast<const uint4*>(v + off) + gl);
+                        }
+                        pair_step(j0, j1, Lq[ii], k0, k1, v0, v1);
                     }
                 }
-            }
-        }
-        // ---- normalise and store
-        if (rvalid) {
-            const float inv = l > 0.f ? 1.f / l : 0.f;
-            uint4* op = reinterpret_cast<uint4*>(out + (size_t)row * rowe + (size_t)h * D);
+                // block part of this row from the transpose buffer, log-sum-exp merge, normalise, store
+                const float* slot = sT + rl * kTS;
+                const float4 b0 = *reinterpret_cast<const float4*>(slot + gl * 8);
+                const float4 b1 = *reinterpret_cast<const float4*>(slot + gl * 8 + 4);
+                const float mb = slot[D], lb = slot[D + 1], lxb = slot[D + 2];
+                const float mm = fmaxf(mb, mr);
+                const float ms = (mm == -INFINITY) ? 0.f : mm;
+                const float cb = ex2(mb - ms), cr = ex2(mr - ms);
+                const float lsum = lb * cb + lr * cr, lxsum = lxb * cb + lr * cr;
+                const float inv = lsum > 0.f ? 1.f / lsum : 0.f;
+                if (cv) {
+                    const float ob[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+                    uint32_t w[4];
 #pragma unroll
-            for (int i = 0; i < CPR; ++i) {
-                uint32_t w[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const __nv_bfloat162 b2 = __floats2bfloat162_rn(acc[8 * i + 2 * j] * inv, acc[8 * i + 2 * j + 1] * inv);
-                    w[j] = *reinterpret_cast<const uint32_t*>(&b2);
+                    for (int jj = 0; jj < 4; ++jj) {
+                        const __nv_bfloat162 b2 = __floats2bfloat162_rn((ob[2 * jj] * cb + a[2 * jj] * cr) * inv,
+                                                                        (ob[2 * jj + 1] * cb + a[2 * jj + 1] * cr) * inv);
+                        w[jj] = *reinterpret_cast<const uint32_t*>(&b2);
+                    }
+                    reinterpret_cast<uint4*>(out + (size_t)rowc * rowe + (size_t)h * D)[gl] = make_uint4(w[0], w[1], w[2], w[3]);
+                    if (gl == 0) lse[(size_t)rowc * H + h] = lxsum > 0.f ? (mm + lg2(lxsum)) * kLn2 : -INFINITY;
                 }
-                op[i] = make_uint4(w[0], w[1], w[2], w[3]);
             }
-            lse[(size_t)row * H + h] = lx > 0.f ? (m + lg2(lx)) * kLn2 : -INFINITY;
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();   // smem operands and TMEM are reused by the next head
