@@ -4,18 +4,22 @@
 // Paper's version: per 16-row window and head, WMMA 16x16x16 on A100: S = Q_win K_blk^T,
 // bitmap mask, FlashAttention-style online softmax, acc += P V_blk.  tcgen05.mma has M in {64, 128}, so here one
 // CTA owns a tile of 128 destination rows = 8 windows and, per head, issues ONE 128x128xd product
-// S = Q_tile K_tile^T (bf16 in, fp32 in TMEM); thread t owns row t (TMEM lane t), reads back only the 16 columns
-// of its own window's diagonal block, masks them with the plan's 16-bit row bitmap (row a11), forms
-// p = 2^(s - m) in registers, writes P (bf16, zero off the diagonal blocks) to shared memory and a second
-// product O = P V_tile (128x128 by 128xd) accumulates the block part in TMEM.  The off-diagonal blocks are wasted
-// tensor work (8x) - far below the HBM time of the tile.  The remainder edges (sources
-// outside the window: the long-range in-edges) are then gathered per row exactly as in the CSR path and merged
-// into the same online-softmax state, so the result equals the plain CSR forward.
+// S = Q_tile K_tile^T (bf16 in, fp32 in TMEM); thread t owns row t (TMEM lane t), reads back only the 32 columns
+// that hold its window's diagonal block, masks its 16 scores with the plan's 16-bit row bitmap (row a11), forms
+// p = 2^(s - m) in registers, writes P (bf16, zero off the diagonal blocks) over the dead Q/K staging area and a
+// second product O = P V_tile (128x128 by 128xd) leaves the block part in the same TMEM columns.  The off-diagonal
+// blocks are wasted tensor work (8x) - far below the memory time of the tile.
 //
-// Operand staging: Q, K (K-major) and V^T (K-major over the source index) are written by the CTA's threads into
-// the canonical no-swizzle core-matrix layout (8 rows x 16 bytes per core matrix; LBO = 128 B between the two
-// K core matrices of one MMA, SBO = bytes per 8-row group), described to the tensor core by 64-bit shared-memory
-// matrix descriptors; completion is signalled with tcgen05.commit on an mbarrier.
+// The block part is then handed to a cooperative layout through a shared-memory transpose (row slots of 272 bytes):
+// 8 lanes per row, each owning 8 channels, gather the row's remainder sources (sources outside the window: the
+// long-range in-edges) as coalesced 128-byte slices, run the same online softmax, merge it with the block part by
+// log-sum-exp and store O coalesced - so the result equals the plain CSR forward.  Per-thread row-wise
+// gathers and stores (32 L1 wavefronts per instruction) made the first version LSU-bound; this layout needs 4.
+//
+// Operand staging: Q, K (K-major) and V (MN-major, no transpose) are written by the CTA's threads into the canonical
+// no-swizzle core-matrix layout (8 x 16-byte core matrices; LBO / SBO = byte distance between core matrices along
+// K / along M,N) and described to the tensor core by 64-bit shared-memory matrix descriptors; completion is
+// signalled with tcgen05.commit on an mbarrier.  48 KB of shared memory and 128 TMEM columns per CTA: 3 CTAs/SM.
 #include <cuda_bf16.h>
 
 #include "internal.h"
