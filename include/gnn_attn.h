@@ -157,7 +157,8 @@ gnn_status_t gnn_gatv2_fwd(const gnn_plan_t* plan, const int32_t* rowptr, const 
  *   z_ij = xl_i + xr_j;  alpha_ij = exp(s_ij - L_i);  dP_ij = <dout_i, xr_j>;  G_i = sum_j alpha_ij dP_ij
  *   de_ij = alpha_ij (dP_ij - G_i);  LeakyReLU'(z) = 1 if z > 0 else slope
  *   dxl_i = sum_j de_ij a . LeakyReLU'(z_ij)                              (dst pass, "AL" kernel)
- *   da    = sum_ij de_ij LeakyReLU(z_ij)    (per-CTA fp32 partials, fixed-order fp64 final reduction)
+ *   da    = sum_ij de_ij LeakyReLU(z_ij)    (= sum_i xl_i . S_i + sum_j xr_j . U_j with S, U the LeakyReLU'-weighted
+ *                                            sums of de of the two passes; per-CTA fp32 partials, fixed-order fp64 final reduction)
  *   dxr_j = sum_i ( alpha_ij dout_i + de_ij a . LeakyReLU'(z_ij) )        (src pass over CSR^T, "R" kernel)
  * g: [n,H] fp32, OUT (holds G on return).  dxl, dxr: [n,H,d] fp32, out.  da: [H,d] fp32, out.     */
 gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,

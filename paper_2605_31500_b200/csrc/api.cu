@@ -59,11 +59,11 @@ bool make_shape(int32_t n, int32_t heads, int32_t head_dim, int dtype, Shape& sh
 
 bool aligned16(const void* p) { return (((uintptr_t)p) & 31) == 0; }  // 256-bit gathers need 32-byte alignment
 
-struct WsLayout { size_t partials, da_part, total; int da_slots; };
+struct WsLayout { size_t partials, da_part, total; int da_slots, da_slots_dst; };
 
 // workspace of one API call = max over its passes of the chunk partials (+ da partials for GATv2 bwd)
 WsLayout ws_layout(const gnn_plan* P, int op, const Shape& sh, int esz) {
-    WsLayout w = {0, 0, 0, 0};
+    WsLayout w = {0, 0, 0, 0, 0};
     size_t part = 0;
     auto need = [&](Pass ps, const BinView& b) {
         const size_t x = (size_t)b.n_chunks * pass_state_floats(ps, sh) * sizeof(float);
@@ -82,7 +82,9 @@ WsLayout ws_layout(const gnn_plan* P, int op, const Shape& sh, int esz) {
     if (op == GNN_OP_GATV2_BWD) {
         LaneCfg lc;
         pick_lane_cfg(kGatBwdDst, esz, sh.H, sh.d, lc);
-        w.da_slots = grid_plan(P->fwd, P->sm_count, lc.g).da_slots();
+        w.da_slots_dst = grid_plan(P->fwd, P->sm_count, lc.g).da_slots();                       // dst pass (CSR bins)
+        pick_lane_cfg(kGatBwdSrc, esz, sh.H, sh.d, lc);
+        w.da_slots = w.da_slots_dst + grid_plan(P->tr, P->sm_count, lc.g).da_slots();          // + src pass (CSR^T bins)
         da = (size_t)w.da_slots * sh.rowe * sizeof(float);
     }
     w.total = w.da_part + da + 256;
@@ -253,8 +255,10 @@ extern "C" gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* P, const int32_t* rowptr
     a.xl = xl; a.xr = xr; a.a = a_; a.dout = dout; a.lse = const_cast<float*>(lse); a.g = g; a.dxl = dxl; a.dxr = dxr;
     a.slope = slope;
     const LaunchCtx c = make_ctx(P, false, ws, w, stream);
-    cudaError_t e = launch_gat_bwd_dst(dtype, sh, c, a);                                   // dxl, G, da partials
+    LaunchCtx ct = make_ctx(P, true, ws, w, stream);
+    ct.da_slot_base = w.da_slots_dst;
+    cudaError_t e = launch_gat_bwd_dst(dtype, sh, c, a);                                   // dxl, G, da partials (xl . S)
+    if (e == cudaSuccess) e = launch_gat_bwd_src(dtype, sh, ct, a);                        // dxr, da partials (xr . U)
     if (e == cudaSuccess) e = launch_da_reduce(c.da_part, w.da_slots, sh.rowe, da, c.stream);  // da
-    if (e == cudaSuccess) e = launch_gat_bwd_src(dtype, sh, make_ctx(P, true, ws, w, stream), a);  // dxr
     return cuda_status(e, who);
 }

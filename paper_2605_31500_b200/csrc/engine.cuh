@@ -41,6 +41,12 @@ namespace gnn {
 #ifndef GNN_BWD_DB
 #define GNN_BWD_DB 0
 #endif
+#ifndef GNN_GAT_DST_MINB
+#define GNN_GAT_DST_MINB 3
+#endif
+#ifndef GNN_GAT_SRC_MINB
+#define GNN_GAT_SRC_MINB 3
+#endif
 constexpr int kCtaThreads = 128;
 constexpr int kWarpsPerCta = kCtaThreads / 32;
 constexpr float kLog2e = 1.4426950408889634f;

@@ -31,7 +31,7 @@ namespace gnn {
 enum Pass { kGtFwd = 0, kGtBwdDst, kGtBwdSrc, kGatFwd, kGatBwdDst, kGatBwdSrc, kNumPass };
 struct PassInfo { int na, ns, softmax, has_da; };
 // must match the NA / NS / SOFTMAX / HAS_DA constants of the Op structs (static_asserted in the dispatch units)
-constexpr PassInfo kPassInfo[kNumPass] = {{1, 1, 1, 0}, {2, 1, 0, 0}, {2, 0, 0, 0}, {1, 1, 1, 0}, {4, 1, 0, 1}, {1, 0, 0, 0}};
+constexpr PassInfo kPassInfo[kNumPass] = {{1, 1, 1, 0}, {2, 1, 0, 0}, {2, 0, 0, 0}, {1, 1, 1, 0}, {2, 1, 0, 1}, {2, 0, 0, 1}};
 
 inline int pass_state_floats(Pass p, const Shape& sh) {
     return kPassInfo[p].na * sh.rowe + (kPassInfo[p].ns + kPassInfo[p].softmax) * sh.H;
@@ -50,7 +50,7 @@ constexpr int pass_inst_max_cb(Pass) { return 32; }
 #define GNN_FWD_KU 4
 #endif
 #ifndef GNN_GAT_DST_KU
-#define GNN_GAT_DST_KU 4
+#define GNN_GAT_DST_KU 2
 #endif
 #ifndef GNN_GAT_SRC_KU
 #define GNN_GAT_SRC_KU 2

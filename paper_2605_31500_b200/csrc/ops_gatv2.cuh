@@ -87,19 +87,23 @@ template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G
 };
 
 // ------------------------------------------------------------- GATv2 backward, dst pass ("AL" kernel)
-// One sweep: with as = a . LeakyReLU'(z), sg = LeakyReLU(z), w = alpha dP:
-//   A1 = sum w as, B1 = sum alpha as, A2 = sum w sg, B2 = sum alpha sg, G = sum w
-//   dxl_i = A1 - G B1;  this row's share of da = A2 - G B2      (== sum_j de_ij ...)
+// With s' = LeakyReLU'(z) in {1, slope} and LeakyReLU(z) = z s'(z), z = xl_i + xr_j, de_ij = alpha_ij (dP_ij - G_i):
+//   dxl_i = a . S_i,              S_i = sum_j de_ij s'_ij                       (this pass)
+//   dxr_j = V_j + a . U_j,        V_j = sum_i alpha_ij dO_i,  U_j = sum_i de_ij s'_ij   (src pass)
+//   da    = sum_ij de_ij z_ij s'_ij = sum_i xl_i . S_i + sum_j xr_j . U_j
+// so the attention-vector gradient needs no accumulators of its own: each pass adds (own row) . (its s'-weighted
+// sum) to the per-lane da partial.  One sweep over the row (G_i is only known at its end):
+//   A = sum w s', B = sum alpha s', G = sum w  with w = alpha dP;  S_i = A - G B.
 template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_, G_, KU_, 1, 0> {
     static constexpr const char* kName = "gatv2_bwd_dst";
-    static constexpr int kMinBlocks = 2;  // resident CTAs per SM the register budget is held to
+    static constexpr int kMinBlocks = GNN_GAT_DST_MINB;  // resident CTAs per SM the register budget is held to
     static constexpr bool kDoubleBuffer = false;
     using B = OpBase<T, CB_, G_, KU_, 1, 0>;
     using typename B::GeoT;
     using typename B::Ck;
     using typename B::Src;
     static constexpr int CH = B::kCH, KU = KU_;
-    static constexpr int NA = 4, NS = 1;
+    static constexpr int NA = 2, NS = 1;
     static constexpr bool SOFTMAX = false, HAS_DA = true;
     using St = State<NA, NS, CH>;
     struct Params {
@@ -145,18 +149,15 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
         for (int u = 0; u < KU; ++u) {
             const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] * kLog2e - o.lp);
             const float w = alpha * r[2 * u + 1];
+            const float ws = w * p.slope, as = alpha * p.slope;
             const Ck& xc = src.c[u][0];
             float z[CH];
             add_chunk(xc, o.xl, z);
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
                 const bool pos = z[c] > 0.f;
-                const float sg = pos ? z[c] : p.slope * z[c];
-                const float as = pos ? o.a[c] : p.slope * o.a[c];
-                st.acc[0][c] = fmaf(w, as, st.acc[0][c]);
-                st.acc[1][c] = fmaf(alpha, as, st.acc[1][c]);
-                st.acc[2][c] = fmaf(w, sg, st.acc[2][c]);
-                st.acc[3][c] = fmaf(alpha, sg, st.acc[3][c]);
+                st.acc[0][c] += pos ? w : ws;
+                st.acc[1][c] += pos ? alpha : as;
             }
             st.sc[0] += w;
         }
@@ -164,11 +165,16 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
                                                     const GeoT& g, float (&da)[CH]) {
         const float gg = st.sc[0];
-        float o[CH];
+        float xl[CH], a[CH], o[CH];
+        Ck c0;
+        c0.load_global(p.xl, (size_t)row * sh.rowe + g.eoff, g.act);
+        c0.to_float(xl);
+        load_f32<CH>(p.a, g.eoff, g.act, a);
 #pragma unroll
         for (int c = 0; c < CH; ++c) {
-            o[c] = st.acc[0][c] - gg * st.acc[1][c];
-            da[c] += st.acc[2][c] - gg * st.acc[3][c];
+            const float sdash = st.acc[0][c] - gg * st.acc[1][c];   // S_i
+            o[c] = a[c] * sdash;
+            da[c] = fmaf(xl[c], sdash, da[c]);
         }
         if (g.act) store_f32<CH>(p.dxl, (size_t)row * sh.rowe + g.eoff, o);
         if (g.lead) p.g[(size_t)row * sh.H + g.hd] = gg;
@@ -176,17 +182,19 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
 };
 
 // ----------------------------------------------------- GATv2 backward, src pass over CSR^T ("R" kernel)
+// V_j = sum_i alpha_ij dO_i and U_j = sum_i de_ij s'_ij accumulate in registers in CSR^T order (deterministic, no
+// atomics); dxr_j = V_j + a . U_j and xr_j . U_j goes to the da partial (see the dst pass for the identities).
 template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_, G_, KU_, 2, 2> {
     static constexpr const char* kName = "gatv2_bwd_src";
-    static constexpr int kMinBlocks = 4;  // resident CTAs per SM the register budget is held to
-    static constexpr bool kDoubleBuffer = GNN_BWD_DB != 0;
+    static constexpr int kMinBlocks = GNN_GAT_SRC_MINB;  // resident CTAs per SM the register budget is held to
+    static constexpr bool kDoubleBuffer = false;
     using B = OpBase<T, CB_, G_, KU_, 2, 2>;
     using typename B::GeoT;
     using typename B::Ck;
     using typename B::Src;
     static constexpr int CH = B::kCH, KU = KU_;
-    static constexpr int NA = 1, NS = 0;
-    static constexpr bool SOFTMAX = false, HAS_DA = false;
+    static constexpr int NA = 2, NS = 0;
+    static constexpr bool SOFTMAX = false, HAS_DA = true;
     using St = State<NA, NS, CH>;
     struct Params {
         const T *xl, *xr, *dout;
@@ -234,19 +242,30 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
             const float li = src.s[u][0], gi = src.s[u][1];
             const float alpha = nbr[u] < 0 ? 0.f : ex2((r[2 * u] - li) * kLog2e);
             const float de = alpha * (r[2 * u + 1] - gi);
+            const float des = de * p.slope;
             const Ck &lc = src.c[u][0], &gc = src.c[u][1];
             float z[CH];
             add_chunk(lc, o.xrf, z);
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-                const float as = z[c] > 0.f ? o.a[c] : p.slope * o.a[c];
-                st.acc[0][c] = fmaf(alpha, gc.get(c), fmaf(de, as, st.acc[0][c]));
+                st.acc[0][c] = fmaf(alpha, gc.get(c), st.acc[0][c]);
+                st.acc[1][c] += z[c] > 0.f ? de : des;
             }
         }
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
-                                                    const GeoT& g, float (&)[CH]) {
-        if (g.act) store_f32<CH>(p.dxr, (size_t)row * sh.rowe + g.eoff, st.acc[0]);
+                                                    const GeoT& g, float (&da)[CH]) {
+        float xr[CH], a[CH], o[CH];
+        Ck c0;
+        c0.load_global(p.xr, (size_t)row * sh.rowe + g.eoff, g.act);
+        c0.to_float(xr);
+        load_f32<CH>(p.a, g.eoff, g.act, a);
+#pragma unroll
+        for (int c = 0; c < CH; ++c) {
+            o[c] = fmaf(a[c], st.acc[1][c], st.acc[0][c]);
+            da[c] = fmaf(xr[c], st.acc[1][c], da[c]);
+        }
+        if (g.act) store_f32<CH>(p.dxr, (size_t)row * sh.rowe + g.eoff, o);
     }
 };
 
