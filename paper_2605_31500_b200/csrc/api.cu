@@ -59,11 +59,11 @@ bool make_shape(int32_t n, int32_t heads, int32_t head_dim, int dtype, Shape& sh
 
 bool aligned16(const void* p) { return (((uintptr_t)p) & 31) == 0; }  // 256-bit gathers need 32-byte alignment
 
-struct WsLayout { size_t partials, da_part, total; int da_slots, da_slots_dst; };
+struct WsLayout { size_t partials, da_part, stat2, total; int da_slots, da_slots_dst; };
 
 // workspace of one API call = max over its passes of the chunk partials (+ da partials for GATv2 bwd)
 WsLayout ws_layout(const gnn_plan* P, int op, const Shape& sh, int esz) {
-    WsLayout w = {0, 0, 0, 0, 0};
+    WsLayout w = {0, 0, 0, 0, 0, 0};
     size_t part = 0;
     auto need = [&](Pass ps, const BinView& b) {
         const size_t x = (size_t)b.n_chunks * pass_state_floats(ps, sh) * sizeof(float);
@@ -87,7 +87,9 @@ WsLayout ws_layout(const gnn_plan* P, int op, const Shape& sh, int esz) {
         w.da_slots = w.da_slots_dst + grid_plan(P->tr, P->sm_count, lc.g).da_slots();          // + src pass (CSR^T bins)
         da = (size_t)w.da_slots * sh.rowe * sizeof(float);
     }
-    w.total = w.da_part + da + 256;
+    w.stat2 = (w.da_part + da + 255) / 256 * 256;
+    const size_t st2 = (op == GNN_OP_GT_BWD) ? (size_t)P->n * sh.H * sizeof(float2) : 0;   // (L log2e, Delta) for the GT src pass
+    w.total = w.stat2 + st2 + 256;
     return w;
 }
 
@@ -205,6 +207,7 @@ extern "C" gnn_status_t gnn_gt_attn_bwd(const gnn_plan_t* P, const int32_t* rowp
     GtArgs a = {};
     a.q = q; a.k = k; a.v = v; a.dout = dout; a.lse = const_cast<float*>(lse); a.delta = delta;
     a.dq = dq; a.dk = dk; a.dv = dv;
+    a.stat2 = (float2*)((char*)ws + w.stat2);
     cudaError_t e = launch_gt_bwd_dst(dtype, sh, make_ctx(P, false, ws, w, stream), a);   // dQ, Delta
     if (e == cudaSuccess) e = launch_gt_bwd_src(dtype, sh, make_ctx(P, true, ws, w, stream), a);  // dK, dV
     return cuda_status(e, who);

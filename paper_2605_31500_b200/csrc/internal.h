@@ -99,6 +99,7 @@ struct GtArgs {
     const void *q, *k, *v, *dout;
     void* out;
     float *lse, *delta, *dq, *dk, *dv;
+    float2* stat2;   // workspace [n,H]: (L * log2(e), Delta) packed by the dst pass for the src pass (one 8-byte gather)
 };
 struct GatArgs {
     const void *xl, *xr, *dout;

@@ -127,6 +127,7 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdDst : OpBase<T, CB_,
         const T *q, *k, *v, *dout;
         const float* lse;
         float *dq, *delta;
+        float2* stat2;
         float qscale, inv_sqrt_d;
     };
     struct Own { Ck q, go; float lp; };
@@ -179,7 +180,10 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdDst : OpBase<T, CB_,
 #pragma unroll
         for (int c = 0; c < CH; ++c) o[c] = (st.acc[0][c] - dl * st.acc[1][c]) * p.inv_sqrt_d;
         if (g.act) store_f32<CH>(p.dq, (size_t)row * sh.rowe + g.eoff, o);
-        if (g.lead) p.delta[(size_t)row * sh.H + g.hd] = dl;
+        if (g.lead) {
+            p.delta[(size_t)row * sh.H + g.hd] = dl;
+            p.stat2[(size_t)row * sh.H + g.hd] = make_float2(__ldg(p.lse + (size_t)row * sh.H + g.hd) * kLog2e, dl);
+        }
     }
 };
 
@@ -200,7 +204,7 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_,
     using St = State<NA, NS, CH>;
     struct Params {
         const T *q, *k, *v, *dout;
-        const float *lse, *delta;
+        const float2* stat2;   // (L * log2(e), Delta) per (node, head), written by the dst pass
         float *dk, *dv;
         float kscale, inv_sqrt_d;
     };
@@ -220,8 +224,9 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_,
             const size_t i = (size_t)(nbr[u] < 0 ? 0 : nbr[u]);
             src.c[u][0].load_global(p.q, i * sh.rowe + g.eoff, pr);
             src.c[u][1].load_global(p.dout, i * sh.rowe + g.eoff, pr);
-            src.s[u][0] = pr ? __ldg(p.lse + i * sh.H + g.hd) : 0.f;
-            src.s[u][1] = pr ? __ldg(p.delta + i * sh.H + g.hd) : 0.f;
+            const float2 t = pr ? __ldg(p.stat2 + i * sh.H + g.hd) : make_float2(0.f, 0.f);
+            src.s[u][0] = t.x;
+            src.s[u][1] = t.y;
         }
     }
     __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
@@ -237,7 +242,7 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_,
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
             const float li = src.s[u][0], di = src.s[u][1];
-            const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] * p.kscale - li * kLog2e);
+            const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] * p.kscale - li);
             const float ds = alpha * (r[2 * u + 1] - di);
             const Ck &qc = src.c[u][0], &gc = src.c[u][1];
 #pragma unroll
