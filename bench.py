@@ -95,6 +95,7 @@ class ClockSampler:
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
+        self.index = index
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
@@ -128,6 +129,17 @@ class ClockSampler:
                 if val.lower().startswith("active"):
                     reasons.add(nm)
         os.unlink(self.f.name)
+        if not sm:   # region shorter than one sampling period: one synchronous query right after it
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=10).stdout
+                parts = [x.strip() for x in out.strip().splitlines()[0].split(",")]
+                sm, mx = [float(parts[0])], [float(parts[1])]
+                for nm, val in zip(names, parts[4:8]):
+                    if val.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(max(mx)) if mx else None,
                 "samples": len(sm), "reasons": sorted(reasons)}
 
@@ -351,10 +363,10 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize()
         return [a.elapsed_time(b) for a, b in evs]
 
+    clocks = ClockSampler(local_rank)     # sampled every 100 ms from the warm-up to the end of the timed regions
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
-    clocks = ClockSampler(local_rank)
     l0 = G.gnn_launch_count()
     ms_steps = timed(step, args.steps)
     launches = G.gnn_launch_count() - l0
