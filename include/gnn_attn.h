@@ -172,7 +172,7 @@ gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* plan, const int32_t* rowptr, const 
  * 16-bit bitmaps of in-window edges; every other edge (the remainder CSR of the plan) is gathered as in
  * gnn_gt_attn_fwd and merged into the same online softmax.  Same result as gnn_gt_attn_fwd up to rounding
  * (P is rounded to bf16 for the second product).  The plan must have been built with build_blocks;
- * bf16 features, head_dim == 64 only (GNN_EUNSUPPORTED otherwise); feature pointers 16-byte aligned; no workspace. */
+ * bf16 features, head_dim == 64 only (GNN_EUNSUPPORTED otherwise); feature pointers 32-byte aligned; no workspace. */
 gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
                                    const void* q, const void* k, const void* v, int32_t heads, int32_t head_dim,
                                    gnn_dtype_t dtype, void* out, float* lse, gnn_stream_t stream);

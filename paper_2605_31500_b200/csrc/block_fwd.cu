@@ -28,6 +28,9 @@
 namespace gnn {
 namespace {
 
+#ifndef GNN_BLOCK_PREFETCH
+#define GNN_BLOCK_PREFETCH 0
+#endif
 constexpr int kTile = 128;  // destination rows per CTA = MMA M = TMEM lanes
 constexpr int kTS = 68;     // floats per row slot of the transpose buffer (64 + m, l, lx + pad): 272 B
 
@@ -163,22 +166,22 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     }
 
     for (int h = 0; h < H; ++h) {
-        // ---- stage Q, K (K-major) and V (MN-major) for this head
-        for (int idx = tid; idx < kTile * CPR; idx += kTile) {
-            int r, kc;
-            stage_rc(idx, r, kc);
-            uint4 a = make_uint4(0, 0, 0, 0), b = a, c = a;
-            if (row0 + r < n) {
-                const size_t off = (size_t)(row0 + r) * rowe + (size_t)h * D + kc * 8;
-                a = __ldg(reinterpret_cast<const uint4*>(q + off));
-                b = __ldg(reinterpret_cast<const uint4*>(k + off));
-                c = __ldg(reinterpret_cast<const uint4*>(v + off));
+        // ---- stage Q, K (K-major) and V (MN-major) for this head: 256-bit loads (two 16-byte chunks of a row per
+        // lane; a warp covers 8 rows x 128 bytes = whole lines), two conflict-free 16-byte shared stores each
+        for (int idx = tid; idx < kTile * (CPR / 2); idx += kTile) {
+            const int r = (idx & 7) + 8 * (idx / (8 * (CPR / 2)));
+            const int kc = 2 * ((idx >> 3) % (CPR / 2));
+            const bool pr = row0 + r < n;
+            const size_t off = (size_t)(pr ? row0 + r : 0) * rowe + (size_t)h * D + kc * 8;
+            const Raw<32> a = ldg_raw<32>(q + off, pr), b = ldg_raw<32>(k + off, pr), c = ldg_raw<32>(v + off, pr);
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                *reinterpret_cast<uint4*>(sQ + canon(r, (kc + t) * 8, SBO_QK)) = make_uint4(a.w[4 * t], a.w[4 * t + 1], a.w[4 * t + 2], a.w[4 * t + 3]);
+                *reinterpret_cast<uint4*>(sK + canon(r, (kc + t) * 8, SBO_QK)) = make_uint4(b.w[4 * t], b.w[4 * t + 1], b.w[4 * t + 2], b.w[4 * t + 3]);
+                *reinterpret_cast<uint4*>(sV + (r & 7) * 16 + (kc + t) * 128 + (r >> 3) * LBO_V) = make_uint4(c.w[4 * t], c.w[4 * t + 1], c.w[4 * t + 2], c.w[4 * t + 3]);
             }
-            *reinterpret_cast<uint4*>(sQ + canon(r, kc * 8, SBO_QK)) = a;
-            *reinterpret_cast<uint4*>(sK + canon(r, kc * 8, SBO_QK)) = b;
-            *reinterpret_cast<uint4*>(sV + (r & 7) * 16 + kc * 128 + (r >> 3) * LBO_V) = c;
         }
-        if (h + 1 < H) prefetch_head(h + 1);
+        if (GNN_BLOCK_PREFETCH && h + 1 < H) prefetch_head(h + 1);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
@@ -390,8 +393,8 @@ extern "C" gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* P, const int32_t
     }
     if (!P->blk_bitmap) { set_error("%s: plan was built without build_blocks", who); return GNN_EINVAL; }
     if (!q || !k || !v || !out || !lse) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
-    if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) != 0) {
-        set_error("%s: feature pointers must be 16-byte aligned", who);
+    if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 31) != 0) {
+        set_error("%s: feature pointers must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
     if (dtype != GNN_BF16 || head_dim != 64 || heads < 1) {
