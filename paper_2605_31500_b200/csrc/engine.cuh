@@ -242,26 +242,44 @@ template <int CH> __device__ __forceinline__ void load_f32(const float* base, si
         o[i] = r.x; o[i + 1] = r.y; o[i + 2] = r.z; o[i + 3] = r.w;
     }
 }
+// 256-bit store (STG.E.256, sm_100): halves the L1 wavefronts of the row-strided output / gradient stores
+__device__ __forceinline__ void stg256(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t e, uint32_t f,
+                                       uint32_t g, uint32_t h) {
+    asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(a), "r"(b), "r"(c), "r"(d), "r"(e),
+                 "r"(f), "r"(g), "r"(h) : "memory");
+}
 template <int CH> __device__ __forceinline__ void store_f32(float* base, size_t elt, const float (&v)[CH]) {
+    if constexpr (CH % 8 == 0) {
 #pragma unroll
-    for (int i = 0; i < CH; i += 4)
-        *reinterpret_cast<float4*>(base + elt + i) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+        for (int i = 0; i < CH; i += 8)
+            stg256(base + elt + i, __float_as_uint(v[i]), __float_as_uint(v[i + 1]), __float_as_uint(v[i + 2]),
+                   __float_as_uint(v[i + 3]), __float_as_uint(v[i + 4]), __float_as_uint(v[i + 5]),
+                   __float_as_uint(v[i + 6]), __float_as_uint(v[i + 7]));
+    } else {
+#pragma unroll
+        for (int i = 0; i < CH; i += 4)
+            *reinterpret_cast<float4*>(base + elt + i) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+    }
 }
 // store CH values in the feature dtype (bf16: round-to-nearest-even)
 template <int CH> __device__ __forceinline__ void store_feat(float* base, size_t elt, const float (&v)[CH]) {
     store_f32<CH>(base, elt, v);
 }
 template <int CH> __device__ __forceinline__ void store_feat(__nv_bfloat16* base, size_t elt, const float (&v)[CH]) {
+    uint32_t w[CH / 2];
 #pragma unroll
-    for (int i = 0; i < CH; i += 8) {
-        uint4 r;
-        uint32_t* w = reinterpret_cast<uint32_t*>(&r);
+    for (int j = 0; j < CH / 2; ++j) {
+        __nv_bfloat162 b = __floats2bfloat162_rn(v[2 * j], v[2 * j + 1]);
+        w[j] = *reinterpret_cast<uint32_t*>(&b);
+    }
+    if constexpr (CH % 16 == 0) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            __nv_bfloat162 b = __floats2bfloat162_rn(v[i + 2 * j], v[i + 2 * j + 1]);
-            w[j] = *reinterpret_cast<uint32_t*>(&b);
-        }
-        *reinterpret_cast<uint4*>(base + elt + i) = r;
+        for (int i = 0; i < CH / 2; i += 8)
+            stg256(base + elt + 2 * i, w[i], w[i + 1], w[i + 2], w[i + 3], w[i + 4], w[i + 5], w[i + 6], w[i + 7]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < CH / 2; i += 4)
+            *reinterpret_cast<uint4*>(base + elt + 2 * i) = make_uint4(w[i], w[i + 1], w[i + 2], w[i + 3]);
     }
 }
 
