@@ -255,7 +255,8 @@ def run_reference(args, rank):
     if rank != 0:
         return
     c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False)
-    arm = OracleArm(c, target_seconds=min(args.cpu_seconds, 20.0))
+    # each step = one bounded sample pass; the whole run (warm-up + steps) is sized to about two minutes of oracle time
+    arm = OracleArm(c, target_seconds=min(args.cpu_seconds, 120.0 / max(args.steps + args.warmup, 1)))
     for _ in range(args.warmup):
         arm.run()
     t0 = time.perf_counter()
