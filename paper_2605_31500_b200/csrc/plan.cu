@@ -146,10 +146,12 @@ struct Layout {
     long long max_chunks, max_hub;
 };
 
-// defaults: warp_max_deg 1024 on large graphs (nnz >= 2^24: enough rows in flight that long single-group rows
-// do not form a tail) and 256 on small ones; cta_max_deg 8192; split_chunk 4096
+// defaults: large graphs (nnz >= 2^24) 1024 / 8192 / 4096 - enough rows in flight that long single-group rows and
+// 4096-edge chunks do not form a tail; small graphs 256 / 1024 / 512 - heavy rows are cut finer so that the few
+// CTAs that own them do not outlast the rest of the launch (profiles/r01_lane_width_sweep.md)
 gnn_plan_opts_t resolve(const gnn_plan_opts_t* o, int64_t nnz) {
-    gnn_plan_opts_t r = {nnz >= (1ll << 24) ? 1024 : 256, 8192, 4096, 0, 0};
+    const bool big = nnz >= (1ll << 24);
+    gnn_plan_opts_t r = {big ? 1024 : 256, big ? 8192 : 1024, big ? 4096 : 512, 0, 0};
     if (o) {
         if (o->warp_max_deg > 0) r.warp_max_deg = o->warp_max_deg;
         if (o->cta_max_deg > 0) r.cta_max_deg = o->cta_max_deg;

@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
 
 SMALL_OPTS = dict(warp_max_deg=6, cta_max_deg=40, split_chunk=24)   # forces CTA rows, hubs, many chunks
 DEFAULT_OPTS = dict(warp_max_deg=0, cta_max_deg=0, split_chunk=0)
-RESOLVED_DEFAULT = dict(warp_max_deg=256, cta_max_deg=8192, split_chunk=4096)   # nnz < 2^24 in these tests
+RESOLVED_DEFAULT = dict(warp_max_deg=256, cta_max_deg=1024, split_chunk=512)   # nnz < 2^24 in these tests
 
 
 def _torch():
