@@ -56,7 +56,7 @@ typedef enum { GNN_F32 = 0, GNN_BF16 = 1 } gnn_dtype_t;
  *   warp_max_deg < deg <= cta_max  : "CTA rows"    - one CTA per row, merged in shared memory
  *   deg > cta_max_deg              : "hub rows"    - cut into ceil(deg/split_chunk) near-equal chunks,
  *                                    one CTA per chunk, partial states merged by a second pass
- * Zero in any threshold selects the default (1024 / 8192 / 4096 if nnz >= 2^24, else 256 / 1024 / 512).
+ * Zero in any threshold selects the default (4096 / 16384 / 4096 if nnz >= 2^24, else 256 / 1024 / 512).
  * build_transpose != 0 also builds CSR^T and its bins (needed by the backward calls).
  * build_blocks != 0 also builds the 16-row block layout (gnn_gt_attn_fwd_block).              */
 typedef struct {

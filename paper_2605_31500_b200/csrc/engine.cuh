@@ -17,7 +17,7 @@
 //                   edge list, states merged through shared memory (the paper's cross-warp merge,
 //                   PAPER.md:492)
 //   hub_merge_kernel                                 : combines the chunk partials of a hub row in
-//                   ascending chunk order (log-sum-exp merge for the forward, plain sums backward)
+//                   a fixed chunk order (log-sum-exp merge for the forward, plain sums backward)
 // Control flow is warp-uniform (masked edges instead of divergent trip counts) so full-mask shuffles
 // are legal everywhere.  No floating-point atomics: every output element has exactly one writer.
 #pragma once

@@ -268,10 +268,16 @@ segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowp
 }
 
 // ------------------------------------------------------------------------------------------------
-// hub rows: merge the chunk partials of hub slot blockIdx.x in ascending chunk order, finalise.
-// smem: state_floats + rowe (da) floats.
+// hub rows: merge the chunk partials of hub slot blockIdx.x in a fixed order, finalise.
+// The merge is latency-bound (one CTA walks up to nnz/split_chunk partial states), so the CTA is wide
+// (kHubThreads) and every lane keeps kHubUnroll independent loads in flight.
+// smem: state_floats + 4 + kHubWarps * (NA*rowe + NS*H) floats.
+constexpr int kHubThreads = 512;
+constexpr int kHubWarps = kHubThreads / 32;
+constexpr int kHubUnroll = 8;
+
 template <class Op>
-__global__ void __launch_bounds__(kCtaThreads)
+__global__ void __launch_bounds__(kHubThreads)
 hub_merge_kernel(typename Op::Params p, Shape sh, BinView bins, const float* __restrict__ partials, float* da_part,
                  int da_slot) {
     constexpr int G = Op::kG, CH = Op::kCH;
@@ -285,27 +291,61 @@ hub_merge_kernel(typename Op::Params p, Shape sh, BinView bins, const float* __r
     const int slot = blockIdx.x;
     const int c0 = __ldg(bins.chunk_ptr + slot), c1 = __ldg(bins.chunk_ptr + slot + 1);
     const int row = __ldg(bins.chunks + 4 * c0);
+    // fixed reduction order: chunk c goes to warp (c - c0) % W, every warp walks its chunks in ascending order
+    // into kHubUnroll round-robin partial sums per element (added as a fixed tree), then the W warp sums are
+    // added in warp order.  s_part: [W][TEp] after s_merged[TE].
+    float* s_part = s_merged + ((TE + 3) & ~3);
     if (Op::SOFTMAX) {
-        for (int h = threadIdx.x; h < sh.H; h += kCtaThreads) {
+        for (int h = warp; h < sh.H; h += kHubWarps) {
             float mg = -INFINITY;
-            for (int c = c0; c < c1; ++c) mg = fmaxf(mg, partials[(size_t)c * TE + TEp + h]);
-            s_merged[TEp + h] = mg;
+            for (int c = c0 + lane; c < c1; c += 32) mg = fmaxf(mg, partials[(size_t)c * TE + TEp + h]);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) mg = fmaxf(mg, __shfl_xor_sync(0xffffffffu, mg, o));
+            if (lane == 0) s_merged[TEp + h] = mg;
         }
         __syncthreads();
     }
-    for (int e = threadIdx.x; e < TEp; e += kCtaThreads) {
+    for (int e = lane; e < TEp; e += 32) {
         const int h = e < Op::NA * sh.rowe ? (e % sh.rowe) / sh.d : (e - Op::NA * sh.rowe) % sh.H;
-        float s = 0.f;
-        if (Op::SOFTMAX) {
-            const float mg = s_merged[TEp + h];
-            for (int c = c0; c < c1; ++c) {
-                const float mc = partials[(size_t)c * TE + TEp + h];
-                const float f = (mc == -INFINITY) ? 0.f : ex2(mc - mg);
-                s += partials[(size_t)c * TE + e] * f;
+        const float mg = Op::SOFTMAX ? s_merged[TEp + h] : 0.f;
+        float su[kHubUnroll];
+#pragma unroll
+        for (int u = 0; u < kHubUnroll; ++u) su[u] = 0.f;
+        int c = c0 + warp;
+        for (; c + (kHubUnroll - 1) * kHubWarps < c1; c += kHubUnroll * kHubWarps) {
+            float v[kHubUnroll], mc[kHubUnroll];
+#pragma unroll
+            for (int u = 0; u < kHubUnroll; ++u) {
+                const size_t cc = (size_t)(c + u * kHubWarps) * TE;
+                v[u] = partials[cc + e];
+                mc[u] = Op::SOFTMAX ? partials[cc + TEp + h] : 0.f;
             }
-        } else {
-            for (int c = c0; c < c1; ++c) s += partials[(size_t)c * TE + e];
+#pragma unroll
+            for (int u = 0; u < kHubUnroll; ++u) {
+                const float f = !Op::SOFTMAX ? 1.f : (mc[u] == -INFINITY) ? 0.f : ex2(mc[u] - mg);
+                su[u] = fmaf(v[u], f, su[u]);
+            }
         }
+#pragma unroll
+        for (int u = 0; u < kHubUnroll; ++u) {
+            const int cu = c + u * kHubWarps;
+            if (cu < c1) {
+                const size_t cc = (size_t)cu * TE;
+                float f = 1.f;
+                if (Op::SOFTMAX) {
+                    const float mc = partials[cc + TEp + h];
+                    f = (mc == -INFINITY) ? 0.f : ex2(mc - mg);
+                }
+                su[u] = fmaf(partials[cc + e], f, su[u]);
+            }
+        }
+        s_part[warp * TEp + e] = ((su[0] + su[1]) + (su[2] + su[3])) + ((su[4] + su[5]) + (su[6] + su[7]));
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < TEp; e += kHubThreads) {
+        float s = 0.f;
+#pragma unroll
+        for (int w = 0; w < kHubWarps; ++w) s += s_part[w * TEp + e];
         s_merged[e] = s;
     }
     __syncthreads();
@@ -385,9 +425,13 @@ template <class Op> inline cudaError_t run_op(const typename Op::Params& p, cons
     }
     slot += gp.grp_grid;
     if (gp.hub_grid > 0) {
-        const size_t smem = 4 * (size_t)state_floats<Op>(sh) + 16;
+        const size_t smem = 4 * ((size_t)state_floats<Op>(sh) + 4 + (size_t)kHubWarps * (Op::NA * sh.rowe + Op::NS * sh.H)) + 16;
+        if (smem > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(hub_merge_kernel<Op>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
         prof_begin(Op::kName, "hub_merge", c.stream);
-        hub_merge_kernel<Op><<<gp.hub_grid, kCtaThreads, smem, c.stream>>>(p, sh, b, c.partials, c.da_part, slot);
+        hub_merge_kernel<Op><<<gp.hub_grid, kHubThreads, smem, c.stream>>>(p, sh, b, c.partials, c.da_part, slot);
         prof_end(c.stream);
         ++g_launches;
     }

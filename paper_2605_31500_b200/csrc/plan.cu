@@ -146,12 +146,12 @@ struct Layout {
     long long max_chunks, max_hub;
 };
 
-// defaults: large graphs (nnz >= 2^24) 1024 / 8192 / 4096 - enough rows in flight that long single-group rows and
+// defaults: large graphs (nnz >= 2^24) 4096 / 16384 / 4096 - enough rows in flight that long single-group rows and
 // 4096-edge chunks do not form a tail; small graphs 256 / 1024 / 512 - heavy rows are cut finer so that the few
 // CTAs that own them do not outlast the rest of the launch (profiles/r01_lane_width_sweep.md)
 gnn_plan_opts_t resolve(const gnn_plan_opts_t* o, int64_t nnz) {
     const bool big = nnz >= (1ll << 24);
-    gnn_plan_opts_t r = {big ? 1024 : 256, big ? 8192 : 1024, big ? 4096 : 512, 0, 0};
+    gnn_plan_opts_t r = {big ? 4096 : 256, big ? 16384 : 1024, big ? 4096 : 512, 0, 0};
     if (o) {
         if (o->warp_max_deg > 0) r.warp_max_deg = o->warp_max_deg;
         if (o->cta_max_deg > 0) r.cta_max_deg = o->cta_max_deg;

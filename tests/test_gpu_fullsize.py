@@ -136,4 +136,4 @@ def test_fullsize_sampled_parity(cfg):
 
 def _resolved_opts(nnz):
     """the library's default thresholds (include/gnn_attn.h)"""
-    return (1024, 8192, 4096) if nnz >= (1 << 24) else (256, 1024, 512)
+    return (4096, 16384, 4096) if nnz >= (1 << 24) else (256, 1024, 512)
