@@ -16,10 +16,15 @@
 // log-sum-exp and store O coalesced - so the result equals the plain CSR forward.  Per-thread row-wise
 // gathers and stores (32 L1 wavefronts per instruction) made the first version LSU-bound; this layout needs 4.
 //
-// Operand staging: Q, K (K-major) and V (MN-major, no transpose) are written by the CTA's threads into the canonical
-// no-swizzle core-matrix layout (8 x 16-byte core matrices; LBO / SBO = byte distance between core matrices along
-// K / along M,N) and described to the tensor core by 64-bit shared-memory matrix descriptors; completion is
-// signalled with tcgen05.commit on an mbarrier.  48 KB of shared memory and 128 TMEM columns per CTA: 3 CTAs/SM.
+// Operand staging: the head slices of Q, K (K-major operands) and V (MN-major B operand, no transpose) of the 128
+// tile rows are 128 x 128-byte boxes of the [n, H*d] tensors: one elected thread fetches them with three TMA tile
+// loads (cp.async.bulk.tensor.2d, 128-byte swizzle, rows past n zero-filled) that complete on an mbarrier, kStages
+// heads ahead of the consumers; the tensor core reads them through 64-bit shared-memory matrix descriptors
+// (SWIZZLE_128B: 8-row groups 1024 bytes apart).  P is written by the threads in the canonical no-swizzle
+// core-matrix layout (8 x 16-byte core matrices; LBO / SBO = byte distance between core matrices along K / along M).
+// MMA completion is signalled with tcgen05.commit on an mbarrier.  48 KB of shared memory per stage and 128 TMEM
+// columns per CTA.
+#include <cuda.h>
 #include <cuda_bf16.h>
 
 #include "internal.h"
@@ -28,9 +33,10 @@
 namespace gnn {
 namespace {
 
-#ifndef GNN_BLOCK_PREFETCH
-#define GNN_BLOCK_PREFETCH 0
+#ifndef GNN_BLOCK_STAGES
+#define GNN_BLOCK_STAGES 1
 #endif
+constexpr int kStages = GNN_BLOCK_STAGES;   // heads of Q/K/V in flight per CTA (1: 3 CTAs/SM, 2: 2 CTAs/SM)
 constexpr int kTile = 128;  // destination rows per CTA = MMA M = TMEM lanes
 constexpr int kTS = 68;     // floats per row slot of the transpose buffer (64 + m, l, lx + pad): 272 B
 
@@ -40,6 +46,11 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)_
 __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
     return (uint64_t)((saddr >> 4) & 0x3fff) | ((uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16) |
            ((uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32) | (1ull << 46);
+}
+// same, SWIZZLE_128B (layout type 2 in bits 61-63): rows of 128 bytes, 8-row groups sbo_bytes apart
+__device__ __forceinline__ uint64_t make_desc_sw128(uint32_t saddr, uint32_t sbo_bytes) {
+    return (uint64_t)((saddr >> 4) & 0x3fff) | (1ull << 16) | ((uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32) | (1ull << 46) |
+           (2ull << 61);
 }
 // instruction descriptor: kind::f16, A = bf16 K-major, B = bf16 K-major or MN-major, D = fp32, M x N
 __host__ __device__ constexpr uint32_t make_idesc(int M, int N, bool b_mn_major) {
@@ -62,6 +73,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     asm volatile("{\n .reg .pred p;\n W_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
                  " @p bra D_%=;\n bra W_%=;\n D_%=:\n}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// TMA: one 2-D box of the tensor map at element coordinates (c0, c1) into shared memory, completing on `bar`
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
     uint32_t r[32];
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -83,23 +102,23 @@ __device__ __forceinline__ uint32_t canon(int r, int k, int sbo) {
 }
 
 template <int D>
-__global__ void __launch_bounds__(kTile, 3)
-gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ k,
-                    const __nv_bfloat16* __restrict__ v, __nv_bfloat16* __restrict__ out, float* __restrict__ lse,
-                    const uint16_t* __restrict__ bitmap, const int32_t* __restrict__ rem_rowptr,
-                    const int32_t* __restrict__ rem_colidx, int n, int H, float sscale) {
-    constexpr int SBO_QK = (D / 8) * 128, SBO_P = (kTile / 8) * 128;
-    constexpr int LBO_V = (D / 8) * 128;   // V stays [source j][channel c] = MN-major B operand: 8x8 core matrices,
-                                           // channel groups 128 B apart (SBO), source groups LBO_V apart
-    constexpr int kBytesQK = kTile * D * 2, kBytesP = kTile * kTile * 2;
+__global__ void __launch_bounds__(kTile, kStages == 1 ? 3 : 2)
+gt_fwd_block_kernel(const __grid_constant__ CUtensorMap tmq, const __grid_constant__ CUtensorMap tmk,
+                    const __grid_constant__ CUtensorMap tmv, const __nv_bfloat16* __restrict__ q,
+                    const __nv_bfloat16* __restrict__ k, const __nv_bfloat16* __restrict__ v,
+                    __nv_bfloat16* __restrict__ out, float* __restrict__ lse, const uint16_t* __restrict__ bitmap,
+                    const int32_t* __restrict__ rem_rowptr, const int32_t* __restrict__ rem_colidx, int n, int H,
+                    float sscale) {
+    static_assert(D == 64, "a head slice must be one 128-byte swizzle row");
+    constexpr int SBO_P = (kTile / 8) * 128;
+    constexpr int kBytesQK = kTile * D * 2, kBytesP = kTile * kTile * 2, kStageBytes = 3 * kBytesQK;
     static_assert(kBytesP <= 2 * kBytesQK, "P aliases the Q and K staging buffers");
-    constexpr int CPR = D / 8;  // 16-byte chunks per row slice
-    extern __shared__ __align__(1024) uint8_t smem[];
-    uint8_t* sQ = smem;
-    uint8_t* sK = sQ + kBytesQK;
-    uint8_t* sP = smem;                      // P overwrites Q and K once S = Q K^T has completed
-    uint8_t* sV = smem + 2 * kBytesQK;
-    uint64_t* bar = reinterpret_cast<uint64_t*>(sV + kBytesQK);
+    static_assert(kTile * kTS * 4 <= kStageBytes, "the transpose buffer aliases one stage");
+    extern __shared__ uint8_t smem_raw[];
+    // 128-byte swizzle atoms (8 rows x 128 bytes) must sit on 1024-byte boundaries
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + kStages * kStageBytes);   // TMA completion, one per stage
+    uint64_t* bar = full + kStages;                                               // tcgen05.commit
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bar + 1);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -108,9 +127,21 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     const size_t rowe = (size_t)H * D;
 
     // ---- one-time setup: barrier, TMEM (128 columns: S, later overwritten by O)
+    // one head's Q, K, V boxes into stage hh % kStages (rows past n arrive as zeros and count as full bytes)
+    auto issue_head = [&](int hh) {
+        uint8_t* st = smem + (hh % kStages) * kStageBytes;
+        uint64_t* fb = full + (hh % kStages);
+        mbar_expect_tx(fb, 3 * kBytesQK);
+        tma_load_2d(st, &tmq, hh * D, row0, fb);
+        tma_load_2d(st + kBytesQK, &tmk, hh * D, row0, fb);
+        tma_load_2d(st + 2 * kBytesQK, &tmv, hh * D, row0, fb);
+    };
     if (tid == 0) {
         mbar_init(bar, 1);
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) mbar_init(full + s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        for (int hh = 0; hh < kStages - 1 && hh < H; ++hh) issue_head(hh);
     }
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" ::"r"(smem_u32(tmem_slot)) : "memory");
@@ -128,29 +159,6 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     const int wl = tid >> 4;  // window of this row inside the tile
     constexpr uint32_t kIdescS = make_idesc(kTile, kTile, false), kIdescO = make_idesc(kTile, D, true);
 
-    // staging map: a warp covers 8 rows x 4 chunks per step, so its 16-byte shared stores fill whole 128-byte
-    // core matrices (conflict-free) while each row still reads 64 contiguous bytes from global memory
-    auto stage_rc = [&](int idx, int& r, int& kc) {
-        r = (idx & 7) + 8 * (idx / (8 * CPR));
-        kc = (idx >> 3) % CPR;
-    };
-    auto prefetch_head = [&](int h) {   // pull the next head's tile slices and remainder rows towards L2
-        {   // the head slice of a row is one (D*2)-byte line: thread t prefetches row t's three slices
-            const int r = tid;
-            if (row0 + r < n) {
-                const size_t off = (size_t)(row0 + r) * rowe + (size_t)h * D;
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(q + off));
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(k + off));
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(v + off));
-            }
-        }
-        for (int e = rb; e < re; ++e) {
-            const size_t off = (size_t)__ldg(rem_colidx + e) * rowe + (size_t)h * D;
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(k + off));
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(v + off));
-        }
-    };
-
     // cooperative role (8 lanes per row, group g4 of the warp takes rows g4 + 4 i): the remainder sources of the
     // group's 8 rows are head-invariant - the first two per row stay in registers
     const int g4 = lane >> 3, gl = lane & 7;
@@ -166,32 +174,21 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     }
 
     for (int h = 0; h < H; ++h) {
-        // ---- stage Q, K (K-major) and V (MN-major) for this head: 256-bit loads (two 16-byte chunks of a row per
-        // lane; a warp covers 8 rows x 128 bytes = whole lines), two conflict-free 16-byte shared stores each
-        for (int idx = tid; idx < kTile * (CPR / 2); idx += kTile) {
-            const int r = (idx & 7) + 8 * (idx / (8 * (CPR / 2)));
-            const int kc = 2 * ((idx >> 3) % (CPR / 2));
-            const bool pr = row0 + r < n;
-            const size_t off = (size_t)(pr ? row0 + r : 0) * rowe + (size_t)h * D + kc * 8;
-            const Raw<32> a = ldg_raw<32>(q + off, pr), b = ldg_raw<32>(k + off, pr), c = ldg_raw<32>(v + off, pr);
-#pragma unroll
-            for (int t = 0; t < 2; ++t) {
-                *reinterpret_cast<uint4*>(sQ + canon(r, (kc + t) * 8, SBO_QK)) = make_uint4(a.w[4 * t], a.w[4 * t + 1], a.w[4 * t + 2], a.w[4 * t + 3]);
-                *reinterpret_cast<uint4*>(sK + canon(r, (kc + t) * 8, SBO_QK)) = make_uint4(b.w[4 * t], b.w[4 * t + 1], b.w[4 * t + 2], b.w[4 * t + 3]);
-                *reinterpret_cast<uint4*>(sV + (r & 7) * 16 + (kc + t) * 128 + (r >> 3) * LBO_V) = make_uint4(c.w[4 * t], c.w[4 * t + 1], c.w[4 * t + 2], c.w[4 * t + 3]);
-            }
-        }
-        if (GNN_BLOCK_PREFETCH && h + 1 < H) prefetch_head(h + 1);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();
+        // ---- operands of this head: issue the TMA loads of the head kStages - 1 ahead (its stage was released by
+        // the barrier that ended the previous head), then wait for this head's boxes
+        uint8_t* sQ = smem + (h % kStages) * kStageBytes;
+        uint8_t* sK = sQ + kBytesQK;
+        uint8_t* sP = sQ;                    // P overwrites Q and K once S = Q K^T has completed
+        uint8_t* sV = sQ + 2 * kBytesQK;
+        if (tid == 0 && h + kStages - 1 < H) issue_head(h + kStages - 1);
+        mbar_wait(full + (h % kStages), (uint32_t)(h / kStages) & 1u);
         // ---- S = Q K^T on the tensor cores (one elected thread issues)
         if (tid == 0) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
             for (int s = 0; s < D / 16; ++s)
-                umma(tmem, make_desc(smem_u32(sQ) + s * 256, 128, SBO_QK), make_desc(smem_u32(sK) + s * 256, 128, SBO_QK),
-                     kIdescS, s > 0);
+                umma(tmem, make_desc_sw128(smem_u32(sQ) + s * 32, 1024), make_desc_sw128(smem_u32(sK) + s * 32, 1024),
+                     kIdescS, s > 0);   // K step = 16 channels = 32 bytes inside the 128-byte swizzle row
             umma_commit(bar);
         }
         mbar_wait(bar, phase);
@@ -237,8 +234,8 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
             for (int s = 0; s < kTile / 16; ++s)
-                umma(tmem, make_desc(smem_u32(sP) + s * 256, 128, SBO_P), make_desc(smem_u32(sV) + s * 2 * LBO_V, LBO_V, 128),
-                     kIdescO, s > 0);
+                umma(tmem, make_desc(smem_u32(sP) + s * 256, 128, SBO_P), make_desc_sw128(smem_u32(sV) + s * 2048, 1024),
+                     kIdescO, s > 0);   // V: [source][channel] rows of 128 bytes = MN-major, K step = 16 sources
             umma_commit(bar);
         }
         mbar_wait(bar, phase);
@@ -247,7 +244,7 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
         // ---- hand the block part over to the cooperative layout: thread t (owner of row t) writes its unnormalised
         // O row and (m, l, lx) into the warp's transpose buffer (aliases the dead Q/K/P/V staging area; 272-byte row
         // slots keep 16-byte accesses conflict-free)
-        float* sT = reinterpret_cast<float*>(smem) + warp * (32 * kTS);
+        float* sT = reinterpret_cast<float*>(sQ) + warp * (32 * kTS);
         {
             float* slot = sT + lane * kTS;
 #pragma unroll
@@ -372,10 +369,39 @@ gt_fwd_block_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
                 }
             }
         }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes (P, transpose) before the next TMA
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();   // smem operands and TMEM are reused by the next head
+        __syncthreads();   // this stage and TMEM are reused by a later head
     }
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" ::"r"(tmem) : "memory");
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point lookup (the library does not link libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+            qres != cudaDriverEntryPointSuccess)
+            p = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(p);
+    }();
+    return fn;
+}
+// [n, H*D] bf16 row-major tensor, boxes of kTile rows x D channels (one head slice), 128-byte swizzle, zero fill
+bool encode_head_tile_map(CUtensorMap* m, const void* base, int n, int H, int D) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return false;
+    const cuuint64_t gdim[2] = {(cuuint64_t)H * D, (cuuint64_t)n};
+    const cuuint64_t gstride[1] = {(cuuint64_t)H * D * 2};
+    const cuuint32_t box[2] = {(cuuint32_t)D, (cuuint32_t)kTile};
+    const cuuint32_t estr[2] = {1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstride, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 }  // namespace
@@ -402,13 +428,20 @@ extern "C" gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* P, const int32_t
         return GNN_EUNSUPPORTED;
     }
     constexpr int D = 64;
-    const size_t smem = 3 * (size_t)kTile * D * 2 + 64;   // Q, K (aliased by P), V, barrier, TMEM slot
+    CUtensorMap tmq, tmk, tmv;
+    if (!encode_head_tile_map(&tmq, q, n, heads, D) || !encode_head_tile_map(&tmk, k, n, heads, D) ||
+        !encode_head_tile_map(&tmv, v, n, heads, D)) {
+        set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who);
+        return GNN_ECUDA;
+    }
+    // kStages x (Q, K (aliased by P), V), barriers, TMEM slot, slack for the 1024-byte alignment
+    const size_t smem = (size_t)kStages * 3 * kTile * D * 2 + 64 + 1024;
     cudaError_t e = cudaFuncSetAttribute(gt_fwd_block_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) {
         const int grid = (n + kTile - 1) / kTile;
         prof_begin("gt_fwd_block", "tile", (cudaStream_t)stream);
         gt_fwd_block_kernel<D><<<grid, kTile, smem, (cudaStream_t)stream>>>(
-            (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, (__nv_bfloat16*)out, lse, P->blk_bitmap,
+            tmq, tmk, tmv, (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, (__nv_bfloat16*)out, lse, P->blk_bitmap,
             P->blk_rem_rowptr, P->blk_rem_colidx, n, heads, kLog2e / sqrtf((float)D));
         prof_end((cudaStream_t)stream);
         ++g_launches;
