@@ -36,6 +36,9 @@ namespace {
 #ifndef GNN_BLOCK_STAGES
 #define GNN_BLOCK_STAGES 1
 #endif
+#ifndef GNN_BLOCK_MINB
+#define GNN_BLOCK_MINB 3
+#endif
 constexpr int kStages = GNN_BLOCK_STAGES;   // heads of Q/K/V in flight per CTA (1: 3 CTAs/SM, 2: 2 CTAs/SM)
 constexpr int kTile = 128;  // destination rows per CTA = MMA M = TMEM lanes
 constexpr int kTS = 68;     // floats per row slot of the transpose buffer (64 + m, l, lx + pad): 272 B
@@ -102,7 +105,7 @@ __device__ __forceinline__ uint32_t canon(int r, int k, int sbo) {
 }
 
 template <int D>
-__global__ void __launch_bounds__(kTile, kStages == 1 ? 3 : 2)
+__global__ void __launch_bounds__(kTile, kStages == 1 ? GNN_BLOCK_MINB : 2)
 gt_fwd_block_kernel(const __grid_constant__ CUtensorMap tmq, const __grid_constant__ CUtensorMap tmk,
                     const __grid_constant__ CUtensorMap tmv, const __nv_bfloat16* __restrict__ q,
                     const __nv_bfloat16* __restrict__ k, const __nv_bfloat16* __restrict__ v,
