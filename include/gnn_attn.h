@@ -147,7 +147,8 @@ gnn_status_t gnn_gt_attn_bwd(const gnn_plan_t* plan, const int32_t* rowptr, cons
 
 /* GATv2 attention, forward:
  *   s_ij = sum_c a[h,c] LeakyReLU_slope(xl[i,h,c] + xr[j,h,c]);  softmax / lse / out as above with
- *   value xr[j,h,:].  xl, xr: [n,H,d] `dtype`, in.  a: [H,d] fp32, in.  out, lse: as gnn_gt_attn_fwd. */
+ *   value xr[j,h,:].  xl, xr: [n,H,d] `dtype`, in.  a: [H,d] fp32, in.  out, lse: as gnn_gt_attn_fwd.
+ *   slope: finite and >= 0 (GNN_EINVAL otherwise; same for gnn_gatv2_bwd).                            */
 gnn_status_t gnn_gatv2_fwd(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
                            const void* xl, const void* xr, const float* a, int32_t heads, int32_t head_dim,
                            gnn_dtype_t dtype, float slope, void* out, float* lse, void* ws, size_t ws_bytes,

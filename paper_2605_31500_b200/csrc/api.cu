@@ -220,6 +220,7 @@ extern "C" gnn_status_t gnn_gatv2_fwd(const gnn_plan_t* P, const int32_t* rowptr
     const char* who = "gnn_gatv2_fwd";
     if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
     if (!xl || !xr || !a_ || !out || !lse || !ws) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
+    if (!(slope >= 0.f) || !(slope < INFINITY)) { set_error("%s: LeakyReLU slope must be finite and >= 0", who); return GNN_EINVAL; }
     if (!aligned16(xl) || !aligned16(xr) || !aligned16(a_) || !aligned16(out) || !aligned16(ws)) {
         set_error("%s: feature pointers, a and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
@@ -245,6 +246,7 @@ extern "C" gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* P, const int32_t* rowptr
         set_error("%s: NULL pointer argument", who);
         return GNN_EINVAL;
     }
+    if (!(slope >= 0.f) || !(slope < INFINITY)) { set_error("%s: LeakyReLU slope must be finite and >= 0", who); return GNN_EINVAL; }
     if (!aligned16(xl) || !aligned16(xr) || !aligned16(a_) || !aligned16(dout) || !aligned16(dxl) || !aligned16(dxr) ||
         !aligned16(ws)) {
         set_error("%s: feature/gradient pointers, a and workspace must be 32-byte aligned", who);

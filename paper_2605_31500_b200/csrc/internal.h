@@ -31,7 +31,7 @@ namespace gnn {
 enum Pass { kGtFwd = 0, kGtBwdDst, kGtBwdSrc, kGatFwd, kGatBwdDst, kGatBwdSrc, kNumPass };
 struct PassInfo { int na, ns, softmax, has_da; };
 // must match the NA / NS / SOFTMAX / HAS_DA constants of the Op structs (static_asserted in the dispatch units)
-constexpr PassInfo kPassInfo[kNumPass] = {{1, 1, 1, 0}, {2, 1, 0, 0}, {2, 0, 0, 0}, {1, 1, 1, 0}, {2, 1, 0, 1}, {2, 0, 0, 1}};
+constexpr PassInfo kPassInfo[kNumPass] = {{1, 1, 1, 0}, {2, 1, 0, 0}, {2, 0, 0, 0}, {1, 1, 1, 0}, {2, 2, 0, 1}, {2, 1, 0, 1}};
 
 inline int pass_state_floats(Pass p, const Shape& sh) {
     return kPassInfo[p].na * sh.rowe + (kPassInfo[p].ns + kPassInfo[p].softmax) * sh.H;

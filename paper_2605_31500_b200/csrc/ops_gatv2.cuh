@@ -5,7 +5,17 @@
 
 namespace gnn {
 
-__device__ __forceinline__ float lrelu(float z, float slope) { return fmaxf(z, 0.f) + slope * fminf(z, 0.f); }
+// LeakyReLU(z) = c1 z + c2 |z| with c1 = (1 + slope) / 2, c2 = (1 - slope) / 2, so with a' = a c1 and k = c2 / c1
+// (|k| <= 1 for slope >= 0, which the entry points require)
+//   sum_c a_c LeakyReLU(z_c) = sum_c a'_c (z_c + k |z_c|):
+// two FFMAs per channel (|z| is an operand modifier) instead of max, min and two FFMAs.
+struct LreluK {
+    float c1, k;
+    __device__ __forceinline__ explicit LreluK(float slope) : c1(0.5f * (1.f + slope)), k((1.f - slope) / (1.f + slope)) {}
+};
+__device__ __forceinline__ float lrelu_dot_step(float a1, float z, float k, float acc) {
+    return fmaf(a1, fmaf(k, fabsf(z), z), acc);
+}
 
 // ------------------------------------------------------------------------------------ GATv2 forward
 template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G_, KU_, 1, 0> {
@@ -27,7 +37,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G
         float* lse;
         float slope;
     };
-    struct Own { float xl[CH], a[CH]; };  // a pre-multiplied by log2(e)
+    struct Own { float xl[CH], a[CH], k; };  // a pre-multiplied by log2(e) (1 + slope) / 2, k = (1 - slope) / (1 + slope)
 
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
@@ -35,8 +45,10 @@ template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G
         c.load_global(p.xl, (size_t)row * sh.rowe + g.eoff, valid && g.act);
         c.to_float(o.xl);
         load_f32<CH>(p.a, g.eoff, g.act, o.a);
+        const LreluK lk(p.slope);
+        o.k = lk.k;
 #pragma unroll
-        for (int i = 0; i < CH; ++i) o.a[i] *= kLog2e;
+        for (int i = 0; i < CH; ++i) o.a[i] *= kLog2e * lk.c1;
     }
     __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
                                                   Src& src) {
@@ -55,8 +67,8 @@ template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G
             float a0 = 0.f, a1 = 0.f;
 #pragma unroll
             for (int c = 0; c < CH; c += 2) {
-                a0 = fmaf(o.a[c], lrelu(z[c], p.slope), a0);
-                a1 = fmaf(o.a[c + 1], lrelu(z[c + 1], p.slope), a1);
+                a0 = lrelu_dot_step(o.a[c], z[c], o.k, a0);
+                a1 = lrelu_dot_step(o.a[c + 1], z[c + 1], o.k, a1);
             }
             s[u] = a0 + a1;
         }
@@ -94,6 +106,8 @@ template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G
 // so the attention-vector gradient needs no accumulators of its own: each pass adds (own row) . (its s'-weighted
 // sum) to the per-lane da partial.  One sweep over the row (G_i is only known at its end):
 //   A = sum w s', B = sum alpha s', G = sum w  with w = alpha dP;  S_i = A - G B.
+// s' takes two values, so A = slope G + (1 - slope) A+ with A+ = sum over {z > 0} of w (likewise B from B+ and
+// sum alpha): the sweep keeps A+, B+ per channel (a compare and two predicated adds) and G, sum alpha per head.
 template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_, G_, KU_, 1, 0> {
     static constexpr const char* kName = "gatv2_bwd_dst";
     static constexpr int kMinBlocks = GNN_GAT_DST_MINB;  // resident CTAs per SM the register budget is held to
@@ -103,7 +117,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
     using typename B::Ck;
     using typename B::Src;
     static constexpr int CH = B::kCH, KU = KU_;
-    static constexpr int NA = 2, NS = 1;
+    static constexpr int NA = 2, NS = 2;
     static constexpr bool SOFTMAX = false, HAS_DA = true;
     using St = State<NA, NS, CH>;
     struct Params {
@@ -112,7 +126,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
         float *dxl, *g;
         float slope;
     };
-    struct Own { float xl[CH], a[CH], lp; Ck go; };
+    struct Own { float xl[CH], a[CH], lp, k; Ck go; };  // a pre-multiplied by log2(e) (1 + slope) / 2
 
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
@@ -122,6 +136,10 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
         c0.to_float(o.xl);
         o.go.load_global(p.dout, (size_t)row * sh.rowe + g.eoff, pr);
         load_f32<CH>(p.a, g.eoff, g.act, o.a);
+        const LreluK lk(p.slope);
+        o.k = lk.k;
+#pragma unroll
+        for (int i = 0; i < CH; ++i) o.a[i] *= kLog2e * lk.c1;
         o.lp = pr ? __ldg(p.lse + (size_t)row * sh.H + g.hd) * kLog2e : 0.f;
     }
     __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
@@ -140,31 +158,33 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
             add_chunk(xc, o.xl, z);
             float a0 = 0.f;
 #pragma unroll
-            for (int c = 0; c < CH; ++c) a0 = fmaf(o.a[c], lrelu(z[c], p.slope), a0);
+            for (int c = 0; c < CH; ++c) a0 = lrelu_dot_step(o.a[c], z[c], o.k, a0);
             r[2 * u] = a0;
             r[2 * u + 1] = dot(o.go, xc);
         }
         head_reduce(r, g.lpl);
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] * kLog2e - o.lp);
+            const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] - o.lp);
             const float w = alpha * r[2 * u + 1];
-            const float ws = w * p.slope, as = alpha * p.slope;
             const Ck& xc = src.c[u][0];
             float z[CH];
             add_chunk(xc, o.xl, z);
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-                const bool pos = z[c] > 0.f;
-                st.acc[0][c] += pos ? w : ws;
-                st.acc[1][c] += pos ? alpha : as;
+                if (z[c] > 0.f) {
+                    st.acc[0][c] += w;
+                    st.acc[1][c] += alpha;
+                }
             }
             st.sc[0] += w;
+            st.sc[1] += alpha;
         }
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
                                                     const GeoT& g, float (&da)[CH]) {
-        const float gg = st.sc[0];
+        const float gg = st.sc[0], om = 1.f - p.slope;
+        const float gs = p.slope * gg, as = p.slope * st.sc[1];
         float xl[CH], a[CH], o[CH];
         Ck c0;
         c0.load_global(p.xl, (size_t)row * sh.rowe + g.eoff, g.act);
@@ -172,7 +192,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
         load_f32<CH>(p.a, g.eoff, g.act, a);
 #pragma unroll
         for (int c = 0; c < CH; ++c) {
-            const float sdash = st.acc[0][c] - gg * st.acc[1][c];   // S_i
+            const float sdash = fmaf(om, st.acc[0][c], gs) - gg * fmaf(om, st.acc[1][c], as);   // S_i = A - G B
             o[c] = a[c] * sdash;
             da[c] = fmaf(xl[c], sdash, da[c]);
         }
@@ -193,7 +213,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
     using typename B::Ck;
     using typename B::Src;
     static constexpr int CH = B::kCH, KU = KU_;
-    static constexpr int NA = 2, NS = 0;
+    static constexpr int NA = 2, NS = 1;   // acc[1] = U+ (sum of de over {z > 0}), sc[0] = sum of de: U = slope sc + (1 - slope) U+
     static constexpr bool SOFTMAX = false, HAS_DA = true;
     using St = State<NA, NS, CH>;
     struct Params {
@@ -202,13 +222,17 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
         float* dxr;
         float slope;
     };
-    struct Own { Ck xr; float xrf[CH], a[CH]; };
+    struct Own { Ck xr; float xrf[CH], a[CH], k; };  // a pre-multiplied by log2(e) (1 + slope) / 2
 
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
         o.xr.load_global(p.xr, (size_t)row * sh.rowe + g.eoff, valid && g.act);
         o.xr.to_float(o.xrf);
         load_f32<CH>(p.a, g.eoff, g.act, o.a);
+        const LreluK lk(p.slope);
+        o.k = lk.k;
+#pragma unroll
+        for (int i = 0; i < CH; ++i) o.a[i] *= kLog2e * lk.c1;
     }
     __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
                                                   Src& src) {
@@ -232,7 +256,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
             add_chunk(lc, o.xrf, z);
             float a0 = 0.f;
 #pragma unroll
-            for (int c = 0; c < CH; ++c) a0 = fmaf(o.a[c], lrelu(z[c], p.slope), a0);
+            for (int c = 0; c < CH; ++c) a0 = lrelu_dot_step(o.a[c], z[c], o.k, a0);
             r[2 * u] = a0;
             r[2 * u + 1] = dot(gc, o.xr);
         }
@@ -240,17 +264,17 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
             const float li = src.s[u][0], gi = src.s[u][1];
-            const float alpha = nbr[u] < 0 ? 0.f : ex2((r[2 * u] - li) * kLog2e);
+            const float alpha = nbr[u] < 0 ? 0.f : ex2(fmaf(-li, kLog2e, r[2 * u]));
             const float de = alpha * (r[2 * u + 1] - gi);
-            const float des = de * p.slope;
             const Ck &lc = src.c[u][0], &gc = src.c[u][1];
             float z[CH];
             add_chunk(lc, o.xrf, z);
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
                 st.acc[0][c] = fmaf(alpha, gc.get(c), st.acc[0][c]);
-                st.acc[1][c] += z[c] > 0.f ? de : des;
+                if (z[c] > 0.f) st.acc[1][c] += de;
             }
+            st.sc[0] += de;
         }
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
@@ -261,9 +285,12 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
         c0.to_float(xr);
         load_f32<CH>(p.a, g.eoff, g.act, a);
 #pragma unroll
+        const float om = 1.f - p.slope, ds = p.slope * st.sc[0];
+#pragma unroll
         for (int c = 0; c < CH; ++c) {
-            o[c] = fmaf(a[c], st.acc[1][c], st.acc[0][c]);
-            da[c] = fmaf(xr[c], st.acc[1][c], da[c]);
+            const float u = fmaf(om, st.acc[1][c], ds);   // U_j
+            o[c] = fmaf(a[c], u, st.acc[0][c]);
+            da[c] = fmaf(xr[c], u, da[c]);
         }
         if (g.act) store_f32<CH>(p.dxr, (size_t)row * sh.rowe + g.eoff, o);
     }
