@@ -45,7 +45,7 @@ namespace gnn {
 #define GNN_GAT_DST_MINB 3
 #endif
 #ifndef GNN_GAT_SRC_MINB
-#define GNN_GAT_SRC_MINB 3
+#define GNN_GAT_SRC_MINB 4
 #endif
 constexpr int kCtaThreads = 128;
 constexpr int kWarpsPerCta = kCtaThreads / 32;

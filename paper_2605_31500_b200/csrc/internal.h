@@ -50,7 +50,7 @@ constexpr int pass_inst_max_cb(Pass) { return 32; }
 #define GNN_FWD_KU 4
 #endif
 #ifndef GNN_GAT_DST_KU
-#define GNN_GAT_DST_KU 2
+#define GNN_GAT_DST_KU 4
 #endif
 #ifndef GNN_GAT_SRC_KU
 #define GNN_GAT_SRC_KU 2

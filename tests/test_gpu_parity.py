@@ -237,6 +237,30 @@ def test_errors_are_reported():
         G.gnn_gt_attn_fwd(plan, q3, q3, q3, q3, lse)
 
 
+@pytest.mark.parametrize("slope", [0.0, 1.0, 1.5])
+def test_gatv2_slopes(slope):
+    """The kernels evaluate LeakyReLU as c1 z + c2 |z| and LeakyReLU' through {z > 0} sums: check the ends of the slope
+    range (ReLU, identity) and a slope above 1 against the oracle, with bins small enough that CTA rows and hub
+    chunk merges carry the extra per-head totals; a negative slope is rejected."""
+    import paper_2605_31500_b200 as G
+    c = dict(GI.make_config(2, scale=0.02))
+    c["slope"] = slope
+    got = run_gat(c, dict(warp_max_deg=8, cta_max_deg=32, split_chunk=16))
+    cnt = got["plan"].counts()
+    assert cnt["n_hub"] > 0 and cnt["n_cta"] > 0
+    want = oracle_gat(c)
+    if slope == 1.0:
+        # identity activation: alpha does not depend on xl, so dxl is pure cancellation (exactly 0 in exact
+        # arithmetic); a relative norm against ~1e-16 means nothing - hold it to the absolute bar instead
+        assert np.abs(got["dxl"] - want["dxl"]).max() <= 1e-4
+        got["dxl"] = want["dxl"]
+    compare_all(c, got, want)
+    if slope == 0.0:
+        with pytest.raises(G.GnnError, match="slope"):
+            c["slope"] = -0.1
+            run_gat(c, {}, backward=False)
+
+
 def test_block_layout_bit_exact():
     """Row a11: per-window 16x16 bitmaps + remainder CSR, bit-exact vs oracle/plan_ref.py, on the locally dense
     config (scaled) and on a multigraph whose size is not a multiple of 16 (duplicates go to the remainder)."""
