@@ -456,3 +456,90 @@ def test_build_blocks_vs_bruteforce():
     np.testing.assert_array_equal(b["rem_colidx"], np.concatenate([np.array(x, np.int32) for x in rem_rows]))
     # every CSR entry is accounted for exactly once
     assert int(sum(bin(int(x)).count("1") for x in bm.ravel())) + b["rem_colidx"].size == ci.size
+
+
+# --------------------------------------------------------------------------- min / max aggregation (row f3)
+from oracle import agg_ref  # noqa: E402
+
+
+@pytest.mark.parametrize("mode", ["min", "max"])
+def test_seg_minmax_vs_bruteforce(mode):
+    """Pin: the definition evaluated pair by pair with Python tuples - lexicographic (value, source id) over the
+    neighbour set, PAPER.md:462/:474 - on a multigraph with empty rows and heavy ties (values drawn from 3 levels)."""
+    rng = np.random.default_rng(5)
+    n, C = 41, 6
+    rp, ci = _rand_graph(rng, n, 4.0, multigraph=True, empty_rows=True)
+    x = rng.integers(-1, 2, size=(n, C)).astype(np.float64)          # many ties
+    x[rng.integers(0, n, 5)] *= 0.5
+    out, arg = agg_ref.seg_minmax_forward(rp, ci, x, mode)
+    sgn = 1.0 if mode == "min" else -1.0
+    for i in range(n):
+        nb = sorted(set(int(j) for j in ci[rp[i]:rp[i + 1]]))
+        for c in range(C):
+            if not nb:
+                assert out[i, c] == 0.0 and arg[i, c] == -1
+                continue
+            v, j = min((sgn * x[j, c], j) for j in nb)
+            assert out[i, c] == sgn * v and arg[i, c] == j
+
+
+def test_seg_minmax_closed_forms():
+    rng = np.random.default_rng(6)
+    n, C = 30, 4
+    rp, ci = _rand_graph(rng, n, 3.0)
+    x = rng.standard_normal((n, C))
+    # degree-1 rows return their neighbour; constant features pick the smallest neighbour id
+    rp1 = np.arange(n + 1, dtype=np.int32)
+    ci1 = rng.permutation(n).astype(np.int32)
+    out, arg = agg_ref.seg_minmax_forward(rp1, ci1, x, "min")
+    np.testing.assert_array_equal(out, x[ci1])
+    np.testing.assert_array_equal(arg, np.repeat(ci1[:, None], C, 1))
+    out, arg = agg_ref.seg_minmax_forward(rp, ci, np.ones((n, C)), "max")
+    for i in range(n):
+        assert np.all(out[i] == 1.0) and np.all(arg[i] == ci[rp[i]:rp[i + 1]].min())
+    # neighbour order and duplicate entries do not matter; max(x) = -min(-x) with the same sources
+    out0, arg0 = agg_ref.seg_minmax_forward(rp, ci, x, "min")
+    ci2 = ci.copy()
+    for i in range(n):
+        ci2[rp[i]:rp[i + 1]] = rng.permutation(ci[rp[i]:rp[i + 1]])
+    out1, arg1 = agg_ref.seg_minmax_forward(rp, ci2, x, "min")
+    np.testing.assert_array_equal(out0, out1)
+    np.testing.assert_array_equal(arg0, arg1)
+    rpd = (2 * rp.astype(np.int64)).astype(np.int32)
+    cid = np.concatenate([np.tile(ci[rp[i]:rp[i + 1]], 2) for i in range(n)]).astype(np.int32)
+    out2, arg2 = agg_ref.seg_minmax_forward(rpd, cid, x, "min")
+    np.testing.assert_array_equal(out0, out2)
+    np.testing.assert_array_equal(arg0, arg2)
+    outm, argm = agg_ref.seg_minmax_forward(rp, ci, -x, "max")
+    np.testing.assert_array_equal(outm, -out0)
+    np.testing.assert_array_equal(argm, arg0)
+    # -0.0 and +0.0 tie: the smaller source id wins
+    rpz, ciz = np.array([0, 2], np.int32), np.array([1, 0], np.int32)
+    oz, az = agg_ref.seg_minmax_forward(np.array([0, 2, 2], np.int32), ciz, np.array([[0.0], [-0.0]]), "min")
+    assert az[0, 0] == 0 and az[1, 0] == -1 and oz[1, 0] == 0.0
+    del rpz
+
+
+@pytest.mark.parametrize("mode", ["min", "max"])
+def test_seg_minmax_backward_vs_autograd(mode):
+    """Pin: gradient of the dense masked amin / amax (continuous values => no ties, so autograd's even split among
+    equal elements never triggers) equals the scatter through the saved indices."""
+    rng = np.random.default_rng(7)
+    n, C = 25, 5
+    rp, ci = _rand_graph(rng, n, 3.0, empty_rows=True)
+    x = rng.standard_normal((n, C))
+    dout = rng.standard_normal((n, C))
+    out, arg = agg_ref.seg_minmax_forward(rp, ci, x, mode)
+    dx = agg_ref.seg_minmax_backward(arg, dout, n)
+    M = torch.from_numpy(_count_matrix(rp, ci) > 0)
+    tx = torch.from_numpy(x).requires_grad_(True)
+    fill = math.inf if mode == "min" else -math.inf
+    dense = torch.where(M[:, :, None], tx[None, :, :], torch.tensor(fill, dtype=torch.float64))
+    red = dense.amin(dim=1) if mode == "min" else dense.amax(dim=1)
+    nonempty = M.any(dim=1)
+    red = torch.where(nonempty[:, None], red, torch.zeros_like(red))
+    np.testing.assert_allclose(red.detach().numpy(), out, rtol=0, atol=0)
+    red.backward(torch.from_numpy(dout))
+    np.testing.assert_allclose(tx.grad.numpy(), dx, rtol=0, atol=1e-15)
+    # gradient mass is conserved: every non-empty (i, c) sends its dout to exactly one source
+    np.testing.assert_allclose(dx.sum(0), dout[nonempty.numpy()].sum(0), rtol=0, atol=1e-12)
