@@ -115,7 +115,8 @@ const int32_t* gnn_plan_colidx_t(const gnn_plan_t* plan);
 /* Workspace (device bytes) a compute call needs: hub-chunk partial states
  * [n_chunks][(n_acc * heads*head_dim + n_scalar * heads)] fp32 and, for gnn_gatv2_bwd, the per-CTA
  * `da` partials.  O(#chunks * H * d), never O(E * H).  `op`:                                         */
-enum { GNN_OP_GT_FWD = 0, GNN_OP_GT_BWD = 1, GNN_OP_GATV2_FWD = 2, GNN_OP_GATV2_BWD = 3, GNN_OP_GT_FWD_BLOCK = 4 };
+enum { GNN_OP_GT_FWD = 0, GNN_OP_GT_BWD = 1, GNN_OP_GATV2_FWD = 2, GNN_OP_GATV2_BWD = 3, GNN_OP_GT_FWD_BLOCK = 4,
+       GNN_OP_SEG_MINMAX_FWD = 5 /* pass heads = 1, head_dim = channels */ };
 gnn_status_t gnn_workspace_bytes(const gnn_plan_t* plan, int op, int32_t heads, int32_t head_dim, gnn_dtype_t dtype,
                                  size_t* bytes);
 
@@ -177,6 +178,26 @@ gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* plan, const int32_t* rowptr, const 
 gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
                                    const void* q, const void* k, const void* v, int32_t heads, int32_t head_dim,
                                    gnn_dtype_t dtype, void* out, float* lse, gnn_stream_t stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Degree-aware min / max neighbourhood aggregation with argmin (PAPER.md:124-151 section 3.1, :452-474 App. D.1):
+ *   out[i,c] = min (mode GNN_AGG_MIN) or max (GNN_AGG_MAX) over the stored in-neighbours j of i of x[j,c]
+ *   arg[i,c] = the source j that attains it; ties go to the smaller j (the paper's packed (value, index)
+ *              atomicMin); values compare as IEEE numbers; rows without entries give 0 / -1.
+ * x, out: [n, channels] `dtype`; arg: [n, channels] int32, out.  channels*sizeof(dtype) must be a multiple of 16 and
+ * at most 1024 (GNN_EUNSUPPORTED otherwise).  Runs on the plan's degree bins (packed rows, CTA rows, hub chunks
+ * merged by the lexicographic (value, index) minimum): no atomics, deterministic.
+ * ws: >= gnn_workspace_bytes(GNN_OP_SEG_MINMAX_FWD, heads = 1, head_dim = channels).  Pointers 32-byte aligned. */
+enum { GNN_AGG_MIN = 0, GNN_AGG_MAX = 1 };
+gnn_status_t gnn_seg_minmax_fwd(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                const void* x, int32_t channels, gnn_dtype_t dtype, int32_t mode, void* out,
+                                int32_t* arg, void* ws, size_t ws_bytes, gnn_stream_t stream);
+/* Backward: dx[arg[i,c], c] += dout[i,c] for every (i,c) with arg >= 0, a sparse scatter-add
+ * through the indices the forward saved.  arg: [n, channels] int32, in; dout: [n, channels] `dtype`, in;
+ * dx: [n, channels] fp32, out (the call zeroes it first).  Uses red.global.add.f32: the order of the additions
+ * into one dx element is not fixed, so dx is reproducible only up to fp32 rounding.  Needs no plan, no workspace. */
+gnn_status_t gnn_seg_minmax_bwd(int32_t n, const int32_t* arg, const void* dout, int32_t channels, gnn_dtype_t dtype,
+                                float* dx, gnn_stream_t stream);
 
 /* Thread-local message describing the last error returned on this thread ("" if none).           */
 const char* gnn_last_error(void);

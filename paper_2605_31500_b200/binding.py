@@ -13,6 +13,8 @@ _LIB_PATH = os.path.join(_HERE, "libgnn_attn.so")
 GNN_OK, GNN_EINVAL, GNN_EUNSUPPORTED, GNN_EWORKSPACE, GNN_ECUDA = range(5)
 GNN_F32, GNN_BF16 = 0, 1
 GNN_OP_GT_FWD, GNN_OP_GT_BWD, GNN_OP_GATV2_FWD, GNN_OP_GATV2_BWD = 0, 1, 2, 3
+GNN_OP_SEG_MINMAX_FWD = 5
+GNN_AGG_MIN, GNN_AGG_MAX = 0, 1
 (GNN_PLAN_COUNTS, GNN_PLAN_PERM, GNN_PLAN_CHUNKS, GNN_PLAN_CHUNK_PTR, GNN_PLAN_ROWPTR_T, GNN_PLAN_COLIDX_T,
  GNN_PLAN_PERM_T, GNN_PLAN_CHUNKS_T, GNN_PLAN_CHUNK_PTR_T, GNN_PLAN_BLOCK_BITMAP, GNN_PLAN_BLOCK_REM_ROWPTR,
  GNN_PLAN_BLOCK_REM_COLIDX) = range(12)
@@ -20,7 +22,7 @@ GNN_OP_GT_FWD, GNN_OP_GT_BWD, GNN_OP_GATV2_FWD, GNN_OP_GATV2_BWD = 0, 1, 2, 3
 EXPORTED_SYMBOLS = [
     "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
     "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
-    "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
+    "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_seg_minmax_fwd", "gnn_seg_minmax_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
     "gnn_profile_collect",
 ]
 
@@ -62,6 +64,8 @@ def lib() -> C.CDLL:
         L.gnn_gatv2_fwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _f, _vp, _vp, _vp, _sz, _vp]
         L.gnn_gatv2_bwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _vp, _vp, _i32, _i32, C.c_int, _f,
                                     _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+        L.gnn_seg_minmax_fwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _i32, C.c_int, _i32, _vp, _vp, _vp, _sz, _vp]
+        L.gnn_seg_minmax_bwd.argtypes = [_i32, _vp, _vp, _i32, C.c_int, _vp, _vp]
         L.gnn_gt_attn_fwd_block.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _vp, _vp, _vp]
         L.gnn_last_error.restype = C.c_char_p
         L.gnn_version.restype = C.c_char_p
@@ -246,3 +250,17 @@ def gnn_gatv2_bwd(plan: Plan, xl, xr, a, lse, dout, slope, g, dxl, dxr, da, stre
     _check(lib().gnn_gatv2_bwd(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(xl), _ptr(xr), _ptr(a),
                                _ptr(lse), _ptr(dout), H, d, _dtype_code(xl), float(slope), _ptr(g), _ptr(dxl), _ptr(dxr),
                                _ptr(da), _ptr(ws), ws.numel(), _stream(stream)))
+
+
+def gnn_seg_minmax_fwd(plan: Plan, x, mode, out, arg, stream=None):
+    """x, out: [n, channels] (fp32 / bf16); arg: [n, channels] int32; mode: GNN_AGG_MIN | GNN_AGG_MAX."""
+    n, ch = x.shape
+    ws = plan.workspace(GNN_OP_SEG_MINMAX_FWD, 1, ch, _dtype_code(x))
+    _check(lib().gnn_seg_minmax_fwd(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(x), ch, _dtype_code(x),
+                                    int(mode), _ptr(out), _ptr(arg), _ptr(ws), ws.numel(), _stream(stream)))
+
+
+def gnn_seg_minmax_bwd(arg, dout, dx, stream=None):
+    """arg: [n, channels] int32 from the forward; dout: [n, channels] (fp32 / bf16); dx: [n, channels] fp32, out."""
+    n, ch = arg.shape
+    _check(lib().gnn_seg_minmax_bwd(n, _ptr(arg), _ptr(dout), ch, _dtype_code(dout), _ptr(dx), _stream(stream)))

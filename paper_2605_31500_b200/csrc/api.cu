@@ -74,6 +74,7 @@ WsLayout ws_layout(const gnn_plan* P, int op, const Shape& sh, int esz) {
         case GNN_OP_GT_BWD: need(kGtBwdDst, P->fwd); need(kGtBwdSrc, P->tr); break;
         case GNN_OP_GATV2_FWD: need(kGatFwd, P->fwd); break;
         case GNN_OP_GATV2_BWD: need(kGatBwdDst, P->fwd); need(kGatBwdSrc, P->tr); break;
+        case GNN_OP_SEG_MINMAX_FWD: need(kMinFwd, P->fwd); break;
         default: break;
     }
     w.partials = 0;
@@ -149,12 +150,19 @@ extern "C" int32_t gnn_profile_collect(char* names, float* ms, int32_t max_recor
     return k;
 }
 
+static bool agg_shape(int32_t n, int32_t channels, int dtype, Shape& sh, const char* who);
+
 extern "C" gnn_status_t gnn_workspace_bytes(const gnn_plan_t* P, int op, int32_t heads, int32_t head_dim,
                                             gnn_dtype_t dtype, size_t* bytes) {
     if (!P || !bytes) { set_error("gnn_workspace_bytes: NULL plan or bytes"); return GNN_EINVAL; }
-    if (op < GNN_OP_GT_FWD || op > GNN_OP_GATV2_BWD) { set_error("gnn_workspace_bytes: unknown op %d", op); return GNN_EINVAL; }
+    if ((op < GNN_OP_GT_FWD || op > GNN_OP_GATV2_BWD) && op != GNN_OP_SEG_MINMAX_FWD) {
+        set_error("gnn_workspace_bytes: unknown op %d", op);
+        return GNN_EINVAL;
+    }
     Shape sh;
-    if (!make_shape(P->n, heads, head_dim, dtype, sh, "gnn_workspace_bytes")) return GNN_EUNSUPPORTED;
+    if (op == GNN_OP_SEG_MINMAX_FWD) {
+        if (heads < 1 || head_dim < 1 || !agg_shape(P->n, heads * head_dim, dtype, sh, "gnn_workspace_bytes")) return GNN_EUNSUPPORTED;
+    } else if (!make_shape(P->n, heads, head_dim, dtype, sh, "gnn_workspace_bytes")) return GNN_EUNSUPPORTED;
     if ((op == GNN_OP_GT_BWD || op == GNN_OP_GATV2_BWD) && !P->opts.build_transpose) {
         set_error("gnn_workspace_bytes: backward needs a plan built with build_transpose");
         return GNN_EINVAL;
@@ -265,5 +273,50 @@ extern "C" gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* P, const int32_t* rowptr
     cudaError_t e = launch_gat_bwd_dst(dtype, sh, c, a);                                   // dxl, G, da partials (xl . S)
     if (e == cudaSuccess) e = launch_gat_bwd_src(dtype, sh, ct, a);                        // dxr, da partials (xr . U)
     if (e == cudaSuccess) e = launch_da_reduce(c.da_part, w.da_slots, sh.rowe, da, c.stream);  // da
+    return cuda_status(e, who);
+}
+
+// ---- row f3: min / max aggregation.  The lane layout wants a power-of-two "head": factor channels = heads * head_dim
+// with head_dim the largest power of two that divides it (the pass has no per-head arithmetic).
+static bool agg_shape(int32_t n, int32_t channels, int dtype, Shape& sh, const char* who) {
+    if (channels < 1) { set_error("%s: channels must be >= 1", who); return false; }
+    const int hd = channels & -channels;
+    return make_shape(n, channels / hd, hd, dtype, sh, who);
+}
+
+extern "C" gnn_status_t gnn_seg_minmax_fwd(const gnn_plan_t* P, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                           const void* x, int32_t channels, gnn_dtype_t dtype, int32_t mode, void* out,
+                                           int32_t* arg, void* ws, size_t ws_bytes, gnn_stream_t stream) {
+    const char* who = "gnn_seg_minmax_fwd";
+    if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
+    if (!x || !out || !arg || !ws) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
+    if (mode != GNN_AGG_MIN && mode != GNN_AGG_MAX) { set_error("%s: unknown mode %d", who, mode); return GNN_EINVAL; }
+    if (!aligned16(x) || !aligned16(out) || !aligned16(arg) || !aligned16(ws)) {
+        set_error("%s: x, out, arg and workspace must be 32-byte aligned", who);
+        return GNN_EINVAL;
+    }
+    Shape sh;
+    if (!agg_shape(n, channels, dtype, sh, who)) return GNN_EUNSUPPORTED;
+    const WsLayout w = ws_layout(P, GNN_OP_SEG_MINMAX_FWD, sh, dtype == GNN_F32 ? 4 : 2);
+    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
+    AggArgs a = {};
+    a.x = x; a.out = out; a.arg = arg; a.sign = mode == GNN_AGG_MIN ? 1.f : -1.f;
+    return cuda_status(launch_min_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a), who);
+}
+
+extern "C" gnn_status_t gnn_seg_minmax_bwd(int32_t n, const int32_t* arg, const void* dout, int32_t channels,
+                                           gnn_dtype_t dtype, float* dx, gnn_stream_t stream) {
+    const char* who = "gnn_seg_minmax_bwd";
+    if (n < 1 || !arg || !dout || !dx) { set_error("%s: n < 1 or NULL pointer argument", who); return GNN_EINVAL; }
+    if (!aligned16(arg) || !aligned16(dout) || !aligned16(dx)) {
+        set_error("%s: arg, dout and dx must be 32-byte aligned", who);
+        return GNN_EINVAL;
+    }
+    Shape sh;
+    if (!agg_shape(n, channels, dtype, sh, who)) return GNN_EUNSUPPORTED;
+    cudaError_t e = cudaMemsetAsync(dx, 0, sizeof(float) * (size_t)n * channels, (cudaStream_t)stream);
+    AggArgs a = {};
+    a.arg = const_cast<int32_t*>(arg); a.dout = dout; a.dx = dx;
+    if (e == cudaSuccess) e = launch_minmax_scatter(dtype, n, channels, a, (cudaStream_t)stream);
     return cuda_status(e, who);
 }

@@ -28,10 +28,10 @@ struct gnn_plan {
 
 namespace gnn {
 
-enum Pass { kGtFwd = 0, kGtBwdDst, kGtBwdSrc, kGatFwd, kGatBwdDst, kGatBwdSrc, kNumPass };
+enum Pass { kGtFwd = 0, kGtBwdDst, kGtBwdSrc, kGatFwd, kGatBwdDst, kGatBwdSrc, kMinFwd, kNumPass };
 struct PassInfo { int na, ns, softmax, has_da; };
 // must match the NA / NS / SOFTMAX / HAS_DA constants of the Op structs (static_asserted in the dispatch units)
-constexpr PassInfo kPassInfo[kNumPass] = {{1, 1, 1, 0}, {2, 1, 0, 0}, {2, 0, 0, 0}, {1, 1, 1, 0}, {2, 2, 0, 1}, {2, 1, 0, 1}};
+constexpr PassInfo kPassInfo[kNumPass] = {{1, 1, 1, 0}, {2, 1, 0, 0}, {2, 0, 0, 0}, {1, 1, 1, 0}, {2, 2, 0, 1}, {2, 1, 0, 1}, {2, 0, 0, 0}};
 
 inline int pass_state_floats(Pass p, const Shape& sh) {
     return kPassInfo[p].na * sh.rowe + (kPassInfo[p].ns + kPassInfo[p].softmax) * sh.H;
@@ -59,7 +59,7 @@ constexpr int pass_inst_max_cb(Pass) { return 32; }
 #define GNN_BWD_KU 4
 #endif
 constexpr int pass_ku(Pass p, int cb) {
-    return (p == kGatFwd || p == kGtFwd) ? (cb == 32 ? GNN_FWD_KU : 4)
+    return (p == kGatFwd || p == kGtFwd || p == kMinFwd) ? (cb == 32 ? GNN_FWD_KU : 4)
          : (p == kGatBwdDst)             ? (cb == 32 ? GNN_GAT_DST_KU : 4)   // four accumulator vectors
          : (p == kGatBwdSrc)             ? (cb == 32 ? GNN_GAT_SRC_KU : 4)
                                          : (cb == 32 ? GNN_BWD_KU : 4);
@@ -67,7 +67,7 @@ constexpr int pass_ku(Pass p, int cb) {
 inline bool pick_lane_cfg(Pass p, int esz, int heads, int head_dim, LaneCfg& lc) {
     const int head_bytes = head_dim * esz, row_bytes = heads * head_bytes;
     int cb = pass_max_cb(p);
-    if (const char* e = getenv((p == kGtFwd || p == kGatFwd) ? "GNN_MAX_CB_FWD" : "GNN_MAX_CB_BWD")) {  // tuning knob
+    if (const char* e = getenv((p == kGtFwd || p == kGatFwd || p == kMinFwd) ? "GNN_MAX_CB_FWD" : "GNN_MAX_CB_BWD")) {  // tuning knob
         const int v = atoi(e);
         if ((v == 16 || v == 32 || v == 64) && v <= pass_inst_max_cb(p)) cb = v;
     }
@@ -108,6 +108,13 @@ struct GatArgs {
     float *lse, *g, *dxl, *dxr;
     float slope;
 };
+struct AggArgs {
+    const void *x, *dout;
+    void* out;
+    int32_t* arg;
+    float* dx;
+    float sign;   // +1: min, -1: max
+};
 // `Shape` passed to the launchers carries n, H, d, rowe; the lane fields are filled per pass inside.
 cudaError_t launch_gt_fwd(int dtype, const Shape&, const LaunchCtx&, const GtArgs&);
 cudaError_t launch_gt_bwd_dst(int dtype, const Shape&, const LaunchCtx&, const GtArgs&);
@@ -115,6 +122,9 @@ cudaError_t launch_gt_bwd_src(int dtype, const Shape&, const LaunchCtx&, const G
 cudaError_t launch_gat_fwd(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
 cudaError_t launch_gat_bwd_dst(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
 cudaError_t launch_gat_bwd_src(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
+cudaError_t launch_min_fwd(int dtype, const Shape&, const LaunchCtx&, const AggArgs&);
+// dx[arg[i,c], c] += dout[i,c] over all (i, c) with arg >= 0 (dx zeroed by the caller); one red.global.add per element
+cudaError_t launch_minmax_scatter(int dtype, long long n, int rowe, const AggArgs&, cudaStream_t);
 // da[e] = sum over slots of da_part[slot][e], fixed order, fp64 accumulation (no atomics)
 cudaError_t launch_da_reduce(const float* da_part, int slots, int rowe, float* da, cudaStream_t);
 

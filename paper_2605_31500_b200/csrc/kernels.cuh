@@ -9,6 +9,11 @@ extern unsigned long long g_launches;  // host-side launch counter (api.cu)
 void prof_begin(const char* pass, const char* kernel, cudaStream_t st);
 void prof_end(cudaStream_t st);
 
+// lexicographic (value, index) order of the MINARG states; index < 0 marks "no candidate yet"
+__device__ __forceinline__ bool minarg_better(float v, int j, float bv, int bj) {
+    return j >= 0 && (bj < 0 || v < bv || (v == bv && j < bj));
+}
+
 // ------------------------------------------------------------------------------------------------
 // state <-> shared memory (serialised layout of state_floats<Op>)
 template <class Op> __device__ __forceinline__ void state_to_smem(const typename Op::St& st, float* dst,
@@ -169,6 +174,7 @@ group_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowptr
         Op::load_own(own, p, sh, valid ? row : 0, valid, g);
         typename Op::St st;
         st.reset();
+        if constexpr (Op::MINARG) Op::init_state(st);
         int maxlen = len;
 #pragma unroll
         for (int o = G; o < 32; o <<= 1) maxlen = max(maxlen, __shfl_xor_sync(0xffffffffu, maxlen, o));
@@ -223,6 +229,7 @@ segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowp
         Op::load_own(own, p, sh, row, true, g);
         typename Op::St st;
         st.reset();
+        if constexpr (Op::MINARG) Op::init_state(st);
         // blocks of G edges are dealt round-robin to the NG groups; this warp's first group takes blocks
         // warp*GPW + k*NG, so its block count / last-block fill bound those of the warp's other groups
         const int nblk_all = (e1 - e0 + G - 1) / G;
@@ -249,10 +256,24 @@ segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowp
         }
         state_to_smem<Op>(st, s_part + gi * TEs, g, sh);
         __syncthreads();
-        for (int e = threadIdx.x; e < TEp; e += kCtaThreads) {
-            float s = 0.f;
-            for (int k = 0; k < NG; ++k) s += s_part[k * TEs + e];
-            s_merged[e] = s;
+        if constexpr (Op::MINARG) {
+            for (int e = threadIdx.x; e < sh.rowe; e += kCtaThreads) {
+                float bv = s_part[e];
+                int bj = __float_as_int(s_part[sh.rowe + e]);
+                for (int k = 1; k < NG; ++k) {
+                    const float v = s_part[k * TEs + e];
+                    const int j = __float_as_int(s_part[k * TEs + sh.rowe + e]);
+                    if (minarg_better(v, j, bv, bj)) { bv = v; bj = j; }
+                }
+                s_merged[e] = bv;
+                s_merged[sh.rowe + e] = __int_as_float(bj);
+            }
+        } else {
+            for (int e = threadIdx.x; e < TEp; e += kCtaThreads) {
+                float s = 0.f;
+                for (int k = 0; k < NG; ++k) s += s_part[k * TEs + e];
+                s_merged[e] = s;
+            }
         }
         if (Op::SOFTMAX && gi == 0 && g.lead) s_merged[TEp + g.hd] = st.m;
         __syncthreads();
@@ -305,6 +326,43 @@ hub_merge_kernel(typename Op::Params p, Shape sh, BinView bins, const float* __r
         }
         __syncthreads();
     }
+    if constexpr (Op::MINARG) {
+        // same chunk-to-warp assignment; every lane keeps four independent (value, index) candidates in flight
+        for (int e = lane; e < sh.rowe; e += 32) {
+            float bv[4];
+            int bj[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { bv[u] = INFINITY; bj[u] = -1; }
+            for (int c = c0 + warp; c < c1; c += 4 * kHubWarps) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int cu = c + u * kHubWarps;
+                    if (cu < c1) {
+                        const float v = partials[(size_t)cu * TE + e];
+                        const int j = __float_as_int(partials[(size_t)cu * TE + sh.rowe + e]);
+                        if (minarg_better(v, j, bv[u], bj[u])) { bv[u] = v; bj[u] = j; }
+                    }
+                }
+            }
+#pragma unroll
+            for (int u = 1; u < 4; ++u)
+                if (minarg_better(bv[u], bj[u], bv[0], bj[0])) { bv[0] = bv[u]; bj[0] = bj[u]; }
+            s_part[warp * TEp + e] = bv[0];
+            s_part[warp * TEp + sh.rowe + e] = __int_as_float(bj[0]);
+        }
+        __syncthreads();
+        for (int e = threadIdx.x; e < sh.rowe; e += kHubThreads) {
+            float bv = s_part[e];
+            int bj = __float_as_int(s_part[sh.rowe + e]);
+            for (int w = 1; w < kHubWarps; ++w) {
+                const float v = s_part[w * TEp + e];
+                const int j = __float_as_int(s_part[w * TEp + sh.rowe + e]);
+                if (minarg_better(v, j, bv, bj)) { bv = v; bj = j; }
+            }
+            s_merged[e] = bv;
+            s_merged[sh.rowe + e] = __int_as_float(bj);
+        }
+    } else {
     for (int e = lane; e < TEp; e += 32) {
         const int h = e < Op::NA * sh.rowe ? (e % sh.rowe) / sh.d : (e - Op::NA * sh.rowe) % sh.H;
         const float mg = Op::SOFTMAX ? s_merged[TEp + h] : 0.f;
@@ -347,6 +405,7 @@ hub_merge_kernel(typename Op::Params p, Shape sh, BinView bins, const float* __r
 #pragma unroll
         for (int w = 0; w < kHubWarps; ++w) s += s_part[w * TEp + e];
         s_merged[e] = s;
+    }
     }
     __syncthreads();
     float da[CH];

@@ -14,6 +14,9 @@ template <typename T, int CB_, int G_, int KU_, int NT_, int NSC_> struct OpBase
     static constexpr int kG = G_, kCB = CB_, kU = KU_, kCH = CB_ / (int)sizeof(T), kNT = NT_, kNSC = NSC_;
     using GeoT = Geo<G_>;
     using Ck = Chunk<T, CB_>;
+    // states are sums merged by addition unless an Op says otherwise: MINARG = pairs (value in acc[0], source index
+    // bits in acc[1]) that start at (+inf, -1) and are merged by the lexicographic minimum (ops_agg.cuh)
+    static constexpr bool MINARG = false;
     // the gathered operands of one batch of KU edges, raw (unconverted) in registers
     struct Src {
         Ck c[KU_][NT_];
