@@ -43,6 +43,7 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-minmax", action="store_true", help="skip the extra row-f3 (min aggregation) measurement of cfg 3 / 5")
     ap.add_argument("--warp-max-deg", type=int, default=0)
     ap.add_argument("--cta-max-deg", type=int, default=0)
     ap.add_argument("--split-chunk", type=int, default=0)
@@ -446,6 +447,44 @@ def run_ours(args, rank, world, local_rank):
                       "traffic": (traffic or {}).get("gt_fwd_block/tile") if traffic else None,
                       "tensor_pipe_pct_of_peak": tp})
 
+    # ---- row f3: degree-aware min aggregation with argmin on the same graph and plan, x = the K / xr tensor
+    # viewed as [n, H*d], dout = the config's upstream gradient; an extra object, not part of `value`
+    minmax = None
+    if args.cfg in (3, 5) and not args.no_minmax:
+        x2 = devt["k" if gt else "xr"].view(n, H * d)
+        do2 = devt["do"].view(n, H * d)
+        mo, ma = torch.empty_like(x2), torch.empty((n, H * d), dtype=torch.int32, device=dev)
+        mdx = torch.empty((n, H * d), **f32)
+
+        def mm_fwd():
+            G.gnn_seg_minmax_fwd(plan, x2, G.GNN_AGG_MIN, mo, ma)
+
+        def mm_bwd():
+            G.gnn_seg_minmax_bwd(ma, do2, mdx)
+
+        for _ in range(3):
+            mm_fwd()
+            mm_bwd()
+        ms_mf, ms_mb = timed(mm_fwd, args.steps), timed(mm_bwd, args.steps)
+        G.gnn_profile_enable(True)
+        mm_fwd()
+        mm_bwd()
+        G.gnn_profile_enable(False)
+        mk = {nm: float(ms) for nm, ms in G.gnn_profile_collect(64)}
+        b_el = x2.element_size()
+        R = H * d
+        # forward: index + one gathered row per edge; per row perm, rowptr, out row, arg row.  backward: arg + dout read,
+        # dx zeroed and one 32-byte sector read-modify-written per 8 scattered floats at best (counted as 4 B read + 4 B write)
+        mm_fwd_bytes = e * (4 + R * b_el) + n * (8 + R * b_el + 4 * R)
+        mm_bwd_bytes = n * R * (4 + b_el + 4 + 8)
+        minmax = {"op": "seg_min + argmin (row f3)", "channels": R, "ms_fwd": float(np.mean(ms_mf)), "ms_bwd": float(np.mean(ms_mb)),
+                  "gedges_fwd": e / (np.mean(ms_mf) * 1e-3) * 1e-9, "kernels_ms": mk,
+                  "algorithmic_bytes_fwd": mm_fwd_bytes, "achieved_gbs_fwd": mm_fwd_bytes / (np.mean(ms_mf) * 1e-3) * 1e-9,
+                  "frac_of_hbm_peak_fwd": mm_fwd_bytes / (np.mean(ms_mf) * 1e-3) * 1e-9 / peak,
+                  "algorithmic_bytes_bwd": mm_bwd_bytes, "achieved_gbs_bwd": mm_bwd_bytes / (np.mean(ms_mb) * 1e-3) * 1e-9,
+                  "frac_of_hbm_peak_bwd": mm_bwd_bytes / (np.mean(ms_mb) * 1e-3) * 1e-9 / peak}
+        del mo, ma, mdx
+
     # ---- end to end: pinned host inputs -> device, step, every output -> pinned host, all inside the events
     e2e = None
     if args.e2e_steps > 0:
@@ -487,7 +526,7 @@ def run_ours(args, rank, world, local_rank):
                 "gedges_fwd": e / (np.mean(ms_fwd) * 1e-3) * 1e-9, "gedges_bwd": e / (np.mean(ms_bwd) * 1e-3) * 1e-9,
                 "peak_device_bytes": peak_mem, "device_bytes_inputs": in_bytes, "device_bytes_outputs": out_bytes,
                 "plan_bytes": plan.plan_bytes, "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
-                "roofline": roof, "block_path": block, "cpu_baseline": cpu}
+                "roofline": roof, "block_path": block, "seg_minmax": minmax, "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

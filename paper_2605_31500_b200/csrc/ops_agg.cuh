@@ -51,12 +51,17 @@ template <typename T, int CB_, int G_, int KU_> struct MinFwd : OpBase<T, CB_, G
         for (int u = 0; u < KU; ++u) {
             const Ck& xc = src.c[u][0];
             const int j = nbr[u];
+            const bool valid = j >= 0;
+            const float jf = __int_as_float(j);
+            // branch-free lexicographic update (bitwise predicate logic keeps the compiler from short-circuit branches);
+            // the state starts at (+inf, -1), so with finite inputs the first candidate always wins the `<`
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
                 const float v = p.sign * xc.get(c);
-                const bool b = minarg_better(v, j, st.acc[0][c], __float_as_int(st.acc[1][c]));
-                st.acc[0][c] = b ? v : st.acc[0][c];
-                st.acc[1][c] = b ? __int_as_float(j) : st.acc[1][c];
+                const float bv = st.acc[0][c];
+                const bool b = valid & ((v < bv) | ((v == bv) & (j < __float_as_int(st.acc[1][c]))));
+                st.acc[0][c] = b ? v : bv;
+                st.acc[1][c] = b ? jf : st.acc[1][c];
             }
         }
     }
