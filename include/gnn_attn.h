@@ -103,7 +103,8 @@ enum {
     GNN_PLAN_CHUNK_PTR_T = 8,
     GNN_PLAN_BLOCK_BITMAP = 9,      /* uint16[n_windows][16]                                         */
     GNN_PLAN_BLOCK_REM_ROWPTR = 10, /* int32[n + 1]                                                  */
-    GNN_PLAN_BLOCK_REM_COLIDX = 11  /* int32[rem_nnz]                                                */
+    GNN_PLAN_BLOCK_REM_COLIDX = 11, /* int32[rem_nnz]                                                */
+    GNN_PLAN_FLAGS = 12             /* int32[1]: 1 if every CSR row lists its sources in ascending order */
 };
 /* Copies the item to HOST memory `host_dst` (synchronous).  *bytes in = capacity, out = size needed;
  * with host_dst == NULL only the size is returned.                                                 */

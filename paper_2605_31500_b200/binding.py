@@ -17,7 +17,7 @@ GNN_OP_SEG_MINMAX_FWD = 5
 GNN_AGG_MIN, GNN_AGG_MAX = 0, 1
 (GNN_PLAN_COUNTS, GNN_PLAN_PERM, GNN_PLAN_CHUNKS, GNN_PLAN_CHUNK_PTR, GNN_PLAN_ROWPTR_T, GNN_PLAN_COLIDX_T,
  GNN_PLAN_PERM_T, GNN_PLAN_CHUNKS_T, GNN_PLAN_CHUNK_PTR_T, GNN_PLAN_BLOCK_BITMAP, GNN_PLAN_BLOCK_REM_ROWPTR,
- GNN_PLAN_BLOCK_REM_COLIDX) = range(12)
+ GNN_PLAN_BLOCK_REM_COLIDX, GNN_PLAN_FLAGS) = range(13)
 
 EXPORTED_SYMBOLS = [
     "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
@@ -200,6 +200,10 @@ class Plan:
         c = self.export(GNN_PLAN_COUNTS)
         keys = ["n_hub", "n_cta", "n_group", "n_chunks"]
         return {**{k: int(v) for k, v in zip(keys, c[:4])}, **{k + "_t": int(v) for k, v in zip(keys, c[4:])}}
+
+    def rows_sorted(self) -> bool:
+        """True if every CSR row lists its sources in ascending order (selects the min / max fast path)."""
+        return bool(self.export(GNN_PLAN_FLAGS)[0])
 
     def workspace(self, op: int, heads: int, head_dim: int, dtype_code: int):
         import torch

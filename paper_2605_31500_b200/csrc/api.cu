@@ -301,7 +301,7 @@ extern "C" gnn_status_t gnn_seg_minmax_fwd(const gnn_plan_t* P, const int32_t* r
     if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
     AggArgs a = {};
     a.x = x; a.out = out; a.arg = arg; a.sign = mode == GNN_AGG_MIN ? 1.f : -1.f;
-    return cuda_status(launch_min_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a), who);
+    return cuda_status(launch_min_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a, P->rows_sorted != 0), who);
 }
 
 extern "C" gnn_status_t gnn_seg_minmax_bwd(int32_t n, const int32_t* arg, const void* dout, int32_t channels,

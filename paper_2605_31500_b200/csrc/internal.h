@@ -24,6 +24,7 @@ struct gnn_plan {
     int32_t* blk_rem_colidx; // [rem_nnz]
     int32_t n_windows;
     int64_t rem_nnz;
+    int32_t rows_sorted;     // 1 if every CSR row lists its sources in ascending order (min / max fast path)
 };
 
 namespace gnn {
@@ -122,7 +123,7 @@ cudaError_t launch_gt_bwd_src(int dtype, const Shape&, const LaunchCtx&, const G
 cudaError_t launch_gat_fwd(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
 cudaError_t launch_gat_bwd_dst(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
 cudaError_t launch_gat_bwd_src(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
-cudaError_t launch_min_fwd(int dtype, const Shape&, const LaunchCtx&, const AggArgs&);
+cudaError_t launch_min_fwd(int dtype, const Shape&, const LaunchCtx&, const AggArgs&, bool rows_sorted);
 // dx[arg[i,c], c] += dout[i,c] over all (i, c) with arg >= 0 (dx zeroed by the caller); one red.global.add per element
 cudaError_t launch_minmax_scatter(int dtype, long long n, int rowe, const AggArgs&, cudaStream_t);
 // da[e] = sum over slots of da_part[slot][e], fixed order, fp64 accumulation (no atomics)

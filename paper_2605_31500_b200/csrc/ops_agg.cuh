@@ -11,7 +11,10 @@
 
 namespace gnn {
 
-template <typename T, int CB_, int G_, int KU_> struct MinFwd : OpBase<T, CB_, G_, KU_, 1, 0> {
+// SORTED: every CSR row lists its sources in ascending order (plan flag).  A lane then meets its candidates in
+// ascending index order, so "first strict minimum wins" is the tie rule and the per-channel update is one compare and
+// two selects; the merges across lane groups and hub chunks always use the full lexicographic order.
+template <typename T, int CB_, int G_, int KU_, bool SORTED> struct MinFwdT : OpBase<T, CB_, G_, KU_, 1, 0> {
     static constexpr const char* kName = "seg_minmax_fwd";
     static constexpr int kMinBlocks = GNN_FWD_MINB;
     static constexpr bool kDoubleBuffer = false;
@@ -59,7 +62,8 @@ template <typename T, int CB_, int G_, int KU_> struct MinFwd : OpBase<T, CB_, G
             for (int c = 0; c < CH; ++c) {
                 const float v = p.sign * xc.get(c);
                 const float bv = st.acc[0][c];
-                const bool b = valid & ((v < bv) | ((v == bv) & (j < __float_as_int(st.acc[1][c]))));
+                const bool b = SORTED ? (valid & (v < bv))
+                                      : (valid & ((v < bv) | ((v == bv) & (j < __float_as_int(st.acc[1][c])))));
                 st.acc[0][c] = b ? v : bv;
                 st.acc[1][c] = b ? jf : st.acc[1][c];
             }
@@ -80,5 +84,8 @@ template <typename T, int CB_, int G_, int KU_> struct MinFwd : OpBase<T, CB_, G
         }
     }
 };
+
+template <typename T, int CB_, int G_, int KU_> using MinFwd = MinFwdT<T, CB_, G_, KU_, false>;
+template <typename T, int CB_, int G_, int KU_> using MinFwdSorted = MinFwdT<T, CB_, G_, KU_, true>;
 
 }  // namespace gnn

@@ -1,10 +1,11 @@
 #include "dispatch.cuh"
 #include "ops_agg.cuh"
 namespace gnn {
-cudaError_t launch_min_fwd(int dtype, const Shape& sh, const LaunchCtx& c, const AggArgs& a) {
-    return dispatch_pass<MinFwd, kMinFwd>(dtype, sh, c, [&](auto& p) {
+cudaError_t launch_min_fwd(int dtype, const Shape& sh, const LaunchCtx& c, const AggArgs& a, bool rows_sorted) {
+    auto fill = [&](auto& p) {
         p.x = (decltype(p.x))a.x; p.out = (decltype(p.out))a.out; p.arg = a.arg; p.sign = a.sign;
-    });
+    };
+    return rows_sorted ? dispatch_pass<MinFwdSorted, kMinFwd>(dtype, sh, c, fill) : dispatch_pass<MinFwd, kMinFwd>(dtype, sh, c, fill);
 }
 
 // Backward of the min / max aggregation: a sparse scatter-add through the saved indices.  One thread

@@ -96,6 +96,20 @@ __global__ void row_of_edge_kernel(const int32_t* __restrict__ rowptr, int n, lo
     row_of_edge[e] = lo;
 }
 
+// flag = 1 if some row lists its sources out of ascending order: a descent colidx[e-1] > colidx[e] is harmless only
+// when e starts a row (binary search in rowptr, reached by ~one entry per row on a sorted CSR)
+__global__ void rows_unsorted_kernel(const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx, int n,
+                                     long long nnz, int32_t* __restrict__ flag) {
+    const long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x + 1;
+    if (e >= nnz || __ldg(colidx + e - 1) <= __ldg(colidx + e)) return;
+    int lo = 0, hi = n;
+    while (lo < hi) {
+        const int mid = (int)(((long long)lo + hi + 1) >> 1);
+        if (__ldg(rowptr + mid) <= e) lo = mid; else hi = mid - 1;
+    }
+    if (__ldg(rowptr + lo) != e) *flag = 1;
+}
+
 // rowptr_t[j] = number of entries with source id < j = lower_bound(sorted source ids, j)
 __global__ void rowptr_t_kernel(const uint32_t* __restrict__ src_sorted, long long nnz, int n,
                                 int32_t* __restrict__ rowptr_t) {
@@ -177,7 +191,7 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
     L.perm = take(sizeof(int32_t) * (size_t)n);
     L.chunks = take(sizeof(int32_t) * 4 * (size_t)L.max_chunks);
     L.chunk_ptr = take(sizeof(int32_t) * (size_t)(L.max_hub + 1));
-    L.counts = take(sizeof(int32_t) * 8);
+    L.counts = take(sizeof(int32_t) * 16);   // 8 bin counts + flags
     L.rowptr_t = L.colidx_t = L.perm_t = L.chunks_t = L.chunk_ptr_t = 0;
     if (o.build_transpose) {
         L.rowptr_t = take(sizeof(int32_t) * ((size_t)n + 1));
@@ -327,6 +341,13 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
                            (int32_t*)(dm + L.chunk_ptr_t), counts_dev + 4, hc + 4, st);
         }
     }
+    int32_t unsorted = 0;
+    if (e == cudaSuccess) e = cudaMemsetAsync(counts_dev + 8, 0, sizeof(int32_t), st);
+    if (e == cudaSuccess && nnz > 1) {
+        rows_unsorted_kernel<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(rowptr, colidx, n, nnz, counts_dev + 8);
+        ++g_launches;
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&unsorted, counts_dev + 8, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
     int32_t rem_nnz = 0;
     if (e == cudaSuccess && o.build_blocks) {
         P->n_windows = (n + 15) / 16;
@@ -348,6 +369,7 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     P->rem_nnz = rem_nnz;
+    P->rows_sorted = unsorted ? 0 : 1;
     if (e != cudaSuccess) {
         set_error("gnn_plan_build: CUDA error: %s", cudaGetErrorString(e));
         delete P;
@@ -372,7 +394,9 @@ extern "C" gnn_status_t gnn_plan_export(const gnn_plan_t* P, int what, void* hos
     int32_t counts[8] = {P->fwd.n_hub, P->fwd.n_cta, P->fwd.n_group, P->fwd.n_chunks,
                          P->tr.n_hub, P->tr.n_cta, P->tr.n_group, P->tr.n_chunks};
     const bool T = P->opts.build_transpose != 0;
+    const int32_t flags[1] = {P->rows_sorted};
     switch (what) {
+        case GNN_PLAN_FLAGS: src = flags; need = sizeof(flags); break;
         case GNN_PLAN_COUNTS: need = sizeof(counts); break;
         case GNN_PLAN_PERM: src = P->fwd.perm; need = 4 * (size_t)P->n; break;
         case GNN_PLAN_CHUNKS: src = P->fwd.chunks; need = 16 * (size_t)P->fwd.n_chunks; break;
@@ -397,6 +421,7 @@ extern "C" gnn_status_t gnn_plan_export(const gnn_plan_t* P, int what, void* hos
     if (!host_dst) return GNN_OK;
     if (cap < need) { set_error("gnn_plan_export: buffer too small (%zu < %zu)", cap, need); return GNN_EWORKSPACE; }
     if (what == GNN_PLAN_COUNTS) { memcpy(host_dst, counts, need); return GNN_OK; }
+    if (what == GNN_PLAN_FLAGS) { memcpy(host_dst, flags, need); return GNN_OK; }
     if (need == 0) return GNN_OK;
     cudaError_t e = cudaMemcpy(host_dst, src, need, cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) { set_error("gnn_plan_export: CUDA error: %s", cudaGetErrorString(e)); return GNN_ECUDA; }

@@ -46,7 +46,11 @@ def test_seg_minmax_parity(dtype, mode, channels, opts):
     c = GI.make_config(2, scale=0.03)
     rp, ci, n = c["rowptr"], c["colidx"], c["n"]
     rng = np.random.default_rng(channels)
-    for ties in (False, True):
+    ci_shuffled = ci.copy()
+    for i in range(n):
+        ci_shuffled[rp[i]:rp[i + 1]] = rng.permutation(ci[rp[i]:rp[i + 1]])
+    for ties, shuffled in ((False, False), (True, False), (True, True)):
+        ci = ci_shuffled if shuffled else c["colidx"]   # sorted rows: strict-minimum fast path; shuffled: general path
         x = rng.standard_normal((n, channels)) if not ties else rng.integers(-1, 2, size=(n, channels)).astype(np.float64)
         if ties:
             x[rng.random((n, channels)) < 0.1] = -0.0
@@ -55,6 +59,7 @@ def test_seg_minmax_parity(dtype, mode, channels, opts):
         dout = rng.standard_normal((n, channels))
         dd = _to_dev(dout, dtype)
         got = _run(rp, ci, xd, mode, opts, dd)
+        assert got["plan"].rows_sorted() == (not shuffled)
         if opts is SMALL_OPTS:
             cnt = got["plan"].counts()
             assert cnt["n_hub"] > 0 and cnt["n_cta"] > 0
@@ -112,7 +117,7 @@ def test_seg_minmax_fullsize_cfg5():
     C = x_st.shape[1]
     xd = torch.from_numpy(np.ascontiguousarray(x_st)).view(torch.bfloat16).cuda()
     plan = G.Plan(torch.from_numpy(rp).cuda(), torch.from_numpy(ci).cuda(), transpose=False, **DEFAULT_OPTS)
-    assert plan.counts()["n_hub"] > 0
+    assert plan.counts()["n_hub"] > 0 and plan.rows_sorted()
     out = torch.empty_like(xd)
     arg = torch.empty((n, C), dtype=torch.int32, device="cuda")
     G.gnn_seg_minmax_fwd(plan, xd, G.GNN_AGG_MIN, out, arg)
