@@ -7,6 +7,8 @@ TEST INFRASTRUCTURE ONLY.  Only ``tests/``, ``__graft_entry__.smoke()`` and ``be
 * ``gnn_oracle.c``  - the layer definitions of PAPER.md section 2.2 (lines 68-76) and the backward
   identities of PAPER.md:494 / :496 / :539 / :563 written out in plain C, all arithmetic in
   double, OpenMP over rows.  Built by ``oracle.build()`` with gcc.
+* ``agg_ref.py``    - the min / max neighbourhood aggregation with argmin (SURVEY 8 row
+  f3) written as its definition in numpy, and its scatter-add backward.
 * ``plan_ref.py``   - numpy reference for the integer metadata (degree bins + hub chunk
   table, transposed CSR, 16-row block layout) that the CUDA plan must reproduce bit-exactly.
 
