@@ -43,6 +43,10 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--natural-ids", action="store_true",
+                    help="cfg 3: keep the natural R-MAT ids instead of the random relabel (locality study, SURVEY 8(d))")
+    ap.add_argument("--directed-plan", action="store_true",
+                    help="cfg 3: build CSR^T instead of reusing the forward CSR in the backward (row f1)")
     ap.add_argument("--no-minmax", action="store_true", help="skip the extra row-f3 (min aggregation) measurement of cfg 3 / 5")
     ap.add_argument("--warp-max-deg", type=int, default=0)
     ap.add_argument("--cta-max-deg", type=int, default=0)
@@ -249,13 +253,14 @@ def job_gedges(edges_per_rank: int, steps: int, world: int, total_ms: float) -> 
 def workload_config(c, args):
     return {"workload": c["name"], "layer": c["layer"], "nodes": c["n"], "edges": c["e"], "heads": c["heads"],
             "head_dim": c["head_dim"], "feature_dtype": c["dtype"], "scale": args.scale,
-            "graph": "synthetic seeded generator (gnn_inputs), stands in for the paper's datasets"}
+            "graph": "synthetic seeded generator (gnn_inputs), stands in for the paper's datasets",
+            "ids": "randomly relabelled" if c.get("relabel", True) else "natural R-MAT ids (locality study, not the headline)"}
 
 
 def run_reference(args, rank):
     if rank != 0:
         return
-    c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False)
+    c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False, relabel=not args.natural_ids)
     # each step = one bounded sample pass; the whole run (warm-up + steps) is sized to about two minutes of oracle time
     arm = OracleArm(c, target_seconds=min(args.cpu_seconds, 120.0 / max(args.steps + args.warmup, 1)))
     for _ in range(args.warmup):
@@ -291,7 +296,7 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False)   # replicas: every rank runs the same workload
+    c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False, relabel=not args.natural_ids)   # replicas: every rank runs the same workload
     n, e, H, d, dt = c["n"], c["e"], c["heads"], c["head_dim"], c["dtype"]
     gt = c["layer"] == "gt"
     names = ("q", "k", "v", "do") if gt else ("xl", "xr", "do")
@@ -306,11 +311,25 @@ def run_ours(args, rank, world, local_rank):
         host["a"] = torch.from_numpy(c["a_f32"])
     devt = {k: v.to(dev) for k, v in host.items()}
     torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    plan = G.Plan(devt["rowptr"], devt["colidx"], warp_max_deg=args.warp_max_deg, cta_max_deg=args.cta_max_deg,
-                  split_chunk=args.split_chunk, transpose=True, blocks=(args.cfg == 4))
-    torch.cuda.synchronize()
-    plan_ms = 1e3 * (time.perf_counter() - t0)
+    # row f1: cfg 3 is undirected by construction, so its backward reuses the forward CSR (the
+    # library verifies that); --directed-plan builds CSR^T instead.  Both plans are built and timed for cfg 3.
+    undirected = args.cfg == 3 and not args.directed_plan
+
+    def build_plan(mode):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        p = G.Plan(devt["rowptr"], devt["colidx"], warp_max_deg=args.warp_max_deg, cta_max_deg=args.cta_max_deg,
+                   split_chunk=args.split_chunk, transpose=mode, blocks=(args.cfg == 4))
+        torch.cuda.synchronize()
+        return p, 1e3 * (time.perf_counter() - t0)
+
+    plan_cmp = None
+    if undirected:
+        build_plan(True)            # untimed first build: module load, allocator warm-up
+        p_dir, ms_dir = build_plan(True)
+        plan_cmp = {"directed_plan_build_ms": ms_dir, "directed_plan_bytes": p_dir.plan_bytes}
+        del p_dir
+    plan, plan_ms = build_plan("undirected" if undirected else True)
 
     f32 = dict(dtype=torch.float32, device=dev)
     out = torch.empty((n, H, d), dtype=devt[names[0]].dtype, device=dev)
@@ -518,7 +537,9 @@ def run_ours(args, rank, world, local_rank):
         cfgd.update({"l2": "L2 flushed between timed steps" if need_flush else "inputs larger than L2 (no flush)",
                      "plan": cnt, "plan_opts": {"warp_max_deg": plan.opts.warp_max_deg, "cta_max_deg": plan.opts.cta_max_deg,
                                                 "split_chunk": plan.opts.split_chunk},
-                     "plan_build_ms": plan_ms, "degree_stats": GI.degree_stats(c["rowptr"], c["colidx"])})
+                     "plan_build_ms": plan_ms,
+                     "backward_csr": "forward CSR reused (undirected graph, PAPER.md:343)" if undirected else "CSR^T built by the plan",
+                     "plan_vs_directed": plan_cmp, "degree_stats": GI.degree_stats(c["rowptr"], c["colidx"])})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfgd,

@@ -57,8 +57,14 @@ typedef enum { GNN_F32 = 0, GNN_BF16 = 1 } gnn_dtype_t;
  *   deg > cta_max_deg              : "hub rows"    - cut into ceil(deg/split_chunk) near-equal chunks,
  *                                    one CTA per chunk, partial states merged by a second pass
  * Zero in any threshold selects the default (4096 / 16384 / 4096 if nnz >= 2^24, else 256 / 1024 / 512).
- * build_transpose != 0 also builds CSR^T and its bins (needed by the backward calls).
+ * build_transpose: GNN_TRANSPOSE_NONE (0) forward only; GNN_TRANSPOSE_BUILD (1) also builds CSR^T and its bins
+ * (needed by the backward calls); GNN_TRANSPOSE_UNDIRECTED (2) is the direction-aware mode of PAPER.md:343: the
+ * caller declares the graph undirected (rows strictly ascending, a mirror (j, i) for every entry (i, j));
+ * gnn_plan_build verifies that on the device (GNN_EINVAL if it does not hold) and the backward calls then traverse
+ * the forward CSR and its bins: no transposed structure is built or stored (plan storage drops by 4*(nnz + n) bytes
+ * plus the second bin set), and the gradients are bit-identical to mode 1, for which CSR^T == CSR bit for bit.
  * build_blocks != 0 also builds the 16-row block layout (gnn_gt_attn_fwd_block).              */
+enum { GNN_TRANSPOSE_NONE = 0, GNN_TRANSPOSE_BUILD = 1, GNN_TRANSPOSE_UNDIRECTED = 2 };
 typedef struct {
     int32_t warp_max_deg;
     int32_t cta_max_deg;
@@ -104,12 +110,14 @@ enum {
     GNN_PLAN_BLOCK_BITMAP = 9,      /* uint16[n_windows][16]                                         */
     GNN_PLAN_BLOCK_REM_ROWPTR = 10, /* int32[n + 1]                                                  */
     GNN_PLAN_BLOCK_REM_COLIDX = 11, /* int32[rem_nnz]                                                */
-    GNN_PLAN_FLAGS = 12             /* int32[1]: 1 if every CSR row lists its sources in ascending order */
+    GNN_PLAN_FLAGS = 12             /* int32[2]: [0] = 1 if every CSR row lists its sources in ascending order;
+                                       [1] = 1 if the backward traverses the forward CSR (GNN_TRANSPOSE_UNDIRECTED) */
 };
 /* Copies the item to HOST memory `host_dst` (synchronous).  *bytes in = capacity, out = size needed;
  * with host_dst == NULL only the size is returned.                                                 */
 gnn_status_t gnn_plan_export(const gnn_plan_t* plan, int what, void* host_dst, size_t* bytes);
-/* Device pointers to CSR^T held by the plan (NULL if build_transpose was 0).                        */
+/* Device pointers to CSR^T held by the plan (NULL if build_transpose was 0; the caller's own rowptr / colidx
+ * in the undirected mode).                                                                          */
 const int32_t* gnn_plan_rowptr_t(const gnn_plan_t* plan);
 const int32_t* gnn_plan_colidx_t(const gnn_plan_t* plan);
 

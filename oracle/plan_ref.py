@@ -16,6 +16,9 @@ a1 - degree bins (paper: light / heavy split with per-bucket warp counts, PAPER.
      (row, e_begin, e_end, hub_slot) in (hub_slot, t) order; hub_chunk_ptr is its row pointer.
 a2 - transposed CSR by a STABLE counting sort on the source id: row j of
      CSR^T lists the destinations i of j's out-edges ordered by (i ascending, original position).
+f1 - direction-aware backward: a CSR is "undirected" iff every row is strictly
+     ascending and its set of (dst, src) pairs equals its set of (src, dst) pairs; then
+     transpose_csr(CSR) == CSR bit for bit, which is why the backward may reuse the forward CSR.
 a11 - 16-row block layout for the locally dense graph (own layout; the paper's WSB, PAPER.md:545,
      is prior art): window w = rows [16w, 16w+16); bitmap[w][r] bit c is set iff the FIRST
      occurrence of edge (dst 16w+r <- src 16w+c) exists; every other entry (sources outside
@@ -80,6 +83,23 @@ def transpose_csr(rowptr, colidx):
     rowptr_t = np.zeros(n + 1, dtype=np.int64)
     np.cumsum(np.bincount(colidx, minlength=n), out=rowptr_t[1:])
     return rowptr_t.astype(np.int32), colidx_t
+
+
+def is_undirected(rowptr, colidx) -> bool:
+    """f1: strictly ascending rows and edge set == mirrored edge set (plain set comparison)."""
+    rowptr = np.asarray(rowptr, dtype=np.int64)
+    colidx = np.asarray(colidx, dtype=np.int64)
+    n = rowptr.size - 1
+    if colidx.size and (colidx.min() < 0 or colidx.max() >= n):
+        return False
+    for i in range(n):
+        row = colidx[rowptr[i]:rowptr[i + 1]]
+        if np.any(np.diff(row) <= 0):
+            return False
+    row_of_edge = np.repeat(np.arange(n, dtype=np.int64), np.diff(rowptr))
+    fwd = np.sort(row_of_edge * n + colidx)
+    rev = np.sort(colidx * n + row_of_edge)
+    return bool(np.array_equal(fwd, rev))
 
 
 def build_blocks(rowptr, colidx) -> dict:

@@ -12,5 +12,6 @@ from .binding import (  # noqa: F401
     gnn_seg_minmax_fwd, gnn_seg_minmax_bwd, GNN_AGG_MIN, GNN_AGG_MAX, GNN_OP_SEG_MINMAX_FWD,
     gnn_last_error, gnn_version, gnn_launch_count, gnn_profile_enable, gnn_profile_collect,
     GNN_F32, GNN_BF16, GNN_OP_GT_FWD, GNN_OP_GT_BWD, GNN_OP_GATV2_FWD, GNN_OP_GATV2_BWD,
+    GNN_TRANSPOSE_NONE, GNN_TRANSPOSE_BUILD, GNN_TRANSPOSE_UNDIRECTED,
     EXPORTED_SYMBOLS,
 )

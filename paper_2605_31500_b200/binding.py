@@ -15,6 +15,7 @@ GNN_F32, GNN_BF16 = 0, 1
 GNN_OP_GT_FWD, GNN_OP_GT_BWD, GNN_OP_GATV2_FWD, GNN_OP_GATV2_BWD = 0, 1, 2, 3
 GNN_OP_SEG_MINMAX_FWD = 5
 GNN_AGG_MIN, GNN_AGG_MAX = 0, 1
+GNN_TRANSPOSE_NONE, GNN_TRANSPOSE_BUILD, GNN_TRANSPOSE_UNDIRECTED = 0, 1, 2
 (GNN_PLAN_COUNTS, GNN_PLAN_PERM, GNN_PLAN_CHUNKS, GNN_PLAN_CHUNK_PTR, GNN_PLAN_ROWPTR_T, GNN_PLAN_COLIDX_T,
  GNN_PLAN_PERM_T, GNN_PLAN_CHUNKS_T, GNN_PLAN_CHUNK_PTR_T, GNN_PLAN_BLOCK_BITMAP, GNN_PLAN_BLOCK_REM_ROWPTR,
  GNN_PLAN_BLOCK_REM_COLIDX, GNN_PLAN_FLAGS) = range(13)
@@ -184,7 +185,10 @@ class Plan:
             raise GnnError("rowptr / colidx must be int32")
         self.rowptr, self.colidx = rowptr.contiguous(), colidx.contiguous()
         self.n, self.nnz = int(rowptr.numel()) - 1, int(colidx.numel())
-        self.opts = PlanOpts(warp_max_deg, cta_max_deg, split_chunk, 1 if transpose else 0, 1 if blocks else 0)
+        # transpose: False (forward only), True (build CSR^T) or "undirected" (the backward reuses
+        # the forward CSR; the library verifies the graph is undirected and raises GnnError if not)
+        mode = GNN_TRANSPOSE_UNDIRECTED if transpose == "undirected" else (GNN_TRANSPOSE_BUILD if transpose else GNN_TRANSPOSE_NONE)
+        self.opts = PlanOpts(warp_max_deg, cta_max_deg, split_chunk, mode, 1 if blocks else 0)
         dev_bytes, scratch_bytes = gnn_plan_bytes(self.n, self.nnz, self.opts)
         self.dev_mem = torch.empty(dev_bytes, dtype=torch.uint8, device=rowptr.device)
         scratch = torch.empty(scratch_bytes, dtype=torch.uint8, device=rowptr.device)
@@ -204,6 +208,10 @@ class Plan:
     def rows_sorted(self) -> bool:
         """True if every CSR row lists its sources in ascending order (selects the min / max fast path)."""
         return bool(self.export(GNN_PLAN_FLAGS)[0])
+
+    def undirected(self) -> bool:
+        """True if the backward traverses the forward CSR (plan built with transpose="undirected")."""
+        return bool(self.export(GNN_PLAN_FLAGS)[1])
 
     def workspace(self, op: int, heads: int, head_dim: int, dtype_code: int):
         import torch

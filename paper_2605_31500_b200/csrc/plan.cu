@@ -110,6 +110,30 @@ __global__ void rows_unsorted_kernel(const int32_t* __restrict__ rowptr, const i
     if (__ldg(rowptr + lo) != e) *flag = 1;
 }
 
+// Undirected check: flag = 1 unless every row is STRICTLY ascending and every entry (i, j) has its
+// mirror (j, i).  For such a CSR the stable transpose is the CSR itself, bit for bit (row j of CSR^T lists the
+// destinations of j ascending = the sources of j ascending = row j of the CSR).  One thread per entry: binary
+// search of its row in rowptr, then of i in row j.
+__global__ void undirected_check_kernel(const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx, int n,
+                                        long long nnz, int32_t* __restrict__ flag) {
+    const long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (e >= nnz) return;
+    int lo = 0, hi = n;
+    while (lo < hi) {
+        const int mid = (int)(((long long)lo + hi + 1) >> 1);
+        if (__ldg(rowptr + mid) <= e) lo = mid; else hi = mid - 1;
+    }
+    const int i = lo, j = __ldg(colidx + e);
+    if ((unsigned)j >= (unsigned)n) { *flag = 1; return; }
+    if (e > __ldg(rowptr + i) && __ldg(colidx + e - 1) >= j) { *flag = 1; return; }
+    int a = __ldg(rowptr + j), b = __ldg(rowptr + j + 1);
+    while (a < b) {
+        const int mid = a + ((b - a) >> 1);
+        if (__ldg(colidx + mid) < i) a = mid + 1; else b = mid;
+    }
+    if (a >= __ldg(rowptr + j + 1) || __ldg(colidx + a) != i) *flag = 1;
+}
+
 // rowptr_t[j] = number of entries with source id < j = lower_bound(sorted source ids, j)
 __global__ void rowptr_t_kernel(const uint32_t* __restrict__ src_sorted, long long nnz, int n,
                                 int32_t* __restrict__ rowptr_t) {
@@ -184,6 +208,7 @@ int n_bits(int n) {
 }
 
 cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout& L) {
+    const bool own_t = o.build_transpose != 0 && o.build_transpose != GNN_TRANSPOSE_UNDIRECTED;  // CSR^T stored in the plan
     L.max_hub = nnz / (o.cta_max_deg + 1) + 1;
     L.max_chunks = nnz / o.split_chunk + L.max_hub + 1;
     size_t off = 0;
@@ -193,7 +218,7 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
     L.chunk_ptr = take(sizeof(int32_t) * (size_t)(L.max_hub + 1));
     L.counts = take(sizeof(int32_t) * 16);   // 8 bin counts + flags
     L.rowptr_t = L.colidx_t = L.perm_t = L.chunks_t = L.chunk_ptr_t = 0;
-    if (o.build_transpose) {
+    if (own_t) {
         L.rowptr_t = take(sizeof(int32_t) * ((size_t)n + 1));
         L.colidx_t = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
         L.perm_t = take(sizeof(int32_t) * (size_t)n);
@@ -211,7 +236,7 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
     cudaError_t e = cub::DeviceRadixSort::SortPairs(nullptr, t1, (const uint32_t*)nullptr, (uint32_t*)nullptr,
                                                     (const int32_t*)nullptr, (int32_t*)nullptr, (long long)n, 0, 7);
     if (e != cudaSuccess) return e;
-    if (o.build_transpose) {
+    if (own_t) {
         e = cub::DeviceRadixSort::SortPairs(nullptr, t2, (const uint32_t*)nullptr, (uint32_t*)nullptr,
                                             (const int32_t*)nullptr, (int32_t*)nullptr, (long long)nnz, 0, n_bits(n));
         if (e != cudaSuccess) return e;
@@ -227,7 +252,7 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
     L.key_sorted = take(sizeof(uint32_t) * (size_t)n);
     L.rowid = take(sizeof(int32_t) * (size_t)n);
     L.ekey_sorted = L.erow = 0;
-    if (o.build_transpose) {
+    if (own_t) {
         L.ekey_sorted = take(sizeof(uint32_t) * (size_t)(nnz > 0 ? nnz : 1));
         L.erow = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
     }
@@ -322,7 +347,20 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
     int32_t hc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     e = build_bins(rowptr, n, o, L, sc, (int32_t*)(dm + L.perm), (int32_t*)(dm + L.chunks),
                    (int32_t*)(dm + L.chunk_ptr), counts_dev, hc, st);
-    if (e == cudaSuccess && o.build_transpose) {
+    int32_t directed = 0;
+    if (e == cudaSuccess && o.build_transpose == GNN_TRANSPOSE_UNDIRECTED) {
+        // direction-aware backward: the caller declares an undirected graph; verified here, then the
+        // backward passes traverse the forward CSR and its bins - no transposed structure is built or stored
+        e = cudaMemsetAsync(counts_dev + 9, 0, sizeof(int32_t), st);
+        if (e == cudaSuccess && nnz > 0) {
+            undirected_check_kernel<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(rowptr, colidx, n, nnz, counts_dev + 9);
+            ++g_launches;
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&directed, counts_dev + 9, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        P->rowptr_t = const_cast<int32_t*>(rowptr);
+        P->colidx_t = const_cast<int32_t*>(colidx);
+        for (int t = 0; t < 4; ++t) hc[4 + t] = hc[t];
+    } else if (e == cudaSuccess && o.build_transpose) {
         P->rowptr_t = (int32_t*)(dm + L.rowptr_t);
         P->colidx_t = (int32_t*)(dm + L.colidx_t);
         uint32_t* ekey_sorted = (uint32_t*)(sc + L.ekey_sorted);
@@ -375,8 +413,15 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
         delete P;
         return GNN_ECUDA;
     }
+    if (directed) {
+        set_error("gnn_plan_build: GNN_TRANSPOSE_UNDIRECTED needs strictly ascending rows and a mirror (j, i) for every entry (i, j)");
+        delete P;
+        return GNN_EINVAL;
+    }
     P->fwd = BinView{(int32_t*)(dm + L.perm), (int32_t*)(dm + L.chunks), (int32_t*)(dm + L.chunk_ptr), hc[0], hc[1], hc[2], hc[3]};
-    if (o.build_transpose)
+    if (o.build_transpose == GNN_TRANSPOSE_UNDIRECTED)
+        P->tr = P->fwd;
+    else if (o.build_transpose)
         P->tr = BinView{(int32_t*)(dm + L.perm_t), (int32_t*)(dm + L.chunks_t), (int32_t*)(dm + L.chunk_ptr_t), hc[4], hc[5], hc[6], hc[7]};
     *plan = P;
     return GNN_OK;
@@ -394,7 +439,7 @@ extern "C" gnn_status_t gnn_plan_export(const gnn_plan_t* P, int what, void* hos
     int32_t counts[8] = {P->fwd.n_hub, P->fwd.n_cta, P->fwd.n_group, P->fwd.n_chunks,
                          P->tr.n_hub, P->tr.n_cta, P->tr.n_group, P->tr.n_chunks};
     const bool T = P->opts.build_transpose != 0;
-    const int32_t flags[1] = {P->rows_sorted};
+    const int32_t flags[2] = {P->rows_sorted, P->opts.build_transpose == GNN_TRANSPOSE_UNDIRECTED ? 1 : 0};
     switch (what) {
         case GNN_PLAN_FLAGS: src = flags; need = sizeof(flags); break;
         case GNN_PLAN_COUNTS: need = sizeof(counts); break;

@@ -40,7 +40,9 @@ def test_fullsize_sampled_parity(cfg):
     c = GI.make_config(cfg, keep_f32=False)
     n, H, d, dt, gt = c["n"], c["heads"], c["head_dim"], c["dtype"], c["layer"] == "gt"
     rp, ci = torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda()
-    plan = G.Plan(rp, ci, transpose=True, blocks=(cfg == 4), **DEFAULT_OPTS)
+    # cfg 3 is undirected: same launch configuration as bench.py (backward over the forward CSR, row f1)
+    plan = G.Plan(rp, ci, transpose="undirected" if cfg == 3 else True, blocks=(cfg == 4), **DEFAULT_OPTS)
+    assert plan.undirected() == (cfg == 3)
     names = ("q", "k", "v", "do") if gt else ("xl", "xr", "do")
     T = {nm: _dev(c[nm + "_st"], dt) for nm in names}
     out = torch.empty_like(T[names[0]])

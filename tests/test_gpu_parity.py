@@ -56,12 +56,12 @@ def check(name, got, want, dtype):
         assert rel <= 5e-3, f"{name}: rel Frobenius err {rel:.3e} > 5e-3"
 
 
-def run_gt(c, opts, backward=True):
+def run_gt(c, opts, backward=True, transpose=True):
     import paper_2605_31500_b200 as G
     torch = _torch()
     n, H, d, dt = c["n"], c["heads"], c["head_dim"], c["dtype"]
     rp, ci = torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda()
-    plan = G.Plan(rp, ci, transpose=True, **opts)
+    plan = G.Plan(rp, ci, transpose=transpose, **opts)
     q, k, v = (_dev(c[x + "_st"], dt) for x in "qkv")
     out = torch.empty_like(q)
     lse = torch.empty((n, H), dtype=torch.float32, device="cuda")
@@ -77,12 +77,12 @@ def run_gt(c, opts, backward=True):
     return res
 
 
-def run_gat(c, opts, backward=True):
+def run_gat(c, opts, backward=True, transpose=True):
     import paper_2605_31500_b200 as G
     torch = _torch()
     n, H, d, dt = c["n"], c["heads"], c["head_dim"], c["dtype"]
     rp, ci = torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda()
-    plan = G.Plan(rp, ci, transpose=True, **opts)
+    plan = G.Plan(rp, ci, transpose=transpose, **opts)
     xl, xr = _dev(c["xl_st"], dt), _dev(c["xr_st"], dt)
     a = torch.from_numpy(c["a_f32"]).cuda()
     out = torch.empty_like(xl)
@@ -167,6 +167,42 @@ def _custom(layer, n, rowptr, colidx, H, d, dtype, seed=1):
     if layer == "gatv2":
         c["a_f32"] = (rng.standard_normal((H, d)) * d ** -0.5).astype(np.float32)
     return c
+
+
+@pytest.mark.parametrize("layer", ["gt", "gatv2"])
+def test_undirected_backward_reuses_forward_csr(layer):
+    """Row f1: on an undirected graph the backward traverses the forward CSR; the plan stores no
+    CSR^T, its exported transpose is still plan_ref's (== the CSR), and the gradients are bit-identical to the
+    directed backward ("numerically identical gradients").  A directed graph or a multigraph is refused."""
+    import paper_2605_31500_b200 as G
+    import paper_2605_31500_b200.binding as B
+    torch = _torch()
+    c3 = GI.make_config(3, scale=0.002)          # symmetrised R-MAT, ascending rows, one self-loop per node
+    rowptr, colidx = c3["rowptr"], c3["colidx"]
+    assert plan_ref.is_undirected(rowptr, colidx)
+    c = c3 if layer == "gt" else _custom("gatv2", c3["n"], rowptr, colidx, 4, 32, "bf16")
+    run = run_gt if layer == "gt" else run_gat
+    keys = ["Delta", "dQ", "dK", "dV"] if layer == "gt" else ["G", "dxl", "dxr", "da"]
+    for opts, resolved in ((SMALL_OPTS, SMALL_OPTS), (DEFAULT_OPTS, RESOLVED_DEFAULT)):
+        directed = run(c, opts, transpose=True)
+        undirected = run(c, opts, transpose="undirected")
+        assert undirected["plan"].undirected() and not directed["plan"].undirected()
+        assert undirected["plan"].plan_bytes + 4 * (colidx.size + rowptr.size) <= directed["plan"].plan_bytes
+        check_plan(undirected["plan"], rowptr, colidx, resolved)     # exported CSR^T / bins == plan_ref's
+        assert np.array_equal(undirected["plan"].export(B.GNN_PLAN_COLIDX_T), colidx)
+        for key in keys:
+            assert np.array_equal(directed[key], undirected[key]), key
+    compare_all(c, undirected, oracle_gt(c) if layer == "gt" else oracle_gat(c))
+    # refused: a directed graph, and a symmetric multigraph (rows not strictly ascending)
+    c1 = GI.make_config(1, scale=0.1)
+    assert not plan_ref.is_undirected(c1["rowptr"], c1["colidx"])
+    dup_dst, dup_src = np.array([0, 0, 1, 1, 1, 2], np.int64), np.array([1, 1, 0, 0, 2, 1], np.int64)
+    rp_m, ci_m = GI.csr_from_pairs(3, dup_dst, dup_src, self_loops=False, dedupe=False)
+    assert not plan_ref.is_undirected(rp_m, ci_m)
+    for rp, ci in ((c1["rowptr"], c1["colidx"]), (rp_m, ci_m)):
+        with pytest.raises(G.GnnError, match="UNDIRECTED"):
+            G.Plan(torch.from_numpy(rp.astype(np.int32)).cuda(), torch.from_numpy(ci.astype(np.int32)).cuda(),
+                   transpose="undirected")
 
 
 @pytest.mark.parametrize("layer", ["gt", "gatv2"])

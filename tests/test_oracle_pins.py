@@ -388,6 +388,45 @@ def test_transpose_csr_vs_bruteforce_and_scipy():
     np.testing.assert_array_equal(cit, A.indices)
 
 
+def test_is_undirected_vs_dense_and_implies_self_transpose():
+    """Row f1: is_undirected == (dense 0/1 adjacency equals its transpose, no repeated entry,
+    ascending rows), and whenever it holds the stable transpose is the CSR itself; one removed mirror entry, one
+    repeated entry or one swapped pair of neighbours breaks it."""
+    import scipy.sparse as sp
+    rng = np.random.default_rng(35)
+    for trial in range(6):
+        n = 23 + trial
+        m = rng.random((n, n)) < 0.15
+        if trial % 2 == 0:
+            m = m | m.T
+        A = sp.csr_matrix(m.astype(np.float64))
+        A.sort_indices()
+        rp, ci = A.indptr.astype(np.int32), A.indices.astype(np.int32)
+        dense = np.zeros((n, n), np.int64)
+        for i in range(n):
+            for e in range(rp[i], rp[i + 1]):
+                dense[i, ci[e]] += 1
+        want = bool(np.array_equal(dense, dense.T) and dense.max() <= 1)
+        assert plan_ref.is_undirected(rp, ci) == want == (trial % 2 == 0)
+        if want:
+            rpt, cit = plan_ref.transpose_csr(rp, ci)
+            np.testing.assert_array_equal(rpt, rp)
+            np.testing.assert_array_equal(cit, ci)
+            i = int(np.argmax(np.diff(rp) >= 2))                      # a row with two neighbours
+            swapped = ci.copy()
+            swapped[rp[i]], swapped[rp[i] + 1] = ci[rp[i] + 1], ci[rp[i]]
+            assert not plan_ref.is_undirected(rp, swapped)            # same edge set, row not ascending
+            e = int(np.argmax(ci != np.repeat(np.arange(n), np.diff(rp))))   # first off-diagonal entry
+            rp_cut = rp.copy()
+            rp_cut[np.searchsorted(rp, e, side="right"):] -= 1
+            assert not plan_ref.is_undirected(rp_cut, np.delete(ci, e))       # mirror entry missing
+            rp_dup = rp.copy()
+            rp_dup[np.searchsorted(rp, e, side="right"):] += 1
+            assert not plan_ref.is_undirected(rp_dup, np.insert(ci, e, ci[e]))  # repeated entry
+    assert plan_ref.is_undirected(np.array([0, 0, 0], np.int32), np.zeros(0, np.int32))   # no edges
+    assert not plan_ref.is_undirected(np.array([0, 1], np.int32), np.array([3], np.int32))  # out-of-range source
+
+
 def test_build_bins_vs_bruteforce():
     rng = np.random.default_rng(32)
     deg = np.concatenate([rng.integers(0, 6, 200), rng.integers(30, 300, 40), [1000, 2500, 4097, 9000, 0, 1, 64, 65]])
