@@ -49,6 +49,17 @@ def test_fullsize_sampled_parity(cfg):
     lse = torch.empty((n, H), dtype=torch.float32, device="cuda")
     stat = torch.empty_like(lse)
     g1, g2 = (torch.empty((n, H, d), dtype=torch.float32, device="cuda") for _ in range(2))
+    # saved state and workspace are O(N*H*d), never O(E*H): the library allocates nothing, the
+    # binding allocates only the workspace the library asks for, and that is far below one E x H fp32 tensor
+    code = B.GNN_BF16 if dt == "bf16" else B.GNN_F32
+    ops = (B.GNN_OP_GT_FWD, B.GNN_OP_GT_BWD) if gt else (B.GNN_OP_GATV2_FWD, B.GNN_OP_GATV2_BWD)
+    ws_need = max(G.gnn_workspace_bytes(plan.handle, op, H, d, code) for op in ops)
+    assert ws_need <= 4 * n * H * d                      # at most one [n,H,d] fp32 tensor
+    if c["e"] >= 20 * n:                                 # cfg 3 / 5: a small fraction of one E x H fp32 tensor
+        assert ws_need <= 0.1 * (4 * c["e"] * H)
+    torch.cuda.synchronize()
+    torch.cuda.reset_peak_memory_stats()
+    mem0 = torch.cuda.memory_allocated()
     if gt:
         g3 = torch.empty((n, H, d), dtype=torch.float32, device="cuda")
         G.gnn_gt_attn_fwd(plan, T["q"], T["k"], T["v"], out, lse)
@@ -59,6 +70,8 @@ def test_fullsize_sampled_parity(cfg):
         G.gnn_gatv2_fwd(plan, T["xl"], T["xr"], a, c["slope"], out, lse)
         G.gnn_gatv2_bwd(plan, T["xl"], T["xr"], a, lse, T["do"], c["slope"], stat, g1, g2, g3)
     torch.cuda.synchronize()
+    extra = torch.cuda.max_memory_allocated() - mem0 - g3.numel() * 4
+    assert extra <= ws_need + (4 << 20), f"forward + backward allocated {extra} bytes beyond the workspace ({ws_need})"
 
     # ---- metadata, bit-exact on the full graph
     rp_t, ci_t = plan_ref.transpose_csr(c["rowptr"], c["colidx"])
