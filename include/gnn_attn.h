@@ -96,6 +96,14 @@ gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t dev_bytes, 
                             const gnn_plan_opts_t* opts, gnn_stream_t stream);
 void gnn_plan_destroy(gnn_plan_t* plan);
 
+/* Optional input check (the compute calls never range-check colidx: a bad index is an out-of-bounds gather).
+ * Verifies on the device that rowptr[0] == 0, rowptr[n] == nnz, rowptr is non-decreasing and every colidx is in
+ * [0, n).  rowptr / colidx: device.  Synchronises the stream.  GNN_EINVAL (message names the first kind of
+ * violation and the smallest offending position) if the CSR is malformed; uses no plan and no workspace
+ * beyond 16 bytes it takes from `scratch` (device, 16-byte aligned).                                 */
+gnn_status_t gnn_csr_validate(int32_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx, void* scratch,
+                              gnn_stream_t stream);
+
 /* Plan introspection for the bit-exact metadata check.  `what`:                                    */
 enum {
     GNN_PLAN_COUNTS = 0,    /* int32[8]: n_hub, n_cta, n_group, n_chunks, then the same 4 for CSR^T  */

@@ -21,7 +21,7 @@ GNN_TRANSPOSE_NONE, GNN_TRANSPOSE_BUILD, GNN_TRANSPOSE_UNDIRECTED = 0, 1, 2
  GNN_PLAN_BLOCK_REM_COLIDX, GNN_PLAN_FLAGS) = range(13)
 
 EXPORTED_SYMBOLS = [
-    "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
+    "gnn_csr_validate", "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
     "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
     "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_seg_minmax_fwd", "gnn_seg_minmax_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
     "gnn_profile_collect",
@@ -49,6 +49,7 @@ def lib() -> C.CDLL:
             raise GnnError(f"{_LIB_PATH} is missing: run `python -m paper_2605_31500_b200.build` "
                            "(there is no CPU fallback)")
         L = C.CDLL(_LIB_PATH)
+        L.gnn_csr_validate.argtypes = [_i32, _i64, _vp, _vp, _vp, _vp]
         L.gnn_plan_bytes.argtypes = [_i32, _i64, C.POINTER(PlanOpts), C.POINTER(_sz), C.POINTER(_sz)]
         L.gnn_plan_build.argtypes = [C.POINTER(_vp), _vp, _sz, _vp, _sz, _i32, _i64, _vp, _vp, C.POINTER(PlanOpts), _vp]
         L.gnn_plan_destroy.argtypes = [_vp]
@@ -154,6 +155,14 @@ def gnn_plan_build(dev_mem, scratch, n: int, nnz: int, rowptr, colidx, opts: Pla
     _check(lib().gnn_plan_build(C.byref(h), _ptr(dev_mem), dev_mem.numel(), _ptr(scratch), scratch.numel(), n, nnz,
                                 _ptr(rowptr), _ptr(colidx), C.byref(opts), _stream(stream)))
     return h
+
+
+def gnn_csr_validate(rowptr, colidx, stream=None):
+    """Raises GnnError unless (rowptr, colidx) is a well-formed int32 CSR with sources in [0, n) (device tensors)."""
+    torch = _require_cuda()
+    scratch = torch.empty(16, dtype=torch.uint8, device=rowptr.device)
+    _check(lib().gnn_csr_validate(int(rowptr.numel()) - 1, int(colidx.numel()), _ptr(rowptr), _ptr(colidx), _ptr(scratch),
+                                  _stream(stream)))
 
 
 def gnn_plan_destroy(handle):

@@ -134,6 +134,15 @@ __global__ void undirected_check_kernel(const int32_t* __restrict__ rowptr, cons
     if (a >= __ldg(rowptr + j + 1) || __ldg(colidx + a) != i) *flag = 1;
 }
 
+// gnn_csr_validate: err[0] = smallest row r with rowptr[r] > rowptr[r+1] (or n if none), err[1] = smallest entry with
+// colidx outside [0, n) (or nnz if none), kept in 64 bits as two atomicMin targets
+__global__ void csr_validate_kernel(const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx, int n,
+                                    long long nnz, unsigned long long* __restrict__ err) {
+    const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t < n && __ldg(rowptr + t) > __ldg(rowptr + t + 1)) atomicMin(err, (unsigned long long)t);
+    if (t < nnz && (unsigned)__ldg(colidx + t) >= (unsigned)n) atomicMin(err + 1, (unsigned long long)t);
+}
+
 // rowptr_t[j] = number of entries with source id < j = lower_bound(sorted source ids, j)
 __global__ void rowptr_t_kernel(const uint32_t* __restrict__ src_sorted, long long nnz, int n,
                                 int32_t* __restrict__ rowptr_t) {
@@ -428,6 +437,41 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
 }
 
 extern "C" void gnn_plan_destroy(gnn_plan_t* plan) { delete plan; }
+
+extern "C" gnn_status_t gnn_csr_validate(int32_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx,
+                                         void* scratch, gnn_stream_t stream) {
+    if (n < 1 || nnz < 0 || nnz >= (1ll << 31) || !rowptr || (!colidx && nnz > 0) || !scratch || ((uintptr_t)scratch & 15)) {
+        set_error("gnn_csr_validate: need n >= 1, 0 <= nnz < 2^31, non-NULL pointers and a 16-byte aligned scratch");
+        return GNN_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long init[2] = {(unsigned long long)n, (unsigned long long)nnz}, got[2];
+    int32_t ends[2] = {0, 0};
+    cudaError_t e = cudaMemcpyAsync(scratch, init, sizeof(init), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        const long long work = nnz > n ? nnz : n;
+        csr_validate_kernel<<<(unsigned)((work + 255) / 256), 256, 0, st>>>(rowptr, colidx, n, nnz, (unsigned long long*)scratch);
+        ++g_launches;
+        e = cudaMemcpyAsync(got, scratch, sizeof(got), cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&ends[0], rowptr, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&ends[1], rowptr + n, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { set_error("gnn_csr_validate: CUDA error: %s", cudaGetErrorString(e)); return GNN_ECUDA; }
+    if (ends[0] != 0 || ends[1] != nnz) {
+        set_error("gnn_csr_validate: rowptr[0] = %d (want 0), rowptr[n] = %d (want nnz = %lld)", ends[0], ends[1], (long long)nnz);
+        return GNN_EINVAL;
+    }
+    if (got[0] != (unsigned long long)n) {
+        set_error("gnn_csr_validate: rowptr decreases after row %llu", got[0]);
+        return GNN_EINVAL;
+    }
+    if (got[1] != (unsigned long long)nnz) {
+        set_error("gnn_csr_validate: colidx[%llu] is outside [0, n)", got[1]);
+        return GNN_EINVAL;
+    }
+    return GNN_OK;
+}
 
 extern "C" const int32_t* gnn_plan_rowptr_t(const gnn_plan_t* plan) { return plan ? plan->rowptr_t : nullptr; }
 extern "C" const int32_t* gnn_plan_colidx_t(const gnn_plan_t* plan) { return plan ? plan->colidx_t : nullptr; }

@@ -169,6 +169,26 @@ def _custom(layer, n, rowptr, colidx, H, d, dtype, seed=1):
     return c
 
 
+def test_csr_validate():
+    """gnn_csr_validate accepts every generated graph and names the first malformed spot of a broken one."""
+    import paper_2605_31500_b200 as G
+    torch = _torch()
+    c = GI.make_config(2, scale=0.03)
+    rp, ci = torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda()
+    G.gnn_csr_validate(rp, ci)
+    bad = ci.clone()
+    bad[1234], bad[777] = c["n"], -1
+    with pytest.raises(G.GnnError, match=r"colidx\[777\]"):
+        G.gnn_csr_validate(rp, bad)
+    bad_rp = rp.clone()
+    bad_rp[50] = bad_rp[51] + 1
+    with pytest.raises(G.GnnError, match="rowptr decreases after row 50"):
+        G.gnn_csr_validate(bad_rp, ci)
+    with pytest.raises(G.GnnError, match="rowptr\\[n\\]"):
+        G.gnn_csr_validate(rp, ci[:-1].contiguous())
+    G.gnn_csr_validate(torch.zeros(5, dtype=torch.int32, device="cuda"), torch.zeros(0, dtype=torch.int32, device="cuda"))
+
+
 @pytest.mark.parametrize("layer", ["gt", "gatv2"])
 def test_undirected_backward_reuses_forward_csr(layer):
     """Row f1: on an undirected graph the backward traverses the forward CSR; the plan stores no
