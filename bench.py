@@ -40,7 +40,7 @@ def parse():
     ap.add_argument("--cfg", type=int, default=3, help="BASELINE.json config 1..5 (default 3: the large power-law GT graph)")
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the workload (debug only; < 1 is not a bench value)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-steps", type=int, default=4)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--natural-ids", action="store_true",
@@ -398,6 +398,8 @@ def run_ours(args, rank, world, local_rank):
     total_ms = max_over_ranks(float(sum(ms_steps)), world, dev)
     value = job_gedges(e, args.steps, world, total_ms)
 
+    peak_mem = int(torch.cuda.max_memory_allocated(dev))   # the layer itself: inputs, outputs, plan, workspace (+ L2 flush buffer)
+
     block = None
     if args.cfg == 4:
         for _ in range(3):
@@ -526,28 +528,71 @@ def run_ours(args, rank, world, local_rank):
                   "frac_of_hbm_peak_bwd": mm_bwd_bytes / (np.mean(ms_mb) * 1e-3) * 1e-9 / peak}
         del mo, ma, mdx
 
-    # ---- end to end: pinned host inputs -> device, step, every output -> pinned host, all inside the events
+    # ---- end to end: pinned host inputs -> device, step, every output -> pinned host, all inside the timed region.
+    # Three streams (H2D, compute, D2H) and two sets of device feature / output buffers, so the copies of step k+1
+    # and k-1 overlap the kernels of step k (PCIe is full duplex); the CSR goes into the plan's own buffers once the
+    # previous step's kernels are done.  Time = first H2D start -> last D2H end, pipeline fill and drain included.
     e2e = None
     if args.e2e_steps > 0:
+        ksteps = args.e2e_steps
         pin_in = {k: v.pin_memory() for k, v in host.items()}
         pin_out = [torch.empty(o.shape, dtype=o.dtype, pin_memory=True) for o in outs]
+        feat = [k for k in host if k not in ("rowptr", "colidx")]
+        dsets = [devt, {**devt, **{k: torch.empty_like(devt[k]) for k in feat}}]
+        osets = [outs, [torch.empty_like(o) for o in outs]]
+        s_in, s_c, s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
 
-        def e2e_step():
-            for k2, v in pin_in.items():
-                devt[k2].copy_(v, non_blocking=True)
-            step()
-            for po, o in zip(pin_out, outs):
-                po.copy_(o, non_blocking=True)
+        def step_on(D, O):
+            o_, l_, st_, a1, a2, a3 = O
+            if gt:
+                G.gnn_gt_attn_fwd(plan, D["q"], D["k"], D["v"], o_, l_)
+                G.gnn_gt_attn_bwd(plan, D["q"], D["k"], D["v"], l_, D["do"], st_, a1, a2, a3)
+            else:
+                G.gnn_gatv2_fwd(plan, D["xl"], D["xr"], D["a"], c["slope"], o_, l_)
+                G.gnn_gatv2_bwd(plan, D["xl"], D["xr"], D["a"], l_, D["do"], c["slope"], st_, a1, a2, a3)
 
-        e2e_step()
+        def e2e_run(k):
+            ev_in, ev_c, ev_out = [], [], []
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(s_in):
+                t0.record()
+            for i in range(k):
+                D, O = dsets[i % 2], osets[i % 2]
+                with torch.cuda.stream(s_in):
+                    if i >= 2:
+                        s_in.wait_event(ev_c[i - 2])          # feature set i % 2 is free again
+                    for k2 in feat:
+                        D[k2].copy_(pin_in[k2], non_blocking=True)
+                    if i >= 1:
+                        s_in.wait_event(ev_c[i - 1])          # the CSR buffers are the plan's: no kernel may be reading
+                    for k2 in ("rowptr", "colidx"):
+                        D[k2].copy_(pin_in[k2], non_blocking=True)
+                    ev_in.append(torch.cuda.Event()); ev_in[-1].record()
+                with torch.cuda.stream(s_c):
+                    s_c.wait_event(ev_in[i])
+                    if i >= 2:
+                        s_c.wait_event(ev_out[i - 2])         # output set i % 2 has been read back
+                    step_on(D, O)
+                    ev_c.append(torch.cuda.Event()); ev_c[-1].record()
+                with torch.cuda.stream(s_out):
+                    s_out.wait_event(ev_c[i])
+                    for po, o in zip(pin_out, O):
+                        po.copy_(o, non_blocking=True)
+                    ev_out.append(torch.cuda.Event()); ev_out[-1].record()
+            with torch.cuda.stream(s_out):
+                t1.record()
+            torch.cuda.synchronize()
+            return t0.elapsed_time(t1)
+
         barrier()
-        ms_e2e = timed(e2e_step, args.e2e_steps)
-        t_e2e = max_over_ranks(float(sum(ms_e2e)), world, dev)
-        e2e = {"value": job_gedges(e, args.e2e_steps, world, t_e2e), "unit": UNIT,
-               "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes, "steps": args.e2e_steps,
-               "ms_per_step": t_e2e / args.e2e_steps}
-        del pin_in, pin_out
-    peak_mem = int(torch.cuda.max_memory_allocated(dev))
+        e2e_run(2)
+        barrier()
+        t_e2e = max_over_ranks(float(e2e_run(ksteps)), world, dev)
+        e2e = {"value": job_gedges(e, ksteps, world, t_e2e), "unit": UNIT,
+               "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes, "steps": ksteps,
+               "ms_per_step": t_e2e / ksteps,
+               "pipeline": "3 streams, double-buffered features and outputs; fill and drain inside the timed region"}
+        del pin_in, pin_out, dsets, osets
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
