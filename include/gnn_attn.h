@@ -24,9 +24,12 @@
  *     [n, heads, head_dim] regardless of the feature dtype (reading A9); the forward
  *     output O has the feature dtype (bf16: round-to-nearest-even of the fp32 accumulator).
  *     All arithmetic is fp32.
- *   - Supported shapes: head_dim a power of two with head_dim*sizeof(elt) >= 16 bytes,
- *     heads*head_dim*sizeof(elt) <= 1024 bytes, and heads*head_dim*sizeof(elt) / min(head_dim*sizeof(elt), 32)
- *     <= 32 (a row must fit one warp at 32 bytes per lane).  Anything else returns GNN_EUNSUPPORTED.
+ *   - Supported shapes: head_dim a power of two with 16 <= head_dim*sizeof(elt) <= 1024 bytes, any heads >= 1.
+ *     One launch covers a row slice of at most 1024 bytes (32 lanes x 32 bytes); wider rows - e.g. the paper's
+ *     fp32 (H, D) = (4, 128), (8, 64), (2, 256) grid points, PAPER.md:126-153 - are processed as consecutive
+ *     head groups (at most 64) through the full-row strides, which changes no result because heads are
+ *     independent in every pass.  Anything else returns GNN_EUNSUPPORTED.  gnn_seg_minmax_fwd and
+ *     gnn_gt_attn_fwd_block state their own limits.
  *   - Every compute call is asynchronous on `stream` and never synchronises.  gnn_plan_build
  *     synchronises `stream` (it reads a few counters back to the host).
  *   - Return value: GNN_OK or an error code; nothing is launched when an error is returned for

@@ -53,9 +53,47 @@ bool make_shape(int32_t n, int32_t heads, int32_t head_dim, int dtype, Shape& sh
         return false;
     }
     sh.n = n; sh.H = heads; sh.d = head_dim; sh.rowe = heads * head_dim;
+    sh.ld = sh.rowe; sh.ldh = heads;
     sh.ch = sh.lanes = sh.lpl = sh.lpl_log2 = 0;  // filled per pass (pass_shape)
     return true;
 }
+
+// One launch covers rows of at most 1024 bytes (32 lanes x 32 bytes).  Wider rows (e.g. the paper's fp32 H=4, D=128
+// grid points) are processed as consecutive HEAD GROUPS: group g runs the same passes on heads
+// [h0, h0 + H_g) through pointers offset by h0 and the full-row strides ld = heads*head_dim, ldh = heads.  Heads
+// are independent in every pass (softmax, gradients and da are per head), so the result is that of one launch.
+struct HeadGroup { Shape sh; int h0; };
+constexpr int kMaxHeadGroups = 64;
+int head_groups(int32_t n, int32_t heads, int32_t head_dim, int dtype, HeadGroup* out, const char* who) {
+    Shape sh;
+    if (dtype != GNN_F32 && dtype != GNN_BF16) { set_error("%s: unknown dtype %d", who, dtype); return 0; }
+    const int esz = dtype == GNN_F32 ? 4 : 2;
+    const long long hb = (long long)head_dim * esz;
+    int hg = 0;
+    if (heads >= 1 && head_dim >= 1 && !(head_dim & (head_dim - 1)) && hb >= 16 && hb <= 1024) {
+        // widest group one launch supports; a group that is not the whole row must keep the 32-byte alignment of
+        // the 256-bit gathers at its byte offset h0 * head_dim * sizeof
+        hg = (int)(1024 / hb) < heads ? (int)(1024 / hb) : heads;
+        while (hg >= 1 && !((hg == heads || (hg * hb) % 32 == 0) && make_shape(n, hg, head_dim, dtype, sh, who))) --hg;
+    }
+    if (hg < 1 || (heads + hg - 1) / hg > kMaxHeadGroups) {
+        set_error("%s: unsupported shape heads=%d head_dim=%d dtype=%d (head_dim must be a power of two with "
+                  "16 <= head_dim*sizeof <= 1024; at most %d head groups)", who, heads, head_dim, dtype, kMaxHeadGroups);
+        return 0;
+    }
+    int ng = 0;
+    for (int h0 = 0; h0 < heads; h0 += hg, ++ng) {
+        const int h = heads - h0 < hg ? heads - h0 : hg;
+        if (!make_shape(n, h, head_dim, dtype, sh, who)) return 0;
+        sh.ld = heads * head_dim;
+        sh.ldh = heads;
+        out[ng] = {sh, h0};
+    }
+    return ng;
+}
+// workspace of a call = max over its head groups
+template <class T> T* off_bytes(T* p, size_t bytes) { return (T*)((char*)p + bytes); }
+template <class T> const T* off_bytes(const T* p, size_t bytes) { return (const T*)((const char*)p + bytes); }
 
 bool aligned16(const void* p) { return (((uintptr_t)p) & 31) == 0; }  // 256-bit gathers need 32-byte alignment
 
@@ -89,9 +127,18 @@ WsLayout ws_layout(const gnn_plan* P, int op, const Shape& sh, int esz) {
         da = (size_t)w.da_slots * sh.rowe * sizeof(float);
     }
     w.stat2 = (w.da_part + da + 255) / 256 * 256;
-    const size_t st2 = (op == GNN_OP_GT_BWD) ? (size_t)P->n * sh.H * sizeof(float2) : 0;   // (L log2e, Delta) for the GT src pass
+    const size_t st2 = (op == GNN_OP_GT_BWD) ? (size_t)P->n * sh.ldh * sizeof(float2) : 0;   // (L log2e, Delta) for the GT src pass
     w.total = w.stat2 + st2 + 256;
     return w;
+}
+
+size_t ws_total(const gnn_plan* P, int op, const HeadGroup* hg, int ng, int esz) {
+    size_t t = 0;
+    for (int g = 0; g < ng; ++g) {
+        const size_t x = ws_layout(P, op, hg[g].sh, esz).total;
+        if (x > t) t = x;
+    }
+    return t;
 }
 
 bool check_common(const gnn_plan* P, const int32_t* rowptr, const int32_t* colidx, int32_t n, const char* who) {
@@ -159,15 +206,16 @@ extern "C" gnn_status_t gnn_workspace_bytes(const gnn_plan_t* P, int op, int32_t
         set_error("gnn_workspace_bytes: unknown op %d", op);
         return GNN_EINVAL;
     }
-    Shape sh;
+    HeadGroup hg[kMaxHeadGroups];
+    int ng = 1;
     if (op == GNN_OP_SEG_MINMAX_FWD) {
-        if (heads < 1 || head_dim < 1 || !agg_shape(P->n, heads * head_dim, dtype, sh, "gnn_workspace_bytes")) return GNN_EUNSUPPORTED;
-    } else if (!make_shape(P->n, heads, head_dim, dtype, sh, "gnn_workspace_bytes")) return GNN_EUNSUPPORTED;
+        if (heads < 1 || head_dim < 1 || !agg_shape(P->n, heads * head_dim, dtype, hg[0].sh, "gnn_workspace_bytes")) return GNN_EUNSUPPORTED;
+    } else if (!(ng = head_groups(P->n, heads, head_dim, dtype, hg, "gnn_workspace_bytes"))) return GNN_EUNSUPPORTED;
     if ((op == GNN_OP_GT_BWD || op == GNN_OP_GATV2_BWD) && !P->opts.build_transpose) {
         set_error("gnn_workspace_bytes: backward needs a plan built with build_transpose");
         return GNN_EINVAL;
     }
-    *bytes = ws_layout(P, op, sh, dtype == GNN_F32 ? 4 : 2).total;
+    *bytes = ws_total(P, op, hg, ng, dtype == GNN_F32 ? 4 : 2);
     return GNN_OK;
 }
 
@@ -182,13 +230,21 @@ extern "C" gnn_status_t gnn_gt_attn_fwd(const gnn_plan_t* P, const int32_t* rowp
         set_error("%s: feature pointers and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
-    Shape sh;
-    if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
-    const WsLayout w = ws_layout(P, GNN_OP_GT_FWD, sh, dtype == GNN_F32 ? 4 : 2);
-    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
-    GtArgs a = {};
-    a.q = q; a.k = k; a.v = v; a.out = out; a.lse = lse;
-    return cuda_status(launch_gt_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a), who);
+    HeadGroup hg[kMaxHeadGroups];
+    const int ng = head_groups(n, heads, head_dim, dtype, hg, who), esz = dtype == GNN_F32 ? 4 : 2;
+    if (!ng) return GNN_EUNSUPPORTED;
+    const size_t need = ws_total(P, GNN_OP_GT_FWD, hg, ng, esz);
+    if (ws_bytes < need) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, need); return GNN_EWORKSPACE; }
+    cudaError_t e = cudaSuccess;
+    for (int g = 0; g < ng && e == cudaSuccess; ++g) {
+        const Shape& sh = hg[g].sh;
+        const size_t fo = (size_t)hg[g].h0 * head_dim * esz;   // byte offset of the group's first head in a feature row
+        const WsLayout w = ws_layout(P, GNN_OP_GT_FWD, sh, esz);
+        GtArgs a = {};
+        a.q = off_bytes(q, fo); a.k = off_bytes(k, fo); a.v = off_bytes(v, fo); a.out = off_bytes(out, fo); a.lse = lse + hg[g].h0;
+        e = launch_gt_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a);
+    }
+    return cuda_status(e, who);
 }
 
 extern "C" gnn_status_t gnn_gt_attn_bwd(const gnn_plan_t* P, const int32_t* rowptr, const int32_t* colidx, int32_t n,
@@ -208,16 +264,25 @@ extern "C" gnn_status_t gnn_gt_attn_bwd(const gnn_plan_t* P, const int32_t* rowp
         set_error("%s: feature/gradient pointers and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
-    Shape sh;
-    if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
-    const WsLayout w = ws_layout(P, GNN_OP_GT_BWD, sh, dtype == GNN_F32 ? 4 : 2);
-    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
-    GtArgs a = {};
-    a.q = q; a.k = k; a.v = v; a.dout = dout; a.lse = const_cast<float*>(lse); a.delta = delta;
-    a.dq = dq; a.dk = dk; a.dv = dv;
-    a.stat2 = (float2*)((char*)ws + w.stat2);
-    cudaError_t e = launch_gt_bwd_dst(dtype, sh, make_ctx(P, false, ws, w, stream), a);   // dQ, Delta
-    if (e == cudaSuccess) e = launch_gt_bwd_src(dtype, sh, make_ctx(P, true, ws, w, stream), a);  // dK, dV
+    HeadGroup hg[kMaxHeadGroups];
+    const int ng = head_groups(n, heads, head_dim, dtype, hg, who), esz = dtype == GNN_F32 ? 4 : 2;
+    if (!ng) return GNN_EUNSUPPORTED;
+    const size_t need = ws_total(P, GNN_OP_GT_BWD, hg, ng, esz);
+    if (ws_bytes < need) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, need); return GNN_EWORKSPACE; }
+    cudaError_t e = cudaSuccess;
+    for (int g = 0; g < ng && e == cudaSuccess; ++g) {
+        const Shape& sh = hg[g].sh;
+        const int h0 = hg[g].h0;
+        const size_t fo = (size_t)h0 * head_dim * esz, go = (size_t)h0 * head_dim;
+        const WsLayout w = ws_layout(P, GNN_OP_GT_BWD, sh, esz);
+        GtArgs a = {};
+        a.q = off_bytes(q, fo); a.k = off_bytes(k, fo); a.v = off_bytes(v, fo); a.dout = off_bytes(dout, fo);
+        a.lse = const_cast<float*>(lse) + h0; a.delta = delta + h0;
+        a.dq = dq + go; a.dk = dk + go; a.dv = dv + go;
+        a.stat2 = (float2*)((char*)ws + w.stat2) + h0;
+        e = launch_gt_bwd_dst(dtype, sh, make_ctx(P, false, ws, w, stream), a);                        // dQ, Delta
+        if (e == cudaSuccess) e = launch_gt_bwd_src(dtype, sh, make_ctx(P, true, ws, w, stream), a);   // dK, dV
+    }
     return cuda_status(e, who);
 }
 
@@ -233,13 +298,22 @@ extern "C" gnn_status_t gnn_gatv2_fwd(const gnn_plan_t* P, const int32_t* rowptr
         set_error("%s: feature pointers, a and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
-    Shape sh;
-    if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
-    const WsLayout w = ws_layout(P, GNN_OP_GATV2_FWD, sh, dtype == GNN_F32 ? 4 : 2);
-    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
-    GatArgs a = {};
-    a.xl = xl; a.xr = xr; a.a = a_; a.out = out; a.lse = lse; a.slope = slope;
-    return cuda_status(launch_gat_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a), who);
+    HeadGroup hg[kMaxHeadGroups];
+    const int ng = head_groups(n, heads, head_dim, dtype, hg, who), esz = dtype == GNN_F32 ? 4 : 2;
+    if (!ng) return GNN_EUNSUPPORTED;
+    const size_t need = ws_total(P, GNN_OP_GATV2_FWD, hg, ng, esz);
+    if (ws_bytes < need) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, need); return GNN_EWORKSPACE; }
+    cudaError_t e = cudaSuccess;
+    for (int g = 0; g < ng && e == cudaSuccess; ++g) {
+        const Shape& sh = hg[g].sh;
+        const size_t fo = (size_t)hg[g].h0 * head_dim * esz;
+        const WsLayout w = ws_layout(P, GNN_OP_GATV2_FWD, sh, esz);
+        GatArgs a = {};
+        a.xl = off_bytes(xl, fo); a.xr = off_bytes(xr, fo); a.a = a_ + (size_t)hg[g].h0 * head_dim;
+        a.out = off_bytes(out, fo); a.lse = lse + hg[g].h0; a.slope = slope;
+        e = launch_gat_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a);
+    }
+    return cuda_status(e, who);
 }
 
 extern "C" gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* P, const int32_t* rowptr, const int32_t* colidx, int32_t n,
@@ -260,19 +334,28 @@ extern "C" gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* P, const int32_t* rowptr
         set_error("%s: feature/gradient pointers, a and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
-    Shape sh;
-    if (!make_shape(n, heads, head_dim, dtype, sh, who)) return GNN_EUNSUPPORTED;
-    const WsLayout w = ws_layout(P, GNN_OP_GATV2_BWD, sh, dtype == GNN_F32 ? 4 : 2);
-    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
-    GatArgs a = {};
-    a.xl = xl; a.xr = xr; a.a = a_; a.dout = dout; a.lse = const_cast<float*>(lse); a.g = g; a.dxl = dxl; a.dxr = dxr;
-    a.slope = slope;
-    const LaunchCtx c = make_ctx(P, false, ws, w, stream);
-    LaunchCtx ct = make_ctx(P, true, ws, w, stream);
-    ct.da_slot_base = w.da_slots_dst;
-    cudaError_t e = launch_gat_bwd_dst(dtype, sh, c, a);                                   // dxl, G, da partials (xl . S)
-    if (e == cudaSuccess) e = launch_gat_bwd_src(dtype, sh, ct, a);                        // dxr, da partials (xr . U)
-    if (e == cudaSuccess) e = launch_da_reduce(c.da_part, w.da_slots, sh.rowe, da, c.stream);  // da
+    HeadGroup hg[kMaxHeadGroups];
+    const int ng = head_groups(n, heads, head_dim, dtype, hg, who), esz = dtype == GNN_F32 ? 4 : 2;
+    if (!ng) return GNN_EUNSUPPORTED;
+    const size_t need = ws_total(P, GNN_OP_GATV2_BWD, hg, ng, esz);
+    if (ws_bytes < need) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, need); return GNN_EWORKSPACE; }
+    cudaError_t e = cudaSuccess;
+    for (int gi = 0; gi < ng && e == cudaSuccess; ++gi) {
+        const Shape& sh = hg[gi].sh;
+        const int h0 = hg[gi].h0;
+        const size_t fo = (size_t)h0 * head_dim * esz, go = (size_t)h0 * head_dim;
+        const WsLayout w = ws_layout(P, GNN_OP_GATV2_BWD, sh, esz);
+        GatArgs a = {};
+        a.xl = off_bytes(xl, fo); a.xr = off_bytes(xr, fo); a.a = a_ + go; a.dout = off_bytes(dout, fo);
+        a.lse = const_cast<float*>(lse) + h0; a.g = g + h0; a.dxl = dxl + go; a.dxr = dxr + go;
+        a.slope = slope;
+        const LaunchCtx c = make_ctx(P, false, ws, w, stream);
+        LaunchCtx ct = make_ctx(P, true, ws, w, stream);
+        ct.da_slot_base = w.da_slots_dst;
+        e = launch_gat_bwd_dst(dtype, sh, c, a);                                                       // dxl, G, da partials (xl . S)
+        if (e == cudaSuccess) e = launch_gat_bwd_src(dtype, sh, ct, a);                                // dxr, da partials (xr . U)
+        if (e == cudaSuccess) e = launch_da_reduce(c.da_part, w.da_slots, sh.rowe, da + go, c.stream);  // da
+    }
     return cuda_status(e, who);
 }
 

@@ -56,7 +56,10 @@ struct Shape {
     int n;          // nodes
     int H;          // heads
     int d;          // head_dim
-    int rowe;       // H * d elements per feature row
+    int rowe;       // H * d elements per feature row (of the heads this launch processes)
+    int ld;         // elements between consecutive rows of the [n, H_total, d] tensors (== rowe unless the call
+                    // was split into head groups, api.cu)
+    int ldh;        // elements between consecutive rows of the [n, H_total] arrays (lse, Delta, G, stat2)
     int ch;         // channels per lane (CH)
     int lanes;      // active lanes per row = rowe / ch
     int lpl;        // lanes per head = d / ch (power of two)

@@ -46,7 +46,7 @@ template <typename T, int CB_, int G_, int KU_, bool SORTED> struct MinFwdT : Op
                                                   Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u)
-            src.c[u][0].load_global(p.x, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff, nbr[u] >= 0 && g.act);
+            src.c[u][0].load_global(p.x, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.ld + g.eoff, nbr[u] >= 0 && g.act);
     }
     __device__ __forceinline__ static void compute(St& st, const Own&, const Params& p, const Shape&,
                                                    const int (&nbr)[KU], const GeoT&, const Src& src) {
@@ -79,8 +79,8 @@ template <typename T, int CB_, int G_, int KU_, bool SORTED> struct MinFwdT : Op
             a[c] = st.acc[1][c];
         }
         if (g.act) {
-            store_feat<CH>(p.out, (size_t)row * sh.rowe + g.eoff, o);
-            store_f32<CH>(reinterpret_cast<float*>(p.arg), (size_t)row * sh.rowe + g.eoff, a);   // bit copies
+            store_feat<CH>(p.out, (size_t)row * sh.ld + g.eoff, o);
+            store_f32<CH>(reinterpret_cast<float*>(p.arg), (size_t)row * sh.ld + g.eoff, a);   // bit copies
         }
     }
 };

@@ -42,7 +42,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
         Ck c;
-        c.load_global(p.xl, (size_t)row * sh.rowe + g.eoff, valid && g.act);
+        c.load_global(p.xl, (size_t)row * sh.ld + g.eoff, valid && g.act);
         c.to_float(o.xl);
         load_f32<CH>(p.a, g.eoff, g.act, o.a);
         const LreluK lk(p.slope);
@@ -54,7 +54,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G
                                                   Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u)
-            src.c[u][0].load_global(p.xr, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff, nbr[u] >= 0 && g.act);
+            src.c[u][0].load_global(p.xr, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.ld + g.eoff, nbr[u] >= 0 && g.act);
     }
     __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
                                                    const int (&nbr)[KU], const GeoT& g, const Src& src) {
@@ -93,8 +93,8 @@ template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G
         float o[CH];
 #pragma unroll
         for (int c = 0; c < CH; ++c) o[c] = st.acc[0][c] * inv;
-        if (g.act) store_feat<CH>(p.out, (size_t)row * sh.rowe + g.eoff, o);
-        if (g.lead) p.lse[(size_t)row * sh.H + g.hd] = l > 0.f ? (st.m + lg2(l)) * kLn2 : -INFINITY;
+        if (g.act) store_feat<CH>(p.out, (size_t)row * sh.ld + g.eoff, o);
+        if (g.lead) p.lse[(size_t)row * sh.ldh + g.hd] = l > 0.f ? (st.m + lg2(l)) * kLn2 : -INFINITY;
     }
 };
 
@@ -132,21 +132,21 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
                                                     const GeoT& g) {
         const bool pr = valid && g.act;
         Ck c0;
-        c0.load_global(p.xl, (size_t)row * sh.rowe + g.eoff, pr);
+        c0.load_global(p.xl, (size_t)row * sh.ld + g.eoff, pr);
         c0.to_float(o.xl);
-        o.go.load_global(p.dout, (size_t)row * sh.rowe + g.eoff, pr);
+        o.go.load_global(p.dout, (size_t)row * sh.ld + g.eoff, pr);
         load_f32<CH>(p.a, g.eoff, g.act, o.a);
         const LreluK lk(p.slope);
         o.k = lk.k;
 #pragma unroll
         for (int i = 0; i < CH; ++i) o.a[i] *= kLog2e * lk.c1;
-        o.lp = pr ? __ldg(p.lse + (size_t)row * sh.H + g.hd) * kLog2e : 0.f;
+        o.lp = pr ? __ldg(p.lse + (size_t)row * sh.ldh + g.hd) * kLog2e : 0.f;
     }
     __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
                                                   Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u)
-            src.c[u][0].load_global(p.xr, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff, nbr[u] >= 0 && g.act);
+            src.c[u][0].load_global(p.xr, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.ld + g.eoff, nbr[u] >= 0 && g.act);
     }
     __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
                                                    const int (&nbr)[KU], const GeoT& g, const Src& src) {
@@ -187,7 +187,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
         const float gs = p.slope * gg, as = p.slope * st.sc[1];
         float xl[CH], a[CH], o[CH];
         Ck c0;
-        c0.load_global(p.xl, (size_t)row * sh.rowe + g.eoff, g.act);
+        c0.load_global(p.xl, (size_t)row * sh.ld + g.eoff, g.act);
         c0.to_float(xl);
         load_f32<CH>(p.a, g.eoff, g.act, a);
 #pragma unroll
@@ -196,8 +196,8 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
             o[c] = a[c] * sdash;
             da[c] = fmaf(xl[c], sdash, da[c]);
         }
-        if (g.act) store_f32<CH>(p.dxl, (size_t)row * sh.rowe + g.eoff, o);
-        if (g.lead) p.g[(size_t)row * sh.H + g.hd] = gg;
+        if (g.act) store_f32<CH>(p.dxl, (size_t)row * sh.ld + g.eoff, o);
+        if (g.lead) p.g[(size_t)row * sh.ldh + g.hd] = gg;
     }
 };
 
@@ -226,7 +226,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
 
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
-        o.xr.load_global(p.xr, (size_t)row * sh.rowe + g.eoff, valid && g.act);
+        o.xr.load_global(p.xr, (size_t)row * sh.ld + g.eoff, valid && g.act);
         o.xr.to_float(o.xrf);
         load_f32<CH>(p.a, g.eoff, g.act, o.a);
         const LreluK lk(p.slope);
@@ -240,10 +240,10 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
         for (int u = 0; u < KU; ++u) {
             const bool pr = nbr[u] >= 0 && g.act;
             const size_t i = (size_t)(nbr[u] < 0 ? 0 : nbr[u]);
-            src.c[u][0].load_global(p.xl, i * sh.rowe + g.eoff, pr);
-            src.c[u][1].load_global(p.dout, i * sh.rowe + g.eoff, pr);
-            src.s[u][0] = pr ? __ldg(p.lse + i * sh.H + g.hd) : 0.f;
-            src.s[u][1] = pr ? __ldg(p.g + i * sh.H + g.hd) : 0.f;
+            src.c[u][0].load_global(p.xl, i * sh.ld + g.eoff, pr);
+            src.c[u][1].load_global(p.dout, i * sh.ld + g.eoff, pr);
+            src.s[u][0] = pr ? __ldg(p.lse + i * sh.ldh + g.hd) : 0.f;
+            src.s[u][1] = pr ? __ldg(p.g + i * sh.ldh + g.hd) : 0.f;
         }
     }
     __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
@@ -281,7 +281,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
                                                     const GeoT& g, float (&da)[CH]) {
         float xr[CH], a[CH], o[CH];
         Ck c0;
-        c0.load_global(p.xr, (size_t)row * sh.rowe + g.eoff, g.act);
+        c0.load_global(p.xr, (size_t)row * sh.ld + g.eoff, g.act);
         c0.to_float(xr);
         load_f32<CH>(p.a, g.eoff, g.act, a);
 #pragma unroll
@@ -292,7 +292,7 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
             o[c] = fmaf(a[c], u, st.acc[0][c]);
             da[c] = fmaf(xr[c], u, da[c]);
         }
-        if (g.act) store_f32<CH>(p.dxr, (size_t)row * sh.rowe + g.eoff, o);
+        if (g.act) store_f32<CH>(p.dxr, (size_t)row * sh.ld + g.eoff, o);
     }
 };
 

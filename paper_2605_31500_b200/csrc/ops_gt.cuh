@@ -65,14 +65,14 @@ template <typename T, int CB_, int G_, int KU_> struct GtFwd : OpBase<T, CB_, G_
 
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
-        o.q.load_global(p.q, (size_t)row * sh.rowe + g.eoff, valid && g.act);
+        o.q.load_global(p.q, (size_t)row * sh.ld + g.eoff, valid && g.act);
     }
     __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
                                                   Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
             const bool pr = nbr[u] >= 0 && g.act;
-            const size_t off = (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff;
+            const size_t off = (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.ld + g.eoff;
             src.c[u][0].load_global(p.k, off, pr);
             src.c[u][1].load_global(p.v, off, pr);
         }
@@ -106,8 +106,8 @@ template <typename T, int CB_, int G_, int KU_> struct GtFwd : OpBase<T, CB_, G_
         float o[CH];
 #pragma unroll
         for (int c = 0; c < CH; ++c) o[c] = st.acc[0][c] * inv;
-        if (g.act) store_feat<CH>(p.out, (size_t)row * sh.rowe + g.eoff, o);
-        if (g.lead) p.lse[(size_t)row * sh.H + g.hd] = l > 0.f ? (st.m + lg2(l)) * kLn2 : -INFINITY;
+        if (g.act) store_feat<CH>(p.out, (size_t)row * sh.ld + g.eoff, o);
+        if (g.lead) p.lse[(size_t)row * sh.ldh + g.hd] = l > 0.f ? (st.m + lg2(l)) * kLn2 : -INFINITY;
     }
 };
 
@@ -138,16 +138,16 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdDst : OpBase<T, CB_,
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
         const bool pr = valid && g.act;
-        o.q.load_global(p.q, (size_t)row * sh.rowe + g.eoff, pr);
-        o.go.load_global(p.dout, (size_t)row * sh.rowe + g.eoff, pr);
-        o.lp = pr ? __ldg(p.lse + (size_t)row * sh.H + g.hd) * kLog2e : 0.f;
+        o.q.load_global(p.q, (size_t)row * sh.ld + g.eoff, pr);
+        o.go.load_global(p.dout, (size_t)row * sh.ld + g.eoff, pr);
+        o.lp = pr ? __ldg(p.lse + (size_t)row * sh.ldh + g.hd) * kLog2e : 0.f;
     }
     __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
                                                   Src& src) {
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
             const bool pr = nbr[u] >= 0 && g.act;
-            const size_t off = (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.rowe + g.eoff;
+            const size_t off = (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.ld + g.eoff;
             src.c[u][0].load_global(p.k, off, pr);
             src.c[u][1].load_global(p.v, off, pr);
         }
@@ -182,10 +182,10 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdDst : OpBase<T, CB_,
         float o[CH];
 #pragma unroll
         for (int c = 0; c < CH; ++c) o[c] = (st.acc[0][c] - dl * st.acc[1][c]) * p.inv_sqrt_d;
-        if (g.act) store_f32<CH>(p.dq, (size_t)row * sh.rowe + g.eoff, o);
+        if (g.act) store_f32<CH>(p.dq, (size_t)row * sh.ld + g.eoff, o);
         if (g.lead) {
-            p.delta[(size_t)row * sh.H + g.hd] = dl;
-            p.stat2[(size_t)row * sh.H + g.hd] = make_float2(__ldg(p.lse + (size_t)row * sh.H + g.hd) * kLog2e, dl);
+            p.delta[(size_t)row * sh.ldh + g.hd] = dl;
+            p.stat2[(size_t)row * sh.ldh + g.hd] = make_float2(__ldg(p.lse + (size_t)row * sh.ldh + g.hd) * kLog2e, dl);
         }
     }
 };
@@ -216,8 +216,8 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_,
     __device__ __forceinline__ static void load_own(Own& o, const Params& p, const Shape& sh, int row, bool valid,
                                                     const GeoT& g) {
         const bool pr = valid && g.act;
-        o.k.load_global(p.k, (size_t)row * sh.rowe + g.eoff, pr);
-        o.v.load_global(p.v, (size_t)row * sh.rowe + g.eoff, pr);
+        o.k.load_global(p.k, (size_t)row * sh.ld + g.eoff, pr);
+        o.v.load_global(p.v, (size_t)row * sh.ld + g.eoff, pr);
     }
     __device__ __forceinline__ static void gather(const Params& p, const Shape& sh, const int (&nbr)[KU], const GeoT& g,
                                                   Src& src) {
@@ -225,9 +225,9 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_,
         for (int u = 0; u < KU; ++u) {
             const bool pr = nbr[u] >= 0 && g.act;
             const size_t i = (size_t)(nbr[u] < 0 ? 0 : nbr[u]);
-            src.c[u][0].load_global(p.q, i * sh.rowe + g.eoff, pr);
-            src.c[u][1].load_global(p.dout, i * sh.rowe + g.eoff, pr);
-            const float2 t = pr ? __ldg(p.stat2 + i * sh.H + g.hd) : make_float2(0.f, 0.f);
+            src.c[u][0].load_global(p.q, i * sh.ld + g.eoff, pr);
+            src.c[u][1].load_global(p.dout, i * sh.ld + g.eoff, pr);
+            const float2 t = pr ? __ldg(p.stat2 + i * sh.ldh + g.hd) : make_float2(0.f, 0.f);
             src.s[u][0] = t.x;
             src.s[u][1] = t.y;
         }
@@ -261,8 +261,8 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_,
 #pragma unroll
         for (int c = 0; c < CH; ++c) o[c] = st.acc[0][c] * p.inv_sqrt_d;
         if (g.act) {
-            store_f32<CH>(p.dk, (size_t)row * sh.rowe + g.eoff, o);
-            store_f32<CH>(p.dv, (size_t)row * sh.rowe + g.eoff, st.acc[1]);
+            store_f32<CH>(p.dk, (size_t)row * sh.ld + g.eoff, o);
+            store_f32<CH>(p.dv, (size_t)row * sh.ld + g.eoff, st.acc[1]);
         }
     }
 };

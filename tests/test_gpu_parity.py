@@ -227,7 +227,12 @@ def test_undirected_backward_reuses_forward_csr(layer):
 
 @pytest.mark.parametrize("layer", ["gt", "gatv2"])
 @pytest.mark.parametrize("dtype,H,d", [("f32", 1, 4), ("f32", 3, 8), ("f32", 2, 128), ("bf16", 1, 8), ("bf16", 3, 16),
-                                       ("bf16", 5, 32), ("bf16", 8, 64), ("bf16", 2, 256), ("f32", 8, 32)])
+                                       ("bf16", 5, 32), ("bf16", 8, 64), ("bf16", 2, 256), ("f32", 8, 32),
+                                       # rows wider than one launch (1024 B): head groups (4,128)/(8,64)/(2,256) fp32
+                                       # are the paper's grid points; (5,256) bf16 = groups of 2+2+1, (5,128) f32 = 2+2+1,
+                                       # (40,8) bf16 = 640 B rows that need 40 lanes -> groups of 32+8
+                                       ("f32", 4, 128), ("f32", 8, 64), ("f32", 2, 256), ("bf16", 5, 256),
+                                       ("f32", 5, 128), ("bf16", 40, 8), ("bf16", 2, 512)])
 def test_shapes(layer, dtype, H, d):
     """All lane-group widths (8/16/32 lanes, 1-2 vectors per lane), non-power-of-two head counts, rows that
     do not fill the lane group, on a skewed multigraph with EMPTY rows and duplicate entries."""
