@@ -204,8 +204,8 @@ gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* plan, const int32_t* rowptr
  *   out[i,c] = min (mode GNN_AGG_MIN) or max (GNN_AGG_MAX) over the stored in-neighbours j of i of x[j,c]
  *   arg[i,c] = the source j that attains it; ties go to the smaller j (the paper's packed (value, index)
  *              atomicMin); values compare as IEEE numbers; rows without entries give 0 / -1.
- * x, out: [n, channels] `dtype`; arg: [n, channels] int32, out.  channels*sizeof(dtype) must be a multiple of 16 and
- * at most 1024 (GNN_EUNSUPPORTED otherwise).  Runs on the plan's degree bins (packed rows, CTA rows, hub chunks
+ * x, out: [n, channels] `dtype`; arg: [n, channels] int32, out.  channels*sizeof(dtype) must be a multiple of 16
+ * (GNN_EUNSUPPORTED otherwise); rows wider than 1024 bytes run as consecutive channel groups (at most 64).  Runs on the plan's degree bins (packed rows, CTA rows, hub chunks
  * merged by the lexicographic (value, index) minimum): no atomics, deterministic.
  * ws: >= gnn_workspace_bytes(GNN_OP_SEG_MINMAX_FWD, heads = 1, head_dim = channels).  Pointers 32-byte aligned. */
 enum { GNN_AGG_MIN = 0, GNN_AGG_MAX = 1 };

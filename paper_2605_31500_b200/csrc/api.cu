@@ -361,10 +361,18 @@ extern "C" gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* P, const int32_t* rowptr
 
 // ---- row f3: min / max aggregation.  The lane layout wants a power-of-two "head": factor channels = heads * head_dim
 // with head_dim the largest power of two that divides it (the pass has no per-head arithmetic).
+static int agg_groups(int32_t n, int32_t channels, int dtype, HeadGroup* hg, const char* who) {
+    if (channels < 1) { set_error("%s: channels must be >= 1", who); return 0; }
+    int hd = channels & -channels;
+    const int cap = 1024 / (dtype == GNN_F32 ? 4 : 2);       // a "head" here is just a slice: keep it within one launch
+    if (hd > cap) hd = cap;
+    return head_groups(n, channels / hd, hd, dtype, hg, who);
+}
 static bool agg_shape(int32_t n, int32_t channels, int dtype, Shape& sh, const char* who) {
-    if (channels < 1) { set_error("%s: channels must be >= 1", who); return false; }
-    const int hd = channels & -channels;
-    return make_shape(n, channels / hd, hd, dtype, sh, who);
+    HeadGroup hg[kMaxHeadGroups];
+    if (!agg_groups(n, channels, dtype, hg, who)) return false;
+    sh = hg[0].sh;    // the widest group: sizes the workspace
+    return true;
 }
 
 extern "C" gnn_status_t gnn_seg_minmax_fwd(const gnn_plan_t* P, const int32_t* rowptr, const int32_t* colidx, int32_t n,
@@ -378,13 +386,22 @@ extern "C" gnn_status_t gnn_seg_minmax_fwd(const gnn_plan_t* P, const int32_t* r
         set_error("%s: x, out, arg and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
-    Shape sh;
-    if (!agg_shape(n, channels, dtype, sh, who)) return GNN_EUNSUPPORTED;
-    const WsLayout w = ws_layout(P, GNN_OP_SEG_MINMAX_FWD, sh, dtype == GNN_F32 ? 4 : 2);
-    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
-    AggArgs a = {};
-    a.x = x; a.out = out; a.arg = arg; a.sign = mode == GNN_AGG_MIN ? 1.f : -1.f;
-    return cuda_status(launch_min_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a, P->rows_sorted != 0), who);
+    HeadGroup hg[kMaxHeadGroups];
+    const int ng = agg_groups(n, channels, dtype, hg, who), esz = dtype == GNN_F32 ? 4 : 2;
+    if (!ng) return GNN_EUNSUPPORTED;
+    const size_t need = ws_total(P, GNN_OP_SEG_MINMAX_FWD, hg, ng, esz);
+    if (ws_bytes < need) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, need); return GNN_EWORKSPACE; }
+    cudaError_t e = cudaSuccess;
+    for (int g = 0; g < ng && e == cudaSuccess; ++g) {      // channel groups of at most 1024 bytes (see head_groups)
+        const Shape& sh = hg[g].sh;
+        const size_t co = (size_t)hg[g].h0 * sh.d;           // first channel of the group
+        const WsLayout w = ws_layout(P, GNN_OP_SEG_MINMAX_FWD, sh, esz);
+        AggArgs a = {};
+        a.x = off_bytes(x, co * esz); a.out = off_bytes(out, co * esz); a.arg = arg + co;
+        a.sign = mode == GNN_AGG_MIN ? 1.f : -1.f;
+        e = launch_min_fwd(dtype, sh, make_ctx(P, false, ws, w, stream), a, P->rows_sorted != 0);
+    }
+    return cuda_status(e, who);
 }
 
 extern "C" gnn_status_t gnn_seg_minmax_bwd(int32_t n, const int32_t* arg, const void* dout, int32_t channels,

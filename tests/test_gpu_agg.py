@@ -37,7 +37,8 @@ def _run(rowptr, colidx, x_dev, mode, opts, dout_dev=None):
 
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 @pytest.mark.parametrize("mode", ["min", "max"])
-@pytest.mark.parametrize("channels,opts", [(128, SMALL_OPTS), (96, SMALL_OPTS), (64, DEFAULT_OPTS), (8, SMALL_OPTS)])
+@pytest.mark.parametrize("channels,opts", [(128, SMALL_OPTS), (96, SMALL_OPTS), (64, DEFAULT_OPTS), (8, SMALL_OPTS),
+                                              (640, SMALL_OPTS), (1024, DEFAULT_OPTS)])   # channel groups (> 1024-byte rows)
 def test_seg_minmax_parity(dtype, mode, channels, opts):
     """Power-law graph (cfg 2 scaled: hubs, CTA rows and packed rows under the small bins), random features AND a
     tie-heavy variant (three value levels, -0.0 included) that exercises the smaller-index rule in every merge."""
