@@ -45,6 +45,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--natural-ids", action="store_true",
                     help="cfg 3: keep the natural R-MAT ids instead of the random relabel (locality study, SURVEY 8(d))")
+    ap.add_argument("--dense", action="store_true",
+                    help="cfg 3 only: variant 3b, 85 M R-MAT samples -> ~124 M stored entries (ogbn-products' shape); not the headline")
     ap.add_argument("--directed-plan", action="store_true",
                     help="cfg 3: build CSR^T instead of reusing the forward CSR in the backward (row f1)")
     ap.add_argument("--no-minmax", action="store_true", help="skip the extra row-f3 (min aggregation) measurement of cfg 3 / 5")
@@ -260,7 +262,7 @@ def workload_config(c, args):
 def run_reference(args, rank):
     if rank != 0:
         return
-    c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False, relabel=not args.natural_ids)
+    c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False, relabel=not args.natural_ids, dense=args.dense)
     # each step = one bounded sample pass; the whole run (warm-up + steps) is sized to about two minutes of oracle time
     arm = OracleArm(c, target_seconds=min(args.cpu_seconds, 120.0 / max(args.steps + args.warmup, 1)))
     for _ in range(args.warmup):
@@ -296,7 +298,7 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False, relabel=not args.natural_ids)   # replicas: every rank runs the same workload
+    c = GI.make_config(args.cfg, scale=args.scale, keep_f32=False, relabel=not args.natural_ids, dense=args.dense)   # replicas: every rank runs the same workload
     n, e, H, d, dt = c["n"], c["e"], c["heads"], c["head_dim"], c["dtype"]
     gt = c["layer"] == "gt"
     names = ("q", "k", "v", "do") if gt else ("xl", "xr", "do")

@@ -30,7 +30,7 @@ def config_name(cfg: int) -> str:
     return CONFIGS[cfg]["name"]
 
 
-def _graph(cfg: int, scale: float, seed: int, relabel: bool = True):
+def _graph(cfg: int, scale: float, seed: int, relabel: bool = True, dense: bool = False):
     c = CONFIGS[cfg]
     n = max(64, int(round(c["n"] * scale)))
     r0, r1, r2, r3 = (rng_for(cfg, s, seed) for s in (0, 1, 2, 3))
@@ -42,7 +42,8 @@ def _graph(cfg: int, scale: float, seed: int, relabel: bool = True):
         return n, G.chung_lu(n, n_pairs, 2.1, w_max, r0, r1)
     if cfg == 3:
         bits = max(7, int(np.ceil(np.log2(n))))
-        return n, G.rmat_symmetric(n, bits, int(round(41_500_000 * scale)), (0.57, 0.19, 0.19), r0, r1 if relabel else None)
+        samples = 85_000_000 if dense else 41_500_000   # dense = "cfg 3b": ~124 M stored entries, average degree ~50 (ogbn-products' shape)
+        return n, G.rmat_symmetric(n, bits, int(round(samples * scale)), (0.57, 0.19, 0.19), r0, r1 if relabel else None)
     if cfg == 4:
         n = (n // 16) * 16
         return n, G.community_graph(n, 16, 0.6, 2, r0, r3)
@@ -54,12 +55,14 @@ def _graph(cfg: int, scale: float, seed: int, relabel: bool = True):
 
 
 def make_config(cfg: int, scale: float = 1.0, seed: int = 0, with_grads: bool = True, keep_f32: bool = True,
-                relabel: bool = True) -> dict:
+                relabel: bool = True, dense: bool = False) -> dict:
     """relabel=False (cfg 3 only) keeps the natural R-MAT ids: the locality study of SURVEY section 8(d), not the headline."""
     c = dict(CONFIGS[cfg])
-    if not relabel and cfg != 3:
-        raise ValueError("relabel=False is defined for cfg 3 only")
-    n, (rowptr, colidx) = _graph(cfg, scale, seed, relabel)
+    if (not relabel or dense) and cfg != 3:
+        raise ValueError("relabel=False / dense=True are defined for cfg 3 only")
+    n, (rowptr, colidx) = _graph(cfg, scale, seed, relabel, dense)
+    if dense:
+        c["name"] = c["name"].replace("cfg3_", "cfg3b_deg50_")
     h, d, dt = c["heads"], c["head_dim"], c["dtype"]
     out = dict(c, cfg=cfg, scale=scale, seed=seed, relabel=relabel, n=n, e=int(colidx.size), rowptr=rowptr, colidx=colidx)
     if c["layer"] == "gt":
