@@ -33,6 +33,7 @@ void prof_begin(const char* pass, const char* kernel, cudaStream_t st) {
     cudaEventRecord(r.a, st);
     g_prof.push_back(r);
 }
+bool prof_enabled() { return g_prof_on; }
 void prof_end(cudaStream_t st) {
     if (!g_prof_on || g_prof.empty()) return;
     cudaEventRecord(g_prof.back().b, st);

@@ -8,6 +8,11 @@ extern unsigned long long g_launches;  // host-side launch counter (api.cu)
 // optional per-launch CUDA-event timing (gnn_profile_enable); no-ops when disabled
 void prof_begin(const char* pass, const char* kernel, cudaStream_t st);
 void prof_end(cudaStream_t st);
+bool prof_enabled();
+// programmatic dependent launch of a pass's group kernel behind its segment kernel (tuning knob, on by default)
+#ifndef GNN_PDL
+#define GNN_PDL 1
+#endif
 
 // lexicographic (value, index) order of the MINARG states; index < 0 marks "no candidate yet"
 __device__ __forceinline__ bool minarg_better(float v, int j, float bv, int bj) {
@@ -197,6 +202,10 @@ segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowp
                BinView bins, float* __restrict__ partials, float* da_part, int da_slot) {
     constexpr int G = Op::kG, CH = Op::kCH;
     constexpr int GPW = 32 / G, NG = kWarpsPerCta * GPW;
+    // programmatic dependent launch: once every CTA of this grid is resident (or done), the group kernel of the same
+    // pass - which touches disjoint rows and waits for nothing from here - may start filling the SMs this grid's
+    // last, partial wave leaves idle (run_op launches it with programmatic stream serialization)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     extern __shared__ float4 smem4[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float* smem = reinterpret_cast<float*>(smem4);
@@ -477,8 +486,18 @@ template <class Op> inline cudaError_t run_op(const typename Op::Params& p, cons
             if (e != cudaSuccess) return e;
         }
         prof_begin(Op::kName, "group", c.stream);
-        group_kernel<Op><<<gp.grp_grid, kCtaThreads, smem, c.stream>>>(p, sh, c.rowptr, c.colidx, b.perm,
-                                                                       b.n_hub + b.n_cta, b.n_group, c.da_part, slot);
+        // overlaps the tail of this pass's segment kernel (see there); never the previous pass, whose results it may
+        // read, and not while the per-kernel event profiler brackets every launch
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(gp.grp_grid); cfg.blockDim = dim3(kCtaThreads); cfg.dynamicSmemBytes = smem; cfg.stream = c.stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = (GNN_PDL && gp.seg_grid > 0 && !prof_enabled()) ? 1 : 0;
+        cudaError_t le = cudaLaunchKernelEx(&cfg, group_kernel<Op>, p, sh, c.rowptr, c.colidx, b.perm, b.n_hub + b.n_cta,
+                                            b.n_group, c.da_part, slot);
+        if (le != cudaSuccess) return le;
         prof_end(c.stream);
         ++g_launches;
     }
