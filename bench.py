@@ -478,6 +478,21 @@ def run_ours(args, rank, world, local_rank):
                            "frac_bwd": comp["bwd"] / (np.mean(ms_bwd) * 1e-3) * 1e-9 / peak,
                            "frac_step": comp_step / (step_ms * 1e-3) * 1e-9 / peak}}
 
+    # third ceiling: plain fp32 ALUs.  Useful flops per (edge, head), d = head_dim, one exp counted as 1:
+    # GT fwd 5d+1 (Eq. 3), bwd dst 8d (one-sweep form), bwd src 8d; GATv2 fwd 7d+1 (Eq. 4), bwd dst 15d,
+    # bwd src 11d.  Peak = SMs x 128 fp32 lanes x 2 flop x the SM clock sampled during the timed region.
+    fl = {"fwd": (5 * d + 1) if gt else (7 * d + 1), "bwd": (16 * d) if gt else (26 * d)}
+    sm_clk = float(clk.get("sm_mhz") or clk.get("sm_max_mhz") or 1965.0)
+    alu_peak = torch.cuda.get_device_properties(dev).multi_processor_count * 128 * 2 * sm_clk * 1e6 * 1e-12   # TFLOP/s
+    tf_fwd = e * H * fl["fwd"] / (np.mean(ms_fwd) * 1e-3) * 1e-12
+    tf_bwd = e * H * fl["bwd"] / (np.mean(ms_bwd) * 1e-3) * 1e-12
+    roof["fp32_alu"] = {"flop_per_edge_head_fwd": fl["fwd"], "flop_per_edge_head_bwd": fl["bwd"], "peak_tflops": alu_peak,
+                        "sm_mhz": sm_clk, "tflops_fwd": tf_fwd, "tflops_bwd": tf_bwd,
+                        "frac_fwd": tf_fwd / alu_peak, "frac_bwd": tf_bwd / alu_peak}
+    roof["binding"] = ("three ceilings are reported: `compulsory` (HBM, each array once), `kernels_algorithmic_gbs` (gather ingest "
+                       "through L2, against the measured HBM peak; values above 1.0 x peak are L2 hits) and `fp32_alu`; the "
+                       "largest fraction is the one that binds")
+
     if block is not None:
         rem = int(plan.export(B.GNN_PLAN_BLOCK_REM_ROWPTR)[-1])
         b_el = 2
