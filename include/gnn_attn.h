@@ -34,8 +34,10 @@
  *     synchronises `stream` (it reads a few counters back to the host).
  *   - Return value: GNN_OK or an error code; nothing is launched when an error is returned for
  *     argument validation.  gnn_last_error() returns a thread-local message for the last error.
- *   - Determinism: no floating-point atomics anywhere; results are bit-reproducible run to run
- *     for the same plan options and device.
+ *   - Determinism: the attention entry points (forward, backward, block / WSB variants) and gnn_seg_minmax_fwd
+ *     use no floating-point atomics; their results are bit-reproducible run to run for the same plan
+ *     options and device.  The one exception is gnn_seg_minmax_bwd, the paper's scatter-add:
+ *     it uses red.global.add.f32, so dx is reproducible only up to fp32 rounding (stated at the call).
  */
 #ifndef GNN_ATTN_H_
 #define GNN_ATTN_H_
@@ -135,8 +137,10 @@ const int32_t* gnn_plan_colidx_t(const gnn_plan_t* plan);
 /* Workspace (device bytes) a compute call needs: hub-chunk partial states
  * [n_chunks][(n_acc * heads*head_dim + n_scalar * heads)] fp32 and, for gnn_gatv2_bwd, the per-CTA
  * `da` partials.  O(#chunks * H * d), never O(E * H).  `op`:                                         */
-enum { GNN_OP_GT_FWD = 0, GNN_OP_GT_BWD = 1, GNN_OP_GATV2_FWD = 2, GNN_OP_GATV2_BWD = 3, GNN_OP_GT_FWD_BLOCK = 4,
-       GNN_OP_SEG_MINMAX_FWD = 5 /* pass heads = 1, head_dim = channels */ };
+enum { GNN_OP_GT_FWD = 0, GNN_OP_GT_BWD = 1, GNN_OP_GATV2_FWD = 2, GNN_OP_GATV2_BWD = 3,
+       GNN_OP_GT_FWD_BLOCK = 4 /* needs no workspace: 0 bytes */,
+       GNN_OP_SEG_MINMAX_FWD = 5 /* pass heads = 1, head_dim = channels */,
+       GNN_OP_WSB_FWD = 6, GNN_OP_WSB_BWD = 7 /* tile-local: 0 bytes */ };
 gnn_status_t gnn_workspace_bytes(const gnn_plan_t* plan, int op, int32_t heads, int32_t head_dim, gnn_dtype_t dtype,
                                  size_t* bytes);
 
@@ -203,7 +207,9 @@ gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* plan, const int32_t* rowptr
  * Degree-aware min / max neighbourhood aggregation with argmin (PAPER.md:124-151 section 3.1, :452-474 App. D.1):
  *   out[i,c] = min (mode GNN_AGG_MIN) or max (GNN_AGG_MAX) over the stored in-neighbours j of i of x[j,c]
  *   arg[i,c] = the source j that attains it; ties go to the smaller j (the paper's packed (value, index)
- *              atomicMin); values compare as IEEE numbers; rows without entries give 0 / -1.
+ *              atomicMin); values compare as IEEE numbers (-0.0 == +0.0; +-inf are ordinary values: a row
+ *              whose candidates are all +inf returns +inf and the smallest such j); NaN inputs are outside the contract
+ *              (result unspecified); rows without entries give 0 / -1.
  * x, out: [n, channels] `dtype`; arg: [n, channels] int32, out.  channels*sizeof(dtype) must be a multiple of 16
  * (GNN_EUNSUPPORTED otherwise); rows wider than 1024 bytes run as consecutive channel groups (at most 64).  Runs on the plan's degree bins (packed rows, CTA rows, hub chunks
  * merged by the lexicographic (value, index) minimum): no atomics, deterministic.
@@ -223,8 +229,12 @@ gnn_status_t gnn_seg_minmax_bwd(int32_t n, const int32_t* arg, const void* dout,
 const char* gnn_last_error(void);
 /* Library version string, e.g. "gnn_attn 0.1 sm_100a".                                            */
 const char* gnn_version(void);
-/* Number of kernel launches the library has issued in this process (all threads).               */
+/* Number of kernel launches the library has issued in this process (all threads; atomic counter). */
 int64_t gnn_launch_count(void);
+/* Test / measurement aid: switches the programmatic-dependent-launch overlap of a pass's two traversal kernels
+ * off (0) or on (1, the default) for the whole process.  Results are bit-identical either way (the overlapped
+ * kernels touch disjoint rows, and the dependent kernel ends in griddepcontrol.wait).      */
+void gnn_pdl_enable(int on);
 
 /* Measurement aid (bench.py): when enabled, every kernel launch of the library is bracketed by two
  * CUDA events on the launch stream.  gnn_profile_collect synchronises on them, writes up to
@@ -233,6 +243,16 @@ int64_t gnn_launch_count(void);
  * thread-safe; off by default (the timed `value` runs have it off).                                */
 void gnn_profile_enable(int on);
 int32_t gnn_profile_collect(char* names, float* ms, int32_t max_records);
+
+/* Measurement aid (bench.py): ONE launch that gathers n_idx rows of row_bytes (256 | 512 | 1024) bytes at the row
+ * indices idx[0..n_idx) (each in [0, table_rows)) from `table` and discards them - the achievable gather-ingest rate
+ * ("ceiling 2" of DESIGN.md section 6: HBM-resident when the table is far larger than L2, L2-resident when it fits),
+ * which the caller times with CUDA events on `stream`.  mode 0: one 256-bit load per lane per row, `depth` (1|2|4|8)
+ * rows in flight per lane group, as the traversal kernels do; mode 1: cp.async.bulk copies into a shared-memory ring,
+ * `depth` (4|8|16) rows per stage.  ctas_per_sm (1..16) CTAs of 128 threads per SM.  table, idx, sink: device;
+ * table 32-byte aligned; sink: one float the kernel never writes for finite table contents.  Asynchronous.        */
+gnn_status_t gnn_probe_gather(const void* table, int64_t table_rows, int32_t row_bytes, const int32_t* idx, int64_t n_idx,
+                              int32_t mode, int32_t depth, int32_t ctas_per_sm, float* sink, gnn_stream_t stream);
 
 #ifdef __cplusplus
 }

@@ -13,7 +13,7 @@ _LIB_PATH = os.path.join(_HERE, "libgnn_attn.so")
 GNN_OK, GNN_EINVAL, GNN_EUNSUPPORTED, GNN_EWORKSPACE, GNN_ECUDA = range(5)
 GNN_F32, GNN_BF16 = 0, 1
 GNN_OP_GT_FWD, GNN_OP_GT_BWD, GNN_OP_GATV2_FWD, GNN_OP_GATV2_BWD = 0, 1, 2, 3
-GNN_OP_SEG_MINMAX_FWD = 5
+GNN_OP_GT_FWD_BLOCK, GNN_OP_SEG_MINMAX_FWD, GNN_OP_WSB_FWD, GNN_OP_WSB_BWD = 4, 5, 6, 7
 GNN_AGG_MIN, GNN_AGG_MAX = 0, 1
 GNN_TRANSPOSE_NONE, GNN_TRANSPOSE_BUILD, GNN_TRANSPOSE_UNDIRECTED = 0, 1, 2
 (GNN_PLAN_COUNTS, GNN_PLAN_PERM, GNN_PLAN_CHUNKS, GNN_PLAN_CHUNK_PTR, GNN_PLAN_ROWPTR_T, GNN_PLAN_COLIDX_T,
@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = [
     "gnn_csr_validate", "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
     "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
     "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_seg_minmax_fwd", "gnn_seg_minmax_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
-    "gnn_profile_collect",
+    "gnn_profile_collect", "gnn_pdl_enable", "gnn_probe_gather",
 ]
 
 
@@ -74,6 +74,9 @@ def lib() -> C.CDLL:
         L.gnn_launch_count.restype = _i64
         L.gnn_profile_enable.argtypes = [C.c_int]
         L.gnn_profile_enable.restype = None
+        L.gnn_probe_gather.argtypes = [_vp, _i64, _i32, _vp, _i64, _i32, _i32, _i32, _vp, _vp]
+        L.gnn_pdl_enable.argtypes = [C.c_int]
+        L.gnn_pdl_enable.restype = None
         L.gnn_profile_collect.argtypes = [_vp, _vp, _i32]
         L.gnn_profile_collect.restype = _i32
         for s in EXPORTED_SYMBOLS:
@@ -96,6 +99,10 @@ def gnn_launch_count() -> int:
 
 def gnn_profile_enable(on: bool) -> None:
     lib().gnn_profile_enable(1 if on else 0)
+
+
+def gnn_pdl_enable(on: bool) -> None:
+    lib().gnn_pdl_enable(1 if on else 0)
 
 
 def gnn_profile_collect(max_records: int = 4096):
@@ -271,6 +278,13 @@ def gnn_gatv2_bwd(plan: Plan, xl, xr, a, lse, dout, slope, g, dxl, dxr, da, stre
     _check(lib().gnn_gatv2_bwd(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(xl), _ptr(xr), _ptr(a),
                                _ptr(lse), _ptr(dout), H, d, _dtype_code(xl), float(slope), _ptr(g), _ptr(dxl), _ptr(dxr),
                                _ptr(da), _ptr(ws), ws.numel(), _stream(stream)))
+
+
+def gnn_probe_gather(table, row_bytes: int, idx, mode: int, depth: int, ctas_per_sm: int, sink, stream=None):
+    """One launch gathering idx.numel() random rows of `row_bytes` from `table` (uint8 [rows * row_bytes]); time it
+    with CUDA events on the stream.  mode 0: 256-bit register gathers; mode 1: cp.async.bulk ring."""
+    _check(lib().gnn_probe_gather(_ptr(table), table.numel() // row_bytes, row_bytes, _ptr(idx), idx.numel(), mode, depth,
+                                  ctas_per_sm, _ptr(sink), _stream(stream)))
 
 
 def gnn_seg_minmax_fwd(plan: Plan, x, mode, out, arg, stream=None):

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgnn_attn.so")
-UNITS = ["api", "plan", "block_fwd", "pass_gt_fwd", "pass_gt_bwd_dst", "pass_gt_bwd_src", "pass_gat_fwd", "pass_gat_bwd_dst", "pass_min_fwd",
+UNITS = ["api", "plan", "probe", "block_fwd", "pass_gt_fwd", "pass_gt_bwd_dst", "pass_gt_bwd_src", "pass_gat_fwd", "pass_gat_bwd_dst", "pass_min_fwd",
          "pass_gat_bwd_src"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
@@ -24,7 +24,7 @@ def _nvcc() -> str:
 
 
 def _deps_mtime() -> float:
-    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if not f.startswith("microbench")]
+    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
     files.append(os.path.join(HERE, "..", "include", "gnn_attn.h"))
     return max(os.path.getmtime(f) for f in files)
 
@@ -55,17 +55,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_microbench() -> str:
-    """Standalone gather-bandwidth microbenchmark (measurement aid, see csrc/microbench_gather.cu)."""
-    out = os.path.join(HERE, "microbench_gather")
-    r = subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-o", out,
-                        os.path.join(CSRC, "microbench_gather.cu")], capture_output=True, text=True)
-    if r.returncode != 0:
-        raise RuntimeError(f"nvcc failed for microbench_gather:\n{r.stdout}\n{r.stderr}")
-    return out
-
-
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
-    if "--microbench" in sys.argv:
-        print(build_microbench())

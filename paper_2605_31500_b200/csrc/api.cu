@@ -1,5 +1,6 @@
 // api.cu - the C-ABI entry points of include/gnn_attn.h: argument validation and pass sequencing.
 // Every step of the path runs in this library's kernels; nothing here computes on the host.
+#include <atomic>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -10,7 +11,10 @@
 
 namespace gnn {
 
-unsigned long long g_launches = 0;
+static std::atomic<unsigned long long> g_launches{0};
+static std::atomic<int> g_pdl_on{1};
+void count_launch(int k) { g_launches.fetch_add((unsigned long long)k, std::memory_order_relaxed); }
+bool pdl_enabled() { return g_pdl_on.load(std::memory_order_relaxed) != 0; }
 static thread_local char t_err[512] = "";
 
 void set_error(const char* fmt, ...) {
@@ -96,7 +100,7 @@ int head_groups(int32_t n, int32_t heads, int32_t head_dim, int dtype, HeadGroup
 template <class T> T* off_bytes(T* p, size_t bytes) { return (T*)((char*)p + bytes); }
 template <class T> const T* off_bytes(const T* p, size_t bytes) { return (const T*)((const char*)p + bytes); }
 
-bool aligned16(const void* p) { return (((uintptr_t)p) & 31) == 0; }  // 256-bit gathers need 32-byte alignment
+bool aligned32(const void* p) { return (((uintptr_t)p) & 31) == 0; }  // 256-bit gathers need 32-byte alignment
 
 struct WsLayout { size_t partials, da_part, stat2, total; int da_slots, da_slots_dst; };
 
@@ -177,7 +181,8 @@ using namespace gnn;
 
 extern "C" const char* gnn_last_error(void) { return t_err; }
 extern "C" const char* gnn_version(void) { return "gnn_attn 0.1 sm_100a"; }
-extern "C" int64_t gnn_launch_count(void) { return (int64_t)g_launches; }
+extern "C" int64_t gnn_launch_count(void) { return (int64_t)g_launches.load(std::memory_order_relaxed); }
+extern "C" void gnn_pdl_enable(int on) { g_pdl_on.store(on != 0, std::memory_order_relaxed); }
 
 extern "C" void gnn_profile_enable(int on) { g_prof_on = on != 0; }
 extern "C" int32_t gnn_profile_collect(char* names, float* ms, int32_t max_records) {
@@ -203,6 +208,7 @@ static bool agg_shape(int32_t n, int32_t channels, int dtype, Shape& sh, const c
 extern "C" gnn_status_t gnn_workspace_bytes(const gnn_plan_t* P, int op, int32_t heads, int32_t head_dim,
                                             gnn_dtype_t dtype, size_t* bytes) {
     if (!P || !bytes) { set_error("gnn_workspace_bytes: NULL plan or bytes"); return GNN_EINVAL; }
+    if (op == GNN_OP_GT_FWD_BLOCK || op == GNN_OP_WSB_FWD || op == GNN_OP_WSB_BWD) { *bytes = 0; return GNN_OK; }   // tile-local: no workspace
     if ((op < GNN_OP_GT_FWD || op > GNN_OP_GATV2_BWD) && op != GNN_OP_SEG_MINMAX_FWD) {
         set_error("gnn_workspace_bytes: unknown op %d", op);
         return GNN_EINVAL;
@@ -227,7 +233,7 @@ extern "C" gnn_status_t gnn_gt_attn_fwd(const gnn_plan_t* P, const int32_t* rowp
     const char* who = "gnn_gt_attn_fwd";
     if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
     if (!q || !k || !v || !out || !lse || !ws) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
-    if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !aligned16(ws)) {
+    if (!aligned32(q) || !aligned32(k) || !aligned32(v) || !aligned32(out) || !aligned32(ws)) {
         set_error("%s: feature pointers and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
@@ -260,8 +266,8 @@ extern "C" gnn_status_t gnn_gt_attn_bwd(const gnn_plan_t* P, const int32_t* rowp
         set_error("%s: NULL pointer argument", who);
         return GNN_EINVAL;
     }
-    if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(dout) || !aligned16(dq) || !aligned16(dk) ||
-        !aligned16(dv) || !aligned16(ws)) {
+    if (!aligned32(q) || !aligned32(k) || !aligned32(v) || !aligned32(dout) || !aligned32(dq) || !aligned32(dk) ||
+        !aligned32(dv) || !aligned32(ws)) {
         set_error("%s: feature/gradient pointers and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
@@ -295,7 +301,7 @@ extern "C" gnn_status_t gnn_gatv2_fwd(const gnn_plan_t* P, const int32_t* rowptr
     if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
     if (!xl || !xr || !a_ || !out || !lse || !ws) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
     if (!(slope >= 0.f) || !(slope < INFINITY)) { set_error("%s: LeakyReLU slope must be finite and >= 0", who); return GNN_EINVAL; }
-    if (!aligned16(xl) || !aligned16(xr) || !aligned16(a_) || !aligned16(out) || !aligned16(ws)) {
+    if (!aligned32(xl) || !aligned32(xr) || !aligned32(a_) || !aligned32(out) || !aligned32(ws)) {
         set_error("%s: feature pointers, a and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
@@ -330,8 +336,8 @@ extern "C" gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* P, const int32_t* rowptr
         return GNN_EINVAL;
     }
     if (!(slope >= 0.f) || !(slope < INFINITY)) { set_error("%s: LeakyReLU slope must be finite and >= 0", who); return GNN_EINVAL; }
-    if (!aligned16(xl) || !aligned16(xr) || !aligned16(a_) || !aligned16(dout) || !aligned16(dxl) || !aligned16(dxr) ||
-        !aligned16(ws)) {
+    if (!aligned32(xl) || !aligned32(xr) || !aligned32(a_) || !aligned32(dout) || !aligned32(dxl) || !aligned32(dxr) ||
+        !aligned32(ws)) {
         set_error("%s: feature/gradient pointers, a and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
@@ -383,7 +389,7 @@ extern "C" gnn_status_t gnn_seg_minmax_fwd(const gnn_plan_t* P, const int32_t* r
     if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
     if (!x || !out || !arg || !ws) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
     if (mode != GNN_AGG_MIN && mode != GNN_AGG_MAX) { set_error("%s: unknown mode %d", who, mode); return GNN_EINVAL; }
-    if (!aligned16(x) || !aligned16(out) || !aligned16(arg) || !aligned16(ws)) {
+    if (!aligned32(x) || !aligned32(out) || !aligned32(arg) || !aligned32(ws)) {
         set_error("%s: x, out, arg and workspace must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
@@ -409,7 +415,7 @@ extern "C" gnn_status_t gnn_seg_minmax_bwd(int32_t n, const int32_t* arg, const 
                                            gnn_dtype_t dtype, float* dx, gnn_stream_t stream) {
     const char* who = "gnn_seg_minmax_bwd";
     if (n < 1 || !arg || !dout || !dx) { set_error("%s: n < 1 or NULL pointer argument", who); return GNN_EINVAL; }
-    if (!aligned16(arg) || !aligned16(dout) || !aligned16(dx)) {
+    if (!aligned32(arg) || !aligned32(dout) || !aligned32(dx)) {
         set_error("%s: arg, dout and dx must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
@@ -418,6 +424,9 @@ extern "C" gnn_status_t gnn_seg_minmax_bwd(int32_t n, const int32_t* arg, const 
     cudaError_t e = cudaMemsetAsync(dx, 0, sizeof(float) * (size_t)n * channels, (cudaStream_t)stream);
     AggArgs a = {};
     a.arg = const_cast<int32_t*>(arg); a.dout = dout; a.dx = dx;
-    if (e == cudaSuccess) e = launch_minmax_scatter(dtype, n, channels, a, (cudaStream_t)stream);
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = launch_minmax_scatter(dtype, n, channels, a, sms, (cudaStream_t)stream);
     return cuda_status(e, who);
 }

@@ -447,7 +447,7 @@ extern "C" gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* P, const int32_t
             tmq, tmk, tmv, (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, (__nv_bfloat16*)out, lse, P->blk_bitmap,
             P->blk_rem_rowptr, P->blk_rem_colidx, n, heads, kLog2e / sqrtf((float)D));
         prof_end((cudaStream_t)stream);
-        ++g_launches;
+        count_launch();
         e = cudaGetLastError();
     }
     if (e != cudaSuccess) { set_error("%s: CUDA error: %s", who, cudaGetErrorString(e)); return GNN_ECUDA; }

@@ -27,6 +27,9 @@
 
 namespace gnn {
 
+void count_launch(int k = 1);   // host-side launch counter, atomic (api.cu; gnn_launch_count)
+bool pdl_enabled();             // run-time switch of the dependent-launch overlap (api.cu; gnn_pdl_enable)
+
 // tuning knobs (profiles/r01_lane_width_sweep.md): resident CTAs per SM the register budget is held to and
 // register double-buffering of the gathers, for the forward and the backward passes
 #ifndef GNN_FWD_MINB
@@ -95,30 +98,6 @@ __device__ __forceinline__ float lg2(float x) {
     return y;
 }
 
-// ---- asynchronous gathers into shared memory (cp.async / LDGSTS).  Every lane copies exactly the bytes it
-// will consume itself, into lane-private slots of a per-warp ring, so completion needs only the lane's own
-// cp.async.wait_group (no barrier) and gathers in flight hold no registers.  pred == false zero-fills.
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool pred) {
-    const int sz = pred ? 16 : 0;
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(sz) : "memory");
-}
-__device__ __forceinline__ void cp_async4(uint32_t dst, const void* src, bool pred) {
-    const int sz = pred ? 4 : 0;
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(sz) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-__device__ __forceinline__ uint4 lds128(uint32_t addr) {
-    uint4 r;
-    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
-    return r;
-}
-__device__ __forceinline__ float lds32(uint32_t addr) {
-    float r;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r) : "r"(addr));
-    return r;
-}
-
 // ---- mixed-precision arithmetic on packed bf16 pairs (sm_100: FHFMA.BF16 / FHADD.BF16 take the .H0/.H1 half
 // of a register directly, so bf16 operands need no unpack instruction; products are exact, sums fp32)
 __device__ __forceinline__ void fma_bf16x2(uint32_t a, uint32_t b, float& acc0, float& acc1) {
@@ -168,8 +147,7 @@ template <> __device__ __forceinline__ float raw_elt<__nv_bfloat16, 32>(const Ra
 }
 
 // A lane's CB contiguous bytes (CH = CB / sizeof(T) channels of one head) of a [*, rowe] tensor of T, kept as raw
-// 32-bit words.  In the per-warp ring the 16-byte pieces of a chunk sit 512 bytes apart (32 lanes x 16 bytes),
-// so both the cp.async writes and the LDS.128 reads of a warp are conflict-free.
+// 32-bit words.
 template <typename T, int CB> struct Chunk {
     static constexpr int CH = CB / (int)sizeof(T), NW = CB / 4, NP = CB / 16;
     uint32_t w[NW];
@@ -185,18 +163,6 @@ template <typename T, int CB> struct Chunk {
             const Raw<16> r = ldg_raw<16>(base + elt, pred);
 #pragma unroll
             for (int i = 0; i < 4; ++i) w[i] = r.w[i];
-        }
-    }
-    // issue the asynchronous copy of this chunk of row `src` into the ring (addr = lane's slot of piece 0)
-    __device__ __forceinline__ static void issue(uint32_t addr, const T* src, bool pred) {
-#pragma unroll
-        for (int v = 0; v < NP; ++v) cp_async16(addr + 512 * v, reinterpret_cast<const char*>(src) + 16 * v, pred);
-    }
-    __device__ __forceinline__ void load_smem(uint32_t addr) {
-#pragma unroll
-        for (int v = 0; v < NP; ++v) {
-            const uint4 r = lds128(addr + 512 * v);
-            w[4 * v] = r.x; w[4 * v + 1] = r.y; w[4 * v + 2] = r.z; w[4 * v + 3] = r.w;
         }
     }
     __device__ __forceinline__ float get(int c) const {

@@ -125,7 +125,7 @@ cudaError_t launch_gat_bwd_dst(int dtype, const Shape&, const LaunchCtx&, const 
 cudaError_t launch_gat_bwd_src(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
 cudaError_t launch_min_fwd(int dtype, const Shape&, const LaunchCtx&, const AggArgs&, bool rows_sorted);
 // dx[arg[i,c], c] += dout[i,c] over all (i, c) with arg >= 0 (dx zeroed by the caller); one red.global.add per element
-cudaError_t launch_minmax_scatter(int dtype, long long n, int rowe, const AggArgs&, cudaStream_t);
+cudaError_t launch_minmax_scatter(int dtype, long long n, int rowe, const AggArgs&, int sm_count, cudaStream_t);
 // da[e] = sum over slots of da_part[slot][e], fixed order, fp64 accumulation (no atomics)
 cudaError_t launch_da_reduce(const float* da_part, int slots, int rowe, float* da, cudaStream_t);
 

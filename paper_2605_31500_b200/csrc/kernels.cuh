@@ -4,7 +4,6 @@
 
 namespace gnn {
 
-extern unsigned long long g_launches;  // host-side launch counter (api.cu)
 // optional per-launch CUDA-event timing (gnn_profile_enable); no-ops when disabled
 void prof_begin(const char* pass, const char* kernel, cudaStream_t st);
 void prof_end(cudaStream_t st);
@@ -190,6 +189,13 @@ group_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowptr
     }
     if (Op::HAS_DA)
         cta_write_da<Op>(da, smem, da_part, da_slot + blockIdx.x, g, sh, warp * GPW + sub, kWarpsPerCta * GPW);
+    // This grid may have been launched programmatically behind the pass's segment grid (run_op).  It reads nothing
+    // from that grid, so the wait sits at its very end: the PTX ISA requires a dependent of a grid that executes
+    // griddepcontrol.launch_dependents to execute griddepcontrol.wait, and with it "this grid has completed" implies
+    // "the segment grid has completed and its writes (partials, stat2, Delta / G, da slots) are visible" - which is
+    // what the ordinary launches that follow in the stream (hub merge, next pass, the caller's kernels) rely on.
+    // A no-op when the launch carried no programmatic dependency.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -203,8 +209,9 @@ segment_kernel(typename Op::Params p, Shape sh, const int32_t* __restrict__ rowp
     constexpr int G = Op::kG, CH = Op::kCH;
     constexpr int GPW = 32 / G, NG = kWarpsPerCta * GPW;
     // programmatic dependent launch: once every CTA of this grid is resident (or done), the group kernel of the same
-    // pass - which touches disjoint rows and waits for nothing from here - may start filling the SMs this grid's
-    // last, partial wave leaves idle (run_op launches it with programmatic stream serialization)
+    // pass - which touches disjoint rows and needs nothing from here - may start filling the SMs this grid's
+    // last, partial wave leaves idle (run_op launches it with programmatic stream serialization; the group kernel
+    // ends with griddepcontrol.wait, which restores full stream order for everything launched after it)
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     extern __shared__ float4 smem4[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -476,7 +483,7 @@ template <class Op> inline cudaError_t run_op(const typename Op::Params& p, cons
         segment_kernel<Op><<<gp.seg_grid, kCtaThreads, smem, c.stream>>>(p, sh, c.rowptr, c.colidx, b, c.partials,
                                                                          c.da_part, slot);
         prof_end(c.stream);
-        ++g_launches;
+        count_launch();
     }
     slot += gp.seg_grid;
     if (gp.grp_grid > 0) {
@@ -494,12 +501,12 @@ template <class Op> inline cudaError_t run_op(const typename Op::Params& p, cons
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at;
-        cfg.numAttrs = (GNN_PDL && gp.seg_grid > 0 && !prof_enabled()) ? 1 : 0;
+        cfg.numAttrs = (GNN_PDL && pdl_enabled() && gp.seg_grid > 0 && !prof_enabled()) ? 1 : 0;
         cudaError_t le = cudaLaunchKernelEx(&cfg, group_kernel<Op>, p, sh, c.rowptr, c.colidx, b.perm, b.n_hub + b.n_cta,
                                             b.n_group, c.da_part, slot);
         if (le != cudaSuccess) return le;
         prof_end(c.stream);
-        ++g_launches;
+        count_launch();
     }
     slot += gp.grp_grid;
     if (gp.hub_grid > 0) {
@@ -511,7 +518,7 @@ template <class Op> inline cudaError_t run_op(const typename Op::Params& p, cons
         prof_begin(Op::kName, "hub_merge", c.stream);
         hub_merge_kernel<Op><<<gp.hub_grid, kHubThreads, smem, c.stream>>>(p, sh, b, c.partials, c.da_part, slot);
         prof_end(c.stream);
-        ++g_launches;
+        count_launch();
     }
     return cudaGetLastError();
 }

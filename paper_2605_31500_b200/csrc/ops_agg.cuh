@@ -37,7 +37,7 @@ template <typename T, int CB_, int G_, int KU_, bool SORTED> struct MinFwdT : Op
     __device__ __forceinline__ static void init_state(St& st) {
 #pragma unroll
         for (int c = 0; c < CH; ++c) {
-            st.acc[0][c] = INFINITY;
+            st.acc[0][c] = __int_as_float(0x7fc00000);   // NaN: "no candidate yet", loses every less-than-or-unordered test
             st.acc[1][c] = __int_as_float(-1);
         }
     }
@@ -56,14 +56,16 @@ template <typename T, int CB_, int G_, int KU_, bool SORTED> struct MinFwdT : Op
             const int j = nbr[u];
             const bool valid = j >= 0;
             const float jf = __int_as_float(j);
-            // branch-free lexicographic update (bitwise predicate logic keeps the compiler from short-circuit branches);
-            // the state starts at (+inf, -1), so with finite inputs the first candidate always wins the `<`
+            // branch-free lexicographic update (bitwise predicate logic keeps the compiler from short-circuit branches).
+            // The state starts at (NaN, -1) and the test is "less than or unordered" (!(v >= bv), one FSETP.LTU), so
+            // the first valid candidate always wins - also a signed value of +inf (x = +inf for min, -inf for max) -
+            // and afterwards it is the plain IEEE `<`.  NaN inputs are outside the contract (include/gnn_attn.h).
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
                 const float v = p.sign * xc.get(c);
                 const float bv = st.acc[0][c];
-                const bool b = SORTED ? (valid & (v < bv))
-                                      : (valid & ((v < bv) | ((v == bv) & (j < __float_as_int(st.acc[1][c])))));
+                const bool b = SORTED ? (valid & !(v >= bv))
+                                      : (valid & (!(v >= bv) | ((v == bv) & (j < __float_as_int(st.acc[1][c])))));
                 st.acc[0][c] = b ? v : bv;
                 st.acc[1][c] = b ? jf : st.acc[1][c];
             }

@@ -284,7 +284,6 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
         c0.load_global(p.xr, (size_t)row * sh.ld + g.eoff, g.act);
         c0.to_float(xr);
         load_f32<CH>(p.a, g.eoff, g.act, a);
-#pragma unroll
         const float om = 1.f - p.slope, ds = p.slope * st.sc[0];
 #pragma unroll
         for (int c = 0; c < CH; ++c) {

@@ -29,7 +29,7 @@ cudaError_t launch_da_reduce(const float* da_part, int slots, int rowe, float* d
     prof_begin("gatv2_bwd_dst", "da_reduce", st);
     da_reduce_kernel<<<rowe, 256, 0, st>>>(da_part, slots, rowe, da);
     prof_end(st);
-    ++g_launches;
+    count_launch();
     return cudaGetLastError();
 }
 }  // namespace gnn

@@ -36,17 +36,17 @@ minmax_scatter_kernel(const int32_t* __restrict__ arg, const T* __restrict__ dou
     }
 }
 
-cudaError_t launch_minmax_scatter(int dtype, long long n, int rowe, const AggArgs& a, cudaStream_t st) {
+cudaError_t launch_minmax_scatter(int dtype, long long n, int rowe, const AggArgs& a, int sm_count, cudaStream_t st) {
     const long long nquads = n * rowe / 4;
     if (nquads == 0) return cudaSuccess;
-    const int grid = (int)std::min<long long>((nquads + 255) / 256, 148LL * 32);
+    const int grid = (int)std::min<long long>((nquads + 255) / 256, (long long)sm_count * 32);
     prof_begin("seg_minmax_bwd", "scatter", st);
     if (dtype == GNN_F32)
         minmax_scatter_kernel<float><<<grid, 256, 0, st>>>(a.arg, (const float*)a.dout, a.dx, nquads, rowe);
     else
         minmax_scatter_kernel<__nv_bfloat16><<<grid, 256, 0, st>>>(a.arg, (const __nv_bfloat16*)a.dout, a.dx, nquads, rowe);
     prof_end(st);
-    ++g_launches;
+    count_launch();
     return cudaGetLastError();
 }
 }  // namespace gnn

@@ -12,7 +12,6 @@
 #include "internal.h"
 
 namespace gnn {
-extern unsigned long long g_launches;
 
 namespace {
 
@@ -285,14 +284,14 @@ cudaError_t build_bins(const int32_t* rowptr, int n, const gnn_plan_opts_t& o, c
                                                     (const int32_t*)rowid, perm, (long long)n, 0, 7, st);
     if (e != cudaSuccess) return e;
     count_kernel<<<1, 32, 0, st>>>(key_sorted, perm, rowptr, n, o.split_chunk, counts_dev, chunk_ptr, (int)L.max_hub);
-    g_launches += 3;
+    count_launch(3);
     e = cudaMemcpyAsync(counts_host, counts_dev, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
     if (e != cudaSuccess) return e;
     e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return e;
     if (counts_host[0] > 0) {
         chunk_kernel<<<counts_host[0], 128, 0, st>>>(perm, rowptr, chunk_ptr, chunks);
-        ++g_launches;
+        count_launch();
     }
     return cudaGetLastError();
 }
@@ -363,7 +362,7 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
         e = cudaMemsetAsync(counts_dev + 9, 0, sizeof(int32_t), st);
         if (e == cudaSuccess && nnz > 0) {
             undirected_check_kernel<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(rowptr, colidx, n, nnz, counts_dev + 9);
-            ++g_launches;
+            count_launch();
         }
         if (e == cudaSuccess) e = cudaMemcpyAsync(&directed, counts_dev + 9, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
         P->rowptr_t = const_cast<int32_t*>(rowptr);
@@ -376,14 +375,14 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
         int32_t* erow = (int32_t*)(sc + L.erow);
         if (nnz > 0) {
             row_of_edge_kernel<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(rowptr, n, nnz, erow);
-            ++g_launches;
+            count_launch();
             size_t cb = L.cub_bytes;
             e = cub::DeviceRadixSort::SortPairs(sc + L.cub, cb, (const uint32_t*)colidx, ekey_sorted,
                                                 (const int32_t*)erow, P->colidx_t, (long long)nnz, 0, n_bits(n), st);
         }
         if (e == cudaSuccess) {
             rowptr_t_kernel<<<(n + 1 + 255) / 256, 256, 0, st>>>(ekey_sorted, nnz, n, P->rowptr_t);
-            ++g_launches;
+            count_launch();
             e = build_bins(P->rowptr_t, n, o, L, sc, (int32_t*)(dm + L.perm_t), (int32_t*)(dm + L.chunks_t),
                            (int32_t*)(dm + L.chunk_ptr_t), counts_dev + 4, hc + 4, st);
         }
@@ -392,7 +391,7 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
     if (e == cudaSuccess) e = cudaMemsetAsync(counts_dev + 8, 0, sizeof(int32_t), st);
     if (e == cudaSuccess && nnz > 1) {
         rows_unsorted_kernel<<<(unsigned)((nnz + 255) / 256), 256, 0, st>>>(rowptr, colidx, n, nnz, counts_dev + 8);
-        ++g_launches;
+        count_launch();
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(&unsorted, counts_dev + 8, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
     int32_t rem_nnz = 0;
@@ -410,7 +409,7 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
         if (e == cudaSuccess) e = cub::DeviceScan::InclusiveSum(sc + L.cub, cb, (const int32_t*)cnt, P->blk_rem_rowptr + 1, n, st);
         if (e == cudaSuccess) {
             block_layout_kernel<<<gb, tb, 0, st>>>(rowptr, colidx, n, 1, nullptr, nullptr, P->blk_rem_rowptr, P->blk_rem_colidx);
-            g_launches += 3;
+            count_launch(3);
             e = cudaMemcpyAsync(&rem_nnz, P->blk_rem_rowptr + n, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
         }
     }
@@ -451,7 +450,7 @@ extern "C" gnn_status_t gnn_csr_validate(int32_t n, int64_t nnz, const int32_t* 
     if (e == cudaSuccess) {
         const long long work = nnz > n ? nnz : n;
         csr_validate_kernel<<<(unsigned)((work + 255) / 256), 256, 0, st>>>(rowptr, colidx, n, nnz, (unsigned long long*)scratch);
-        ++g_launches;
+        count_launch();
         e = cudaMemcpyAsync(got, scratch, sizeof(got), cudaMemcpyDeviceToHost, st);
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(&ends[0], rowptr, sizeof(int32_t), cudaMemcpyDeviceToHost, st);

@@ -105,6 +105,36 @@ def test_seg_minmax_degenerate():
         G.gnn_seg_minmax_fwd(plan, xd, 7, torch.empty_like(xd), torch.empty((n, C), dtype=torch.int32, device="cuda"))
 
 
+@pytest.mark.parametrize("mode", ["min", "max"])
+@pytest.mark.parametrize("shuffled", [False, True])
+def test_seg_minmax_infinite_values(mode, shuffled):
+    """+-inf are ordinary IEEE values (include/gnn_attn.h): a candidate whose signed value is +inf (x = +inf for min,
+    -inf for max) must still beat "no candidate yet" - rows whose sources are all +inf return +inf and the smallest
+    such source, not the empty-row answer 0 / -1 - through the per-lane update, the CTA-row merge and the hub merge."""
+    c = GI.make_config(2, scale=0.03)
+    rp, ci, n = c["rowptr"], c["colidx"].copy(), c["n"]
+    rng = np.random.default_rng(5)
+    if shuffled:
+        for i in range(n):
+            ci[rp[i]:rp[i + 1]] = rng.permutation(ci[rp[i]:rp[i + 1]])
+    C = 64
+    x = rng.standard_normal((n, C))
+    bad = np.inf if mode == "min" else -np.inf
+    x[:, :16] = bad                                    # whole channels: every row, hubs included, sees only +-inf there
+    x[rng.random((n, C)) < 0.3] = bad                  # scattered: some rows see only +-inf, most see a mix
+    x[rng.random((n, C)) < 0.05] = -bad                # and the value that must always win
+    for dtype in ("f32", "bf16"):
+        xd = _to_dev(x, dtype)
+        got = _run(rp, ci, xd, mode, SMALL_OPTS)
+        cnt = got["plan"].counts()
+        assert cnt["n_hub"] > 0 and cnt["n_cta"] > 0
+        want_out, want_arg = agg_ref.seg_minmax_forward(rp, ci, _host(xd), mode)
+        assert np.array_equal(got["arg"], want_arg)
+        assert np.array_equal(got["out"], want_out)
+        deg = np.diff(rp)
+        assert np.all(got["arg"][deg > 0] >= 0) and np.all(got["out"][deg > 0][:, :16] == bad)
+
+
 @pytest.mark.slow
 def test_seg_minmax_fullsize_cfg5():
     """BASELINE.json cfg 5 graph (4 M nodes, 94 M edges, hubs of in-degree up to 3 M = 733 chunks each) with the default

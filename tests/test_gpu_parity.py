@@ -283,6 +283,50 @@ def test_split_row_equals_unsplit_and_deterministic():
         np.testing.assert_allclose(a[key], u[key], rtol=0, atol=2e-2 if key == "O" else 2e-3)
 
 
+@pytest.mark.parametrize("layer", ["gt", "gatv2"])
+def test_pdl_ordering_when_the_group_grid_finishes_first(layer):
+    """A pass launches its group kernel programmatically behind its segment kernel (CTA rows + hub chunks) so the two
+    overlap; the group kernel ends with griddepcontrol.wait, which is what orders the hub merge, the next pass and the
+    caller's kernels behind the SEGMENT grid too.  The case to fear is a group grid that
+    finishes long before the segment grid: here ~all rows are CTA rows or hubs (degree 24..3000 against thresholds
+    8 / 256 / 64) and only a handful are group rows.  50 repetitions with the overlap on must be bit-identical to the
+    serialised launch order (gnn_pdl_enable(0)) - forward and backward, incl. the (L, Delta) / G hand-over between
+    the dst and the src pass and the da slots - and within tolerance of the oracle."""
+    import paper_2605_31500_b200 as G
+    torch = _torch()
+    rng = np.random.default_rng(21)
+    n = 1500
+    deg = rng.integers(24, 200, size=n)
+    deg[rng.choice(n, 40, replace=False)] = rng.integers(800, 3000, size=40)      # hubs: 13..47 chunks each
+    deg[:6] = rng.integers(1, 8, size=6)                                          # the only group rows
+    dst = np.repeat(np.arange(n), deg)
+    src = rng.integers(0, n, size=dst.size)
+    # out-degrees must look the same for the src pass over CSR^T: route most edges to few sources
+    heavy = rng.choice(n, 30, replace=False)
+    src = np.where(rng.random(dst.size) < 0.5, heavy[rng.integers(0, 30, size=dst.size)], src)
+    lone = np.arange(n - 6, n)                                                    # the only group rows of CSR^T
+    src = np.where(np.isin(src, lone), heavy[0], src)
+    dst, src = np.concatenate([dst, rng.integers(6, n - 6, size=6)]), np.concatenate([src, lone])
+    rowptr, colidx = GI.csr_from_pairs(n, dst, src, self_loops=False, dedupe=False)
+    c = _custom(layer, n, rowptr, colidx, 4, 32, "bf16", seed=4)
+    opts = dict(warp_max_deg=8, cta_max_deg=256, split_chunk=64)
+    run = run_gt if layer == "gt" else run_gat
+    keys = ["O", "L", "Delta", "dQ", "dK", "dV"] if layer == "gt" else ["O", "L", "G", "dxl", "dxr", "da"]
+    try:
+        G.gnn_pdl_enable(False)
+        base = run(c, opts)
+    finally:
+        G.gnn_pdl_enable(True)
+    cnt = base["plan"].counts()
+    assert cnt["n_group"] <= 8 and cnt["n_cta"] > 1000 and cnt["n_hub"] >= 30 and cnt["n_chunks"] > 400
+    assert 0 < cnt["n_group_t"] <= 8 and cnt["n_cta_t"] > 1000 and cnt["n_hub_t"] >= 20 and cnt["n_chunks_t"] > 400
+    compare_all(c, base, oracle_gt(c) if layer == "gt" else oracle_gat(c))
+    for rep in range(50):
+        got = run(c, opts)
+        for key in keys:
+            assert np.array_equal(got[key], base[key]), f"{key} differs from the serialised run at repetition {rep}"
+
+
 def test_errors_are_reported():
     import paper_2605_31500_b200 as G
     torch = _torch()
