@@ -105,6 +105,62 @@ __device__ __forceinline__ void fma_bf16x2(uint32_t a, uint32_t b, float& acc0, 
         " fma.rn.f32.bf16 %0, al, bl, %0;\n fma.rn.f32.bf16 %1, ah, bh, %1;\n}"
         : "+f"(acc0), "+f"(acc1) : "r"(a), "r"(b));
 }
+// first products of a dot: the accumulator operand is the zero register, so no register pair has to be cleared first
+__device__ __forceinline__ void mul_bf16x2(uint32_t a, uint32_t b, float& acc0, float& acc1) {
+    asm("{\n .reg .b16 al, ah, bl, bh;\n mov.b32 {al, ah}, %2;\n mov.b32 {bl, bh}, %3;\n"
+        " fma.rn.f32.bf16 %0, al, bl, 0f00000000;\n fma.rn.f32.bf16 %1, ah, bh, 0f00000000;\n}"
+        : "=f"(acc0), "=f"(acc1) : "r"(a), "r"(b));
+}
+// ---- packed fp32 pairs (sm_100 FFMA2 / FADD2 / FMUL2: two fp32 lanes of a 64-bit register pair per instruction;
+// a scalar operand is broadcast by the instruction itself).  The pairs are named as two floats; ptxas allocates them
+// to aligned register pairs, so the mov.b64 packs below cost nothing.
+__device__ __forceinline__ void fma2(float& a0, float& a1, float w, float x0, float x1) {            // a += w * x
+    asm("{\n .reg .b64 ww, xx, cc;\n mov.b64 ww, {%2, %2};\n mov.b64 xx, {%3, %4};\n mov.b64 cc, {%0, %1};\n"
+        " fma.rn.f32x2 cc, ww, xx, cc;\n mov.b64 {%0, %1}, cc;\n}" : "+f"(a0), "+f"(a1) : "f"(w), "f"(x0), "f"(x1));
+}
+__device__ __forceinline__ void fma2v(float& a0, float& a1, float w0, float w1, float x0, float x1) {  // a += w .* x
+    asm("{\n .reg .b64 ww, xx, cc;\n mov.b64 ww, {%2, %3};\n mov.b64 xx, {%4, %5};\n mov.b64 cc, {%0, %1};\n"
+        " fma.rn.f32x2 cc, ww, xx, cc;\n mov.b64 {%0, %1}, cc;\n}" : "+f"(a0), "+f"(a1) : "f"(w0), "f"(w1), "f"(x0), "f"(x1));
+}
+__device__ __forceinline__ void mul2(float& a0, float& a1, float w) {                                 // a *= w
+    asm("{\n .reg .b64 ww, cc;\n mov.b64 ww, {%2, %2};\n mov.b64 cc, {%0, %1};\n"
+        " mul.rn.f32x2 cc, cc, ww;\n mov.b64 {%0, %1}, cc;\n}" : "+f"(a0), "+f"(a1) : "f"(w));
+}
+__device__ __forceinline__ void mul2v(float& o0, float& o1, float w0, float w1, float x0, float x1) {  // o = w .* x
+    asm("{\n .reg .b64 ww, xx, cc;\n mov.b64 ww, {%2, %3};\n mov.b64 xx, {%4, %5};\n"
+        " mul.rn.f32x2 cc, ww, xx;\n mov.b64 {%0, %1}, cc;\n}" : "=f"(o0), "=f"(o1) : "f"(w0), "f"(w1), "f"(x0), "f"(x1));
+}
+// predicated pair add: (a0, a1) += (x0, x1) if pred (one FADD2 under a predicate)
+__device__ __forceinline__ void add2_if(bool pred, float& a0, float& a1, float x0, float x1) {
+    asm("{\n .reg .pred q;\n .reg .b64 xx, cc;\n setp.ne.b32 q, %4, 0;\n mov.b64 xx, {%2, %3};\n mov.b64 cc, {%0, %1};\n"
+        " @q add.rn.f32x2 cc, cc, xx;\n mov.b64 {%0, %1}, cc;\n}" : "+f"(a0), "+f"(a1) : "f"(x0), "f"(x1), "r"((int)pred));
+}
+// a[c] += w * x[c] and a[c] *= w over a lane's channels
+template <int CH> __device__ __forceinline__ void axpy(float (&a)[CH], float w, const float (&x)[CH]) {
+#pragma unroll
+    for (int c = 0; c < CH; c += 2) fma2(a[c], a[c + 1], w, x[c], x[c + 1]);
+}
+template <int CH> __device__ __forceinline__ void scale(float (&a)[CH], float w) {
+#pragma unroll
+    for (int c = 0; c < CH; c += 2) mul2(a[c], a[c + 1], w);
+}
+
+// ---- L2 prefetch of a feature row that a later batch will gather (run_edges): no destination register, so the
+// bytes in flight are not bounded by the register file.  GNN_PF_MODE 0: off (default); 1: one prefetch.global.L2 per
+// 128-byte line (SASS CCTL.E.PF2); 2: one cp.async.bulk.prefetch.L2 per row (TMA unit).  Measured on B200
+// (profiles/r02_csr_experiments.md): both modes are SLOWER than no prefetch (cfg 3 step +8 % / +17 %, cfg 5 +4 % /
+// +29 %) - the extra requests cost more in the memory pipeline than the shorter latency returns - so the knob
+// stays off; it is kept for the record.
+#ifndef GNN_PF_MODE
+#define GNN_PF_MODE 0
+#endif
+__device__ __forceinline__ void prefetch_row_l2(const void* row, int bytes) {
+#if GNN_PF_MODE == 1
+    for (int o = 0; o < bytes; o += 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(row) + o));
+#elif GNN_PF_MODE == 2
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(row), "r"(bytes) : "memory");
+#endif
+}
 // (lo, hi) halves of a packed bf16 pair, each added to an fp32 value: z = bf16 + f32
 __device__ __forceinline__ void add_bf16x2(uint32_t a, float x0, float x1, float& z0, float& z1) {
     // volatile: stops the compiler from keeping z alive across the head reduction instead of recomputing it
@@ -177,16 +233,16 @@ template <typename T, int CB> struct Chunk {
 
 // <a, b> over the lane's channels: fp32 accumulation of exact products (bf16: FHFMA on packed halves)
 template <typename T, int CB> __device__ __forceinline__ float dot(const Chunk<T, CB>& a, const Chunk<T, CB>& b) {
-    float s0 = 0.f, s1 = 0.f;
+    float s0, s1;
     if constexpr (sizeof(T) == 4) {
+        mul2v(s0, s1, __uint_as_float(a.w[0]), __uint_as_float(a.w[1]), __uint_as_float(b.w[0]), __uint_as_float(b.w[1]));
 #pragma unroll
-        for (int i = 0; i < CB / 4; i += 2) {
-            s0 = fmaf(__uint_as_float(a.w[i]), __uint_as_float(b.w[i]), s0);
-            s1 = fmaf(__uint_as_float(a.w[i + 1]), __uint_as_float(b.w[i + 1]), s1);
-        }
+        for (int i = 2; i < CB / 4; i += 2)
+            fma2v(s0, s1, __uint_as_float(a.w[i]), __uint_as_float(a.w[i + 1]), __uint_as_float(b.w[i]), __uint_as_float(b.w[i + 1]));
     } else {
+        mul_bf16x2(a.w[0], b.w[0], s0, s1);
 #pragma unroll
-        for (int i = 0; i < CB / 4; ++i) fma_bf16x2(a.w[i], b.w[i], s0, s1);
+        for (int i = 1; i < CB / 4; ++i) fma_bf16x2(a.w[i], b.w[i], s0, s1);
     }
     return s0 + s1;
 }

@@ -102,6 +102,9 @@ __device__ __forceinline__ void run_edges(typename Op::St& st, const typename Op
             nbrs(t, kc, na);
             typename Op::Src sa;
             Op::gather(p, sh, na, g, sa);
+            // while the first batch of block kc is in flight: this lane's neighbour of block kc + 1 (my_next, loaded one
+            // block ago) -> its rows into L2, so the gathers of that block find them there instead of in DRAM
+            if (GNN_PF_MODE != 0 && (t % BPB) == 0 && kc + 1 < nblk && my_next >= 0) Op::prefetch(p, sh, my_next);
             Op::compute(st, own, p, sh, na, g, sa);
             if ((t % BPB) == BPB - 1) { my_cur = my_next; my_next = ldidx(kc + 2); }
         }

@@ -48,6 +48,9 @@ template <typename T, int CB_, int G_, int KU_, bool SORTED> struct MinFwdT : Op
         for (int u = 0; u < KU; ++u)
             src.c[u][0].load_global(p.x, (size_t)(nbr[u] < 0 ? 0 : nbr[u]) * sh.ld + g.eoff, nbr[u] >= 0 && g.act);
     }
+    __device__ __forceinline__ static void prefetch(const Params& p, const Shape& sh, int nbr) {
+        prefetch_row_l2(p.x + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
+    }
     __device__ __forceinline__ static void compute(St& st, const Own&, const Params& p, const Shape&,
                                                    const int (&nbr)[KU], const GeoT&, const Src& src) {
 #pragma unroll

@@ -77,14 +77,16 @@ template <typename T, int CB_, int G_, int KU_> struct GatFwd : OpBase<T, CB_, G
 #pragma unroll
         for (int u = 0; u < KU; ++u) s[u] = nbr[u] < 0 ? -INFINITY : s[u];
         const float corr = softmax_step<KU>(st.m, st.sc[0], s, pw);
-#pragma unroll
-        for (int c = 0; c < CH; ++c) st.acc[0][c] *= corr;
+        scale<CH>(st.acc[0], corr);
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            const Ck& xc = src.c[u][0];
-#pragma unroll
-            for (int c = 0; c < CH; ++c) st.acc[0][c] = fmaf(pw[u], xc.get(c), st.acc[0][c]);
+            float xf[CH];
+            src.c[u][0].to_float(xf);
+            axpy<CH>(st.acc[0], pw[u], xf);
         }
+    }
+    __device__ __forceinline__ static void prefetch(const Params& p, const Shape& sh, int nbr) {
+        prefetch_row_l2(p.xr + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
                                                     const GeoT& g, float (&)[CH]) {
@@ -171,15 +173,13 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdDst : OpBase<T, CB_
             float z[CH];
             add_chunk(xc, o.xl, z);
 #pragma unroll
-            for (int c = 0; c < CH; ++c) {
-                if (z[c] > 0.f) {
-                    st.acc[0][c] += w;
-                    st.acc[1][c] += alpha;
-                }
-            }
+            for (int c = 0; c < CH; ++c) add2_if(z[c] > 0.f, st.acc[0][c], st.acc[1][c], w, alpha);   // (A+, B+) += (w, alpha)
             st.sc[0] += w;
             st.sc[1] += alpha;
         }
+    }
+    __device__ __forceinline__ static void prefetch(const Params& p, const Shape& sh, int nbr) {
+        prefetch_row_l2(p.xr + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
                                                     const GeoT& g, float (&da)[CH]) {
@@ -269,13 +269,21 @@ template <typename T, int CB_, int G_, int KU_> struct GatBwdSrc : OpBase<T, CB_
             const Ck &lc = src.c[u][0], &gc = src.c[u][1];
             float z[CH];
             add_chunk(lc, o.xrf, z);
+            float gf[CH];
+            gc.to_float(gf);
+            axpy<CH>(st.acc[0], alpha, gf);
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-                st.acc[0][c] = fmaf(alpha, gc.get(c), st.acc[0][c]);
                 if (z[c] > 0.f) st.acc[1][c] += de;
             }
             st.sc[0] += de;
         }
+    }
+    __device__ __forceinline__ static void prefetch(const Params& p, const Shape& sh, int nbr) {
+        prefetch_row_l2(p.xl + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
+        prefetch_row_l2(p.dout + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
+        prefetch_row_l2(p.lse + (size_t)nbr * sh.ldh, sh.H * (int)sizeof(float));
+        prefetch_row_l2(p.g + (size_t)nbr * sh.ldh, sh.H * (int)sizeof(float));
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
                                                     const GeoT& g, float (&da)[CH]) {

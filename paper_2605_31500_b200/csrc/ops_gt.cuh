@@ -77,6 +77,11 @@ template <typename T, int CB_, int G_, int KU_> struct GtFwd : OpBase<T, CB_, G_
             src.c[u][1].load_global(p.v, off, pr);
         }
     }
+    // this lane's neighbour of the NEXT edge block: its K and V rows into L2 (see run_edges)
+    __device__ __forceinline__ static void prefetch(const Params& p, const Shape& sh, int nbr) {
+        prefetch_row_l2(p.k + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
+        prefetch_row_l2(p.v + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
+    }
     __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
                                                    const int (&nbr)[KU], const GeoT& g, const Src& src) {
         float s[KU];
@@ -90,13 +95,12 @@ template <typename T, int CB_, int G_, int KU_> struct GtFwd : OpBase<T, CB_, G_
 #pragma unroll
         for (int u = 0; u < KU; ++u) s[u] = nbr[u] < 0 ? -INFINITY : s[u] * p.qscale;
         const float corr = softmax_step<KU>(st.m, st.sc[0], s, pw);
-#pragma unroll
-        for (int c = 0; c < CH; ++c) st.acc[0][c] *= corr;
+        scale<CH>(st.acc[0], corr);
 #pragma unroll
         for (int u = 0; u < KU; ++u) {
-            const Ck& vc = src.c[u][1];
-#pragma unroll
-            for (int c = 0; c < CH; ++c) st.acc[0][c] = fmaf(pw[u], vc.get(c), st.acc[0][c]);
+            float vf[CH];
+            src.c[u][1].to_float(vf);
+            axpy<CH>(st.acc[0], pw[u], vf);
         }
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
@@ -152,6 +156,10 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdDst : OpBase<T, CB_,
             src.c[u][1].load_global(p.v, off, pr);
         }
     }
+    __device__ __forceinline__ static void prefetch(const Params& p, const Shape& sh, int nbr) {
+        prefetch_row_l2(p.k + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
+        prefetch_row_l2(p.v + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
+    }
     __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
                                                    const int (&nbr)[KU], const GeoT& g, const Src& src) {
         float r[2 * KU];
@@ -166,13 +174,10 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdDst : OpBase<T, CB_,
         for (int u = 0; u < KU; ++u) {
             const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] * p.qscale - o.lp);
             const float w = alpha * r[2 * u + 1];
-            const Ck& kc = src.c[u][0];
-#pragma unroll
-            for (int c = 0; c < CH; ++c) {
-                const float kf = kc.get(c);
-                st.acc[0][c] = fmaf(w, kf, st.acc[0][c]);
-                st.acc[1][c] = fmaf(alpha, kf, st.acc[1][c]);
-            }
+            float kf[CH];
+            src.c[u][0].to_float(kf);
+            axpy<CH>(st.acc[0], w, kf);
+            axpy<CH>(st.acc[1], alpha, kf);
             st.sc[0] += w;
         }
     }
@@ -232,6 +237,11 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_,
             src.s[u][1] = t.y;
         }
     }
+    __device__ __forceinline__ static void prefetch(const Params& p, const Shape& sh, int nbr) {
+        prefetch_row_l2(p.q + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
+        prefetch_row_l2(p.dout + (size_t)nbr * sh.ld, sh.rowe * (int)sizeof(T));
+        prefetch_row_l2(p.stat2 + (size_t)nbr * sh.ldh, sh.H * (int)sizeof(float2));
+    }
     __device__ __forceinline__ static void compute(St& st, const Own& o, const Params& p, const Shape&,
                                                    const int (&nbr)[KU], const GeoT& g, const Src& src) {
         float r[2 * KU];
@@ -247,12 +257,11 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_,
             const float li = src.s[u][0], di = src.s[u][1];
             const float alpha = nbr[u] < 0 ? 0.f : ex2(r[2 * u] * p.kscale - li);
             const float ds = alpha * (r[2 * u + 1] - di);
-            const Ck &qc = src.c[u][0], &gc = src.c[u][1];
-#pragma unroll
-            for (int c = 0; c < CH; ++c) {
-                st.acc[0][c] = fmaf(ds, qc.get(c), st.acc[0][c]);
-                st.acc[1][c] = fmaf(alpha, gc.get(c), st.acc[1][c]);
-            }
+            float xf[CH];
+            src.c[u][0].to_float(xf);
+            axpy<CH>(st.acc[0], ds, xf);
+            src.c[u][1].to_float(xf);
+            axpy<CH>(st.acc[1], alpha, xf);
         }
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,

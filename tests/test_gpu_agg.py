@@ -120,9 +120,9 @@ def test_seg_minmax_infinite_values(mode, shuffled):
     C = 64
     x = rng.standard_normal((n, C))
     bad = np.inf if mode == "min" else -np.inf
-    x[:, :16] = bad                                    # whole channels: every row, hubs included, sees only +-inf there
     x[rng.random((n, C)) < 0.3] = bad                  # scattered: some rows see only +-inf, most see a mix
     x[rng.random((n, C)) < 0.05] = -bad                # and the value that must always win
+    x[:, :16] = bad                                    # whole channels: every row, hubs included, sees only +-inf there
     for dtype in ("f32", "bf16"):
         xd = _to_dev(x, dtype)
         got = _run(rp, ci, xd, mode, SMALL_OPTS)
