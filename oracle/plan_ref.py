@@ -23,6 +23,14 @@ a11 - 16-row block layout for the locally dense graph (own layout; the paper's W
      is prior art): window w = rows [16w, 16w+16); bitmap[w][r] bit c is set iff the FIRST
      occurrence of edge (dst 16w+r <- src 16w+c) exists; every other entry (sources outside
      the window, and duplicate in-window entries) goes to a remainder CSR in original order.
+f2 - general WSB layout ("WSB format and TCB construction", storage PAPER.md:573): destination rows are cut
+     into row windows of R = 16; for each window the UNIQUE source columns of all its edges are sorted ascending and
+     split into Tensor Core Blocks (TCBs) of width W = 8; a TCB stores its 8 global column indices (padded with zeros
+     if fewer than 8) and a 128-bit bitmap of which of its 16 x 8 edges exist; tcb_row_offset maps each row window to
+     its contiguous range of TCBs.  Bitmap layout here: 16 bytes per TCB, byte r = row r of the window, bit c = column
+     c of the TCB (read as two little-endian 64-bit words: word 0 = rows 0-7, word 1 = rows 8-15).  A bitmap cannot
+     say that an entry occurs twice: n_dup counts the CSR entries beyond the first of each (dst, src) pair (0 for a
+     simple graph; the CUDA WSB entry points refuse plans with n_dup > 0).
 """
 from __future__ import annotations
 
@@ -124,3 +132,34 @@ def build_blocks(rowptr, colidx) -> dict:
     np.cumsum(np.bincount(row_of_edge[rem], minlength=n), out=rem_rowptr[1:])
     return dict(n_windows=nw, bitmap=bitmap.reshape(nw, 16), rem_rowptr=rem_rowptr.astype(np.int32),
                 rem_colidx=rem_colidx)
+
+
+def build_wsb(rowptr, colidx) -> dict:
+    """f2: the paper's WSB layout for the attention path (no weight tiles)."""
+    rowptr = np.asarray(rowptr, dtype=np.int64)
+    colidx = np.asarray(colidx, dtype=np.int64)
+    n = rowptr.size - 1
+    nw = (n + 15) // 16
+    row_of_edge = np.repeat(np.arange(n, dtype=np.int64), np.diff(rowptr))
+    win = row_of_edge // 16
+    # unique (window, column) pairs in (window, column) order = per window the sorted unique columns
+    pair = np.unique(win * n + colidx) if colidx.size else np.zeros(0, np.int64)
+    uwin, ucol = pair // max(n, 1), pair % max(n, 1)
+    ucount = np.bincount(uwin, minlength=nw) if pair.size else np.zeros(nw, np.int64)
+    ntcb = (ucount + 7) // 8
+    tcb_row_offset = np.zeros(nw + 1, dtype=np.int64)
+    np.cumsum(ntcb, out=tcb_row_offset[1:])
+    total = int(tcb_row_offset[-1])
+    ustart = np.zeros(nw + 1, dtype=np.int64)
+    np.cumsum(ucount, out=ustart[1:])
+    pos = np.arange(pair.size, dtype=np.int64) - ustart[uwin]          # rank of the column inside its window
+    cols = np.zeros(total * 8, dtype=np.int32)                          # padded with zeros (PAPER.md:545)
+    cols[tcb_row_offset[uwin] * 8 + pos] = ucol
+    # bitmap: one bit per distinct (dst, src) pair
+    bitmap = np.zeros(total * 16, dtype=np.uint8)
+    epos = np.searchsorted(pair, win * n + colidx) - ustart[win] if colidx.size else np.zeros(0, np.int64)
+    byte = (tcb_row_offset[win] + epos // 8) * 16 + (row_of_edge % 16)
+    np.bitwise_or.at(bitmap, byte, (np.uint8(1) << (epos % 8).astype(np.uint8)))
+    nbits = int(np.unpackbits(bitmap).sum())
+    return dict(n_windows=nw, n_tcb=total, tcb_row_offset=tcb_row_offset.astype(np.int32), tcb_cols=cols.reshape(total, 8),
+                tcb_bitmap=bitmap.reshape(total, 16), n_dup=int(colidx.size) - nbits)

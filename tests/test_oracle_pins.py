@@ -497,6 +497,75 @@ def test_build_blocks_vs_bruteforce():
     assert int(sum(bin(int(x)).count("1") for x in bm.ravel())) + b["rem_colidx"].size == ci.size
 
 
+def _wsb_bruteforce(rp, ci, n):
+    """PAPER.md:545 read literally, with Python sets and loops."""
+    nw = (n + 15) // 16
+    offs, cols, bms = [0], [], []
+    for w in range(nw):
+        rows = range(16 * w, min(n, 16 * w + 16))
+        uniq = sorted({int(ci[e]) for i in rows for e in range(rp[i], rp[i + 1])})
+        for t in range(0, len(uniq), 8):
+            blk = uniq[t:t + 8]
+            cols.append(blk + [0] * (8 - len(blk)))
+            bm = [0] * 16
+            for i in rows:
+                present = {int(ci[e]) for e in range(rp[i], rp[i + 1])}
+                for c, j in enumerate(blk):
+                    if j in present:
+                        bm[i - 16 * w] |= 1 << c
+            bms.append(bm)
+        offs.append(len(cols))
+    return np.array(offs, np.int32), np.array(cols, np.int32).reshape(-1, 8), np.array(bms, np.uint8).reshape(-1, 16)
+
+
+@pytest.mark.parametrize("multigraph", [False, True])
+def test_build_wsb_vs_bruteforce_and_roundtrip(multigraph):
+    """Row f2 layout: per 16-row window the sorted unique source columns cut into width-8 TCBs,
+    zero-padded column lists, 128-bit bitmaps, tcb_row_offset - against a literal set-and-loop construction, and
+    expanding the layout back gives exactly the set of distinct (dst, src) pairs of the CSR."""
+    rng = np.random.default_rng(41 + multigraph)
+    n = 103                                   # ragged last window (103 = 6*16 + 7)
+    rp, ci = _rand_graph(rng, n, 5.0, multigraph=multigraph, empty_rows=True)
+    # overlapping column sets between windows + a dense window + a row with > 8 * 3 distinct sources
+    extra_d = np.concatenate([rng.integers(0, n, 400), np.full(40, 17), rng.integers(32, 48, 200)])
+    extra_s = np.concatenate([rng.integers(0, 12, 400), rng.integers(0, n, 40), rng.integers(32, 48, 200)])
+    d_all = np.concatenate([np.repeat(np.arange(n), np.diff(rp)), extra_d])
+    s_all = np.concatenate([ci, extra_s])
+    if not multigraph:
+        key = np.unique(d_all.astype(np.int64) * n + s_all)
+        d_all, s_all = key // n, key % n
+    o = np.lexsort((s_all, d_all)) if not multigraph else np.argsort(d_all, kind="stable")
+    d_all, s_all = d_all[o], s_all[o]
+    rp = np.concatenate([[0], np.cumsum(np.bincount(d_all, minlength=n))]).astype(np.int32)
+    ci = s_all.astype(np.int32)
+    w = plan_ref.build_wsb(rp, ci)
+    offs, cols, bms = _wsb_bruteforce(rp, ci, n)
+    np.testing.assert_array_equal(w["tcb_row_offset"], offs)
+    np.testing.assert_array_equal(w["tcb_cols"], cols)
+    np.testing.assert_array_equal(w["tcb_bitmap"], bms)
+    assert w["n_windows"] == 7 and w["n_tcb"] == cols.shape[0]
+    # round trip: the layout encodes exactly the distinct (dst, src) pairs
+    pairs = set()
+    for win in range(w["n_windows"]):
+        for t in range(w["tcb_row_offset"][win], w["tcb_row_offset"][win + 1]):
+            for r in range(16):
+                for c in range(8):
+                    if (int(w["tcb_bitmap"][t, r]) >> c) & 1:
+                        pairs.add((16 * win + r, int(w["tcb_cols"][t, c])))
+    want = {(i, int(ci[e])) for i in range(n) for e in range(rp[i], rp[i + 1])}
+    assert pairs == want
+    assert w["n_dup"] == ci.size - len(want) and (w["n_dup"] > 0) == multigraph
+    # columns inside a window ascend across its TCBs; padding sits only at the end of a window's last TCB
+    for win in range(w["n_windows"]):
+        t0, t1 = w["tcb_row_offset"][win], w["tcb_row_offset"][win + 1]
+        used = w["tcb_bitmap"][t0:t1].reshape(t1 - t0, 16)
+        colmask = np.bitwise_or.reduce(used, axis=1) if t1 > t0 else np.zeros(0, np.uint8)
+        flat = [(int(w["tcb_cols"][t0 + k, c]), (int(colmask[k]) >> c) & 1) for k in range(t1 - t0) for c in range(8)]
+        valid = [j for j, u in flat if u]
+        assert valid == sorted(set(valid))
+        assert all(u for _, u in flat[:len(valid)]) and all(j == 0 and not u for j, u in flat[len(valid):])
+
+
 # --------------------------------------------------------------------------- min / max aggregation (row f3)
 from oracle import agg_ref  # noqa: E402
 
