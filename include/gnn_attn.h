@@ -68,8 +68,11 @@ typedef enum { GNN_F32 = 0, GNN_BF16 = 1 } gnn_dtype_t;
  * gnn_plan_build verifies that on the device (GNN_EINVAL if it does not hold) and the backward calls then traverse
  * the forward CSR and its bins: no transposed structure is built or stored (plan storage drops by 4*(nnz + n) bytes
  * plus the second bin set), and the gradients are bit-identical to mode 1, for which CSR^T == CSR bit for bit.
- * build_blocks != 0 also builds the 16-row block layout (gnn_gt_attn_fwd_block).              */
+ * build_blocks: bit mask.  GNN_BLOCKS_DIAG (1) also builds the diagonal 16-row block layout (gnn_gt_attn_fwd_block);
+ * GNN_BLOCKS_WSB (2) also builds the general WSB layout of PAPER.md:545 (gnn_gt_attn_fwd_wsb / _bwd_wsb) for the CSR
+ * and - with build_transpose - for CSR^T (in the undirected mode the two coincide and one copy is stored).       */
 enum { GNN_TRANSPOSE_NONE = 0, GNN_TRANSPOSE_BUILD = 1, GNN_TRANSPOSE_UNDIRECTED = 2 };
+enum { GNN_BLOCKS_NONE = 0, GNN_BLOCKS_DIAG = 1, GNN_BLOCKS_WSB = 2 };
 typedef struct {
     int32_t warp_max_deg;
     int32_t cta_max_deg;
@@ -94,6 +97,9 @@ gnn_status_t gnn_plan_bytes(int32_t n, int64_t nnz, const gnn_plan_opts_t* opts,
  *   CSR^T  : rowptr_t[n+1], colidx_t[nnz] by a STABLE sort on the source id,
  *            plus the same bins / chunks for CSR^T (out-degrees)
  *   blocks : see gnn_gt_attn_fwd_block
+ *   WSB    : per 16-row window the sorted unique source columns cut into Tensor Core Blocks of width 8; per TCB
+ *            8 column ids (zero padded) and a 128-bit bitmap of its 16 x 8 edges; tcb_row_offset per window
+ *            (PAPER.md:545).  n_dup = entries beyond the first of their (dst, src) pair (not representable).
  * rowptr/colidx: device, must outlive the plan (the plan keeps the pointers, not a copy).
  * On success *plan is a host handle to free with gnn_plan_destroy (device storage stays the caller's). */
 gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t dev_bytes, void* scratch, size_t scratch_bytes,
@@ -123,8 +129,16 @@ enum {
     GNN_PLAN_BLOCK_BITMAP = 9,      /* uint16[n_windows][16]                                         */
     GNN_PLAN_BLOCK_REM_ROWPTR = 10, /* int32[n + 1]                                                  */
     GNN_PLAN_BLOCK_REM_COLIDX = 11, /* int32[rem_nnz]                                                */
-    GNN_PLAN_FLAGS = 12             /* int32[2]: [0] = 1 if every CSR row lists its sources in ascending order;
+    GNN_PLAN_FLAGS = 12,            /* int32[2]: [0] = 1 if every CSR row lists its sources in ascending order;
                                        [1] = 1 if the backward traverses the forward CSR (GNN_TRANSPOSE_UNDIRECTED) */
+    /* general WSB layout, bit-exact against oracle/plan_ref.py::build_wsb:                  */
+    GNN_PLAN_WSB_INFO = 13,         /* int32[6]: has_wsb, n_windows, n_tcb, n_dup, n_tcb of CSR^T, n_dup of CSR^T   */
+    GNN_PLAN_WSB_ROW_OFFSET = 14,   /* int32[n_windows + 1]: tcb_row_offset                                        */
+    GNN_PLAN_WSB_COLS = 15,         /* int32[n_tcb][8]: global column ids of each TCB, zero padded                 */
+    GNN_PLAN_WSB_BITMAP = 16,       /* uint8[n_tcb][16]: byte r = row r of the window, bit c = column c of the TCB */
+    GNN_PLAN_WSB_ROW_OFFSET_T = 17, /* the same three for CSR^T (source windows x destination columns)             */
+    GNN_PLAN_WSB_COLS_T = 18,
+    GNN_PLAN_WSB_BITMAP_T = 19
 };
 /* Copies the item to HOST memory `host_dst` (synchronous).  *bytes in = capacity, out = size needed;
  * with host_dst == NULL only the size is returned.                                                 */

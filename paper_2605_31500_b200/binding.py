@@ -18,7 +18,9 @@ GNN_AGG_MIN, GNN_AGG_MAX = 0, 1
 GNN_TRANSPOSE_NONE, GNN_TRANSPOSE_BUILD, GNN_TRANSPOSE_UNDIRECTED = 0, 1, 2
 (GNN_PLAN_COUNTS, GNN_PLAN_PERM, GNN_PLAN_CHUNKS, GNN_PLAN_CHUNK_PTR, GNN_PLAN_ROWPTR_T, GNN_PLAN_COLIDX_T,
  GNN_PLAN_PERM_T, GNN_PLAN_CHUNKS_T, GNN_PLAN_CHUNK_PTR_T, GNN_PLAN_BLOCK_BITMAP, GNN_PLAN_BLOCK_REM_ROWPTR,
- GNN_PLAN_BLOCK_REM_COLIDX, GNN_PLAN_FLAGS) = range(13)
+ GNN_PLAN_BLOCK_REM_COLIDX, GNN_PLAN_FLAGS, GNN_PLAN_WSB_INFO, GNN_PLAN_WSB_ROW_OFFSET, GNN_PLAN_WSB_COLS,
+ GNN_PLAN_WSB_BITMAP, GNN_PLAN_WSB_ROW_OFFSET_T, GNN_PLAN_WSB_COLS_T, GNN_PLAN_WSB_BITMAP_T) = range(20)
+GNN_BLOCKS_NONE, GNN_BLOCKS_DIAG, GNN_BLOCKS_WSB = 0, 1, 2
 
 EXPORTED_SYMBOLS = [
     "gnn_csr_validate", "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
@@ -195,7 +197,7 @@ class Plan:
     """Owns the torch allocations behind a gnn_plan_t (plan storage, workspace) for one CSR graph."""
 
     def __init__(self, rowptr, colidx, warp_max_deg=0, cta_max_deg=0, split_chunk=0, transpose=True, blocks=False,
-                 stream=None):
+                 wsb=False, stream=None):
         torch = _require_cuda()
         if rowptr.dtype != torch.int32 or colidx.dtype != torch.int32:
             raise GnnError("rowptr / colidx must be int32")
@@ -204,7 +206,9 @@ class Plan:
         # transpose: False (forward only), True (build CSR^T) or "undirected" (the backward reuses
         # the forward CSR; the library verifies the graph is undirected and raises GnnError if not)
         mode = GNN_TRANSPOSE_UNDIRECTED if transpose == "undirected" else (GNN_TRANSPOSE_BUILD if transpose else GNN_TRANSPOSE_NONE)
-        self.opts = PlanOpts(warp_max_deg, cta_max_deg, split_chunk, mode, 1 if blocks else 0)
+        # blocks: the diagonal 16-row block layout (gnn_gt_attn_fwd_block); wsb: the general WSB layout
+        self.opts = PlanOpts(warp_max_deg, cta_max_deg, split_chunk, mode,
+                             (GNN_BLOCKS_DIAG if blocks else 0) | (GNN_BLOCKS_WSB if wsb else 0))
         dev_bytes, scratch_bytes = gnn_plan_bytes(self.n, self.nnz, self.opts)
         self.dev_mem = torch.empty(dev_bytes, dtype=torch.uint8, device=rowptr.device)
         scratch = torch.empty(scratch_bytes, dtype=torch.uint8, device=rowptr.device)
@@ -220,6 +224,10 @@ class Plan:
         c = self.export(GNN_PLAN_COUNTS)
         keys = ["n_hub", "n_cta", "n_group", "n_chunks"]
         return {**{k: int(v) for k, v in zip(keys, c[:4])}, **{k + "_t": int(v) for k, v in zip(keys, c[4:])}}
+
+    def wsb_info(self) -> dict:
+        v = self.export(GNN_PLAN_WSB_INFO)
+        return dict(zip(("has_wsb", "n_windows", "n_tcb", "n_dup", "n_tcb_t", "n_dup_t"), (int(x) for x in v)))
 
     def rows_sorted(self) -> bool:
         """True if every CSR row lists its sources in ascending order (selects the min / max fast path)."""

@@ -7,6 +7,17 @@
 #include "../../include/gnn_attn.h"
 #include "engine.cuh"
 
+namespace gnn {
+// general WSB layout (row f2): per 16-row window the sorted unique source columns in width-8 TCBs
+struct WsbView {
+    const int32_t* row_offset;   // [n_windows + 1] first TCB of every row window
+    const int32_t* cols;         // [n_tcb][8] global column ids, zero padded
+    const uint8_t* bitmap;       // [n_tcb][16] byte r = row r of the window, bit c = column c of the TCB
+    int32_t n_tcb;
+    int32_t n_dup;               // CSR entries beyond the first of their (dst, src) pair (the bitmap cannot hold them)
+};
+}  // namespace gnn
+
 struct gnn_plan {
     int32_t n;
     int64_t nnz;
@@ -25,6 +36,9 @@ struct gnn_plan {
     int32_t n_windows;
     int64_t rem_nnz;
     int32_t rows_sorted;     // 1 if every CSR row lists its sources in ascending order (min / max fast path)
+    int32_t has_wsb;         // build_blocks & GNN_BLOCKS_WSB
+    gnn::WsbView wsb;        // of the CSR (destination windows x source columns)
+    gnn::WsbView wsb_t;      // of CSR^T (source windows x destination columns); == wsb in the undirected mode
 };
 
 namespace gnn {

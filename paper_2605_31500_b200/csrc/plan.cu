@@ -6,6 +6,7 @@
 // preprocessing outside the timed layer, like the paper's format construction).
 #include <cub/device/device_radix_sort.cuh>
 #include <cub/device/device_scan.cuh>
+#include <cub/device/device_select.cuh>
 
 #include <new>
 
@@ -182,10 +183,75 @@ __global__ void pad_bitmap_kernel(uint16_t* bitmap, int n, int n_pad) {
     if (i < n_pad) bitmap[i] = 0;
 }
 
+// ---- row f2: general WSB layout.  key = (row window << 32) | source column per CSR entry
+__global__ void wsb_key_kernel(const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx, int n, long long nnz,
+                               unsigned long long* __restrict__ key) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= nnz) return;
+    int lo = 0, hi = n;  // last row with rowptr[row] <= e
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if ((long long)__ldg(rowptr + mid) <= e) lo = mid; else hi = mid;
+    }
+    key[e] = ((unsigned long long)(lo >> 4) << 32) | (unsigned int)__ldg(colidx + e);
+}
+__device__ __forceinline__ long long lower_bound_u64(const unsigned long long* a, long long lo, long long hi, unsigned long long v) {
+    while (lo < hi) {
+        const long long mid = (lo + hi) >> 1;
+        if (a[mid] < v) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+// win_uptr[w] = first unique (window, column) key of window w, w = 0 .. n_win
+__global__ void wsb_winptr_kernel(const unsigned long long* __restrict__ ukey, const int* __restrict__ n_unique, int n_win,
+                                  int32_t* __restrict__ win_uptr) {
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w > n_win) return;
+    win_uptr[w] = (int32_t)lower_bound_u64(ukey, 0, *n_unique, (unsigned long long)w << 32);
+}
+__global__ void wsb_ntcb_kernel(const int32_t* __restrict__ win_uptr, int n_win, int32_t* __restrict__ ntcb) {
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w < n_win) ntcb[w] = (win_uptr[w + 1] - win_uptr[w] + 7) >> 3;
+}
+// the k-th unique column of window w goes to slot k of the window's TCB range (cols is zero-filled beforehand)
+__global__ void wsb_cols_kernel(const unsigned long long* __restrict__ ukey, const int* __restrict__ n_unique,
+                                const int32_t* __restrict__ win_uptr, const int32_t* __restrict__ row_offset,
+                                int32_t* __restrict__ cols) {
+    const long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= *n_unique) return;
+    const unsigned long long k = ukey[u];
+    const int w = (int)(k >> 32);
+    cols[(long long)row_offset[w] * 8 + (u - win_uptr[w])] = (int32_t)(unsigned int)k;
+}
+// one bit per CSR entry (integer atomicOr: the result does not depend on the order); a bit found set = duplicate entry
+__global__ void wsb_bitmap_kernel(const int32_t* __restrict__ rowptr, const int32_t* __restrict__ colidx, int n, long long nnz,
+                                  const unsigned long long* __restrict__ ukey, const int32_t* __restrict__ win_uptr,
+                                  const int32_t* __restrict__ row_offset, unsigned int* __restrict__ bitmap32,
+                                  int32_t* __restrict__ n_dup) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= nnz) return;
+    int lo = 0, hi = n;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if ((long long)__ldg(rowptr + mid) <= e) lo = mid; else hi = mid;
+    }
+    const int w = lo >> 4, r = lo & 15;
+    const unsigned long long k = ((unsigned long long)w << 32) | (unsigned int)__ldg(colidx + e);
+    const long long pos = lower_bound_u64(ukey, win_uptr[w], win_uptr[w + 1], k) - win_uptr[w];
+    const long long byte = ((long long)row_offset[w] + (pos >> 3)) * 16 + r;
+    const unsigned int bit = 1u << ((pos & 7) + 8 * (byte & 3));
+    const unsigned int old = atomicOr(bitmap32 + (byte >> 2), bit);
+    if (old & bit) atomicAdd(n_dup, 1);
+}
+
 struct Layout {
     // persistent
     size_t perm, chunks, chunk_ptr, counts, rowptr_t, colidx_t, perm_t, chunks_t, chunk_ptr_t, dev_total;
     size_t blk_bitmap, blk_rem_rowptr, blk_rem_colidx, blk_cnt;
+    size_t wsb_row_offset[2], wsb_cols[2], wsb_bitmap[2];          // [0] CSR, [1] CSR^T (only when the plan stores CSR^T)
+    size_t wsb_key, wsb_key_sorted, wsb_nuniq, wsb_win_uptr, wsb_ntcb;  // scratch
+    long long max_tcb;
+    int n_win;
     // scratch
     size_t key, key_sorted, rowid, ekey_sorted, erow, cub, scratch_total;
     size_t cub_bytes;
@@ -224,7 +290,7 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
     L.perm = take(sizeof(int32_t) * (size_t)n);
     L.chunks = take(sizeof(int32_t) * 4 * (size_t)L.max_chunks);
     L.chunk_ptr = take(sizeof(int32_t) * (size_t)(L.max_hub + 1));
-    L.counts = take(sizeof(int32_t) * 16);   // 8 bin counts + flags
+    L.counts = take(sizeof(int32_t) * 16);   // 8 bin counts + flags + WSB info
     L.rowptr_t = L.colidx_t = L.perm_t = L.chunks_t = L.chunk_ptr_t = 0;
     if (own_t) {
         L.rowptr_t = take(sizeof(int32_t) * ((size_t)n + 1));
@@ -234,13 +300,23 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
         L.chunk_ptr_t = take(sizeof(int32_t) * (size_t)(L.max_hub + 1));
     }
     L.blk_bitmap = L.blk_rem_rowptr = L.blk_rem_colidx = 0;
-    if (o.build_blocks) {
+    L.n_win = (n + 15) / 16;
+    L.max_tcb = nnz / 8 + L.n_win + 1;          // sum over windows of ceil(unique_w / 8) <= nnz / 8 + n_windows
+    for (int t = 0; t < 2; ++t) L.wsb_row_offset[t] = L.wsb_cols[t] = L.wsb_bitmap[t] = 0;
+    if (o.build_blocks & GNN_BLOCKS_WSB) {
+        for (int t = 0; t < (own_t ? 2 : 1); ++t) {
+            L.wsb_row_offset[t] = take(sizeof(int32_t) * ((size_t)L.n_win + 1));
+            L.wsb_cols[t] = take(sizeof(int32_t) * 8 * (size_t)L.max_tcb);
+            L.wsb_bitmap[t] = take(16 * (size_t)L.max_tcb);
+        }
+    }
+    if (o.build_blocks & GNN_BLOCKS_DIAG) {
         L.blk_bitmap = take(sizeof(uint16_t) * (((size_t)n + 15) / 16 * 16));
         L.blk_rem_rowptr = take(sizeof(int32_t) * ((size_t)n + 1));
         L.blk_rem_colidx = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
     }
     L.dev_total = off;
-    size_t t1 = 0, t2 = 0, t3 = 0;
+    size_t t1 = 0, t2 = 0, t3 = 0, t4 = 0, t5 = 0, t6 = 0;
     cudaError_t e = cub::DeviceRadixSort::SortPairs(nullptr, t1, (const uint32_t*)nullptr, (uint32_t*)nullptr,
                                                     (const int32_t*)nullptr, (int32_t*)nullptr, (long long)n, 0, 7);
     if (e != cudaSuccess) return e;
@@ -249,12 +325,22 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
                                             (const int32_t*)nullptr, (int32_t*)nullptr, (long long)nnz, 0, n_bits(n));
         if (e != cudaSuccess) return e;
     }
-    if (o.build_blocks) {
+    if (o.build_blocks & GNN_BLOCKS_DIAG) {
         e = cub::DeviceScan::InclusiveSum(nullptr, t3, (const int32_t*)nullptr, (int32_t*)nullptr, n);
         if (e != cudaSuccess) return e;
     }
+    if (o.build_blocks & GNN_BLOCKS_WSB) {
+        e = cub::DeviceRadixSort::SortKeys(nullptr, t4, (const unsigned long long*)nullptr, (unsigned long long*)nullptr,
+                                           (long long)nnz, 0, 32 + n_bits(L.n_win + 1));
+        if (e == cudaSuccess)
+            e = cub::DeviceSelect::Unique(nullptr, t5, (const unsigned long long*)nullptr, (unsigned long long*)nullptr,
+                                          (int*)nullptr, (long long)nnz);
+        if (e == cudaSuccess) e = cub::DeviceScan::InclusiveSum(nullptr, t6, (const int32_t*)nullptr, (int32_t*)nullptr, L.n_win);
+        if (e != cudaSuccess) return e;
+    }
     L.cub_bytes = t1 > t2 ? t1 : t2;
-    if (t3 > L.cub_bytes) L.cub_bytes = t3;
+    for (size_t t : {t3, t4, t5, t6})
+        if (t > L.cub_bytes) L.cub_bytes = t;
     off = 0;
     L.key = take(sizeof(uint32_t) * (size_t)n);
     L.key_sorted = take(sizeof(uint32_t) * (size_t)n);
@@ -264,7 +350,15 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
         L.ekey_sorted = take(sizeof(uint32_t) * (size_t)(nnz > 0 ? nnz : 1));
         L.erow = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
     }
-    L.blk_cnt = o.build_blocks ? take(sizeof(int32_t) * (size_t)n) : 0;
+    L.blk_cnt = (o.build_blocks & GNN_BLOCKS_DIAG) ? take(sizeof(int32_t) * (size_t)n) : 0;
+    L.wsb_key = L.wsb_key_sorted = L.wsb_nuniq = L.wsb_win_uptr = L.wsb_ntcb = 0;
+    if (o.build_blocks & GNN_BLOCKS_WSB) {
+        L.wsb_key = take(sizeof(unsigned long long) * (size_t)(nnz > 0 ? nnz : 1));        // keys, later the unique keys
+        L.wsb_key_sorted = take(sizeof(unsigned long long) * (size_t)(nnz > 0 ? nnz : 1));
+        L.wsb_nuniq = take(16);
+        L.wsb_win_uptr = take(sizeof(int32_t) * ((size_t)L.n_win + 1));
+        L.wsb_ntcb = take(sizeof(int32_t) * (size_t)L.n_win);
+    }
     L.cub = take(L.cub_bytes + 16);
     L.scratch_total = off;
     return cudaSuccess;
@@ -294,6 +388,43 @@ cudaError_t build_bins(const int32_t* rowptr, int n, const gnn_plan_opts_t& o, c
         count_launch();
     }
     return cudaGetLastError();
+}
+
+// WSB of one CSR (row f2): everything on the device; info_dev[0] = n_tcb, info_dev[1] = n_dup on return (async)
+cudaError_t build_wsb(const int32_t* rowptr, const int32_t* colidx, int n, long long nnz, const Layout& L, char* sc,
+                      int32_t* row_offset, int32_t* cols, uint8_t* bitmap, int32_t* info_dev, cudaStream_t st) {
+    unsigned long long* key = (unsigned long long*)(sc + L.wsb_key);
+    unsigned long long* key_sorted = (unsigned long long*)(sc + L.wsb_key_sorted);
+    int* n_unique = (int*)(sc + L.wsb_nuniq);
+    int32_t* win_uptr = (int32_t*)(sc + L.wsb_win_uptr);
+    int32_t* ntcb = (int32_t*)(sc + L.wsb_ntcb);
+    const int n_win = L.n_win, tb = 256;
+    cudaError_t e = cudaMemsetAsync(cols, 0, sizeof(int32_t) * 8 * (size_t)L.max_tcb, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(bitmap, 0, 16 * (size_t)L.max_tcb, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(n_unique, 0, 16, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(row_offset, 0, sizeof(int32_t) * ((size_t)n_win + 1), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(info_dev, 0, 2 * sizeof(int32_t), st);
+    if (e != cudaSuccess) return e;
+    if (nnz > 0) {
+        const unsigned nb = (unsigned)((nnz + tb - 1) / tb);
+        wsb_key_kernel<<<nb, tb, 0, st>>>(rowptr, colidx, n, nnz, key);
+        size_t cb = L.cub_bytes;
+        e = cub::DeviceRadixSort::SortKeys(sc + L.cub, cb, (const unsigned long long*)key, key_sorted, nnz, 0,
+                                           32 + n_bits(n_win + 1), st);
+        if (e != cudaSuccess) return e;
+        cb = L.cub_bytes;
+        e = cub::DeviceSelect::Unique(sc + L.cub, cb, (const unsigned long long*)key_sorted, key, n_unique, nnz, st);   // key := unique keys
+        if (e != cudaSuccess) return e;
+        wsb_winptr_kernel<<<(n_win + 1 + tb - 1) / tb, tb, 0, st>>>(key, n_unique, n_win, win_uptr);
+        wsb_ntcb_kernel<<<(n_win + tb - 1) / tb, tb, 0, st>>>(win_uptr, n_win, ntcb);
+        cb = L.cub_bytes;
+        e = cub::DeviceScan::InclusiveSum(sc + L.cub, cb, (const int32_t*)ntcb, row_offset + 1, n_win, st);
+        if (e != cudaSuccess) return e;
+        wsb_cols_kernel<<<nb, tb, 0, st>>>(key, n_unique, win_uptr, row_offset, cols);
+        wsb_bitmap_kernel<<<nb, tb, 0, st>>>(rowptr, colidx, n, nnz, key, win_uptr, row_offset, (unsigned int*)bitmap, info_dev + 1);
+        count_launch(7);
+    }
+    return cudaMemcpyAsync(info_dev, row_offset + n_win, sizeof(int32_t), cudaMemcpyDeviceToDevice, st);
 }
 
 }  // namespace
@@ -394,8 +525,19 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
         count_launch();
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(&unsorted, counts_dev + 8, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    int32_t wsb_info[4] = {0, 0, 0, 0};
+    if (e == cudaSuccess && (o.build_blocks & GNN_BLOCKS_WSB)) {
+        const bool own_t = o.build_transpose == GNN_TRANSPOSE_BUILD;
+        P->has_wsb = 1;
+        e = build_wsb(rowptr, colidx, n, nnz, L, sc, (int32_t*)(dm + L.wsb_row_offset[0]), (int32_t*)(dm + L.wsb_cols[0]),
+                      (uint8_t*)(dm + L.wsb_bitmap[0]), counts_dev + 10, st);
+        if (e == cudaSuccess && own_t)
+            e = build_wsb(P->rowptr_t, P->colidx_t, n, nnz, L, sc, (int32_t*)(dm + L.wsb_row_offset[1]),
+                          (int32_t*)(dm + L.wsb_cols[1]), (uint8_t*)(dm + L.wsb_bitmap[1]), counts_dev + 12, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(wsb_info, counts_dev + 10, (own_t ? 4 : 2) * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    }
     int32_t rem_nnz = 0;
-    if (e == cudaSuccess && o.build_blocks) {
+    if (e == cudaSuccess && (o.build_blocks & GNN_BLOCKS_DIAG)) {
         P->n_windows = (n + 15) / 16;
         P->blk_bitmap = (uint16_t*)(dm + L.blk_bitmap);
         P->blk_rem_rowptr = (int32_t*)(dm + L.blk_rem_rowptr);
@@ -416,6 +558,15 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     P->rem_nnz = rem_nnz;
     P->rows_sorted = unsorted ? 0 : 1;
+    if (P->has_wsb) {
+        P->wsb = WsbView{(int32_t*)(dm + L.wsb_row_offset[0]), (int32_t*)(dm + L.wsb_cols[0]), (uint8_t*)(dm + L.wsb_bitmap[0]),
+                         wsb_info[0], wsb_info[1]};
+        if (o.build_transpose == GNN_TRANSPOSE_BUILD)
+            P->wsb_t = WsbView{(int32_t*)(dm + L.wsb_row_offset[1]), (int32_t*)(dm + L.wsb_cols[1]),
+                               (uint8_t*)(dm + L.wsb_bitmap[1]), wsb_info[2], wsb_info[3]};
+        else if (o.build_transpose == GNN_TRANSPOSE_UNDIRECTED)
+            P->wsb_t = P->wsb;          // the stable transpose of an undirected CSR is the CSR itself
+    }
     if (e != cudaSuccess) {
         set_error("gnn_plan_build: CUDA error: %s", cudaGetErrorString(e));
         delete P;
@@ -483,6 +634,7 @@ extern "C" gnn_status_t gnn_plan_export(const gnn_plan_t* P, int what, void* hos
                          P->tr.n_hub, P->tr.n_cta, P->tr.n_group, P->tr.n_chunks};
     const bool T = P->opts.build_transpose != 0;
     const int32_t flags[2] = {P->rows_sorted, P->opts.build_transpose == GNN_TRANSPOSE_UNDIRECTED ? 1 : 0};
+    const int32_t wsbinfo[6] = {P->has_wsb, (P->n + 15) / 16, P->wsb.n_tcb, P->wsb.n_dup, P->wsb_t.n_tcb, P->wsb_t.n_dup};
     switch (what) {
         case GNN_PLAN_FLAGS: src = flags; need = sizeof(flags); break;
         case GNN_PLAN_COUNTS: need = sizeof(counts); break;
@@ -494,12 +646,29 @@ extern "C" gnn_status_t gnn_plan_export(const gnn_plan_t* P, int what, void* hos
         case GNN_PLAN_PERM_T: if (T) { src = P->tr.perm; need = 4 * (size_t)P->n; } break;
         case GNN_PLAN_CHUNKS_T: if (T) { src = P->tr.chunks; need = 16 * (size_t)P->tr.n_chunks; } break;
         case GNN_PLAN_CHUNK_PTR_T: if (T) { src = P->tr.chunk_ptr; need = 4 * ((size_t)P->tr.n_hub + 1); } break;
+        case GNN_PLAN_WSB_INFO: need = sizeof(wsbinfo); break;
+        case GNN_PLAN_WSB_ROW_OFFSET: if (P->has_wsb) { src = P->wsb.row_offset; need = 4 * ((size_t)(P->n + 15) / 16 + 1); } break;
+        case GNN_PLAN_WSB_COLS: if (P->has_wsb) { src = P->wsb.cols; need = 32 * (size_t)P->wsb.n_tcb; } break;
+        case GNN_PLAN_WSB_BITMAP: if (P->has_wsb) { src = P->wsb.bitmap; need = 16 * (size_t)P->wsb.n_tcb; } break;
+        case GNN_PLAN_WSB_ROW_OFFSET_T: if (P->has_wsb && T) { src = P->wsb_t.row_offset; need = 4 * ((size_t)(P->n + 15) / 16 + 1); } break;
+        case GNN_PLAN_WSB_COLS_T: if (P->has_wsb && T) { src = P->wsb_t.cols; need = 32 * (size_t)P->wsb_t.n_tcb; } break;
+        case GNN_PLAN_WSB_BITMAP_T: if (P->has_wsb && T) { src = P->wsb_t.bitmap; need = 16 * (size_t)P->wsb_t.n_tcb; } break;
         case GNN_PLAN_BLOCK_BITMAP: if (P->blk_bitmap) { src = P->blk_bitmap; need = 2 * 16 * (size_t)P->n_windows; } break;
         case GNN_PLAN_BLOCK_REM_ROWPTR: if (P->blk_bitmap) { src = P->blk_rem_rowptr; need = 4 * ((size_t)P->n + 1); } break;
         case GNN_PLAN_BLOCK_REM_COLIDX: if (P->blk_bitmap) { src = P->blk_rem_colidx; need = 4 * (size_t)P->rem_nnz; } break;
         default: break;
     }
     if (what == GNN_PLAN_BLOCK_REM_COLIDX && P->blk_bitmap && P->rem_nnz == 0) { *bytes = 0; return GNN_OK; }
+    if (what == GNN_PLAN_WSB_INFO) {
+        const size_t cap0 = *bytes;
+        *bytes = need;
+        if (!host_dst) return GNN_OK;
+        if (cap0 < need) { set_error("gnn_plan_export: buffer too small (%zu < %zu)", cap0, need); return GNN_EWORKSPACE; }
+        memcpy(host_dst, wsbinfo, need);
+        return GNN_OK;
+    }
+    if ((what == GNN_PLAN_WSB_COLS || what == GNN_PLAN_WSB_BITMAP) && P->has_wsb && P->wsb.n_tcb == 0) { *bytes = 0; return GNN_OK; }
+    if ((what == GNN_PLAN_WSB_COLS_T || what == GNN_PLAN_WSB_BITMAP_T) && P->has_wsb && T && P->wsb_t.n_tcb == 0) { *bytes = 0; return GNN_OK; }
     if (what != GNN_PLAN_COUNTS && !src) {
         set_error("gnn_plan_export: item %d is not part of this plan", what);
         return GNN_EINVAL;

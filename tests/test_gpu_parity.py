@@ -388,6 +388,65 @@ def test_block_layout_bit_exact():
         assert int(ref["rem_rowptr"][-1]) + int(np.unpackbits(ref["bitmap"].view(np.uint8)).sum()) == colidx.size
 
 
+def _wsb_test_graphs():
+    """(name, n, rowptr, colidx): the locally dense config scaled; a simple graph with heavily overlapping column sets
+    between windows, a dense window, rows with > 24 distinct sources, empty rows and a ragged last window; a directed
+    power-law graph (cfg 2 scaled: hubs -> windows with hundreds of TCBs)."""
+    c4 = GI.make_config(4, scale=0.0041)
+    rng = np.random.default_rng(17)
+    n = 1003
+    dst = np.concatenate([rng.integers(0, n, 9000), np.full(60, 17), rng.integers(32, 48, 300)])
+    src = np.concatenate([np.where(rng.random(9000) < 0.5, rng.integers(0, 40, 9000), rng.integers(0, n, 9000)),
+                          rng.integers(0, n, 60), rng.integers(32, 48, 300)])
+    keep = dst % 11 != 0
+    rp_o, ci_o = GI.csr_from_pairs(n, dst[keep], src[keep], self_loops=False, dedupe=True)
+    c2 = GI.make_config(2, scale=0.03)
+    return [("cfg4", c4["n"], c4["rowptr"], c4["colidx"]), ("overlap", n, rp_o, ci_o), ("cfg2", c2["n"], c2["rowptr"], c2["colidx"])]
+
+
+def test_wsb_layout_bit_exact():
+    """Row f2 metadata: tcb_row_offset, zero-padded column lists and 128-bit bitmaps of the CSR and of CSR^T, bit-exact
+    vs oracle/plan_ref.py::build_wsb (PAPER.md:545); the undirected mode stores one copy; duplicates are counted."""
+    import paper_2605_31500_b200 as G
+    import paper_2605_31500_b200.binding as B
+    torch = _torch()
+
+    def check_wsb(plan, rp, ci, t):
+        ref = plan_ref.build_wsb(rp, ci)
+        ro, co, bm = ((B.GNN_PLAN_WSB_ROW_OFFSET_T, B.GNN_PLAN_WSB_COLS_T, B.GNN_PLAN_WSB_BITMAP_T) if t else
+                      (B.GNN_PLAN_WSB_ROW_OFFSET, B.GNN_PLAN_WSB_COLS, B.GNN_PLAN_WSB_BITMAP))
+        assert np.array_equal(plan.export(ro), ref["tcb_row_offset"])
+        assert np.array_equal(plan.export(co).reshape(-1, 8), ref["tcb_cols"])
+        assert np.array_equal(plan.export(bm, np.uint8).reshape(-1, 16), ref["tcb_bitmap"])
+        info = plan.wsb_info()
+        assert info["has_wsb"] == 1 and info["n_windows"] == ref["n_windows"]
+        assert (info["n_tcb_t"], info["n_dup_t"]) == (ref["n_tcb"], ref["n_dup"]) if t else (info["n_tcb"], info["n_dup"]) == (ref["n_tcb"], ref["n_dup"])
+        return ref
+
+    for name, n, rp, ci in _wsb_test_graphs():
+        plan = G.Plan(torch.from_numpy(rp).cuda(), torch.from_numpy(ci).cuda(), transpose=True, wsb=True)
+        ref = check_wsb(plan, rp, ci, False)
+        assert ref["n_dup"] == 0
+        rp_t, ci_t = plan_ref.transpose_csr(rp, ci)
+        check_wsb(plan, rp_t, ci_t, True)
+    # undirected: one copy serves both directions
+    c3 = GI.make_config(3, scale=0.002)
+    plan = G.Plan(torch.from_numpy(c3["rowptr"]).cuda(), torch.from_numpy(c3["colidx"]).cuda(), transpose="undirected", wsb=True)
+    check_wsb(plan, c3["rowptr"], c3["colidx"], False)
+    check_wsb(plan, c3["rowptr"], c3["colidx"], True)
+    # multigraph: duplicates are counted, the bitmap holds each pair once
+    rng = np.random.default_rng(3)
+    dst, src = rng.integers(0, 200, 3000), rng.integers(0, 200, 3000)
+    rp_m, ci_m = GI.csr_from_pairs(200, dst, src, self_loops=False, dedupe=False)
+    plan = G.Plan(torch.from_numpy(rp_m).cuda(), torch.from_numpy(ci_m).cuda(), transpose=False, wsb=True)
+    ref = check_wsb(plan, rp_m, ci_m, False)
+    assert ref["n_dup"] > 0
+    # a graph without edges
+    plan = G.Plan(torch.zeros(41, dtype=torch.int32, device="cuda"), torch.zeros(0, dtype=torch.int32, device="cuda"),
+                  transpose=False, wsb=True)
+    assert plan.wsb_info()["n_tcb"] == 0 and not plan.export(B.GNN_PLAN_WSB_ROW_OFFSET).any()
+
+
 @pytest.mark.parametrize("heads", [1, 8])
 def test_block_tensor_core_forward(heads):
     """Row a12: the tcgen05/TMEM block-sparse forward (+ CSR remainder merge) against the oracle, on the locally
