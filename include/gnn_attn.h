@@ -218,6 +218,29 @@ gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* plan, const int32_t* rowptr
                                    gnn_dtype_t dtype, void* out, float* lse, gnn_stream_t stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Graph Transformer attention on the general WSB block-sparse layout, forward and backward on the
+ * tensor cores (tcgen05 / TMEM).  Same functions as gnn_gt_attn_fwd / _bwd up to rounding (the softmax weights P and
+ * the score gradients dS are rounded to bf16 before their second products).  A CTA owns 128 rows = 8 row windows and
+ * walks the windows' TCB pairs: S = Q K_blk^T, bitmap mask, online softmax, acc += P V_blk (forward);
+ * P = exp(S - L), dV = P^T dO, dP = dO V^T, dS = P o (dP - Delta), dQ = dS K, dK = dS^T Q (backward) - with the
+ * source-side gradients computed over the WSB layout of the TRANSPOSED graph, so that no atomics are needed (the
+ * paper accumulates dK / dV with atomicAdd; on an undirected graph both layouts are the same arrays).
+ * The plan must have been built with GNN_BLOCKS_WSB (and build_transpose for the backward) from a CSR WITHOUT duplicate
+ * entries (a bitmap stores each (dst, src) pair once: GNN_EUNSUPPORTED otherwise).  bf16 features, head_dim 64 or 128
+ * (GNN_EUNSUPPORTED otherwise); feature / gradient pointers 32-byte aligned; no workspace; asynchronous on `stream`.
+ *   forward : q, k, v [n,H,d] bf16 in; out [n,H,d] bf16, lse [n,H] fp32 out.
+ *   backward: q, k, v, dout in; out = the forward output O (bf16, in: its row dot <O_i, dO_i> centres the bf16-staged
+ *             products; Delta itself is accumulated in fp32 and the result does not depend on O's rounding); lse in;
+ *             delta [n,H] fp32 OUT; dq, dk, dv [n,H,d] fp32 out.                                                  */
+gnn_status_t gnn_gt_attn_fwd_wsb(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                 const void* q, const void* k, const void* v, int32_t heads, int32_t head_dim,
+                                 gnn_dtype_t dtype, void* out, float* lse, gnn_stream_t stream);
+gnn_status_t gnn_gt_attn_bwd_wsb(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                 const void* q, const void* k, const void* v, const void* out, const float* lse,
+                                 const void* dout, int32_t heads, int32_t head_dim, gnn_dtype_t dtype, float* delta,
+                                 float* dq, float* dk, float* dv, gnn_stream_t stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Degree-aware min / max neighbourhood aggregation with argmin (PAPER.md:124-151 section 3.1, :452-474 App. D.1):
  *   out[i,c] = min (mode GNN_AGG_MIN) or max (GNN_AGG_MAX) over the stored in-neighbours j of i of x[j,c]
  *   arg[i,c] = the source j that attains it; ties go to the smaller j (the paper's packed (value, index)

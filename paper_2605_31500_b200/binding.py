@@ -25,7 +25,7 @@ GNN_BLOCKS_NONE, GNN_BLOCKS_DIAG, GNN_BLOCKS_WSB = 0, 1, 2
 EXPORTED_SYMBOLS = [
     "gnn_csr_validate", "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
     "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
-    "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_seg_minmax_fwd", "gnn_seg_minmax_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
+    "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_gt_attn_fwd_wsb", "gnn_gt_attn_bwd_wsb", "gnn_seg_minmax_fwd", "gnn_seg_minmax_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
     "gnn_profile_collect", "gnn_pdl_enable", "gnn_probe_gather",
 ]
 
@@ -71,6 +71,9 @@ def lib() -> C.CDLL:
         L.gnn_seg_minmax_fwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _i32, C.c_int, _i32, _vp, _vp, _vp, _sz, _vp]
         L.gnn_seg_minmax_bwd.argtypes = [_i32, _vp, _vp, _i32, C.c_int, _vp, _vp]
         L.gnn_gt_attn_fwd_block.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _vp, _vp, _vp]
+        L.gnn_gt_attn_fwd_wsb.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _vp, _vp, _vp]
+        L.gnn_gt_attn_bwd_wsb.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, C.c_int,
+                                          _vp, _vp, _vp, _vp, _vp]
         L.gnn_last_error.restype = C.c_char_p
         L.gnn_version.restype = C.c_char_p
         L.gnn_launch_count.restype = _i64
@@ -263,6 +266,19 @@ def gnn_gt_attn_fwd_block(plan: Plan, q, k, v, out, lse, stream=None):
     n, H, d = q.shape
     _check(lib().gnn_gt_attn_fwd_block(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v), H, d,
                                        _dtype_code(q), _ptr(out), _ptr(lse), _stream(stream)))
+
+
+def gnn_gt_attn_fwd_wsb(plan: Plan, q, k, v, out, lse, stream=None):
+    n, H, d = q.shape
+    _check(lib().gnn_gt_attn_fwd_wsb(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v), H, d,
+                                     _dtype_code(q), _ptr(out), _ptr(lse), _stream(stream)))
+
+
+def gnn_gt_attn_bwd_wsb(plan: Plan, q, k, v, out, lse, dout, delta, dq, dk, dv, stream=None):
+    n, H, d = q.shape
+    _check(lib().gnn_gt_attn_bwd_wsb(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v),
+                                     _ptr(out), _ptr(lse), _ptr(dout), H, d, _dtype_code(q), _ptr(delta), _ptr(dq), _ptr(dk),
+                                     _ptr(dv), _stream(stream)))
 
 
 def gnn_gt_attn_bwd(plan: Plan, q, k, v, lse, dout, delta, dq, dk, dv, stream=None):

@@ -29,6 +29,7 @@
 
 #include "internal.h"
 #include "kernels.cuh"
+#include "tc_common.cuh"
 
 namespace gnn {
 namespace {
@@ -43,66 +44,7 @@ constexpr int kStages = GNN_BLOCK_STAGES;   // heads of Q/K/V in flight per CTA 
 constexpr int kTile = 128;  // destination rows per CTA = MMA M = TMEM lanes
 constexpr int kTS = 68;     // floats per row slot of the transpose buffer (64 + m, l, lx + pad): 272 B
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-// 64-bit shared-memory matrix descriptor, SWIZZLE_NONE, version 1 (sm_100)
-__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-    return (uint64_t)((saddr >> 4) & 0x3fff) | ((uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16) |
-           ((uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32) | (1ull << 46);
-}
-// same, SWIZZLE_128B (layout type 2 in bits 61-63): rows of 128 bytes, 8-row groups sbo_bytes apart
-__device__ __forceinline__ uint64_t make_desc_sw128(uint32_t saddr, uint32_t sbo_bytes) {
-    return (uint64_t)((saddr >> 4) & 0x3fff) | (1ull << 16) | ((uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32) | (1ull << 46) |
-           (2ull << 61);
-}
-// instruction descriptor: kind::f16, A = bf16 K-major, B = bf16 K-major or MN-major, D = fp32, M x N
-__host__ __device__ constexpr uint32_t make_idesc(int M, int N, bool b_mn_major) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(N >> 3) << 17) |
-           ((uint32_t)(M >> 4) << 24);
-}
-__device__ __forceinline__ void umma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
-    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n"
-                 " tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
-                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint64_t* bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                 ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile("{\n .reg .pred p;\n W_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-                 " @p bra D_%=;\n bra W_%=;\n D_%=:\n}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-// TMA: one 2-D box of the tensor map at element coordinates (c0, c1) into shared memory, completing on `bar`
-__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
-    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                 ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
-    uint32_t r[32];
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-                 "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
-                 "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
-                   "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
-                   "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-                 : "r"(taddr) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
-}
-
-// byte offset of element (r, k) in the canonical no-swizzle K-major layout (core matrix = 8 rows x 16 bytes)
-__device__ __forceinline__ uint32_t canon(int r, int k, int sbo) {
-    return (uint32_t)((r & 7) * 16 + (r >> 3) * sbo + (k & 7) * 2 + (k >> 3) * 128);
-}
+using namespace tc;
 
 template <int D>
 __global__ void __launch_bounds__(kTile, kStages == 1 ? GNN_BLOCK_MINB : 2)
@@ -379,34 +321,6 @@ gt_fwd_block_kernel(const __grid_constant__ CUtensorMap tmq, const __grid_consta
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" ::"r"(tmem) : "memory");
 }
 
-// cuTensorMapEncodeTiled through the runtime's driver entry point lookup (the library does not link libcuda)
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-EncodeTiledFn encode_tiled_fn() {
-    static EncodeTiledFn fn = [] {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
-            qres != cudaDriverEntryPointSuccess)
-            p = nullptr;
-        return reinterpret_cast<EncodeTiledFn>(p);
-    }();
-    return fn;
-}
-// [n, H*D] bf16 row-major tensor, boxes of kTile rows x D channels (one head slice), 128-byte swizzle, zero fill
-bool encode_head_tile_map(CUtensorMap* m, const void* base, int n, int H, int D) {
-    EncodeTiledFn fn = encode_tiled_fn();
-    if (!fn) return false;
-    const cuuint64_t gdim[2] = {(cuuint64_t)H * D, (cuuint64_t)n};
-    const cuuint64_t gstride[1] = {(cuuint64_t)H * D * 2};
-    const cuuint32_t box[2] = {(cuuint32_t)D, (cuuint32_t)kTile};
-    const cuuint32_t estr[2] = {1, 1};
-    return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstride, box, estr,
-              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
 }  // namespace
 }  // namespace gnn
 
@@ -432,8 +346,8 @@ extern "C" gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* P, const int32_t
     }
     constexpr int D = 64;
     CUtensorMap tmq, tmk, tmv;
-    if (!encode_head_tile_map(&tmq, q, n, heads, D) || !encode_head_tile_map(&tmk, k, n, heads, D) ||
-        !encode_head_tile_map(&tmv, v, n, heads, D)) {
+    if (!tc::encode_row_tile_map(&tmq, q, n, heads * D, D, kTile) || !tc::encode_row_tile_map(&tmk, k, n, heads * D, D, kTile) ||
+        !tc::encode_row_tile_map(&tmv, v, n, heads * D, D, kTile)) {
         set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who);
         return GNN_ECUDA;
     }

@@ -447,6 +447,59 @@ def test_wsb_layout_bit_exact():
     assert plan.wsb_info()["n_tcb"] == 0 and not plan.export(B.GNN_PLAN_WSB_ROW_OFFSET).any()
 
 
+@pytest.mark.parametrize("heads,d", [(1, 64), (8, 64), (3, 128)])
+def test_wsb_tensor_core_forward_backward(heads, d):
+    """Row f2: GT attention on the general WSB layout, forward and tensor-core backward, against the
+    fp64 oracle (the same functions as the CSR entry points): the locally dense config scaled (ragged last tile), a graph
+    whose windows share columns / have many TCBs / have none, and a directed power-law graph (hub windows with hundreds
+    of TCBs; the src side runs on the WSB of CSR^T).  Outputs are NaN-prefilled; the run is repeated to show it is
+    bit-reproducible (no atomics); an undirected graph uses one layout for both sides; a multigraph is refused."""
+    import paper_2605_31500_b200 as G
+    torch = _torch()
+
+    def run(c, transpose=True):
+        nn, H, dd = c["n"], c["heads"], c["head_dim"]
+        plan = G.Plan(torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda(), transpose=transpose, wsb=True)
+        q, k, v, do = (_dev(c[x + "_st"], "bf16") for x in ("q", "k", "v", "do"))
+        out = torch.full_like(q, float("nan"))
+        lse = torch.full((nn, H), float("nan"), dtype=torch.float32, device="cuda")
+        G.gnn_gt_attn_fwd_wsb(plan, q, k, v, out, lse)
+        delta = torch.full_like(lse, float("nan"))
+        dq, dk, dv = (torch.full((nn, H, dd), float("nan"), dtype=torch.float32, device="cuda") for _ in range(3))
+        G.gnn_gt_attn_bwd_wsb(plan, q, k, v, out, lse, do, delta, dq, dk, dv)
+        torch.cuda.synchronize()
+        return dict(O=_host(out), L=_host(lse), Delta=_host(delta), dQ=_host(dq), dK=_host(dk), dV=_host(dv), plan=plan)
+
+    for name, n, rp, ci in _wsb_test_graphs():
+        c = _custom("gt", n, rp, ci, heads, d, "bf16", seed=31)
+        c["name"] = f"wsb_{name}_H{heads}_d{d}"
+        got = run(c)
+        compare_all(c, got, oracle_gt(c))
+        again = run(c)
+        for key in ("O", "L", "Delta", "dQ", "dK", "dV"):
+            assert np.array_equal(got[key], again[key], equal_nan=True), key
+    # undirected graph: one WSB layout serves the dst and the src side (PAPER.md:343)
+    c3 = GI.make_config(3, scale=0.002)
+    c = _custom("gt", c3["n"], c3["rowptr"], c3["colidx"], heads, d, "bf16", seed=32)
+    und = run(c, transpose="undirected")
+    compare_all(c, und, oracle_gt(c))
+    assert und["plan"].plan_bytes < run(c)["plan"].plan_bytes
+    # refused: duplicates, unsupported shapes, a plan without the layout
+    rng = np.random.default_rng(3)
+    rp_m, ci_m = GI.csr_from_pairs(200, rng.integers(0, 200, 3000), rng.integers(0, 200, 3000), self_loops=False, dedupe=False)
+    cm = _custom("gt", 200, rp_m, ci_m, heads, d, "bf16")
+    with pytest.raises(G.GnnError, match="duplicate"):
+        run(cm)
+    plan = G.Plan(torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda(), transpose=True)
+    q = _dev(c["q_st"], "bf16")
+    with pytest.raises(G.GnnError, match="GNN_BLOCKS_WSB"):
+        G.gnn_gt_attn_fwd_wsb(plan, q, q, q, torch.empty_like(q), torch.empty((c["n"], heads), device="cuda"))
+    planw = und["plan"]
+    q3 = torch.zeros((c["n"], 2, 32), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(G.GnnError, match="unsupported shape"):
+        G.gnn_gt_attn_fwd_wsb(planw, q3, q3, q3, torch.empty_like(q3), torch.empty((c["n"], 2), device="cuda"))
+
+
 @pytest.mark.parametrize("heads", [1, 8])
 def test_block_tensor_core_forward(heads):
     """Row a12: the tcgen05/TMEM block-sparse forward (+ CSR remainder merge) against the oracle, on the locally
