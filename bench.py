@@ -321,7 +321,7 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         p = G.Plan(devt["rowptr"], devt["colidx"], warp_max_deg=args.warp_max_deg, cta_max_deg=args.cta_max_deg,
-                   split_chunk=args.split_chunk, transpose=mode, blocks=(args.cfg == 4))
+                   split_chunk=args.split_chunk, transpose=mode, blocks=(args.cfg == 4), wsb=(args.cfg == 4))
         torch.cuda.synchronize()
         return p, 1e3 * (time.perf_counter() - t0)
 
@@ -401,6 +401,26 @@ def run_ours(args, rank, world, local_rank):
     value = job_gedges(e, args.steps, world, total_ms)
 
     peak_mem = int(torch.cuda.max_memory_allocated(dev))   # the layer itself: inputs, outputs, plan, workspace (+ L2 flush buffer)
+
+    def fwd_wsb():     # cfg 4 only: general WSB layout, tcgen05 forward (row f2)
+        G.gnn_gt_attn_fwd_wsb(plan, devt["q"], devt["k"], devt["v"], out, lse)
+
+    def bwd_wsb():     # cfg 4 only: tensor-core backward on the WSB layouts of the CSR and of CSR^T (row f2)
+        G.gnn_gt_attn_bwd_wsb(plan, devt["q"], devt["k"], devt["v"], out, lse, devt["do"], stat, g1, g2, g3)
+
+    wsb = None
+    if args.cfg == 4:
+        for _ in range(3):
+            fwd_wsb()
+            bwd_wsb()
+        ms_wf, ms_wb = timed(fwd_wsb, args.steps), timed(bwd_wsb, args.steps)
+        G.gnn_profile_enable(True)
+        fwd_wsb()
+        bwd_wsb()
+        G.gnn_profile_enable(False)
+        wk = {nm: float(ms) for nm, ms in G.gnn_profile_collect(64)}
+        wsb = {"ms_fwd": float(np.mean(ms_wf)), "ms_bwd": float(np.mean(ms_wb)), "kernels_ms": wk, "info": plan.wsb_info()}
+        fwd()   # restore the CSR forward's out / lse for what follows
 
     block = None
     if args.cfg == 4:
@@ -633,7 +653,7 @@ def run_ours(args, rank, world, local_rank):
                 "gedges_fwd": e / (np.mean(ms_fwd) * 1e-3) * 1e-9, "gedges_bwd": e / (np.mean(ms_bwd) * 1e-3) * 1e-9,
                 "peak_device_bytes": peak_mem, "device_bytes_inputs": in_bytes, "device_bytes_outputs": out_bytes,
                 "plan_bytes": plan.plan_bytes, "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
-                "roofline": roof, "block_path": block, "cuda_graph": graph, "seg_minmax": minmax, "cpu_baseline": cpu}
+                "roofline": roof, "block_path": block, "wsb_path": wsb, "cuda_graph": graph, "seg_minmax": minmax, "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

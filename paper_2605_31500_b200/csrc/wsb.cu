@@ -41,6 +41,9 @@ namespace gnn {
 namespace {
 using namespace tc;
 
+#ifndef GNN_WSB_PF
+#define GNN_WSB_PF 1
+#endif
 constexpr int kTile = 128;      // rows per CTA = MMA M = TMEM lanes
 constexpr int kHT = 16384;      // bytes of a half tile: 128 rows x 64 channels bf16, 128-byte swizzled rows
 constexpr int kWBytes = 32768;  // bytes of the block-diagonal 128 x 128 bf16 weight tile (P / dS)
@@ -265,6 +268,22 @@ wsb_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUte
             if (ta + 1 < t1) bits |= (uint32_t)__ldg(p.bitmap + (size_t)(ta + 1) * 16 + rr) << 8;
             if (!rvalid) bits = 0;
             __syncthreads();
+            // ---- the row slices the NEXT step (or the next head's first step) will gather: into L2 now, so that its
+            // gathers do not pay the DRAM latency inside the serial phase chain (every gathered line is a DRAM miss:
+            // each (row, head) slice is one 128-byte line used by one window; GNN_WSB_PF=0 switches this off)
+            if (GNN_WSB_PF) {
+                const bool nh = s + 1 >= n_steps;               // wraps to the next head
+                const int sn = nh ? 0 : s + 1, hn = nh ? hoff + D : hoff;
+                const int tcb = t0 + 2 * sn + (rr >> 3);
+                if (tcb < t1 && (!nh || h + 1 < p.H)) {
+                    const size_t off = (size_t)__ldg(p.cols + (size_t)tcb * 8 + (rr & 7)) * rowe + hn;
+#pragma unroll
+                    for (int hf = 0; hf < NH; ++hf) {
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(p.gx + off + hf * 64));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(p.gy + off + hf * 64));
+                    }
+                }
+            }
             // ---- gathered tiles
             gather_tile<NH>(sGx, p.gx, s_col, rowe, hoff, tid);
             gather_tile<NH>(sGy, p.gy, s_col, rowe, hoff, tid);
