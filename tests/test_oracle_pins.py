@@ -651,3 +651,61 @@ def test_seg_minmax_backward_vs_autograd(mode):
     np.testing.assert_allclose(tx.grad.numpy(), dx, rtol=0, atol=1e-15)
     # gradient mass is conserved: every non-empty (i, c) sends its dout to exactly one source
     np.testing.assert_allclose(dx.sum(0), dout[nonempty.numpy()].sum(0), rtol=0, atol=1e-12)
+
+
+# --------------------------------------------------------------------------- row f4: LayerNorm + QKV projection, dot-aggr
+from oracle import block_ref  # noqa: E402
+
+
+def test_layer_norm_vs_library_and_closed_forms():
+    """block_ref.layer_norm against the library routine (torch.nn.functional.layer_norm, fp64) and closed forms: with
+    gamma = 1, beta = 0 every row has mean 0 and variance var / (var + eps); a constant row maps to beta; the result
+    is invariant to a per-row shift and (up to eps) to a per-row positive scale."""
+    rng = np.random.default_rng(5)
+    x = rng.standard_normal((37, 96)) * rng.uniform(0.1, 5.0, (37, 1)) + rng.standard_normal((37, 1))
+    g, b = rng.standard_normal(96), rng.standard_normal(96)
+    got = block_ref.layer_norm(x, g, b, 1e-5)
+    want = torch.nn.functional.layer_norm(torch.from_numpy(x), (96,), torch.from_numpy(g), torch.from_numpy(b), 1e-5).numpy()
+    np.testing.assert_allclose(got, want, rtol=1e-12, atol=1e-12)
+    y = block_ref.layer_norm(x, np.ones(96), np.zeros(96), 1e-5)
+    var = x.var(axis=1)
+    np.testing.assert_allclose(y.mean(axis=1), 0.0, atol=1e-12)
+    np.testing.assert_allclose(y.var(axis=1), var / (var + 1e-5), rtol=1e-10)
+    np.testing.assert_allclose(block_ref.layer_norm(np.full((3, 96), 7.25), g, b), np.tile(b, (3, 1)), atol=1e-12)
+    np.testing.assert_allclose(block_ref.layer_norm(x + 3.0, g, b), got, atol=1e-10)
+    np.testing.assert_allclose(block_ref.layer_norm(x * 1e3, g, b, 0.0), block_ref.layer_norm(x, g, b, 0.0), atol=1e-9)
+
+
+def test_ln_qkv_vs_loops_and_library():
+    """block_ref.ln_qkv: the projection against explicit loops on a tiny case (which row block of W feeds Q, K, V; the
+    head / channel order of the outputs) and against torch layer_norm + linear in fp64."""
+    rng = np.random.default_rng(6)
+    n, C, H, d = 5, 16, 2, 4
+    x, g, b = rng.standard_normal((n, C)), rng.standard_normal(C), rng.standard_normal(C)
+    w, bias = rng.standard_normal((3 * H * d, C)), rng.standard_normal(3 * H * d)
+    q, k, v = block_ref.ln_qkv(x, g, b, w, bias, H, d)
+    y = torch.nn.functional.layer_norm(torch.from_numpy(x), (C,), torch.from_numpy(g), torch.from_numpy(b), 1e-5).numpy()
+    for t, out in enumerate((q, k, v)):
+        for i in range(n):
+            for h in range(H):
+                for c in range(d):
+                    row = t * H * d + h * d + c
+                    want = sum(y[i, m] * w[row, m] for m in range(C)) + bias[row]
+                    assert abs(out[i, h, c] - want) < 1e-12
+    lin = torch.nn.functional.linear(torch.from_numpy(y), torch.from_numpy(w), torch.from_numpy(bias)).numpy()
+    np.testing.assert_allclose(np.concatenate([q.reshape(n, -1), k.reshape(n, -1), v.reshape(n, -1)], axis=1), lin, atol=1e-12)
+    q0, _, _ = block_ref.ln_qkv(x, g, b, w, None, H, d)
+    np.testing.assert_allclose(q0, q - bias[:H * d].reshape(1, H, d), atol=1e-12)
+
+
+def test_dot_aggr_vs_dense():
+    """block_ref.dot_aggr against the dense form diag(C X X^T) with C the edge-count matrix (multigraph), and the
+    closed form on a graph of self-loops only (out[i] = |x_i|^2)."""
+    rng = np.random.default_rng(7)
+    n = 23
+    rp, ci = _rand_graph(rng, n, 3.0, multigraph=True, empty_rows=True)
+    x = rng.standard_normal((n, 12))
+    C = _count_matrix(rp, ci)
+    np.testing.assert_allclose(block_ref.dot_aggr(rp, ci, x), np.einsum("ij,ij->i", C, x @ x.T), atol=1e-12)
+    rp1, ci1 = np.arange(n + 1), np.arange(n)
+    np.testing.assert_allclose(block_ref.dot_aggr(rp1, ci1, x), (x * x).sum(axis=1), atol=1e-12)
