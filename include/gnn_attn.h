@@ -281,6 +281,18 @@ void gnn_pdl_enable(int on);
 void gnn_profile_enable(int on);
 int32_t gnn_profile_collect(char* names, float* ms, int32_t max_records);
 
+/* ---------------------------------------------------------------------------------------------
+ * The rest of the Graph Transformer block the paper timed: LayerNorm fused into the QKV projection.
+ *   y[i,:] = (x[i,:] - mean_i) / sqrt(var_i + eps) * gamma + beta    (over the c_in features, biased variance)
+ *   q | k | v [i,:] = y[i,:] W^T + bias,  W = [W_Q; W_K; W_V]: [3*heads*head_dim, c_in] row-major
+ * One tcgen05 GEMM whose A operand is normalised on the way into shared memory: y never exists in HBM.
+ * x: [n, c_in] bf16; gamma, beta: [c_in] fp32; w: bf16; bias: [3*heads*head_dim] fp32 or NULL; q, k, v: [n,H,d] bf16 out
+ * (fp32 accumulation, one bf16 rounding of y and one of the outputs).  c_in a multiple of 64 in [64, 512],
+ * heads*head_dim a multiple of 128 (GNN_EUNSUPPORTED otherwise); x, w, q, k, v 32-byte aligned; no workspace; async. */
+gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, int32_t head_dim, const void* x, const float* gamma,
+                            const float* beta, float eps, const void* w, const float* bias, void* q, void* k, void* v,
+                            gnn_stream_t stream);
+
 /* Measurement aid (bench.py): ONE launch that gathers n_idx rows of row_bytes (256 | 512 | 1024) bytes at the row
  * indices idx[0..n_idx) (each in [0, table_rows)) from `table` and discards them - the achievable gather-ingest rate
  * ("ceiling 2" of DESIGN.md section 6: HBM-resident when the table is far larger than L2, L2-resident when it fits),

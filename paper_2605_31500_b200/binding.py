@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = [
     "gnn_csr_validate", "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
     "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
     "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_gt_attn_fwd_wsb", "gnn_gt_attn_bwd_wsb", "gnn_seg_minmax_fwd", "gnn_seg_minmax_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
-    "gnn_profile_collect", "gnn_pdl_enable", "gnn_probe_gather",
+    "gnn_profile_collect", "gnn_pdl_enable", "gnn_probe_gather", "gnn_ln_qkv_fwd",
 ]
 
 
@@ -80,6 +80,7 @@ def lib() -> C.CDLL:
         L.gnn_profile_enable.argtypes = [C.c_int]
         L.gnn_profile_enable.restype = None
         L.gnn_probe_gather.argtypes = [_vp, _i64, _i32, _vp, _i64, _i32, _i32, _i32, _vp, _vp]
+        L.gnn_ln_qkv_fwd.argtypes = [_i32, _i32, _i32, _i32, _vp, _vp, _vp, _f, _vp, _vp, _vp, _vp, _vp, _vp]
         L.gnn_pdl_enable.argtypes = [C.c_int]
         L.gnn_pdl_enable.restype = None
         L.gnn_profile_collect.argtypes = [_vp, _vp, _i32]
@@ -302,6 +303,14 @@ def gnn_gatv2_bwd(plan: Plan, xl, xr, a, lse, dout, slope, g, dxl, dxr, da, stre
     _check(lib().gnn_gatv2_bwd(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(xl), _ptr(xr), _ptr(a),
                                _ptr(lse), _ptr(dout), H, d, _dtype_code(xl), float(slope), _ptr(g), _ptr(dxl), _ptr(dxr),
                                _ptr(da), _ptr(ws), ws.numel(), _stream(stream)))
+
+
+def gnn_ln_qkv_fwd(x, gamma, beta, eps, w, bias, q, k, v, stream=None):
+    """x [n, C] bf16; gamma, beta [C] fp32; w [3*H*d, C] bf16; bias [3*H*d] fp32 or None; q, k, v [n, H, d] bf16 out."""
+    n, c_in = x.shape
+    _, H, d = q.shape
+    _check(lib().gnn_ln_qkv_fwd(n, c_in, H, d, _ptr(x), _ptr(gamma), _ptr(beta), float(eps), _ptr(w), _ptr(bias), _ptr(q),
+                                _ptr(k), _ptr(v), _stream(stream)))
 
 
 def gnn_probe_gather(table, row_bytes: int, idx, mode: int, depth: int, ctas_per_sm: int, sink, stream=None):

@@ -1,0 +1,292 @@
+// ln_qkv.cu - row f4: the rest of the block the paper timed in front of the Graph Transformer attention
+// ("layer normalization, QKV projection, and the attention mechanism itself"): LayerNorm fused into the
+// A-operand staging of a tcgen05 GEMM that writes Q, K, V.
+//
+//   y[i, :] = (x[i, :] - mean_i) / sqrt(var_i + eps) * gamma + beta        (biased variance over the C features)
+//   [Q | K | V][i, :] = y[i, :] W^T + bias,   W = [W_Q; W_K; W_V] of shape [3*H*d, C]
+//
+// The paper runs these as stock PyTorch ops (LayerNorm kernel, cuBLAS GEMM: one write and one read of the normalised
+// activations in HBM).  Here one CTA owns 128 rows: warps 0-3 normalise their rows in registers (a warp per row,
+// 16-byte loads, shuffle reductions) and write them as bf16 straight into the 128-byte-swizzled K-major shared-memory
+// tile the tensor core reads - the normalised activations never touch HBM.  Then, warp-specialised: warp 4 streams the
+// weight tiles (128 outputs x 64 channels, 16 KB) through a TMA ring, warp 5 issues tcgen05.mma (128 x 128 x 16) into
+// one of two 128-column TMEM accumulators, and warps 0-3 drain the other one (tcgen05.ld, + bias, bf16, per-warp
+// transpose, coalesced stores) - full / empty mbarriers between the three roles, so the epilogue of output chunk c
+// overlaps the products of chunk c + 1.
+#include <cuda.h>
+#include <cuda_bf16.h>
+
+#include "internal.h"
+#include "kernels.cuh"
+#include "tc_common.cuh"
+
+namespace gnn {
+namespace {
+using namespace tc;
+
+constexpr int kRows = 128;          // rows per CTA = MMA M
+constexpr int kNC = 128;            // output columns per chunk = MMA N
+constexpr int kStage = 16384;       // bytes of a weight stage / of a 64-channel half tile of A
+constexpr int kThreads = 192;       // warps 0-3: LayerNorm + epilogue, warp 4: TMA, warp 5: MMA
+constexpr int kSlot = 272;          // bytes of a transpose slot: 128 bf16 + 16 (conflict-free 16-byte accesses)
+
+struct LnQkvParams {
+    const __nv_bfloat16* x;
+    const float *gamma, *beta, *bias;
+    __nv_bfloat16 *q, *k, *v;
+    int n, C, R;                    // rows, input features, H * d
+    float eps;
+    int n_stages;
+};
+
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    const int KC = p.C / 64, NS = p.n_stages;
+    uint8_t* sA = smem;                                   // [KC] half tiles, 128 rows x 128 bytes, SWIZZLE_128B
+    uint8_t* sB = sA + KC * kStage;                       // [NS] weight stages
+    uint8_t* sT = sB + NS * kStage;                       // [128] transpose slots
+    uint64_t* full = reinterpret_cast<uint64_t*>(sT + kRows * kSlot);   // [NS] TMA landed
+    uint64_t* empty = full + 8;                           // [NS] stage consumed (tcgen05.commit)
+    uint64_t* tfull = empty + 8;                          // [2] accumulator complete
+    uint64_t* tempty = tfull + 2;                         // [2] accumulator drained
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int row0 = blockIdx.x * kRows;
+    const int n_chunks = 3 * p.R / kNC;
+
+    if (tid == 0) {
+        for (int s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(tfull + b, 1); mbar_init(tempty + b, 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 5) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp == 4) {
+        // ===== TMA producer: weight stage i = (chunk c, channel block kk) -> ring slot i % NS
+        // (the first NS stages go out now and overlap the LayerNorm; the rest after the A tile barrier below, because
+        // their slots are only released by the MMA warp, which starts behind that barrier)
+        if (lane == 0) {
+            const int items = n_chunks * KC;
+            for (int i = 0; i < items && i < NS; ++i) {
+                mbar_expect_tx(full + i, kStage);
+                tma_load_2d(sB + i * kStage, &tmw, (i % KC) * 64, (i / KC) * kNC, full + i);
+            }
+        }
+    } else if (warp < 4) {
+        // ===== LayerNorm of this warp's 32 rows into the A tile (lane <-> 16-byte chunks lane, lane + 32)
+        const int nchunk = p.C / 8;
+        float g[2][8], b[2][8];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int cc = lane + 32 * j;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                g[j][i] = cc < nchunk ? __ldg(p.gamma + cc * 8 + i) : 0.f;
+                b[j][i] = cc < nchunk ? __ldg(p.beta + cc * 8 + i) : 0.f;
+            }
+        }
+        const float inv_c = 1.f / (float)p.C;
+        for (int rl = 0; rl < 32; rl += 2) {
+            uint4 raw[2][2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const int row = row0 + warp * 32 + rl + u, cc = lane + 32 * j;
+                    raw[u][j] = make_uint4(0, 0, 0, 0);
+                    if (row < p.n && cc < nchunk) raw[u][j] = __ldg(reinterpret_cast<const uint4*>(p.x + (size_t)row * p.C) + cc);
+                }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int r = warp * 32 + rl + u;
+                float v[2][8];
+                float s = 0.f;
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const uint32_t w[4] = {raw[u][j].x, raw[u][j].y, raw[u][j].z, raw[u][j].w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        v[j][2 * i] = __uint_as_float(w[i] << 16);
+                        v[j][2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+                        s += v[j][2 * i] + v[j][2 * i + 1];
+                    }
+                }
+                const float mean = warp_sum(s) * inv_c;
+                float ss = 0.f;
+#pragma unroll
+                for (int j = 0; j < 2; ++j)
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const bool on = lane + 32 * j < nchunk;
+                        v[j][i] = on ? v[j][i] - mean : 0.f;
+                        ss = fmaf(v[j][i], v[j][i], ss);
+                    }
+                const float rstd = 1.f / sqrtf(warp_sum(ss) * inv_c + p.eps);
+                const bool rv = row0 + r < p.n;
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const int cc = lane + 32 * j;
+                    if (cc < nchunk) {
+                        uint32_t o[4];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const float y0 = rv ? fmaf(v[j][2 * i] * rstd, g[j][2 * i], b[j][2 * i]) : 0.f;
+                            const float y1 = rv ? fmaf(v[j][2 * i + 1] * rstd, g[j][2 * i + 1], b[j][2 * i + 1]) : 0.f;
+                            const __nv_bfloat162 yb = __floats2bfloat162_rn(y0, y1);
+                            o[i] = *reinterpret_cast<const uint32_t*>(&yb);
+                        }
+                        const int hf = cc >> 3, c8 = cc & 7;
+                        *reinterpret_cast<uint4*>(sA + hf * kStage + (r >> 3) * 1024 + (r & 7) * 128 + ((c8 ^ (r & 7)) << 4)) =
+                            make_uint4(o[0], o[1], o[2], o[3]);
+                    }
+                }
+            }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();   // the A tile is complete and visible to the tensor core
+
+    if (warp == 4) {
+        if (lane == 0) {
+            const int items = n_chunks * KC;
+            for (int i = NS; i < items; ++i) {
+                const int s = i % NS, c = i / KC, kk = i % KC;
+                mbar_wait(empty + s, (uint32_t)((i / NS) & 1) ^ 1u);
+                mbar_expect_tx(full + s, kStage);
+                tma_load_2d(sB + s * kStage, &tmw, kk * 64, c * kNC, full + s);
+            }
+        }
+    } else if (warp == 5) {
+        // ===== MMA issuer
+        if (lane == 0) {
+            constexpr uint32_t kIdesc = make_idesc(kRows, kNC, false);
+            int i = 0;
+            for (int c = 0; c < n_chunks; ++c) {
+                const int bsel = c & 1;
+                mbar_wait(tempty + bsel, (uint32_t)((c >> 1) & 1) ^ 1u);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                for (int kk = 0; kk < KC; ++kk, ++i) {
+                    const int s = i % NS;
+                    mbar_wait(full + s, (uint32_t)((i / NS) & 1));
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+                    for (int ks = 0; ks < 4; ++ks)
+                        umma(tmem + bsel * kNC, make_desc_sw128(smem_u32(sA + kk * kStage) + ks * 32, 1024),
+                             make_desc_sw128(smem_u32(sB + s * kStage) + ks * 32, 1024), kIdesc, (kk | ks) > 0);
+                    umma_commit(empty + s);
+                }
+                umma_commit(tfull + bsel);
+            }
+        }
+    } else if (warp < 4) {
+        // ===== epilogue: accumulator -> + bias -> bf16 -> transpose slot -> coalesced 16-byte stores
+        const uint32_t t_lane = tmem + ((uint32_t)(warp * 32) << 16);
+        uint8_t* slot = sT + tid * kSlot;
+        for (int c = 0; c < n_chunks; ++c) {
+            const int bsel = c & 1;
+            mbar_wait(tfull + bsel, (uint32_t)((c >> 1) & 1));
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const int col0 = c * kNC;
+#pragma unroll
+            for (int c0 = 0; c0 < kNC; c0 += 32) {
+                float t32[32];
+                tmem_ld32(t_lane + bsel * kNC + c0, t32);
+                uint32_t o[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    const float b0 = p.bias ? __ldg(p.bias + col0 + c0 + 2 * i) : 0.f;
+                    const float b1 = p.bias ? __ldg(p.bias + col0 + c0 + 2 * i + 1) : 0.f;
+                    const __nv_bfloat162 yb = __floats2bfloat162_rn(t32[2 * i] + b0, t32[2 * i + 1] + b1);
+                    o[i] = *reinterpret_cast<const uint32_t*>(&yb);
+                }
+#pragma unroll
+                for (int i = 0; i < 16; i += 4)
+                    *reinterpret_cast<uint4*>(slot + c0 * 2 + i * 4) = make_uint4(o[i], o[i + 1], o[i + 2], o[i + 3]);
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty + bsel);          // this warp's 32 lanes of the accumulator are drained
+            // rows of this warp, 16 lanes per 256-byte row piece
+            const int t = col0 / p.R, off = col0 - t * p.R;
+            __nv_bfloat16* dst = (t == 0 ? p.q : (t == 1 ? p.k : p.v)) + off;
+            const int ch = lane & 15, rsub = lane >> 4;
+#pragma unroll 4
+            for (int it = 0; it < 16; ++it) {
+                const int rl = it * 2 + rsub;
+                const int row = row0 + warp * 32 + rl;
+                if (row < p.n) {
+                    const uint4 w = *reinterpret_cast<const uint4*>(sT + (warp * 32 + rl) * kSlot + ch * 16);
+                    *reinterpret_cast<uint4*>(dst + (size_t)row * p.R + ch * 8) = w;
+                }
+            }
+            __syncwarp();
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 5) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(tmem) : "memory");
+}
+
+}  // namespace
+}  // namespace gnn
+
+using namespace gnn;
+
+extern "C" gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, int32_t head_dim, const void* x,
+                                       const float* gamma, const float* beta, float eps, const void* w, const float* bias,
+                                       void* q, void* k, void* v, gnn_stream_t stream) {
+    const char* who = "gnn_ln_qkv_fwd";
+    if (n < 1 || !x || !gamma || !beta || !w || !q || !k || !v) { set_error("%s: n < 1 or NULL pointer argument", who); return GNN_EINVAL; }
+    if ((((uintptr_t)x | (uintptr_t)w | (uintptr_t)q | (uintptr_t)k | (uintptr_t)v) & 31) != 0) {
+        set_error("%s: x, w, q, k, v must be 32-byte aligned", who);
+        return GNN_EINVAL;
+    }
+    if (!(eps >= 0.f)) { set_error("%s: eps must be >= 0", who); return GNN_EINVAL; }
+    const long long R = (long long)heads * head_dim;
+    if (heads < 1 || head_dim < 1 || c_in < 64 || c_in > 512 || c_in % 64 != 0 || R % kNC != 0 || R > 8192) {
+        set_error("%s: unsupported shape c_in=%d heads=%d head_dim=%d (c_in a multiple of 64 in [64, 512], heads*head_dim a multiple of 128)",
+                  who, c_in, heads, head_dim);
+        return GNN_EUNSUPPORTED;
+    }
+    CUtensorMap tmw;
+    if (!tc::encode_row_tile_map(&tmw, w, (int)(3 * R), c_in, 64, kNC)) {
+        set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who);
+        return GNN_ECUDA;
+    }
+    LnQkvParams p = {};
+    p.x = (const __nv_bfloat16*)x; p.gamma = gamma; p.beta = beta; p.bias = bias;
+    p.q = (__nv_bfloat16*)q; p.k = (__nv_bfloat16*)k; p.v = (__nv_bfloat16*)v;
+    p.n = n; p.C = c_in; p.R = (int)R; p.eps = eps;
+    p.n_stages = c_in <= 256 ? 6 : 3;
+    const size_t smem = (size_t)(c_in / 64) * kStage + (size_t)p.n_stages * kStage + (size_t)kRows * kSlot + 256 + 1024;
+    cudaError_t e = cudaFuncSetAttribute(ln_qkv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) {
+        cudaStream_t st = (cudaStream_t)stream;
+        prof_begin("ln_qkv", "gemm", st);
+        ln_qkv_kernel<<<(n + kRows - 1) / kRows, kThreads, smem, st>>>(tmw, p);
+        prof_end(st);
+        count_launch();
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) { set_error("%s: CUDA error: %s", who, cudaGetErrorString(e)); return GNN_ECUDA; }
+    return GNN_OK;
+}
