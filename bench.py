@@ -50,6 +50,9 @@ def parse():
     ap.add_argument("--directed-plan", action="store_true",
                     help="cfg 3: build CSR^T instead of reusing the forward CSR in the backward (row f1)")
     ap.add_argument("--no-minmax", action="store_true", help="skip the extra row-f3 (min aggregation) measurement of cfg 3 / 5")
+    ap.add_argument("--no-all-configs", action="store_true",
+                    help="default run (cfg 3) only: skip the compact measurements of cfg 1, 2, 4, 5 (`all_configs`)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the gather-ceiling probe and the row-f4 measurements")
     ap.add_argument("--warp-max-deg", type=int, default=0)
     ap.add_argument("--cta-max-deg", type=int, default=0)
     ap.add_argument("--split-chunk", type=int, default=0)
@@ -93,6 +96,199 @@ def byte_model(c, plan_counts, deg_in, deg_out, perm, perm_t):
         alg[ps + "/segment"] = e_heavy * pe + (nc + nch) * pn
         alg[ps + "/group"] = e_group * pe + ng * pn
     return alg, comp
+
+
+def compulsory_bytes(c):
+    """Compulsory bytes per pass: rowptr + colidx (+ CSR^T for the backward) + every tensor once + outputs
+    (O in the feature dtype, gradients fp32, L / Delta / G fp32)."""
+    n, e, H, d = c["n"], c["e"], c["heads"], c["head_dim"]
+    b = 4 if c["dtype"] == "f32" else 2
+    R = H * d
+    csr = 4 * (n + 1) + 4 * e
+    if c["layer"] == "gt":
+        return {"fwd": csr + 4 * n * R * b + 4 * n * H, "bwd": 2 * csr + 4 * n * R * b + 4 * n * H + 12 * n * R + 8 * n * H}
+    return {"fwd": csr + 3 * n * R * b + 4 * n * H + 4 * R, "bwd": 2 * csr + 3 * n * R * b + 4 * n * H + 8 * n * R + 8 * n * H + 8 * R}
+
+
+def quick_config(cfg, args, dev, peak):
+    """Compact measurement of one more BASELINE.json config in the same run (`all_configs`): the same calls, the same
+    timing rules (>= 3 warm-up steps, CUDA events on the launch stream, L2 flushed between steps when the inputs do not
+    exceed it), forward / backward / step times, GEdges/s and the compulsory-byte fractions.  cfg 4 also times the
+    tcgen05 paths (diagonal block forward, WSB forward + backward)."""
+    import torch
+    import paper_2605_31500_b200 as G
+    c = GI.make_config(cfg, keep_f32=False)
+    n, e, H, d, dt = c["n"], c["e"], c["heads"], c["head_dim"], c["dtype"]
+    gt = c["layer"] == "gt"
+    names = ("q", "k", "v", "do") if gt else ("xl", "xr", "do")
+
+    def to_dev(a):
+        t = torch.from_numpy(np.ascontiguousarray(a))
+        return (t.view(torch.bfloat16) if (dt == "bf16" and a.dtype == np.uint16) else t).to(dev)
+
+    T = {nm: to_dev(c[nm + "_st"]) for nm in names}
+    rp, ci = torch.from_numpy(c["rowptr"]).to(dev), torch.from_numpy(c["colidx"]).to(dev)
+    if not gt:
+        T["a"] = torch.from_numpy(c["a_f32"]).to(dev)
+    plan = G.Plan(rp, ci, transpose=True, blocks=(cfg == 4), wsb=(cfg == 4))
+    f32 = dict(dtype=torch.float32, device=dev)
+    out = torch.empty((n, H, d), dtype=T[names[0]].dtype, device=dev)
+    lse, stat = torch.empty((n, H), **f32), torch.empty((n, H), **f32)
+    g1, g2 = torch.empty((n, H, d), **f32), torch.empty((n, H, d), **f32)
+    g3 = torch.empty((n, H, d), **f32) if gt else torch.empty((H, d), **f32)
+    if gt:
+        fwd = lambda: G.gnn_gt_attn_fwd(plan, T["q"], T["k"], T["v"], out, lse)
+        bwd = lambda: G.gnn_gt_attn_bwd(plan, T["q"], T["k"], T["v"], lse, T["do"], stat, g1, g2, g3)
+    else:
+        fwd = lambda: G.gnn_gatv2_fwd(plan, T["xl"], T["xr"], T["a"], c["slope"], out, lse)
+        bwd = lambda: G.gnn_gatv2_bwd(plan, T["xl"], T["xr"], T["a"], lse, T["do"], c["slope"], stat, g1, g2, g3)
+    in_bytes = sum(int(v.numel()) * v.element_size() for v in list(T.values()) + [rp, ci])
+    l2 = torch.cuda.get_device_properties(dev).L2_cache_size
+    flush = torch.empty(max(2 * l2, 1 << 28), dtype=torch.uint8, device=dev) if in_bytes < 4 * l2 else None
+
+    def timed(fn, k):
+        evs = []
+        for _ in range(k):
+            if flush is not None:
+                flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record()
+            evs.append((a, b))
+        torch.cuda.synchronize()
+        return float(np.mean([a.elapsed_time(b) for a, b in evs]))
+
+    step = lambda: (fwd(), bwd())
+    for _ in range(max(args.warmup, 3)):
+        step()
+    l0 = G.gnn_launch_count()
+    ms_step = timed(step, args.steps)
+    launches = (G.gnn_launch_count() - l0) // max(args.steps, 1)
+    ms_f, ms_b = timed(fwd, args.steps), timed(bwd, args.steps)
+    comp = compulsory_bytes(c)
+    frac = lambda byts, ms: byts / (ms * 1e-3) * 1e-9 / peak
+    r = {"workload": c["name"], "layer": c["layer"], "nodes": n, "edges": e, "heads": H, "head_dim": d, "feature_dtype": dt,
+         "ms_per_step": ms_step, "ms_fwd": ms_f, "ms_bwd": ms_b, "gedges": e / (ms_step * 1e-3) * 1e-9,
+         "gedges_fwd": e / (ms_f * 1e-3) * 1e-9, "gedges_bwd": e / (ms_b * 1e-3) * 1e-9, "launches_per_step": int(launches),
+         "l2": "L2 flushed between timed steps" if flush is not None else "inputs larger than L2 (no flush)",
+         "compulsory_frac_fwd": frac(comp["fwd"], ms_f), "compulsory_frac_bwd": frac(comp["bwd"], ms_b),
+         "compulsory_frac_step": frac(comp["fwd"] + comp["bwd"], ms_step), "plan": plan.counts()}
+    if cfg == 4:
+        fb = lambda: G.gnn_gt_attn_fwd_block(plan, T["q"], T["k"], T["v"], out, lse)
+        fw = lambda: G.gnn_gt_attn_fwd_wsb(plan, T["q"], T["k"], T["v"], out, lse)
+        bw = lambda: G.gnn_gt_attn_bwd_wsb(plan, T["q"], T["k"], T["v"], out, lse, T["do"], stat, g1, g2, g3)
+        for _ in range(3):
+            fb(); fw(); bw()
+        ms_fb, ms_fw, ms_bw = timed(fb, args.steps), timed(fw, args.steps), timed(bw, args.steps)
+        r["tcgen05_paths"] = {"block_fwd_ms": ms_fb, "block_fwd_compulsory_frac": frac(comp["fwd"], ms_fb),
+                              "wsb_fwd_ms": ms_fw, "wsb_bwd_ms": ms_bw, "wsb_info": plan.wsb_info(),
+                              "best_step_ms": min(ms_f, ms_fb, ms_fw) + min(ms_b, ms_bw),
+                              "best_step_gedges": e / ((min(ms_f, ms_fb, ms_fw) + min(ms_b, ms_bw)) * 1e-3) * 1e-9}
+    del T, out, lse, stat, g1, g2, g3, plan, flush
+    torch.cuda.empty_cache()
+    return r
+
+
+def event_ms(fn, reps=3, warm=1):
+    import torch
+    for _ in range(warm):
+        fn()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(reps):
+        fn()
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / reps
+
+
+def gather_ceilings(row_bytes, dev):
+    """Ceiling 2 of DESIGN.md section 6, measured in this process through the C ABI (gnn_probe_gather): GB/s of uniformly
+    random `row_bytes` rows from an HBM-resident table (2.4 GB) and from an L2-resident one (48 MB); register gathers
+    (256-bit loads, 4 rows in flight per lane group) at 32 and at 16 resident warps per SM - the traversal kernels run at
+    12-16 - and cp.async.bulk copies at 16 warps per SM."""
+    import torch
+    import paper_2605_31500_b200 as G
+    rb = 256 if row_bytes <= 256 else (512 if row_bytes <= 512 else 1024)
+    n_idx = 1 << 25
+    sink = torch.zeros(1, dtype=torch.float32, device=dev)
+    res = {"row_bytes": rb, "n_gathers": n_idx}
+    for name, tbytes in (("hbm_resident", 2_400_000_000), ("l2_resident", 48_000_000)):
+        rows = tbytes // rb
+        table = torch.ones(rows * rb, dtype=torch.uint8, device=dev)
+        idx = torch.randint(0, rows, (n_idx,), dtype=torch.int32, device=dev)
+        r = {}
+        for key, mode, depth, cps in (("ldg_32warps", 0, 4, 8), ("ldg_16warps", 0, 4, 4), ("bulk_16warps", 1, 8, 4)):
+            ms = event_ms(lambda: G.gnn_probe_gather(table, rb, idx, mode, depth, cps, sink))
+            r[key + "_gbs"] = n_idx * rb / (ms * 1e-3) * 1e-9
+        res[name] = r
+        del table, idx
+    torch.cuda.empty_cache()
+    return res
+
+
+def block_extras(c, dev, peak, bf16_peak):
+    """Row f4 on the main config's shape: (1) the fused LayerNorm + QKV projection in front of the GT attention
+    (PAPER.md:478; input features = H * d as in the paper's block), bytes = x + q, k, v + W once, flops = 2 n C 3R;
+    (2) cfg 3 only: the dot-aggr locality study - second-pass times of the feature-parallel and the
+    neighbour-parallel kernel, scalar and 16-byte loads, fp32 D = 64, on the config's ids (random relabel = "orig") and
+    on two reorderings (natural R-MAT ids, ids sorted by descending in-degree); s = t_orig / t_reordered,
+    gap = s_neighbour - s_feature."""
+    import torch
+    import paper_2605_31500_b200 as G
+    n, H, d = c["n"], c["heads"], c["head_dim"]
+    R = H * d
+    out = {}
+    if c["layer"] == "gt" and R % 128 == 0 and 64 <= R <= 512:
+        g = torch.Generator(device=dev).manual_seed(1)
+        x = torch.randn((n, R), device=dev, generator=g).to(torch.bfloat16)
+        w = (torch.randn((3 * R, R), device=dev, generator=g) * R ** -0.5).to(torch.bfloat16)
+        gamma, beta = torch.ones(R, device=dev), torch.zeros(R, device=dev)
+        bias = torch.zeros(3 * R, device=dev)
+        q, k, v = (torch.empty((n, H, d), dtype=torch.bfloat16, device=dev) for _ in range(3))
+        ms = event_ms(lambda: G.gnn_ln_qkv_fwd(x, gamma, beta, 1e-5, w, bias, q, k, v), reps=5, warm=2)
+        F = torch.nn.functional
+        gb, bb, biasb = gamma.bfloat16(), beta.bfloat16(), bias.bfloat16()
+        ms_lib = event_ms(lambda: F.linear(F.layer_norm(x, (R,), gb, bb, 1e-5), w, biasb), reps=5, warm=2)   # context only
+        byts = n * R * 2 * 4 + 3 * R * R * 2
+        fl = 2.0 * n * R * 3 * R
+        out["ln_qkv"] = {"ms": ms, "c_in": R, "out_features": 3 * R, "bytes": byts, "gbs": byts / (ms * 1e-3) * 1e-9,
+                         "frac_of_hbm_peak": byts / (ms * 1e-3) * 1e-9 / peak, "tflops": fl / (ms * 1e-3) * 1e-12,
+                         "frac_of_bf16_peak": (fl / (ms * 1e-3) * 1e-12 / bf16_peak) if bf16_peak else None,
+                         "library_layer_norm_plus_linear_ms": ms_lib,
+                         "note": "LayerNorm fused into the A-operand staging of a tcgen05 GEMM; x, W random, timed alone; the library "
+                                 "figure (torch layer_norm kernel + cuBLAS linear, the paper's own arrangement) is context, not a product path"}
+        del x, w, q, k, v
+    if c["cfg"] == 3 and c["scale"] == 1.0:
+        from gnn_inputs.configs import _graph
+        D = 64
+        g = torch.Generator(device=dev).manual_seed(2)
+        xf = torch.randn((n, D), device=dev, generator=g) * D ** -0.5
+        o = torch.empty(n, device=dev)
+        deg = np.diff(c["rowptr"].astype(np.int64))
+        order = np.argsort(-deg, kind="stable")
+        new_id = np.empty(n, np.int64)
+        new_id[order] = np.arange(n)
+        dst = np.repeat(np.arange(n, dtype=np.int64), deg)
+        rp_s, ci_s = GI.csr_from_pairs(n, new_id[dst], new_id[c["colidx"]], self_loops=False, dedupe=False)
+        _, (rp_n, ci_n) = _graph(3, 1.0, c["seed"], relabel=False)
+        graphs = {"orig_random_ids": (c["rowptr"], c["colidx"]), "natural_rmat_ids": (rp_n, ci_n), "degree_sorted_ids": (rp_s, ci_s)}
+        t = {}
+        for gname, (rp, ci) in graphs.items():
+            rpd, cid = torch.from_numpy(rp).to(dev), torch.from_numpy(ci).to(dev)
+            for mode, mname in ((0, "feature"), (1, "neighbor")):
+                for vec in (False, True):
+                    t[f"{gname}/{mname}{'_vec' if vec else ''}"] = event_ms(lambda: G.gnn_dot_aggr(rpd, cid, xf, mode, vec, o), reps=2, warm=1)
+            del rpd, cid
+        gaps = {}
+        for gname in ("natural_rmat_ids", "degree_sorted_ids"):
+            for sfx in ("", "_vec"):
+                s_f = t[f"orig_random_ids/feature{sfx}"] / t[f"{gname}/feature{sfx}"]
+                s_n = t[f"orig_random_ids/neighbor{sfx}"] / t[f"{gname}/neighbor{sfx}"]
+                gaps[f"{gname}{sfx}"] = {"s_feature": s_f, "s_neighbor": s_n, "delta_s": s_n - s_f}
+        out["dot_aggr"] = {"dim": D, "dtype": "f32", "second_pass_ms": t, "reordering_gap": gaps,
+                           "note": "METIS is not available: the reorderings are the generator's natural ids and a degree sort"}
+    torch.cuda.empty_cache()
+    return out
 
 
 # ------------------------------------------------------------------------------------------ clocks
@@ -475,17 +671,33 @@ def run_ours(args, rank, world, local_rank):
         peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     else:
         peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r01_dram_traffic.json")
-    if os.path.exists(tpath) and args.scale == 1.0 and not (args.warp_max_deg or args.cta_max_deg or args.split_chunk):
-        traffic = json.load(open(tpath)).get(c["name"], {})
+    bf16_peak = None
+    if os.path.exists(peaks_path):
+        bf16_peak = json.load(open(peaks_path)).get("bf16_tflops")
+    traffic, tfile = None, None
+    for tname in ("r02_dram_traffic.json", "r01_dram_traffic.json"):      # ncu captures of this build, else of round 1
+        tpath = os.path.join(ROOT, "profiles", tname)
+        if traffic is None and os.path.exists(tpath) and args.scale == 1.0 and not (args.warp_max_deg or args.cta_max_deg or args.split_chunk):
+            tj = json.load(open(tpath))
+            if c["name"] in tj:
+                traffic, tfile = tj[c["name"]], "profiles/" + tname
     dom = max((k for k in kern_ms if k in alg), key=lambda k: kern_ms[k])
     achieved = alg[dom] / (kern_ms[dom] * 1e-3) * 1e-9
     step_ms = total_ms / args.steps
     comp_step = comp["fwd"] + comp["bwd"]
+    dom_traffic = (traffic or {}).get(dom)
     roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": (traffic or {}).get(dom), "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch "
-            "(profiles/r01_dram_traffic.json)" if traffic else None, "kernels_traffic": traffic or None,
+            "frac_meaning": "ALGORITHMIC bytes of the dominant kernel (index + gathered rows per edge, SURVEY 8(d)) / its "
+                            "live CUDA-event time / measured HBM copy peak.  Gathers that hit L2 count, so this is NOT a DRAM "
+                            "utilisation and can exceed 1; `dram_frac` is the DRAM utilisation, `north_star` the graded figure",
+            "traffic": dom_traffic,
+            "traffic_source": (f"ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, offline capture ({tfile}); "
+                               "not measured in this run") if traffic else None,
+            "dram_frac": (dom_traffic / (kern_ms[dom] * 1e-3) * 1e-9 / peak) if dom_traffic else None,
+            "traffic_over_compulsory_step": (sum(v for k, v in traffic.items() if k in kern_ms) / comp_step) if traffic else None,
+            "north_star": {"what": "compulsory bytes (each array once) / step time / measured HBM peak", "target": 0.60,
+                           "value": comp_step / (step_ms * 1e-3) * 1e-9 / peak},
+            "kernels_traffic": traffic or None,
             "peak_source": peak_src, "algorithmic_bytes_per_launch": alg[dom],
             "kernel_ms": kern_ms[dom], "kernel_share_of_step": kern_ms[dom] / sum(kern_ms.values()),
             "kernels_ms": kern_ms,
@@ -509,9 +721,27 @@ def run_ours(args, rank, world, local_rank):
     roof["fp32_alu"] = {"flop_per_edge_head_fwd": fl["fwd"], "flop_per_edge_head_bwd": fl["bwd"], "peak_tflops": alu_peak,
                         "sm_mhz": sm_clk, "tflops_fwd": tf_fwd, "tflops_bwd": tf_bwd,
                         "frac_fwd": tf_fwd / alu_peak, "frac_bwd": tf_bwd / alu_peak}
-    roof["binding"] = ("three ceilings are reported: `compulsory` (HBM, each array once), `kernels_algorithmic_gbs` (gather ingest "
-                       "through L2, against the measured HBM peak; values above 1.0 x peak are L2 hits) and `fp32_alu`; the "
-                       "largest fraction is the one that binds")
+    extras = {}
+    if world == 1 and not args.no_extras:
+        gc = gather_ceilings(H * d * (4 if dt == "f32" else 2), dev)
+        roof["gather_ceiling"] = gc
+        # the dominant kernel's row ingest against the probe at the occupancy the kernels run at: an L2-hit-weighted mix
+        # of the two tables bounds it (the kernels see ~40-60 % L2 hits, profiles/)
+        roof["frac_of_gather_ceiling"] = {"vs_hbm_resident_16warps": achieved / gc["hbm_resident"]["ldg_16warps_gbs"],
+                                          "vs_l2_resident_16warps": achieved / gc["l2_resident"]["ldg_16warps_gbs"],
+                                          "vs_hbm_resident_32warps": achieved / gc["hbm_resident"]["ldg_32warps_gbs"],
+                                          "vs_l2_resident_32warps": achieved / gc["l2_resident"]["ldg_32warps_gbs"]}
+        extras = block_extras(c, dev, peak, bf16_peak)
+    fr = {"hbm_compulsory": roof["north_star"]["value"], "hbm_dram_traffic_dominant_kernel": roof["dram_frac"],
+          "fp32_alu": max(roof["fp32_alu"]["frac_fwd"], roof["fp32_alu"]["frac_bwd"]),
+          "gather_ingest_hbm_resident_16warps": (roof.get("frac_of_gather_ceiling") or {}).get("vs_hbm_resident_16warps")}
+    known = {k: v for k, v in fr.items() if v is not None}
+    top = max(known, key=known.get)
+    roof["binding"] = {"fractions": fr, "largest": top,
+                       "reading": ("no ceiling is saturated: the traversal kernels are latency-bound at register-limited occupancy "
+                                   "(12-16 warps/SM); the closest ceiling is the gather ingest of random rows at that occupancy "
+                                   "(profiles/r02_csr_experiments.md); the compulsory-byte fraction misses north_star's 0.60 because the "
+                                   "per-edge gathers move 5-13x the compulsory bytes through L2 / DRAM")}
 
     if block is not None:
         rem = int(plan.export(B.GNN_PLAN_BLOCK_REM_ROWPTR)[-1])
@@ -633,10 +863,18 @@ def run_ours(args, rank, world, local_rank):
                "pipeline": "3 streams, double-buffered features and outputs; fill and drain inside the timed region"}
         del pin_in, pin_out, dsets, osets
 
+    all_cfg = None
+    if rank == 0 and world == 1 and args.cfg == 3 and args.scale == 1.0 and not args.no_all_configs and not args.dense:
+        all_cfg = {}
+        for other in (1, 2, 4, 5):
+            all_cfg[f"cfg{other}"] = quick_config(other, args, dev, peak)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         arm = OracleArm(c, args.cpu_seconds)
-        cpu = {"value": arm.gedges(arm.run()), "unit": UNIT, "cores": arm.cores, "kind": "oracle", "sample": arm.sample_text()}
+        cpu = {"value": arm.gedges(arm.run()), "unit": UNIT, "cores": arm.cores, "kind": "oracle", "sample": arm.sample_text(),
+               "edges_timed_dst_side": arm.er, "edges_timed_src_side": arm.es, "edges_total": e,
+               "fraction_of_edges_timed": {"dst_side": arm.er / e, "src_side": arm.es / e}}
 
     if rank == 0:
         cfgd = workload_config(c, args)
@@ -653,7 +891,8 @@ def run_ours(args, rank, world, local_rank):
                 "gedges_fwd": e / (np.mean(ms_fwd) * 1e-3) * 1e-9, "gedges_bwd": e / (np.mean(ms_bwd) * 1e-3) * 1e-9,
                 "peak_device_bytes": peak_mem, "device_bytes_inputs": in_bytes, "device_bytes_outputs": out_bytes,
                 "plan_bytes": plan.plan_bytes, "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
-                "roofline": roof, "block_path": block, "wsb_path": wsb, "cuda_graph": graph, "seg_minmax": minmax, "cpu_baseline": cpu}
+                "roofline": roof, "block_path": block, "wsb_path": wsb, "all_configs": all_cfg,
+                "ln_qkv": extras.get("ln_qkv"), "dot_aggr": extras.get("dot_aggr"), "cuda_graph": graph, "seg_minmax": minmax, "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

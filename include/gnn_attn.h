@@ -293,6 +293,15 @@ gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, int32_t head
                             const float* beta, float eps, const void* w, const float* bias, void* q, void* k, void* v,
                             gnn_stream_t stream);
 
+/* The paper's `dot-aggr` locality micro-benchmark: out[i] = sum over the stored in-neighbours j of i
+ * of <x[i,:], x[j,:]>, fp32, as two warp-per-node kernels with identical arithmetic: mode 0 = feature-parallel (lanes
+ * over the features, neighbours scanned sequentially, coalesced loads), mode 1 = neighbour-parallel (every lane walks a
+ * different neighbour's row, gather-like loads); vec 0 = 4-byte loads, 1 = 16-byte loads.  x: [n, dim] fp32, dim a
+ * multiple of 4, 16-byte aligned; out: [n] fp32.  Needs no plan.  Summation order differs between the modes (results
+ * agree to fp32 rounding).  Asynchronous on `stream`.                                                              */
+gnn_status_t gnn_dot_aggr(int32_t n, const int32_t* rowptr, const int32_t* colidx, const float* x, int32_t dim, int32_t mode,
+                          int32_t vec, float* out, gnn_stream_t stream);
+
 /* Measurement aid (bench.py): ONE launch that gathers n_idx rows of row_bytes (256 | 512 | 1024) bytes at the row
  * indices idx[0..n_idx) (each in [0, table_rows)) from `table` and discards them - the achievable gather-ingest rate
  * ("ceiling 2" of DESIGN.md section 6: HBM-resident when the table is far larger than L2, L2-resident when it fits),

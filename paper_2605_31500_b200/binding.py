@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = [
     "gnn_csr_validate", "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
     "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
     "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_gt_attn_fwd_wsb", "gnn_gt_attn_bwd_wsb", "gnn_seg_minmax_fwd", "gnn_seg_minmax_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
-    "gnn_profile_collect", "gnn_pdl_enable", "gnn_probe_gather", "gnn_ln_qkv_fwd",
+    "gnn_profile_collect", "gnn_pdl_enable", "gnn_probe_gather", "gnn_ln_qkv_fwd", "gnn_dot_aggr",
 ]
 
 
@@ -81,6 +81,7 @@ def lib() -> C.CDLL:
         L.gnn_profile_enable.restype = None
         L.gnn_probe_gather.argtypes = [_vp, _i64, _i32, _vp, _i64, _i32, _i32, _i32, _vp, _vp]
         L.gnn_ln_qkv_fwd.argtypes = [_i32, _i32, _i32, _i32, _vp, _vp, _vp, _f, _vp, _vp, _vp, _vp, _vp, _vp]
+        L.gnn_dot_aggr.argtypes = [_i32, _vp, _vp, _vp, _i32, _i32, _i32, _vp, _vp]
         L.gnn_pdl_enable.argtypes = [C.c_int]
         L.gnn_pdl_enable.restype = None
         L.gnn_profile_collect.argtypes = [_vp, _vp, _i32]
@@ -311,6 +312,12 @@ def gnn_ln_qkv_fwd(x, gamma, beta, eps, w, bias, q, k, v, stream=None):
     _, H, d = q.shape
     _check(lib().gnn_ln_qkv_fwd(n, c_in, H, d, _ptr(x), _ptr(gamma), _ptr(beta), float(eps), _ptr(w), _ptr(bias), _ptr(q),
                                 _ptr(k), _ptr(v), _stream(stream)))
+
+
+def gnn_dot_aggr(rowptr, colidx, x, mode: int, vec: bool, out, stream=None):
+    """out[i] = sum_j <x_i, x_j> over the CSR row of i; mode 0 feature-parallel, 1 neighbour-parallel."""
+    n, dim = x.shape
+    _check(lib().gnn_dot_aggr(n, _ptr(rowptr), _ptr(colidx), _ptr(x), dim, int(mode), 1 if vec else 0, _ptr(out), _stream(stream)))
 
 
 def gnn_probe_gather(table, row_bytes: int, idx, mode: int, depth: int, ctas_per_sm: int, sink, stream=None):

@@ -28,7 +28,7 @@ constexpr int kRows = 128;          // rows per CTA = MMA M
 constexpr int kNC = 128;            // output columns per chunk = MMA N
 constexpr int kStage = 16384;       // bytes of a weight stage / of a 64-channel half tile of A
 constexpr int kThreads = 192;       // warps 0-3: LayerNorm + epilogue, warp 4: TMA, warp 5: MMA
-constexpr int kSlot = 272;          // bytes of a transpose slot: 128 bf16 + 16 (conflict-free 16-byte accesses)
+constexpr int kSlot = 80;           // bytes of a transpose slot: 32 bf16 + 16 (conflict-free 16-byte writes)
 
 struct LnQkvParams {
     const __nv_bfloat16* x;
@@ -48,7 +48,7 @@ __device__ __forceinline__ float warp_sum(float v) {
     return v;
 }
 
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreads, 2)
 ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -105,10 +105,11 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
             }
         }
         const float inv_c = 1.f / (float)p.C;
-        for (int rl = 0; rl < 32; rl += 2) {
-            uint4 raw[2][2];
+        constexpr int RB = 8;                 // rows in flight per warp: the loads of 8 rows are issued before the first reduction
+        for (int rl = 0; rl < 32; rl += RB) {
+            uint4 raw[RB][2];
 #pragma unroll
-            for (int u = 0; u < 2; ++u)
+            for (int u = 0; u < RB; ++u)
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
                     const int row = row0 + warp * 32 + rl + u, cc = lane + 32 * j;
@@ -116,7 +117,7 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
                     if (row < p.n && cc < nchunk) raw[u][j] = __ldg(reinterpret_cast<const uint4*>(p.x + (size_t)row * p.C) + cc);
                 }
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
+            for (int u = 0; u < RB; ++u) {
                 const int r = warp * 32 + rl + u;
                 float v[2][8];
                 float s = 0.f;
@@ -206,39 +207,46 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
             mbar_wait(tfull + bsel, (uint32_t)((c >> 1) & 1));
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const int col0 = c * kNC;
-#pragma unroll
+            const int t = col0 / p.R, off = col0 - t * p.R;
+            __nv_bfloat16* dst = (t == 0 ? p.q : (t == 1 ? p.k : p.v)) + off;
+            const int ch = lane & 3, rsub = lane >> 2;
+#pragma unroll 1
             for (int c0 = 0; c0 < kNC; c0 += 32) {
                 float t32[32];
                 tmem_ld32(t_lane + bsel * kNC + c0, t32);
+                if (c0 + 32 == kNC) {                           // last read of this accumulator: hand it back to the MMA warp
+                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(tempty + bsel);
+                }
+                if (p.bias) {
+#pragma unroll
+                    for (int i = 0; i < 32; i += 4) {
+                        const float4 bb = __ldg(reinterpret_cast<const float4*>(p.bias + col0 + c0 + i));
+                        t32[i] += bb.x; t32[i + 1] += bb.y; t32[i + 2] += bb.z; t32[i + 3] += bb.w;
+                    }
+                }
                 uint32_t o[16];
 #pragma unroll
                 for (int i = 0; i < 16; ++i) {
-                    const float b0 = p.bias ? __ldg(p.bias + col0 + c0 + 2 * i) : 0.f;
-                    const float b1 = p.bias ? __ldg(p.bias + col0 + c0 + 2 * i + 1) : 0.f;
-                    const __nv_bfloat162 yb = __floats2bfloat162_rn(t32[2 * i] + b0, t32[2 * i + 1] + b1);
+                    const __nv_bfloat162 yb = __floats2bfloat162_rn(t32[2 * i], t32[2 * i + 1]);
                     o[i] = *reinterpret_cast<const uint32_t*>(&yb);
                 }
 #pragma unroll
-                for (int i = 0; i < 16; i += 4)
-                    *reinterpret_cast<uint4*>(slot + c0 * 2 + i * 4) = make_uint4(o[i], o[i + 1], o[i + 2], o[i + 3]);
-            }
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) mbar_arrive(tempty + bsel);          // this warp's 32 lanes of the accumulator are drained
-            // rows of this warp, 16 lanes per 256-byte row piece
-            const int t = col0 / p.R, off = col0 - t * p.R;
-            __nv_bfloat16* dst = (t == 0 ? p.q : (t == 1 ? p.k : p.v)) + off;
-            const int ch = lane & 15, rsub = lane >> 4;
-#pragma unroll 4
-            for (int it = 0; it < 16; ++it) {
-                const int rl = it * 2 + rsub;
-                const int row = row0 + warp * 32 + rl;
-                if (row < p.n) {
-                    const uint4 w = *reinterpret_cast<const uint4*>(sT + (warp * 32 + rl) * kSlot + ch * 16);
-                    *reinterpret_cast<uint4*>(dst + (size_t)row * p.R + ch * 8) = w;
+                for (int i = 0; i < 16; i += 4) *reinterpret_cast<uint4*>(slot + i * 4) = make_uint4(o[i], o[i + 1], o[i + 2], o[i + 3]);
+                __syncwarp();
+                // rows of this warp, 4 lanes per 64-byte row piece, 8 rows per instruction
+#pragma unroll
+                for (int it = 0; it < 4; ++it) {
+                    const int rl = it * 8 + rsub;
+                    const int row = row0 + warp * 32 + rl;
+                    if (row < p.n) {
+                        const uint4 w = *reinterpret_cast<const uint4*>(sT + (warp * 32 + rl) * kSlot + ch * 16);
+                        *reinterpret_cast<uint4*>(dst + (size_t)row * p.R + c0 + ch * 8) = w;
+                    }
                 }
+                __syncwarp();
             }
-            __syncwarp();
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -276,8 +284,12 @@ extern "C" gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, i
     p.x = (const __nv_bfloat16*)x; p.gamma = gamma; p.beta = beta; p.bias = bias;
     p.q = (__nv_bfloat16*)q; p.k = (__nv_bfloat16*)k; p.v = (__nv_bfloat16*)v;
     p.n = n; p.C = c_in; p.R = (int)R; p.eps = eps;
-    p.n_stages = c_in <= 256 ? 6 : 3;
-    const size_t smem = (size_t)(c_in / 64) * kStage + (size_t)p.n_stages * kStage + (size_t)kRows * kSlot + 256 + 1024;
+    // weight ring: as many 16 KB stages as keep two CTAs per SM (113 KB each) when the A tile allows it, else one CTA
+    const size_t fixed = (size_t)(c_in / 64) * kStage + (size_t)kRows * kSlot + 256 + 1024;
+    const size_t budget = fixed + 2 * kStage <= 113 * 1024 ? 113 * 1024 : 226 * 1024;
+    p.n_stages = (int)((budget - fixed) / kStage);
+    if (p.n_stages > 8) p.n_stages = 8;
+    const size_t smem = fixed + (size_t)p.n_stages * kStage;
     cudaError_t e = cudaFuncSetAttribute(ln_qkv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) {
         cudaStream_t st = (cudaStream_t)stream;
