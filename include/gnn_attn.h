@@ -138,7 +138,9 @@ enum {
     GNN_PLAN_WSB_BITMAP = 16,       /* uint8[n_tcb][16]: byte r = row r of the window, bit c = column c of the TCB */
     GNN_PLAN_WSB_ROW_OFFSET_T = 17, /* the same three for CSR^T (source windows x destination columns)             */
     GNN_PLAN_WSB_COLS_T = 18,
-    GNN_PLAN_WSB_BITMAP_T = 19
+    GNN_PLAN_WSB_BITMAP_T = 19,
+    GNN_PLAN_BLOCK_REM_ROWPTR_T = 20, /* int32[n + 1]: stable transpose of the remainder CSR of the diagonal block layout   */
+    GNN_PLAN_BLOCK_REM_COLIDX_T = 21  /* int32[rem_nnz] (plans built with GNN_BLOCKS_DIAG and build_transpose)             */
 };
 /* Copies the item to HOST memory `host_dst` (synchronous).  *bytes in = capacity, out = size needed;
  * with host_dst == NULL only the size is returned.                                                 */
@@ -154,7 +156,8 @@ const int32_t* gnn_plan_colidx_t(const gnn_plan_t* plan);
 enum { GNN_OP_GT_FWD = 0, GNN_OP_GT_BWD = 1, GNN_OP_GATV2_FWD = 2, GNN_OP_GATV2_BWD = 3,
        GNN_OP_GT_FWD_BLOCK = 4 /* needs no workspace: 0 bytes */,
        GNN_OP_SEG_MINMAX_FWD = 5 /* pass heads = 1, head_dim = channels */,
-       GNN_OP_WSB_FWD = 6, GNN_OP_WSB_BWD = 7 /* tile-local: 0 bytes */ };
+       GNN_OP_WSB_FWD = 6, GNN_OP_WSB_BWD = 7 /* tile-local: 0 bytes */,
+       GNN_OP_GT_BWD_BLOCK = 8 };
 gnn_status_t gnn_workspace_bytes(const gnn_plan_t* plan, int op, int32_t heads, int32_t head_dim, gnn_dtype_t dtype,
                                  size_t* bytes);
 
@@ -216,6 +219,18 @@ gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* plan, const int32_t* rowptr, const 
 gnn_status_t gnn_gt_attn_fwd_block(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
                                    const void* q, const void* k, const void* v, int32_t heads, int32_t head_dim,
                                    gnn_dtype_t dtype, void* out, float* lse, gnn_stream_t stream);
+
+/* Backward of the same function on the diagonal block layout, tensor cores for the in-window edges (PAPER.md:563:
+ * P = exp(S - L), dV = P^T dO, dP = dO V^T, dS = P o (dP - Delta), dQ = dS K, dK = dS^T Q) - tile-local, hence no atomics
+ * - and the remainder CSR for every other edge: its dst-side terms (Delta, dQ) inside the tile kernel, its src-side terms
+ * (dK, dV) through the CSR src pass over the transposed remainder CSR of the plan, added to the tile-local part.
+ * Same results as gnn_gt_attn_bwd up to rounding (dS / P rounded to bf16 for the in-window products; Delta fp32).
+ * Plan: GNN_BLOCKS_DIAG and build_transpose != 0.  bf16, head_dim == 64.  Arguments as gnn_gt_attn_bwd;
+ * ws >= gnn_workspace_bytes(GNN_OP_GT_BWD_BLOCK).                                                                  */
+gnn_status_t gnn_gt_attn_bwd_block(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                   const void* q, const void* k, const void* v, const float* lse, const void* dout,
+                                   int32_t heads, int32_t head_dim, gnn_dtype_t dtype, float* delta, float* dq, float* dk,
+                                   float* dv, void* ws, size_t ws_bytes, gnn_stream_t stream);
 
 /* ---------------------------------------------------------------------------------------------
  * Graph Transformer attention on the general WSB block-sparse layout, forward and backward on the

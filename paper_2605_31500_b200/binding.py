@@ -13,19 +13,20 @@ _LIB_PATH = os.path.join(_HERE, "libgnn_attn.so")
 GNN_OK, GNN_EINVAL, GNN_EUNSUPPORTED, GNN_EWORKSPACE, GNN_ECUDA = range(5)
 GNN_F32, GNN_BF16 = 0, 1
 GNN_OP_GT_FWD, GNN_OP_GT_BWD, GNN_OP_GATV2_FWD, GNN_OP_GATV2_BWD = 0, 1, 2, 3
-GNN_OP_GT_FWD_BLOCK, GNN_OP_SEG_MINMAX_FWD, GNN_OP_WSB_FWD, GNN_OP_WSB_BWD = 4, 5, 6, 7
+GNN_OP_GT_FWD_BLOCK, GNN_OP_SEG_MINMAX_FWD, GNN_OP_WSB_FWD, GNN_OP_WSB_BWD, GNN_OP_GT_BWD_BLOCK = 4, 5, 6, 7, 8
 GNN_AGG_MIN, GNN_AGG_MAX = 0, 1
 GNN_TRANSPOSE_NONE, GNN_TRANSPOSE_BUILD, GNN_TRANSPOSE_UNDIRECTED = 0, 1, 2
 (GNN_PLAN_COUNTS, GNN_PLAN_PERM, GNN_PLAN_CHUNKS, GNN_PLAN_CHUNK_PTR, GNN_PLAN_ROWPTR_T, GNN_PLAN_COLIDX_T,
  GNN_PLAN_PERM_T, GNN_PLAN_CHUNKS_T, GNN_PLAN_CHUNK_PTR_T, GNN_PLAN_BLOCK_BITMAP, GNN_PLAN_BLOCK_REM_ROWPTR,
  GNN_PLAN_BLOCK_REM_COLIDX, GNN_PLAN_FLAGS, GNN_PLAN_WSB_INFO, GNN_PLAN_WSB_ROW_OFFSET, GNN_PLAN_WSB_COLS,
- GNN_PLAN_WSB_BITMAP, GNN_PLAN_WSB_ROW_OFFSET_T, GNN_PLAN_WSB_COLS_T, GNN_PLAN_WSB_BITMAP_T) = range(20)
+ GNN_PLAN_WSB_BITMAP, GNN_PLAN_WSB_ROW_OFFSET_T, GNN_PLAN_WSB_COLS_T, GNN_PLAN_WSB_BITMAP_T,
+ GNN_PLAN_BLOCK_REM_ROWPTR_T, GNN_PLAN_BLOCK_REM_COLIDX_T) = range(22)
 GNN_BLOCKS_NONE, GNN_BLOCKS_DIAG, GNN_BLOCKS_WSB = 0, 1, 2
 
 EXPORTED_SYMBOLS = [
     "gnn_csr_validate", "gnn_plan_bytes", "gnn_plan_build", "gnn_plan_destroy", "gnn_plan_export", "gnn_plan_rowptr_t",
     "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
-    "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_gt_attn_fwd_wsb", "gnn_gt_attn_bwd_wsb", "gnn_seg_minmax_fwd", "gnn_seg_minmax_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
+    "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_gt_attn_fwd_wsb", "gnn_gt_attn_bwd_wsb", "gnn_gt_attn_bwd_block", "gnn_seg_minmax_fwd", "gnn_seg_minmax_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
     "gnn_profile_collect", "gnn_pdl_enable", "gnn_probe_gather", "gnn_ln_qkv_fwd", "gnn_dot_aggr",
 ]
 
@@ -71,6 +72,8 @@ def lib() -> C.CDLL:
         L.gnn_seg_minmax_fwd.argtypes = [_vp, _vp, _vp, _i32, _vp, _i32, C.c_int, _i32, _vp, _vp, _vp, _sz, _vp]
         L.gnn_seg_minmax_bwd.argtypes = [_i32, _vp, _vp, _i32, C.c_int, _vp, _vp]
         L.gnn_gt_attn_fwd_block.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _vp, _vp, _vp]
+        L.gnn_gt_attn_bwd_block.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _vp, _vp, _i32, _i32, C.c_int,
+                                            _vp, _vp, _vp, _vp, _vp, _sz, _vp]
         L.gnn_gt_attn_fwd_wsb.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _vp, _vp, _vp]
         L.gnn_gt_attn_bwd_wsb.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _i32, C.c_int,
                                           _vp, _vp, _vp, _vp, _vp]
@@ -268,6 +271,14 @@ def gnn_gt_attn_fwd_block(plan: Plan, q, k, v, out, lse, stream=None):
     n, H, d = q.shape
     _check(lib().gnn_gt_attn_fwd_block(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v), H, d,
                                        _dtype_code(q), _ptr(out), _ptr(lse), _stream(stream)))
+
+
+def gnn_gt_attn_bwd_block(plan: Plan, q, k, v, lse, dout, delta, dq, dk, dv, stream=None):
+    n, H, d = q.shape
+    ws = plan.workspace(GNN_OP_GT_BWD_BLOCK, H, d, _dtype_code(q))
+    _check(lib().gnn_gt_attn_bwd_block(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v),
+                                       _ptr(lse), _ptr(dout), H, d, _dtype_code(q), _ptr(delta), _ptr(dq), _ptr(dk), _ptr(dv),
+                                       _ptr(ws), ws.numel(), _stream(stream)))
 
 
 def gnn_gt_attn_fwd_wsb(plan: Plan, q, k, v, out, lse, stream=None):

@@ -146,6 +146,20 @@ size_t ws_total(const gnn_plan* P, int op, const HeadGroup* hg, int ng, int esz)
     return t;
 }
 
+// workspace of gnn_gt_attn_bwd_block: hub-chunk partials of the remainder src pass, then (L log2e, Delta) per (node, head)
+struct BlockWs { size_t stat2, total; };
+BlockWs block_bwd_ws(const gnn_plan* P, const HeadGroup* hg, int ng, int heads) {
+    size_t part = 0;
+    for (int g = 0; g < ng; ++g) {
+        const size_t x = (size_t)P->rem_tr.n_chunks * pass_state_floats(kGtBwdSrc, hg[g].sh) * sizeof(float);
+        if (x > part) part = x;
+    }
+    BlockWs w;
+    w.stat2 = (part + 255) / 256 * 256;
+    w.total = w.stat2 + (size_t)P->n * heads * sizeof(float2) + 256;
+    return w;
+}
+
 bool check_common(const gnn_plan* P, const int32_t* rowptr, const int32_t* colidx, int32_t n, const char* who) {
     if (!P) { set_error("%s: NULL plan", who); return false; }
     if (rowptr != P->rowptr || colidx != P->colidx || n != P->n) {
@@ -209,6 +223,14 @@ extern "C" gnn_status_t gnn_workspace_bytes(const gnn_plan_t* P, int op, int32_t
                                             gnn_dtype_t dtype, size_t* bytes) {
     if (!P || !bytes) { set_error("gnn_workspace_bytes: NULL plan or bytes"); return GNN_EINVAL; }
     if (op == GNN_OP_GT_FWD_BLOCK || op == GNN_OP_WSB_FWD || op == GNN_OP_WSB_BWD) { *bytes = 0; return GNN_OK; }   // tile-local: no workspace
+    if (op == GNN_OP_GT_BWD_BLOCK) {
+        if (!P->rem_rowptr_t) { set_error("gnn_workspace_bytes: plan lacks GNN_BLOCKS_DIAG with build_transpose"); return GNN_EINVAL; }
+        HeadGroup hgb[kMaxHeadGroups];
+        const int ngb = head_groups(P->n, heads, head_dim, dtype, hgb, "gnn_workspace_bytes");
+        if (!ngb) return GNN_EUNSUPPORTED;
+        *bytes = block_bwd_ws(P, hgb, ngb, heads).total;
+        return GNN_OK;
+    }
     if ((op < GNN_OP_GT_FWD || op > GNN_OP_GATV2_BWD) && op != GNN_OP_SEG_MINMAX_FWD) {
         set_error("gnn_workspace_bytes: unknown op %d", op);
         return GNN_EINVAL;
@@ -362,6 +384,50 @@ extern "C" gnn_status_t gnn_gatv2_bwd(const gnn_plan_t* P, const int32_t* rowptr
         e = launch_gat_bwd_dst(dtype, sh, c, a);                                                       // dxl, G, da partials (xl . S)
         if (e == cudaSuccess) e = launch_gat_bwd_src(dtype, sh, ct, a);                                // dxr, da partials (xr . U)
         if (e == cudaSuccess) e = launch_da_reduce(c.da_part, w.da_slots, sh.rowe, da + go, c.stream);  // da
+    }
+    return cuda_status(e, who);
+}
+
+extern "C" gnn_status_t gnn_gt_attn_bwd_block(const gnn_plan_t* P, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                              const void* q, const void* k, const void* v, const float* lse, const void* dout,
+                                              int32_t heads, int32_t head_dim, gnn_dtype_t dtype, float* delta, float* dq,
+                                              float* dk, float* dv, void* ws, size_t ws_bytes, gnn_stream_t stream) {
+    const char* who = "gnn_gt_attn_bwd_block";
+    if (!check_common(P, rowptr, colidx, n, who)) return GNN_EINVAL;
+    if (!P->blk_bitmap || !P->rem_rowptr_t) { set_error("%s: plan was built without GNN_BLOCKS_DIAG and build_transpose", who); return GNN_EINVAL; }
+    if (!q || !k || !v || !lse || !dout || !delta || !dq || !dk || !dv || !ws) { set_error("%s: NULL pointer argument", who); return GNN_EINVAL; }
+    if (!aligned32(q) || !aligned32(k) || !aligned32(v) || !aligned32(dout) || !aligned32(dq) || !aligned32(dk) || !aligned32(dv) ||
+        !aligned32(ws)) {
+        set_error("%s: feature / gradient pointers and workspace must be 32-byte aligned", who);
+        return GNN_EINVAL;
+    }
+    if (dtype != GNN_BF16 || head_dim != 64 || heads < 1) {
+        set_error("%s: unsupported shape heads=%d head_dim=%d dtype=%d (bf16, head_dim 64 only)", who, heads, head_dim, dtype);
+        return GNN_EUNSUPPORTED;
+    }
+    HeadGroup hg[kMaxHeadGroups];
+    const int ng = head_groups(n, heads, head_dim, dtype, hg, who);
+    if (!ng) return GNN_EUNSUPPORTED;
+    const BlockWs w = block_bwd_ws(P, hg, ng, heads);
+    if (ws_bytes < w.total) { set_error("%s: workspace too small (%zu < %zu)", who, ws_bytes, w.total); return GNN_EWORKSPACE; }
+    cudaStream_t st = (cudaStream_t)stream;
+    GtArgs a = {};
+    a.q = q; a.k = k; a.v = v; a.dout = dout; a.lse = const_cast<float*>(lse); a.delta = delta; a.dq = dq; a.dk = dk; a.dv = dv;
+    a.stat2 = (float2*)((char*)ws + w.stat2);
+    cudaError_t e = launch_gt_bwd_block(P, a, heads, st);         // Delta, dQ; tile-local dK, dV; (L, Delta) pairs
+    if (e == cudaErrorNotSupported) { set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who); return GNN_ECUDA; }
+    // out-of-window edges of the source side: CSR src pass over the transposed remainder CSR, adding to dK / dV
+    for (int g = 0; g < ng && e == cudaSuccess; ++g) {
+        const Shape& sh = hg[g].sh;
+        const int h0 = hg[g].h0;
+        const size_t fo = (size_t)h0 * head_dim * 2, go = (size_t)h0 * head_dim;
+        GtArgs b = {};
+        b.q = off_bytes(q, fo); b.k = off_bytes(k, fo); b.v = off_bytes(v, fo); b.dout = off_bytes(dout, fo);
+        b.dk = dk + go; b.dv = dv + go; b.stat2 = a.stat2 + h0; b.accumulate = 1;
+        LaunchCtx c;
+        c.stream = st; c.sm_count = P->sm_count; c.rowptr = P->rem_rowptr_t; c.colidx = P->rem_colidx_t; c.bins = P->rem_tr;
+        c.partials = (float*)ws; c.da_part = nullptr; c.da_slot_base = 0;
+        e = launch_gt_bwd_src(dtype, sh, c, b);
     }
     return cuda_status(e, who);
 }

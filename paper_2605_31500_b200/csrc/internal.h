@@ -35,6 +35,9 @@ struct gnn_plan {
     int32_t* blk_rem_colidx; // [rem_nnz]
     int32_t n_windows;
     int64_t rem_nnz;
+    int32_t* rem_rowptr_t;   // stable transpose of the remainder CSR + its bins (build_blocks DIAG with build_transpose)
+    int32_t* rem_colidx_t;
+    gnn::BinView rem_tr;
     int32_t rows_sorted;     // 1 if every CSR row lists its sources in ascending order (min / max fast path)
     int32_t has_wsb;         // build_blocks & GNN_BLOCKS_WSB
     gnn::WsbView wsb;        // of the CSR (destination windows x source columns)
@@ -115,6 +118,7 @@ struct GtArgs {
     void* out;
     float *lse, *delta, *dq, *dk, *dv;
     float2* stat2;   // workspace [n,H]: (L * log2(e), Delta) packed by the dst pass for the src pass (one 8-byte gather)
+    int accumulate;  // src pass: add to the dk / dv already stored (block backward: tile-local part first, remainder second)
 };
 struct GatArgs {
     const void *xl, *xr, *dout;
@@ -134,6 +138,8 @@ struct AggArgs {
 cudaError_t launch_gt_fwd(int dtype, const Shape&, const LaunchCtx&, const GtArgs&);
 cudaError_t launch_gt_bwd_dst(int dtype, const Shape&, const LaunchCtx&, const GtArgs&);
 cudaError_t launch_gt_bwd_src(int dtype, const Shape&, const LaunchCtx&, const GtArgs&);
+// tile-local tensor-core part of the block backward (block_bwd.cu): Delta, dQ complete; dK, dV in-window terms; stat2
+cudaError_t launch_gt_bwd_block(const gnn_plan* P, const GtArgs&, int heads, cudaStream_t);
 cudaError_t launch_gat_fwd(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
 cudaError_t launch_gat_bwd_dst(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
 cudaError_t launch_gat_bwd_src(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);

@@ -215,6 +215,7 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_,
         const float2* stat2;   // (L * log2(e), Delta) per (node, head), written by the dst pass
         float *dk, *dv;
         float kscale, inv_sqrt_d;
+        int accumulate;        // 1: dk / dv already hold a partial result (the tile-local part of the block backward): add to it
     };
     struct Own { Ck k, v; };
 
@@ -266,12 +267,19 @@ template <typename T, int CB_, int G_, int KU_> struct GtBwdSrc : OpBase<T, CB_,
     }
     __device__ __forceinline__ static void finalize(const St& st, const Params& p, const Shape& sh, int row,
                                                     const GeoT& g, float (&)[CH]) {
-        float o[CH];
+        float o[CH], o2[CH];
 #pragma unroll
-        for (int c = 0; c < CH; ++c) o[c] = st.acc[0][c] * p.inv_sqrt_d;
+        for (int c = 0; c < CH; ++c) { o[c] = st.acc[0][c] * p.inv_sqrt_d; o2[c] = st.acc[1][c]; }
+        if (p.accumulate) {      // fixed order (partial already stored + this row's sum): still deterministic, one writer
+            float a[CH], b[CH];
+            load_f32<CH>(p.dk, (size_t)row * sh.ld + g.eoff, g.act, a);
+            load_f32<CH>(p.dv, (size_t)row * sh.ld + g.eoff, g.act, b);
+#pragma unroll
+            for (int c = 0; c < CH; ++c) { o[c] += a[c]; o2[c] += b[c]; }
+        }
         if (g.act) {
             store_f32<CH>(p.dk, (size_t)row * sh.ld + g.eoff, o);
-            store_f32<CH>(p.dv, (size_t)row * sh.ld + g.eoff, st.acc[1]);
+            store_f32<CH>(p.dv, (size_t)row * sh.ld + g.eoff, o2);
         }
     }
 };

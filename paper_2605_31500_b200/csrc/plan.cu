@@ -248,6 +248,7 @@ struct Layout {
     // persistent
     size_t perm, chunks, chunk_ptr, counts, rowptr_t, colidx_t, perm_t, chunks_t, chunk_ptr_t, dev_total;
     size_t blk_bitmap, blk_rem_rowptr, blk_rem_colidx, blk_cnt;
+    size_t rem_rowptr_t, rem_colidx_t, rem_perm_t, rem_chunks_t, rem_chunk_ptr_t;
     size_t wsb_row_offset[2], wsb_cols[2], wsb_bitmap[2];          // [0] CSR, [1] CSR^T (only when the plan stores CSR^T)
     size_t wsb_key, wsb_key_sorted, wsb_nuniq, wsb_win_uptr, wsb_ntcb;  // scratch
     long long max_tcb;
@@ -315,12 +316,23 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
         L.blk_rem_rowptr = take(sizeof(int32_t) * ((size_t)n + 1));
         L.blk_rem_colidx = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
     }
+    // transposed remainder CSR + its bins (tensor-core backward on the diagonal layout: the out-of-window edges of the
+    // source side run through the CSR src pass restricted to this structure)
+    L.rem_rowptr_t = L.rem_colidx_t = L.rem_perm_t = L.rem_chunks_t = L.rem_chunk_ptr_t = 0;
+    const bool rem_t = (o.build_blocks & GNN_BLOCKS_DIAG) && o.build_transpose != 0;
+    if (rem_t) {
+        L.rem_rowptr_t = take(sizeof(int32_t) * ((size_t)n + 1));
+        L.rem_colidx_t = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
+        L.rem_perm_t = take(sizeof(int32_t) * (size_t)n);
+        L.rem_chunks_t = take(sizeof(int32_t) * 4 * (size_t)L.max_chunks);
+        L.rem_chunk_ptr_t = take(sizeof(int32_t) * (size_t)(L.max_hub + 1));
+    }
     L.dev_total = off;
     size_t t1 = 0, t2 = 0, t3 = 0, t4 = 0, t5 = 0, t6 = 0;
     cudaError_t e = cub::DeviceRadixSort::SortPairs(nullptr, t1, (const uint32_t*)nullptr, (uint32_t*)nullptr,
                                                     (const int32_t*)nullptr, (int32_t*)nullptr, (long long)n, 0, 7);
     if (e != cudaSuccess) return e;
-    if (own_t) {
+    if (own_t || rem_t) {
         e = cub::DeviceRadixSort::SortPairs(nullptr, t2, (const uint32_t*)nullptr, (uint32_t*)nullptr,
                                             (const int32_t*)nullptr, (int32_t*)nullptr, (long long)nnz, 0, n_bits(n));
         if (e != cudaSuccess) return e;
@@ -346,7 +358,7 @@ cudaError_t make_layout(int32_t n, int64_t nnz, const gnn_plan_opts_t& o, Layout
     L.key_sorted = take(sizeof(uint32_t) * (size_t)n);
     L.rowid = take(sizeof(int32_t) * (size_t)n);
     L.ekey_sorted = L.erow = 0;
-    if (own_t) {
+    if (own_t || rem_t) {
         L.ekey_sorted = take(sizeof(uint32_t) * (size_t)(nnz > 0 ? nnz : 1));
         L.erow = take(sizeof(int32_t) * (size_t)(nnz > 0 ? nnz : 1));
     }
@@ -558,6 +570,30 @@ extern "C" gnn_status_t gnn_plan_build(gnn_plan_t** plan, void* dev_mem, size_t 
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     P->rem_nnz = rem_nnz;
     P->rows_sorted = unsorted ? 0 : 1;
+    int32_t hr[4] = {0, 0, 0, 0};
+    if (e == cudaSuccess && (o.build_blocks & GNN_BLOCKS_DIAG) && o.build_transpose != 0) {
+        // stable transpose of the remainder CSR (same construction as CSR^T above) and its out-degree bins
+        P->rem_rowptr_t = (int32_t*)(dm + L.rem_rowptr_t);
+        P->rem_colidx_t = (int32_t*)(dm + L.rem_colidx_t);
+        uint32_t* ekey_sorted = (uint32_t*)(sc + L.ekey_sorted);
+        int32_t* erow = (int32_t*)(sc + L.erow);
+        if (rem_nnz > 0) {
+            row_of_edge_kernel<<<(unsigned)((rem_nnz + 255) / 256), 256, 0, st>>>(P->blk_rem_rowptr, n, rem_nnz, erow);
+            count_launch();
+            size_t cb = L.cub_bytes;
+            e = cub::DeviceRadixSort::SortPairs(sc + L.cub, cb, (const uint32_t*)P->blk_rem_colidx, ekey_sorted,
+                                                (const int32_t*)erow, P->rem_colidx_t, (long long)rem_nnz, 0, n_bits(n), st);
+        }
+        if (e == cudaSuccess) {
+            rowptr_t_kernel<<<(n + 1 + 255) / 256, 256, 0, st>>>(ekey_sorted, rem_nnz, n, P->rem_rowptr_t);
+            count_launch();
+            e = build_bins(P->rem_rowptr_t, n, o, L, sc, (int32_t*)(dm + L.rem_perm_t), (int32_t*)(dm + L.rem_chunks_t),
+                           (int32_t*)(dm + L.rem_chunk_ptr_t), counts_dev + 4, hr, st);   // counts slot reused (already read back)
+        }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        P->rem_tr = BinView{(int32_t*)(dm + L.rem_perm_t), (int32_t*)(dm + L.rem_chunks_t), (int32_t*)(dm + L.rem_chunk_ptr_t),
+                            hr[0], hr[1], hr[2], hr[3]};
+    }
     if (P->has_wsb) {
         P->wsb = WsbView{(int32_t*)(dm + L.wsb_row_offset[0]), (int32_t*)(dm + L.wsb_cols[0]), (uint8_t*)(dm + L.wsb_bitmap[0]),
                          wsb_info[0], wsb_info[1]};
@@ -653,12 +689,15 @@ extern "C" gnn_status_t gnn_plan_export(const gnn_plan_t* P, int what, void* hos
         case GNN_PLAN_WSB_ROW_OFFSET_T: if (P->has_wsb && T) { src = P->wsb_t.row_offset; need = 4 * ((size_t)(P->n + 15) / 16 + 1); } break;
         case GNN_PLAN_WSB_COLS_T: if (P->has_wsb && T) { src = P->wsb_t.cols; need = 32 * (size_t)P->wsb_t.n_tcb; } break;
         case GNN_PLAN_WSB_BITMAP_T: if (P->has_wsb && T) { src = P->wsb_t.bitmap; need = 16 * (size_t)P->wsb_t.n_tcb; } break;
+        case GNN_PLAN_BLOCK_REM_ROWPTR_T: if (P->rem_rowptr_t) { src = P->rem_rowptr_t; need = 4 * ((size_t)P->n + 1); } break;
+        case GNN_PLAN_BLOCK_REM_COLIDX_T: if (P->rem_rowptr_t) { src = P->rem_colidx_t; need = 4 * (size_t)P->rem_nnz; } break;
         case GNN_PLAN_BLOCK_BITMAP: if (P->blk_bitmap) { src = P->blk_bitmap; need = 2 * 16 * (size_t)P->n_windows; } break;
         case GNN_PLAN_BLOCK_REM_ROWPTR: if (P->blk_bitmap) { src = P->blk_rem_rowptr; need = 4 * ((size_t)P->n + 1); } break;
         case GNN_PLAN_BLOCK_REM_COLIDX: if (P->blk_bitmap) { src = P->blk_rem_colidx; need = 4 * (size_t)P->rem_nnz; } break;
         default: break;
     }
     if (what == GNN_PLAN_BLOCK_REM_COLIDX && P->blk_bitmap && P->rem_nnz == 0) { *bytes = 0; return GNN_OK; }
+    if (what == GNN_PLAN_BLOCK_REM_COLIDX_T && P->rem_rowptr_t && P->rem_nnz == 0) { *bytes = 0; return GNN_OK; }
     if (what == GNN_PLAN_WSB_INFO) {
         const size_t cap0 = *bytes;
         *bytes = need;

@@ -76,6 +76,42 @@ __device__ __forceinline__ uint32_t canon(int r, int k, int sbo) {
     return (uint32_t)((r & 7) * 16 + (r >> 3) * sbo + (k & 7) * 2 + (k >> 3) * 128);
 }
 
+// Thread-row values leave through the warp's transpose slots (32 slots of D + 4 floats) so that global stores are
+// coalesced 16-byte pieces: every thread fills its slot, then LPR lanes per row write the rows out.  TOUT = float | bf16.
+template <int D, typename TOUT>
+__device__ __forceinline__ void flush_rows(float* sTw, TOUT* __restrict__ dst, size_t ld, int row0w, int n, int lane) {
+    constexpr int TS = D + 4;
+    __syncwarp();
+    constexpr int LPR = D * (int)sizeof(TOUT) / 16;   // lanes per row, 16 bytes each
+    constexpr int RPI = 32 / LPR;                      // rows per iteration
+    const int ch = lane % LPR, rsub = lane / LPR;
+#pragma unroll
+    for (int it = 0; it < LPR; ++it) {
+        const int rl = it * RPI + rsub;
+        const int row = row0w + rl;
+        if (row < n) {
+            if constexpr (sizeof(TOUT) == 4) {
+                const float4 x = *reinterpret_cast<const float4*>(sTw + rl * TS + ch * 4);
+                *reinterpret_cast<float4*>(reinterpret_cast<float*>(dst) + (size_t)row * ld + ch * 4) = x;
+            } else {
+                const float4 x = *reinterpret_cast<const float4*>(sTw + rl * TS + ch * 8);
+                const float4 y = *reinterpret_cast<const float4*>(sTw + rl * TS + ch * 8 + 4);
+                __nv_bfloat162 a = __floats2bfloat162_rn(x.x, x.y), b = __floats2bfloat162_rn(x.z, x.w);
+                __nv_bfloat162 c2 = __floats2bfloat162_rn(y.x, y.y), d2 = __floats2bfloat162_rn(y.z, y.w);
+                uint4 w;
+                w.x = *reinterpret_cast<uint32_t*>(&a); w.y = *reinterpret_cast<uint32_t*>(&b);
+                w.z = *reinterpret_cast<uint32_t*>(&c2); w.w = *reinterpret_cast<uint32_t*>(&d2);
+                *reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(dst) + (size_t)row * ld + ch * 8) = w;
+            }
+        }
+    }
+    __syncwarp();
+}
+__device__ __forceinline__ void slot_write32(float* slot, int c0, const float (&v)[32]) {
+#pragma unroll
+    for (int i = 0; i < 32; i += 4) *reinterpret_cast<float4*>(slot + c0 + i) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+}
+
 // cuTensorMapEncodeTiled through the runtime's driver entry point lookup (the library does not link libcuda)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,

@@ -388,6 +388,50 @@ def test_block_layout_bit_exact():
         assert int(ref["rem_rowptr"][-1]) + int(np.unpackbits(ref["bitmap"].view(np.uint8)).sum()) == colidx.size
 
 
+@pytest.mark.parametrize("heads", [1, 8])
+def test_block_tensor_core_backward(heads):
+    """Tensor-core backward on the diagonal block layout (in-window edges tile-local on tcgen05, every other
+    edge through the remainder CSR / its transpose): Delta, dQ, dK, dV against the oracle on the locally dense config
+    scaled (ragged last tile) and on a multigraph with empty rows, rows without in-window edges, rows with many remainder
+    edges and duplicate entries; the transposed remainder CSR bit-exact vs plan_ref; bit-reproducible."""
+    import paper_2605_31500_b200 as G
+    import paper_2605_31500_b200.binding as B
+    torch = _torch()
+    c4 = GI.make_config(4, scale=0.0041)
+    rng = np.random.default_rng(5)
+    n = 1000
+    dst = rng.integers(0, n, size=9000)
+    src = np.where(rng.random(9000) < 0.6, (dst // 16) * 16 + rng.integers(0, 16, size=9000), rng.integers(0, n, size=9000))
+    src = np.minimum(src, n - 1)
+    keep = (dst % 7 != 0)
+    rp_m, ci_m = GI.csr_from_pairs(n, dst[keep], src[keep], self_loops=False, dedupe=False)
+    cm = _custom("gt", n, rp_m, ci_m, heads, 64, "bf16", seed=11)
+    c4h = _custom("gt", c4["n"], c4["rowptr"], c4["colidx"], heads, 64, "bf16", seed=12)
+    for c in (c4h, cm):
+        nn, H, d = c["n"], c["heads"], c["head_dim"]
+        plan = G.Plan(torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda(), transpose=True, blocks=True)
+        ref = plan_ref.build_blocks(c["rowptr"], c["colidx"])
+        rp_rt, ci_rt = plan_ref.transpose_csr(ref["rem_rowptr"], ref["rem_colidx"])
+        assert np.array_equal(plan.export(B.GNN_PLAN_BLOCK_REM_ROWPTR_T), rp_rt)
+        assert np.array_equal(plan.export(B.GNN_PLAN_BLOCK_REM_COLIDX_T), ci_rt)
+        q, k, v, do = (_dev(c[x + "_st"], "bf16") for x in ("q", "k", "v", "do"))
+        want = oracle_gt(c)
+        lse = torch.from_numpy(want["L"].astype(np.float32)).cuda()       # the backward consumes the forward's L
+        runs = []
+        for _ in range(2):
+            delta = torch.full((nn, H), float("nan"), dtype=torch.float32, device="cuda")
+            dq, dk, dv = (torch.full((nn, H, d), float("nan"), dtype=torch.float32, device="cuda") for _ in range(3))
+            G.gnn_gt_attn_bwd_block(plan, q, k, v, lse, do, delta, dq, dk, dv)
+            torch.cuda.synchronize()
+            runs.append(dict(Delta=_host(delta), dQ=_host(dq), dK=_host(dk), dV=_host(dv)))
+        for key in ("Delta", "dQ", "dK", "dV"):
+            check(f"{c['name']}:block_bwd:{key}", runs[0][key], want[key], "bf16")
+            assert np.array_equal(runs[0][key], runs[1][key]), key
+    plan_nt = G.Plan(torch.from_numpy(c["rowptr"]).cuda(), torch.from_numpy(c["colidx"]).cuda(), transpose=False, blocks=True)
+    with pytest.raises(G.GnnError, match="build_transpose"):
+        G.gnn_gt_attn_bwd_block(plan_nt, q, k, v, lse, do, delta, dq, dk, dv)
+
+
 def _wsb_test_graphs():
     """(name, n, rowptr, colidx): the locally dense config scaled; a simple graph with heavily overlapping column sets
     between windows, a dense window, rows with > 24 distinct sources, empty rows and a ragged last window; a directed
