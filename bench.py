@@ -176,13 +176,17 @@ def quick_config(cfg, args, dev, peak):
         fb = lambda: G.gnn_gt_attn_fwd_block(plan, T["q"], T["k"], T["v"], out, lse)
         fw = lambda: G.gnn_gt_attn_fwd_wsb(plan, T["q"], T["k"], T["v"], out, lse)
         bw = lambda: G.gnn_gt_attn_bwd_wsb(plan, T["q"], T["k"], T["v"], out, lse, T["do"], stat, g1, g2, g3)
+        bb = lambda: G.gnn_gt_attn_bwd_block(plan, T["q"], T["k"], T["v"], lse, T["do"], stat, g1, g2, g3)
         for _ in range(3):
-            fb(); fw(); bw()
+            fb(); fw(); bw(); bb()
         ms_fb, ms_fw, ms_bw = timed(fb, args.steps), timed(fw, args.steps), timed(bw, args.steps)
+        ms_bb, ms_sb = timed(bb, args.steps), timed(lambda: (fb(), bb()), args.steps)
         r["tcgen05_paths"] = {"block_fwd_ms": ms_fb, "block_fwd_compulsory_frac": frac(comp["fwd"], ms_fb),
+                              "block_bwd_ms": ms_bb, "block_bwd_compulsory_frac": frac(comp["bwd"], ms_bb),
+                              "block_step_ms": ms_sb, "block_step_gedges": e / (ms_sb * 1e-3) * 1e-9,
+                              "block_step_compulsory_frac": frac(comp["fwd"] + comp["bwd"], ms_sb),
                               "wsb_fwd_ms": ms_fw, "wsb_bwd_ms": ms_bw, "wsb_info": plan.wsb_info(),
-                              "best_step_ms": min(ms_f, ms_fb, ms_fw) + min(ms_b, ms_bw),
-                              "best_step_gedges": e / ((min(ms_f, ms_fb, ms_fw) + min(ms_b, ms_bw)) * 1e-3) * 1e-9}
+                              "note": "block_* = diagonal block layout (tile-local tcgen05 + remainder CSR), wsb_* = general WSB layout"}
     del T, out, lse, stat, g1, g2, g3, plan, flush
     torch.cuda.empty_cache()
     return r
@@ -618,12 +622,25 @@ def run_ours(args, rank, world, local_rank):
         wsb = {"ms_fwd": float(np.mean(ms_wf)), "ms_bwd": float(np.mean(ms_wb)), "kernels_ms": wk, "info": plan.wsb_info()}
         fwd()   # restore the CSR forward's out / lse for what follows
 
+    def bwd_block():   # cfg 4 only: tensor-core backward on the diagonal block layout (+ remainder CSR passes)
+        G.gnn_gt_attn_bwd_block(plan, devt["q"], devt["k"], devt["v"], lse, devt["do"], stat, g1, g2, g3)
+
     block = None
     if args.cfg == 4:
         for _ in range(3):
             fwd_block()
+            bwd_block()
         ms_blk = timed(fwd_block, args.steps)
-        block = {"ms_fwd": float(np.mean(ms_blk)), "gedges_fwd": e / (np.mean(ms_blk) * 1e-3) * 1e-9}
+        ms_bblk = timed(bwd_block, args.steps)
+        ms_sblk = timed(lambda: (fwd_block(), bwd_block()), args.steps)
+        G.gnn_profile_enable(True)
+        fwd_block()
+        bwd_block()
+        G.gnn_profile_enable(False)
+        bk = {nm: float(ms) for nm, ms in G.gnn_profile_collect(64)}
+        block = {"ms_fwd": float(np.mean(ms_blk)), "gedges_fwd": e / (np.mean(ms_blk) * 1e-3) * 1e-9,
+                 "ms_bwd": float(np.mean(ms_bblk)), "ms_step": float(np.mean(ms_sblk)),
+                 "gedges_step": e / (np.mean(ms_sblk) * 1e-3) * 1e-9, "kernels_ms": bk}
 
     # ---- cfg 1 / 2 are launch-bound (a step is 7-9 launches of a few microseconds each): the same step captured
     # once in a CUDA graph of 100 back-to-back layers and replayed (SURVEY 8(d) timing protocol).  Warm L2 by
