@@ -64,9 +64,7 @@ __device__ __forceinline__ void axpy8(float (&acc)[8], float w, const uint4& r) 
     }
 }
 
-// SRC_LOCAL = true: also the tile-local dK / dV (completed afterwards by the accumulating CSR src pass over the
-// transposed remainder); false: dst side only (Delta, dQ, stat2) - the src side then runs in gt_bwd_block_src_kernel
-template <int D, bool SRC_LOCAL>
+template <int D>
 __global__ void __launch_bounds__(kTile, 2)
 gt_bwd_block_kernel(const __grid_constant__ CUtensorMap tmq, const __grid_constant__ CUtensorMap tmk,
                     const __grid_constant__ CUtensorMap tmv, const __grid_constant__ CUtensorMap tmdo,
@@ -259,17 +257,15 @@ gt_bwd_block_kernel(const __grid_constant__ CUtensorMap tmq, const __grid_consta
             *reinterpret_cast<uint4*>(prow + 128) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
         }
         mma2(sK, 0);
-        if constexpr (SRC_LOCAL) {
-            // dK_block = dS^T Q and dV_block = P^T dO: this row's weights as a COLUMN of the window's block
+        // dK_block = dS^T Q and dV_block = P^T dO: this row's weights as a COLUMN of the window's block
 #pragma unroll
-            for (int c = 0; c < 16; ++c)
-                *reinterpret_cast<__nv_bfloat16*>(sW + canon(16 * wl + c, tid, SBO_W)) = __float2bfloat16_rn(w16[c]);
-            mma2(sQ, 64);
+        for (int c = 0; c < 16; ++c)
+            *reinterpret_cast<__nv_bfloat16*>(sW + canon(16 * wl + c, tid, SBO_W)) = __float2bfloat16_rn(w16[c]);
+        mma2(sQ, 64);
 #pragma unroll
-            for (int c = 0; c < 16; ++c)
-                *reinterpret_cast<__nv_bfloat16*>(sW + canon(16 * wl + c, tid, SBO_W)) = __float2bfloat16_rn(p16[c]);
-            mma2(sdO, 128);
-        }
+        for (int c = 0; c < 16; ++c)
+            *reinterpret_cast<__nv_bfloat16*>(sW + canon(16 * wl + c, tid, SBO_W)) = __float2bfloat16_rn(p16[c]);
+        mma2(sdO, 128);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
         // ---- dQ: block part through the transpose slots, remainder terms and the store by 8 lanes per row
@@ -339,7 +335,7 @@ gt_bwd_block_kernel(const __grid_constant__ CUtensorMap tmq, const __grid_consta
         __syncwarp();
         // ---- tile-local dK, dV (the remainder src pass adds the out-of-window terms afterwards)
 #pragma unroll
-        for (int which = 0; which < (SRC_LOCAL ? 2 : 0); ++which) {
+        for (int which = 0; which < 2; ++which) {
 #pragma unroll
             for (int c0 = 0; c0 < D; c0 += 32) {
                 float t32[32];
@@ -359,10 +355,9 @@ gt_bwd_block_kernel(const __grid_constant__ CUtensorMap tmq, const __grid_consta
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(tmem) : "memory");
 }
 
-//@@KERNELB@@
 }  // namespace
 
-cudaError_t launch_gt_bwd_block(const gnn_plan* P, const GtArgs& a, int heads, bool src_local, cudaStream_t st) {
+cudaError_t launch_gt_bwd_block(const gnn_plan* P, const GtArgs& a, int heads, cudaStream_t st) {
     constexpr int D = 64;
     const int n = P->n;
     CUtensorMap tmq, tmk, tmv, tmdo;
@@ -375,30 +370,13 @@ cudaError_t launch_gt_bwd_block(const gnn_plan* P, const GtArgs& a, int heads, b
     p.rem_rowptr = P->blk_rem_rowptr; p.rem_colidx = P->blk_rem_colidx;
     p.dq = a.dq; p.dk = a.dk; p.dv = a.dv; p.delta = a.delta; p.stat2 = a.stat2;
     p.n = n; p.H = heads; p.sscale = kLog2e / sqrtf((float)D); p.inv_sqrt_d = 1.f / sqrtf((float)D);
-    const size_t smem = 4 * (size_t)kHT + kWBytes + 32 + 2 * kTile * 8 + 1024;
-    const int grid = (n + kTile - 1) / kTile;
-    cudaError_t e;
-    if (src_local) {
-        e = cudaFuncSetAttribute(gt_bwd_block_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        prof_begin("gt_bwd_block", "tile", st);
-        gt_bwd_block_kernel<D, true><<<grid, kTile, smem, st>>>(tmq, tmk, tmv, tmdo, p);
-        prof_end(st);
-        count_launch();
-        return cudaGetLastError();
-    }
-    e = cudaFuncSetAttribute(gt_bwd_block_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(gt_bwd_block_src_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const size_t smem = 4 * (size_t)kHT + kWBytes + 32 + 2 * kTile * 4 + 1024;
+    cudaError_t e = cudaFuncSetAttribute(gt_bwd_block_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    prof_begin("gt_bwd_block", "tile_dst", st);
-    gt_bwd_block_kernel<D, false><<<grid, kTile, smem, st>>>(tmq, tmk, tmv, tmdo, p);
+    prof_begin("gt_bwd_block", "tile", st);
+    gt_bwd_block_kernel<D><<<(n + kTile - 1) / kTile, kTile, smem, st>>>(tmq, tmk, tmv, tmdo, p);
     prof_end(st);
-    p.rem_rowptr = P->rem_rowptr_t;      // the src side walks the transposed remainder
-    p.rem_colidx = P->rem_colidx_t;
-    prof_begin("gt_bwd_block", "tile_src", st);
-    gt_bwd_block_src_kernel<D><<<grid, kTile, smem, st>>>(tmq, tmk, tmv, tmdo, p);
-    prof_end(st);
-    count_launch(2);
+    count_launch();
     return cudaGetLastError();
 }
 

@@ -139,8 +139,7 @@ cudaError_t launch_gt_fwd(int dtype, const Shape&, const LaunchCtx&, const GtArg
 cudaError_t launch_gt_bwd_dst(int dtype, const Shape&, const LaunchCtx&, const GtArgs&);
 cudaError_t launch_gt_bwd_src(int dtype, const Shape&, const LaunchCtx&, const GtArgs&);
 // tile-local tensor-core part of the block backward (block_bwd.cu): Delta, dQ complete; dK, dV in-window terms; stat2
-// src_local = false: two tile kernels (dst side; src side over the transposed remainder), dK / dV written once
-cudaError_t launch_gt_bwd_block(const gnn_plan* P, const GtArgs&, int heads, bool src_local, cudaStream_t);
+cudaError_t launch_gt_bwd_block(const gnn_plan* P, const GtArgs&, int heads, cudaStream_t);
 cudaError_t launch_gat_fwd(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
 cudaError_t launch_gat_bwd_dst(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
 cudaError_t launch_gat_bwd_src(int dtype, const Shape&, const LaunchCtx&, const GatArgs&);
