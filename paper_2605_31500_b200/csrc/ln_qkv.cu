@@ -5,6 +5,7 @@
 //   y[i, :] = (x[i, :] - mean_i) / sqrt(var_i + eps) * gamma + beta        (biased variance over the C features)
 //   [Q | K | V][i, :] = y[i, :] W^T + bias,   W = [W_Q; W_K; W_V] of shape [3*H*d, C]
 //
+// (Round-2 layout: 320 threads - eight LayerNorm / epilogue warps, two per TMEM lane quarter - see below.)
 // The paper runs these as stock PyTorch ops (LayerNorm kernel, cuBLAS GEMM: one write and one read of the normalised
 // activations in HBM).  Here one CTA owns 128 rows: warps 0-3 normalise their rows in registers (a warp per row,
 // 16-byte loads, shuffle reductions) and write them as bf16 straight into the 128-byte-swizzled K-major shared-memory
@@ -27,8 +28,9 @@ using namespace tc;
 constexpr int kRows = 128;          // rows per CTA = MMA M
 constexpr int kNC = 128;            // output columns per chunk = MMA N
 constexpr int kStage = 16384;       // bytes of a weight stage / of a 64-channel half tile of A
-constexpr int kThreads = 192;       // warps 0-3: LayerNorm + epilogue, warp 4: TMA, warp 5: MMA
-constexpr int kSlot = 80;           // bytes of a transpose slot: 32 bf16 + 16 (conflict-free 16-byte writes)
+constexpr int kWorkWarps = 8;        // warps 0-7: LayerNorm + epilogue (two warps per TMEM lane quarter, one column half each)
+constexpr int kThreads = 320;       // + warp 8: TMA, warp 9: MMA
+constexpr int kSlot = 48;           // bytes of a transpose slot: 16 bf16 + 16 (conflict-free 16-byte writes)
 
 struct LnQkvParams {
     const __nv_bfloat16* x;
@@ -56,7 +58,7 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
     uint8_t* sA = smem;                                   // [KC] half tiles, 128 rows x 128 bytes, SWIZZLE_128B
     uint8_t* sB = sA + KC * kStage;                       // [NS] weight stages
     uint8_t* sT = sB + NS * kStage;                       // [128] transpose slots
-    uint64_t* full = reinterpret_cast<uint64_t*>(sT + kRows * kSlot);   // [NS] TMA landed
+    uint64_t* full = reinterpret_cast<uint64_t*>(sT + kWorkWarps * 32 * kSlot);   // [NS] TMA landed
     uint64_t* empty = full + 8;                           // [NS] stage consumed (tcgen05.commit)
     uint64_t* tfull = empty + 8;                          // [2] accumulator complete
     uint64_t* tempty = tfull + 2;                         // [2] accumulator drained
@@ -68,10 +70,10 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
 
     if (tid == 0) {
         for (int s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
-        for (int b = 0; b < 2; ++b) { mbar_init(tfull + b, 1); mbar_init(tempty + b, 4); }
+        for (int b = 0; b < 2; ++b) { mbar_init(tfull + b, 1); mbar_init(tempty + b, kWorkWarps); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 5) {
+    if (warp == 9) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" ::"r"(smem_u32(tmem_slot)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -80,7 +82,7 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = *tmem_slot;
 
-    if (warp == 4) {
+    if (warp == 8) {
         // ===== TMA producer: weight stage i = (chunk c, channel block kk) -> ring slot i % NS
         // (the first NS stages go out now and overlap the LayerNorm; the rest after the A tile barrier below, because
         // their slots are only released by the MMA warp, which starts behind that barrier)
@@ -91,8 +93,8 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
                 tma_load_2d(sB + i * kStage, &tmw, (i % KC) * 64, (i / KC) * kNC, full + i);
             }
         }
-    } else if (warp < 4) {
-        // ===== LayerNorm of this warp's 32 rows into the A tile (lane <-> 16-byte chunks lane, lane + 32)
+    } else if (warp < kWorkWarps) {
+        // ===== LayerNorm of this warp's 16 rows into the A tile (lane <-> 16-byte chunks lane, lane + 32)
         const int nchunk = p.C / 8;
         float g[2][8], b[2][8];
 #pragma unroll
@@ -105,20 +107,20 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
             }
         }
         const float inv_c = 1.f / (float)p.C;
-        constexpr int RB = 8;                 // rows in flight per warp: the loads of 8 rows are issued before the first reduction
-        for (int rl = 0; rl < 32; rl += RB) {
+        constexpr int RB = 4;                 // rows in flight per warp: the loads of 4 rows are issued before the first reduction
+        for (int rl = 0; rl < 16; rl += RB) {
             uint4 raw[RB][2];
 #pragma unroll
             for (int u = 0; u < RB; ++u)
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
-                    const int row = row0 + warp * 32 + rl + u, cc = lane + 32 * j;
+                    const int row = row0 + warp * 16 + rl + u, cc = lane + 32 * j;
                     raw[u][j] = make_uint4(0, 0, 0, 0);
                     if (row < p.n && cc < nchunk) raw[u][j] = __ldg(reinterpret_cast<const uint4*>(p.x + (size_t)row * p.C) + cc);
                 }
 #pragma unroll
             for (int u = 0; u < RB; ++u) {
-                const int r = warp * 32 + rl + u;
+                const int r = warp * 16 + rl + u;
                 float v[2][8];
                 float s = 0.f;
 #pragma unroll
@@ -166,7 +168,7 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
     }
     __syncthreads();   // the A tile is complete and visible to the tensor core
 
-    if (warp == 4) {
+    if (warp == 8) {
         if (lane == 0) {
             const int items = n_chunks * KC;
             for (int i = NS; i < items; ++i) {
@@ -176,7 +178,7 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
                 tma_load_2d(sB + s * kStage, &tmw, kk * 64, c * kNC, full + s);
             }
         }
-    } else if (warp == 5) {
+    } else if (warp == 9) {
         // ===== MMA issuer
         if (lane == 0) {
             constexpr uint32_t kIdesc = make_idesc(kRows, kNC, false);
@@ -198,23 +200,26 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
                 umma_commit(tfull + bsel);
             }
         }
-    } else if (warp < 4) {
-        // ===== epilogue: accumulator -> + bias -> bf16 -> transpose slot -> coalesced 16-byte stores
-        const uint32_t t_lane = tmem + ((uint32_t)(warp * 32) << 16);
-        uint8_t* slot = sT + tid * kSlot;
+    } else if (warp < kWorkWarps) {
+        // ===== epilogue: warp w drains TMEM lanes 32 (w & 3) .. +31 (tile rows) of column half w >> 2 of every chunk:
+        // accumulator -> + bias -> bf16 -> 16-column transpose slots -> coalesced 16-byte stores
+        const int q4 = warp & 3, hsel = warp >> 2;
+        const uint32_t t_lane = tmem + ((uint32_t)(q4 * 32) << 16);
+        uint8_t* slots = sT + warp * 32 * kSlot;
+        uint8_t* slot = slots + lane * kSlot;
+        const int ch = lane & 1, rsub = lane >> 1;
         for (int c = 0; c < n_chunks; ++c) {
             const int bsel = c & 1;
             mbar_wait(tfull + bsel, (uint32_t)((c >> 1) & 1));
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const int col0 = c * kNC;
+            const int col0 = c * kNC + 64 * hsel;
             const int t = col0 / p.R, off = col0 - t * p.R;
             __nv_bfloat16* dst = (t == 0 ? p.q : (t == 1 ? p.k : p.v)) + off;
-            const int ch = lane & 3, rsub = lane >> 2;
 #pragma unroll 1
-            for (int c0 = 0; c0 < kNC; c0 += 32) {
+            for (int c0 = 0; c0 < 64; c0 += 32) {
                 float t32[32];
-                tmem_ld32(t_lane + bsel * kNC + c0, t32);
-                if (c0 + 32 == kNC) {                           // last read of this accumulator: hand it back to the MMA warp
+                tmem_ld32(t_lane + bsel * kNC + 64 * hsel + c0, t32);
+                if (c0 == 32) {                                 // last read of this accumulator half: hand it back to the MMA warp
                     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
                     __syncwarp();
                     if (lane == 0) mbar_arrive(tempty + bsel);
@@ -226,32 +231,35 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
                         t32[i] += bb.x; t32[i + 1] += bb.y; t32[i + 2] += bb.z; t32[i + 3] += bb.w;
                     }
                 }
-                uint32_t o[16];
 #pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    const __nv_bfloat162 yb = __floats2bfloat162_rn(t32[2 * i], t32[2 * i + 1]);
-                    o[i] = *reinterpret_cast<const uint32_t*>(&yb);
-                }
+                for (int g16 = 0; g16 < 2; ++g16) {
+                    uint32_t o[8];
 #pragma unroll
-                for (int i = 0; i < 16; i += 4) *reinterpret_cast<uint4*>(slot + i * 4) = make_uint4(o[i], o[i + 1], o[i + 2], o[i + 3]);
-                __syncwarp();
-                // rows of this warp, 4 lanes per 64-byte row piece, 8 rows per instruction
-#pragma unroll
-                for (int it = 0; it < 4; ++it) {
-                    const int rl = it * 8 + rsub;
-                    const int row = row0 + warp * 32 + rl;
-                    if (row < p.n) {
-                        const uint4 w = *reinterpret_cast<const uint4*>(sT + (warp * 32 + rl) * kSlot + ch * 16);
-                        *reinterpret_cast<uint4*>(dst + (size_t)row * p.R + c0 + ch * 8) = w;
+                    for (int i = 0; i < 8; ++i) {
+                        const __nv_bfloat162 yb = __floats2bfloat162_rn(t32[16 * g16 + 2 * i], t32[16 * g16 + 2 * i + 1]);
+                        o[i] = *reinterpret_cast<const uint32_t*>(&yb);
                     }
+                    *reinterpret_cast<uint4*>(slot) = make_uint4(o[0], o[1], o[2], o[3]);
+                    *reinterpret_cast<uint4*>(slot + 16) = make_uint4(o[4], o[5], o[6], o[7]);
+                    __syncwarp();
+                    // 2 lanes per 32-byte row piece, 16 rows per instruction
+#pragma unroll
+                    for (int it = 0; it < 2; ++it) {
+                        const int rl = it * 16 + rsub;
+                        const int row = row0 + q4 * 32 + rl;
+                        if (row < p.n) {
+                            const uint4 w = *reinterpret_cast<const uint4*>(slots + rl * kSlot + ch * 16);
+                            *reinterpret_cast<uint4*>(dst + (size_t)row * p.R + c0 + 16 * g16 + ch * 8) = w;
+                        }
+                    }
+                    __syncwarp();
                 }
-                __syncwarp();
             }
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 5) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(tmem) : "memory");
+    if (warp == 9) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(tmem) : "memory");
 }
 
 }  // namespace
@@ -285,7 +293,7 @@ extern "C" gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, i
     p.q = (__nv_bfloat16*)q; p.k = (__nv_bfloat16*)k; p.v = (__nv_bfloat16*)v;
     p.n = n; p.C = c_in; p.R = (int)R; p.eps = eps;
     // weight ring: as many 16 KB stages as keep two CTAs per SM (113 KB each) when the A tile allows it, else one CTA
-    const size_t fixed = (size_t)(c_in / 64) * kStage + (size_t)kRows * kSlot + 256 + 1024;
+    const size_t fixed = (size_t)(c_in / 64) * kStage + (size_t)kWorkWarps * 32 * kSlot + 256 + 1024;
     const size_t budget = fixed + 2 * kStage <= 113 * 1024 ? 113 * 1024 : 226 * 1024;
     p.n_stages = (int)((budget - fixed) / kStage);
     if (p.n_stages > 8) p.n_stages = 8;
