@@ -30,7 +30,8 @@ constexpr int kNC = 128;            // output columns per chunk = MMA N
 constexpr int kStage = 16384;       // bytes of a weight stage / of a 64-channel half tile of A
 constexpr int kWorkWarps = 8;        // warps 0-7: LayerNorm + epilogue (two warps per TMEM lane quarter, one column half each)
 constexpr int kThreads = 320;       // + warp 8: TMA, warp 9: MMA
-constexpr int kSlot = 48;           // bytes of a transpose slot: 16 bf16 + 16 (conflict-free 16-byte writes)
+constexpr int kOut = 1024;          // bytes of an output staging buffer: 32 rows x 16 bf16 columns (two per worker warp)
+constexpr int kBars = 256;          // mbarriers + TMEM slot, in front of the 1024-byte aligned tiles
 
 struct LnQkvParams {
     const __nv_bfloat16* x;
@@ -51,26 +52,36 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 __global__ void __launch_bounds__(kThreads, 2)
-ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
+ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmw,
+              const __grid_constant__ CUtensorMap tmq, const __grid_constant__ CUtensorMap tmk,
+              const __grid_constant__ CUtensorMap tmv, const LnQkvParams p) {
     extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    // [barriers, kBars bytes][pad to 1024][A: KC half tiles][NS weight stages][16 output staging buffers]
+    uint8_t* smem = smem_raw + kBars + ((1024u - ((smem_u32(smem_raw) + kBars) & 1023u)) & 1023u);
     const int KC = p.C / 64, NS = p.n_stages;
     uint8_t* sA = smem;                                   // [KC] half tiles, 128 rows x 128 bytes, SWIZZLE_128B
     uint8_t* sB = sA + KC * kStage;                       // [NS] weight stages
-    uint8_t* sT = sB + NS * kStage;                       // [128] transpose slots
-    uint64_t* full = reinterpret_cast<uint64_t*>(sT + kWorkWarps * 32 * kSlot);   // [NS] TMA landed
+    uint8_t* sT = sB + NS * kStage;                       // [kWorkWarps][2] staging buffers, 32 rows x 32 bytes, SWIZZLE_32B
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);   // [NS] TMA landed
     uint64_t* empty = full + 8;                           // [NS] stage consumed (tcgen05.commit)
     uint64_t* tfull = empty + 8;                          // [2] accumulator complete
     uint64_t* tempty = tfull + 2;                         // [2] accumulator drained
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+    uint64_t* xfull = tempty + 2;                         // raw x tile landed
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(xfull + 1);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int row0 = blockIdx.x * kRows;
+    {   // the host sizes the allocation for a 1024-byte aligned base (pad + barriers = 1024); refuse anything else loudly
+        uint32_t dyn;
+        asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
+        if ((uint32_t)(sT + kWorkWarps * 2 * kOut - smem_raw) > dyn) __trap();
+    }
     const int n_chunks = 3 * p.R / kNC;
 
     if (tid == 0) {
         for (int s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
         for (int b = 0; b < 2; ++b) { mbar_init(tfull + b, 1); mbar_init(tempty + b, kWorkWarps); }
+        mbar_init(xfull, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 9) {
@@ -87,6 +98,9 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
         // (the first NS stages go out now and overlap the LayerNorm; the rest after the A tile barrier below, because
         // their slots are only released by the MMA warp, which starts behind that barrier)
         if (lane == 0) {
+            // the raw x tile lands in the A tile's own layout (TMA applies the 128-byte swizzle); it is normalised in place
+            mbar_expect_tx(xfull, KC * kStage);
+            for (int kk = 0; kk < KC; ++kk) tma_load_2d(sA + kk * kStage, &tmx, kk * 64, row0, xfull);
             const int items = n_chunks * KC;
             for (int i = 0; i < items && i < NS; ++i) {
                 mbar_expect_tx(full + i, kStage);
@@ -107,16 +121,19 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
             }
         }
         const float inv_c = 1.f / (float)p.C;
-        constexpr int RB = 4;                 // rows in flight per warp: the loads of 4 rows are issued before the first reduction
+        mbar_wait(xfull, 0);
+        constexpr int RB = 4;                 // rows per batch (independent shuffle-reduction chains)
         for (int rl = 0; rl < 16; rl += RB) {
             uint4 raw[RB][2];
 #pragma unroll
             for (int u = 0; u < RB; ++u)
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
-                    const int row = row0 + warp * 16 + rl + u, cc = lane + 32 * j;
+                    const int r = warp * 16 + rl + u, cc = lane + 32 * j;
                     raw[u][j] = make_uint4(0, 0, 0, 0);
-                    if (row < p.n && cc < nchunk) raw[u][j] = __ldg(reinterpret_cast<const uint4*>(p.x + (size_t)row * p.C) + cc);
+                    if (cc < nchunk)
+                        raw[u][j] = *reinterpret_cast<const uint4*>(sA + (cc >> 3) * kStage + (r >> 3) * 1024 + (r & 7) * 128 +
+                                                                    (((cc & 7) ^ (r & 7)) << 4));
                 }
 #pragma unroll
             for (int u = 0; u < RB; ++u) {
@@ -202,21 +219,27 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
         }
     } else if (warp < kWorkWarps) {
         // ===== epilogue: warp w drains TMEM lanes 32 (w & 3) .. +31 (tile rows) of column half w >> 2 of every chunk:
-        // accumulator -> + bias -> bf16 -> 16-column transpose slots -> coalesced 16-byte stores
+        // accumulator -> + bias -> bf16 -> 32-row x 16-column staging buffer (the layout TMA's 32-byte swizzle expects)
+        // -> one TMA store per buffer (rows past n are clipped by the unit); two buffers per warp alternate
         const int q4 = warp & 3, hsel = warp >> 2;
         const uint32_t t_lane = tmem + ((uint32_t)(q4 * 32) << 16);
-        uint8_t* slots = sT + warp * 32 * kSlot;
-        uint8_t* slot = slots + lane * kSlot;
-        const int ch = lane & 1, rsub = lane >> 1;
+        uint8_t* stage = sT + warp * 2 * kOut;
+        const uint32_t my = (uint32_t)lane * 32, sw = ((uint32_t)(lane >> 2) & 1u) << 4;
+        int n_st = 0;
         for (int c = 0; c < n_chunks; ++c) {
             const int bsel = c & 1;
-            mbar_wait(tfull + bsel, (uint32_t)((c >> 1) & 1));
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const int col0 = c * kNC + 64 * hsel;
             const int t = col0 / p.R, off = col0 - t * p.R;
-            __nv_bfloat16* dst = (t == 0 ? p.q : (t == 1 ? p.k : p.v)) + off;
+            const CUtensorMap* tmo = t == 0 ? &tmq : (t == 1 ? &tmk : &tmv);
+            mbar_wait(tfull + bsel, (uint32_t)((c >> 1) & 1));
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
             for (int c0 = 0; c0 < 64; c0 += 32) {
+                float4 bb[8];
+                if (p.bias) {
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) bb[i] = __ldg(reinterpret_cast<const float4*>(p.bias + col0 + c0) + i);
+                }
                 float t32[32];
                 tmem_ld32(t_lane + bsel * kNC + 64 * hsel + c0, t32);
                 if (c0 == 32) {                                 // last read of this accumulator half: hand it back to the MMA warp
@@ -226,36 +249,35 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmw, const LnQkvParams p) {
                 }
                 if (p.bias) {
 #pragma unroll
-                    for (int i = 0; i < 32; i += 4) {
-                        const float4 bb = __ldg(reinterpret_cast<const float4*>(p.bias + col0 + c0 + i));
-                        t32[i] += bb.x; t32[i + 1] += bb.y; t32[i + 2] += bb.z; t32[i + 3] += bb.w;
+                    for (int i = 0; i < 8; ++i) {
+                        t32[4 * i] += bb[i].x; t32[4 * i + 1] += bb[i].y; t32[4 * i + 2] += bb[i].z; t32[4 * i + 3] += bb[i].w;
                     }
                 }
 #pragma unroll
-                for (int g16 = 0; g16 < 2; ++g16) {
+                for (int g16 = 0; g16 < 2; ++g16, ++n_st) {
+                    uint8_t* buf = stage + (n_st & 1) * kOut;
+                    if (n_st >= 2) {                            // the store issued from this buffer two groups ago has read it
+                        if (lane == 0) tma_store_wait_read<1>();
+                        __syncwarp();
+                    }
                     uint32_t o[8];
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         const __nv_bfloat162 yb = __floats2bfloat162_rn(t32[16 * g16 + 2 * i], t32[16 * g16 + 2 * i + 1]);
                         o[i] = *reinterpret_cast<const uint32_t*>(&yb);
                     }
-                    *reinterpret_cast<uint4*>(slot) = make_uint4(o[0], o[1], o[2], o[3]);
-                    *reinterpret_cast<uint4*>(slot + 16) = make_uint4(o[4], o[5], o[6], o[7]);
+                    *reinterpret_cast<uint4*>(buf + my + sw) = make_uint4(o[0], o[1], o[2], o[3]);
+                    *reinterpret_cast<uint4*>(buf + my + (sw ^ 16u)) = make_uint4(o[4], o[5], o[6], o[7]);
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                     __syncwarp();
-                    // 2 lanes per 32-byte row piece, 16 rows per instruction
-#pragma unroll
-                    for (int it = 0; it < 2; ++it) {
-                        const int rl = it * 16 + rsub;
-                        const int row = row0 + q4 * 32 + rl;
-                        if (row < p.n) {
-                            const uint4 w = *reinterpret_cast<const uint4*>(slots + rl * kSlot + ch * 16);
-                            *reinterpret_cast<uint4*>(dst + (size_t)row * p.R + c0 + 16 * g16 + ch * 8) = w;
-                        }
+                    if (lane == 0) {
+                        tma_store_2d(tmo, off + c0 + 16 * g16, row0 + 32 * q4, buf);
+                        tma_store_commit();
                     }
-                    __syncwarp();
                 }
             }
         }
+        if (lane == 0) tma_store_wait<0>();
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -283,8 +305,11 @@ extern "C" gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, i
                   who, c_in, heads, head_dim);
         return GNN_EUNSUPPORTED;
     }
-    CUtensorMap tmw;
-    if (!tc::encode_row_tile_map(&tmw, w, (int)(3 * R), c_in, 64, kNC)) {
+    CUtensorMap tmx, tmw, tmq, tmk, tmv;
+    if (!tc::encode_row_tile_map(&tmx, x, n, c_in, 64, kRows) || !tc::encode_row_tile_map(&tmw, w, (int)(3 * R), c_in, 64, kNC) ||
+        !tc::encode_row_tile_map(&tmq, q, n, (int)R, 16, 32, CU_TENSOR_MAP_SWIZZLE_32B) ||
+        !tc::encode_row_tile_map(&tmk, k, n, (int)R, 16, 32, CU_TENSOR_MAP_SWIZZLE_32B) ||
+        !tc::encode_row_tile_map(&tmv, v, n, (int)R, 16, 32, CU_TENSOR_MAP_SWIZZLE_32B)) {
         set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who);
         return GNN_ECUDA;
     }
@@ -293,7 +318,7 @@ extern "C" gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, i
     p.q = (__nv_bfloat16*)q; p.k = (__nv_bfloat16*)k; p.v = (__nv_bfloat16*)v;
     p.n = n; p.C = c_in; p.R = (int)R; p.eps = eps;
     // weight ring: as many 16 KB stages as keep two CTAs per SM (113 KB each) when the A tile allows it, else one CTA
-    const size_t fixed = (size_t)(c_in / 64) * kStage + (size_t)kWorkWarps * 32 * kSlot + 256 + 1024;
+    const size_t fixed = (size_t)(c_in / 64) * kStage + (size_t)kWorkWarps * 2 * kOut + 1024;   // 1024 = barriers + alignment pad
     const size_t budget = fixed + 2 * kStage <= 113 * 1024 ? 113 * 1024 : 226 * 1024;
     p.n_stages = (int)((budget - fixed) / kStage);
     if (p.n_stages > 8) p.n_stages = 8;
@@ -302,7 +327,7 @@ extern "C" gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, i
     if (e == cudaSuccess) {
         cudaStream_t st = (cudaStream_t)stream;
         prof_begin("ln_qkv", "gemm", st);
-        ln_qkv_kernel<<<(n + kRows - 1) / kRows, kThreads, smem, st>>>(tmw, p);
+        ln_qkv_kernel<<<(n + kRows - 1) / kRows, kThreads, smem, st>>>(tmx, tmw, tmq, tmk, tmv, p);
         prof_end(st);
         count_launch();
         e = cudaGetLastError();
