@@ -45,12 +45,12 @@ struct LnQkvParams {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ float warp_sum(float v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
+__device__ __forceinline__ void add2(float& a0, float& a1, float x0, float x1) {      // (a0, a1) += (x0, x1), one FADD2
+    asm("{\n .reg .b64 xx, cc;\n mov.b64 xx, {%2, %3};\n mov.b64 cc, {%0, %1};\n add.rn.f32x2 cc, cc, xx;\n mov.b64 {%0, %1}, cc;\n}"
+        : "+f"(a0), "+f"(a1) : "f"(x0), "f"(x1));
 }
 
+template <int NJ>     // 16-byte chunks of a row per lane: 1 for C <= 256, 2 for C <= 512
 __global__ void __launch_bounds__(kThreads, 2)
 ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmw,
               const __grid_constant__ CUtensorMap tmq, const __grid_constant__ CUtensorMap tmk,
@@ -108,75 +108,89 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ C
             }
         }
     } else if (warp < kWorkWarps) {
-        // ===== LayerNorm of this warp's 16 rows into the A tile (lane <-> 16-byte chunks lane, lane + 32)
+        // ===== LayerNorm of this warp's 16 rows, in place in the A tile (lane <-> 16-byte chunks lane [, lane + 32]).
+        // bf16 operands enter the fp32 sums directly (FHADD takes a register half: no unpack); squares, scale and shift
+        // run as packed fp32 pairs (FFMA2 / FMUL2).
         const int nchunk = p.C / 8;
-        float g[2][8], b[2][8];
+        float g[NJ][8], b[NJ][8];
+        bool on[NJ];
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
+        for (int j = 0; j < NJ; ++j) {
             const int cc = lane + 32 * j;
+            on[j] = cc < nchunk;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                g[j][i] = cc < nchunk ? __ldg(p.gamma + cc * 8 + i) : 0.f;
-                b[j][i] = cc < nchunk ? __ldg(p.beta + cc * 8 + i) : 0.f;
+                g[j][i] = on[j] ? __ldg(p.gamma + cc * 8 + i) : 0.f;
+                b[j][i] = on[j] ? __ldg(p.beta + cc * 8 + i) : 0.f;
             }
         }
         const float inv_c = 1.f / (float)p.C;
         mbar_wait(xfull, 0);
-        constexpr int RB = 4;                 // rows per batch (independent shuffle-reduction chains)
+        constexpr int RB = NJ == 1 ? 4 : 2;   // rows per batch (independent shuffle-reduction chains)
         for (int rl = 0; rl < 16; rl += RB) {
-            uint4 raw[RB][2];
+            uint4 raw[RB][NJ];
+            uint32_t addr[RB][NJ];
+            float s[RB];
 #pragma unroll
-            for (int u = 0; u < RB; ++u)
+            for (int u = 0; u < RB; ++u) {
+                float s0 = 0.f, s1 = 0.f;
 #pragma unroll
-                for (int j = 0; j < 2; ++j) {
+                for (int j = 0; j < NJ; ++j) {
                     const int r = warp * 16 + rl + u, cc = lane + 32 * j;
+                    addr[u][j] = (uint32_t)((cc >> 3) * kStage + (r >> 3) * 1024 + (r & 7) * 128 + (((cc & 7) ^ (r & 7)) << 4));
                     raw[u][j] = make_uint4(0, 0, 0, 0);
-                    if (cc < nchunk)
-                        raw[u][j] = *reinterpret_cast<const uint4*>(sA + (cc >> 3) * kStage + (r >> 3) * 1024 + (r & 7) * 128 +
-                                                                    (((cc & 7) ^ (r & 7)) << 4));
+                    if (on[j]) raw[u][j] = *reinterpret_cast<const uint4*>(sA + addr[u][j]);
+                    add_bf16x2(raw[u][j].x, s0, s1, s0, s1);
+                    add_bf16x2(raw[u][j].y, s0, s1, s0, s1);
+                    add_bf16x2(raw[u][j].z, s0, s1, s0, s1);
+                    add_bf16x2(raw[u][j].w, s0, s1, s0, s1);
                 }
+                s[u] = s0 + s1;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                for (int u = 0; u < RB; ++u) s[u] += __shfl_xor_sync(0xffffffffu, s[u], o);
+            float v[RB][NJ][8], ss[RB];
+#pragma unroll
+            for (int u = 0; u < RB; ++u) {
+                const float nmean = -s[u] * inv_c;
+                float q0 = 0.f, q1 = 0.f;
+#pragma unroll
+                for (int j = 0; j < NJ; ++j) {
+                    const uint32_t w[4] = {raw[u][j].x, raw[u][j].y, raw[u][j].z, raw[u][j].w};
+                    const float nm = on[j] ? nmean : 0.f;     // lanes past the row's last chunk hold zeros and stay zero
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        add_bf16x2(w[i], nm, nm, v[u][j][2 * i], v[u][j][2 * i + 1]);
+                        fma2v(q0, q1, v[u][j][2 * i], v[u][j][2 * i + 1], v[u][j][2 * i], v[u][j][2 * i + 1]);
+                    }
+                }
+                ss[u] = q0 + q1;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                for (int u = 0; u < RB; ++u) ss[u] += __shfl_xor_sync(0xffffffffu, ss[u], o);
 #pragma unroll
             for (int u = 0; u < RB; ++u) {
                 const int r = warp * 16 + rl + u;
-                float v[2][8];
-                float s = 0.f;
-#pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    const uint32_t w[4] = {raw[u][j].x, raw[u][j].y, raw[u][j].z, raw[u][j].w};
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        v[j][2 * i] = __uint_as_float(w[i] << 16);
-                        v[j][2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
-                        s += v[j][2 * i] + v[j][2 * i + 1];
-                    }
-                }
-                const float mean = warp_sum(s) * inv_c;
-                float ss = 0.f;
-#pragma unroll
-                for (int j = 0; j < 2; ++j)
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const bool on = lane + 32 * j < nchunk;
-                        v[j][i] = on ? v[j][i] - mean : 0.f;
-                        ss = fmaf(v[j][i], v[j][i], ss);
-                    }
-                const float rstd = 1.f / sqrtf(warp_sum(ss) * inv_c + p.eps);
+                const float rstd = row0 + r < p.n ? 1.f / sqrtf(ss[u] * inv_c + p.eps) : 0.f;
                 const bool rv = row0 + r < p.n;
 #pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    const int cc = lane + 32 * j;
-                    if (cc < nchunk) {
+                for (int j = 0; j < NJ; ++j) {
+                    if (on[j]) {
                         uint32_t o[4];
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
-                            const float y0 = rv ? fmaf(v[j][2 * i] * rstd, g[j][2 * i], b[j][2 * i]) : 0.f;
-                            const float y1 = rv ? fmaf(v[j][2 * i + 1] * rstd, g[j][2 * i + 1], b[j][2 * i + 1]) : 0.f;
-                            const __nv_bfloat162 yb = __floats2bfloat162_rn(y0, y1);
+                            float y0 = v[u][j][2 * i], y1 = v[u][j][2 * i + 1];
+                            mul2(y0, y1, rstd);
+                            float z0 = rv ? b[j][2 * i] : 0.f, z1 = rv ? b[j][2 * i + 1] : 0.f;
+                            fma2v(z0, z1, y0, y1, g[j][2 * i], g[j][2 * i + 1]);
+                            const __nv_bfloat162 yb = __floats2bfloat162_rn(z0, z1);
                             o[i] = *reinterpret_cast<const uint32_t*>(&yb);
                         }
-                        const int hf = cc >> 3, c8 = cc & 7;
-                        *reinterpret_cast<uint4*>(sA + hf * kStage + (r >> 3) * 1024 + (r & 7) * 128 + ((c8 ^ (r & 7)) << 4)) =
-                            make_uint4(o[0], o[1], o[2], o[3]);
+                        *reinterpret_cast<uint4*>(sA + addr[u][j]) = make_uint4(o[0], o[1], o[2], o[3]);
                     }
                 }
             }
@@ -226,6 +240,11 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ C
         uint8_t* stage = sT + warp * 2 * kOut;
         const uint32_t my = (uint32_t)lane * 32, sw = ((uint32_t)(lane >> 2) & 1u) << 4;
         int n_st = 0;
+        float4 bb[8];
+        if (p.bias) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) bb[i] = __ldg(reinterpret_cast<const float4*>(p.bias + 64 * hsel) + i);
+        }
         for (int c = 0; c < n_chunks; ++c) {
             const int bsel = c & 1;
             const int col0 = c * kNC + 64 * hsel;
@@ -235,11 +254,6 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ C
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
             for (int c0 = 0; c0 < 64; c0 += 32) {
-                float4 bb[8];
-                if (p.bias) {
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) bb[i] = __ldg(reinterpret_cast<const float4*>(p.bias + col0 + c0) + i);
-                }
                 float t32[32];
                 tmem_ld32(t_lane + bsel * kNC + 64 * hsel + c0, t32);
                 if (c0 == 32) {                                 // last read of this accumulator half: hand it back to the MMA warp
@@ -250,8 +264,13 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ C
                 if (p.bias) {
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
-                        t32[4 * i] += bb[i].x; t32[4 * i + 1] += bb[i].y; t32[4 * i + 2] += bb[i].z; t32[4 * i + 3] += bb[i].w;
+                        add2(t32[4 * i], t32[4 * i + 1], bb[i].x, bb[i].y);
+                        add2(t32[4 * i + 2], t32[4 * i + 3], bb[i].z, bb[i].w);
                     }
+                    // the next pass's bias values travel while this pass is packed and stored
+                    const int nxt = c0 == 0 ? col0 + 32 : (c + 1 < n_chunks ? (c + 1) * kNC + 64 * hsel : col0);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) bb[i] = __ldg(reinterpret_cast<const float4*>(p.bias + nxt) + i);
                 }
 #pragma unroll
                 for (int g16 = 0; g16 < 2; ++g16, ++n_st) {
@@ -323,11 +342,12 @@ extern "C" gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, i
     p.n_stages = (int)((budget - fixed) / kStage);
     if (p.n_stages > 8) p.n_stages = 8;
     const size_t smem = fixed + (size_t)p.n_stages * kStage;
-    cudaError_t e = cudaFuncSetAttribute(ln_qkv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    auto kern = c_in <= 256 ? ln_qkv_kernel<1> : ln_qkv_kernel<2>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) {
         cudaStream_t st = (cudaStream_t)stream;
         prof_begin("ln_qkv", "gemm", st);
-        ln_qkv_kernel<<<(n + kRows - 1) / kRows, kThreads, smem, st>>>(tmx, tmw, tmq, tmk, tmv, p);
+        kern<<<(n + kRows - 1) / kRows, kThreads, smem, st>>>(tmx, tmw, tmq, tmk, tmv, p);
         prof_end(st);
         count_launch();
         e = cudaGetLastError();
