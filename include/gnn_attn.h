@@ -327,6 +327,20 @@ gnn_status_t gnn_dot_aggr(int32_t n, const int32_t* rowptr, const int32_t* colid
 gnn_status_t gnn_probe_gather(const void* table, int64_t table_rows, int32_t row_bytes, const int32_t* idx, int64_t n_idx,
                               int32_t mode, int32_t depth, int32_t ctas_per_sm, float* sink, gnn_stream_t stream);
 
+/* Graph Transformer attention forward WITHOUT any caller-supplied or allocated scratch: gnn_gt_attn_fwd (same operation,
+ * same arguments and layouts) with the pass's scratch - the per-chunk partial softmax states of
+ * split hub rows - in a file-scope __device__ array inside the library, for callers that cannot
+ * call cudaMalloc (CUDA graph capture, serving loops).  The array holds gnn_static_workspace_limit() bytes (16 MiB; every
+ * GPU that loads the library holds it until exit); a graph / shape whose gnn_workspace_bytes(GNN_OP_GT_FWD) exceeds it is
+ * refused with GNN_EWORKSPACE and a message.  The call allocates and frees nothing on host or device.  ALL calls on a
+ * device share the array (it keeps the previous call's contents; nothing in it needs clearing - every partial is
+ * written before it is read within a call): calls that may overlap on the GPU (unordered streams, two host threads)
+ * RACE on it - order them.  The plan must live on the current device.  Asynchronous on `stream`.                    */
+size_t gnn_static_workspace_limit(void);
+gnn_status_t gnn_gt_attn_fwd_static(const gnn_plan_t* plan, const int32_t* rowptr, const int32_t* colidx, int32_t n,
+                                    const void* q, const void* k, const void* v, int32_t heads, int32_t head_dim,
+                                    gnn_dtype_t dtype, void* out, float* lse, gnn_stream_t stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -28,6 +28,7 @@ EXPORTED_SYMBOLS = [
     "gnn_plan_colidx_t", "gnn_workspace_bytes", "gnn_gt_attn_fwd", "gnn_gt_attn_bwd", "gnn_gatv2_fwd",
     "gnn_gatv2_bwd", "gnn_gt_attn_fwd_block", "gnn_gt_attn_fwd_wsb", "gnn_gt_attn_bwd_wsb", "gnn_gt_attn_bwd_block", "gnn_seg_minmax_fwd", "gnn_seg_minmax_bwd", "gnn_last_error", "gnn_version", "gnn_launch_count", "gnn_profile_enable",
     "gnn_profile_collect", "gnn_pdl_enable", "gnn_probe_gather", "gnn_ln_qkv_fwd", "gnn_dot_aggr",
+    "gnn_static_workspace_limit", "gnn_gt_attn_fwd_static",
 ]
 
 
@@ -85,6 +86,8 @@ def lib() -> C.CDLL:
         L.gnn_probe_gather.argtypes = [_vp, _i64, _i32, _vp, _i64, _i32, _i32, _i32, _vp, _vp]
         L.gnn_ln_qkv_fwd.argtypes = [_i32, _i32, _i32, _i32, _vp, _vp, _vp, _f, _vp, _vp, _vp, _vp, _vp, _vp]
         L.gnn_dot_aggr.argtypes = [_i32, _vp, _vp, _vp, _i32, _i32, _i32, _vp, _vp]
+        L.gnn_static_workspace_limit.restype = _sz
+        L.gnn_gt_attn_fwd_static.argtypes = [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32, _i32, C.c_int, _vp, _vp, _vp]
         L.gnn_pdl_enable.argtypes = [C.c_int]
         L.gnn_pdl_enable.restype = None
         L.gnn_profile_collect.argtypes = [_vp, _vp, _i32]
@@ -265,6 +268,17 @@ def gnn_gt_attn_fwd(plan: Plan, q, k, v, out, lse, stream=None):
     ws = plan.workspace(GNN_OP_GT_FWD, H, d, _dtype_code(q))
     _check(lib().gnn_gt_attn_fwd(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v), H, d,
                                  _dtype_code(q), _ptr(out), _ptr(lse), _ptr(ws), ws.numel(), _stream(stream)))
+
+
+def gnn_static_workspace_limit() -> int:
+    return int(lib().gnn_static_workspace_limit())
+
+
+def gnn_gt_attn_fwd_static(plan: Plan, q, k, v, out, lse, stream=None):
+    """gnn_gt_attn_fwd with the scratch in the library's built-in device array: no workspace tensor, no allocation."""
+    n, H, d = q.shape
+    _check(lib().gnn_gt_attn_fwd_static(plan.handle, _ptr(plan.rowptr), _ptr(plan.colidx), n, _ptr(q), _ptr(k), _ptr(v), H, d,
+                                        _dtype_code(q), _ptr(out), _ptr(lse), _stream(stream)))
 
 
 def gnn_gt_attn_fwd_block(plan: Plan, q, k, v, out, lse, stream=None):

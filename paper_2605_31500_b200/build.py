@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgnn_attn.so")
-UNITS = ["api", "plan", "probe", "block_fwd", "block_bwd", "wsb", "ln_qkv", "dot_aggr", "pass_gt_fwd", "pass_gt_bwd_dst", "pass_gt_bwd_src", "pass_gat_fwd", "pass_gat_bwd_dst", "pass_min_fwd",
+UNITS = ["api", "plan", "probe", "static_ws", "block_fwd", "block_bwd", "wsb", "ln_qkv", "dot_aggr", "pass_gt_fwd", "pass_gt_bwd_dst", "pass_gt_bwd_src", "pass_gat_fwd", "pass_gat_bwd_dst", "pass_min_fwd",
          "pass_gat_bwd_src"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
