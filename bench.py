@@ -187,12 +187,16 @@ def quick_config(cfg, args, dev, peak):
             fb(); fw(); bw(); bb()
         ms_fb, ms_fw, ms_bw = timed(fb, args.steps), timed(fw, args.steps), timed(bw, args.steps)
         ms_bb, ms_sb = timed(bb, args.steps), timed(lambda: (fb(), bb()), args.steps)
+        ms_mx = timed(lambda: (fb(), bwd()), args.steps)     # fastest measured composition: tcgen05 forward + CSR backward
         r["tcgen05_paths"] = {"block_fwd_ms": ms_fb, "block_fwd_compulsory_frac": frac(comp["fwd"], ms_fb),
                               "block_bwd_ms": ms_bb, "block_bwd_compulsory_frac": frac(comp["bwd"], ms_bb),
                               "block_step_ms": ms_sb, "block_step_gedges": e / (ms_sb * 1e-3) * 1e-9,
                               "block_step_compulsory_frac": frac(comp["fwd"] + comp["bwd"], ms_sb),
+                              "mixed_step_ms": ms_mx, "mixed_step_gedges": e / (ms_mx * 1e-3) * 1e-9,
+                              "mixed_step_compulsory_frac": frac(comp["fwd"] + comp["bwd"], ms_mx),
                               "wsb_fwd_ms": ms_fw, "wsb_bwd_ms": ms_bw, "wsb_info": plan.wsb_info(),
-                              "note": "block_* = diagonal block layout (tile-local tcgen05 + remainder CSR), wsb_* = general WSB layout"}
+                              "note": "block_* = diagonal block layout (tile-local tcgen05 + remainder CSR), wsb_* = general WSB layout, "
+                                      "mixed_* = block forward + CSR backward"}
     del T, out, lse, stat, g1, g2, g3, plan, flush
     torch.cuda.empty_cache()
     return r
