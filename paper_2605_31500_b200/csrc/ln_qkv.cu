@@ -5,15 +5,21 @@
 //   y[i, :] = (x[i, :] - mean_i) / sqrt(var_i + eps) * gamma + beta        (biased variance over the C features)
 //   [Q | K | V][i, :] = y[i, :] W^T + bias,   W = [W_Q; W_K; W_V] of shape [3*H*d, C]
 //
-// (Round-2 layout: 320 threads - eight LayerNorm / epilogue warps, two per TMEM lane quarter - see below.)
 // The paper runs these as stock PyTorch ops (LayerNorm kernel, cuBLAS GEMM: one write and one read of the normalised
-// activations in HBM).  Here one CTA owns 128 rows: warps 0-3 normalise their rows in registers (a warp per row,
-// 16-byte loads, shuffle reductions) and write them as bf16 straight into the 128-byte-swizzled K-major shared-memory
-// tile the tensor core reads - the normalised activations never touch HBM.  Then, warp-specialised: warp 4 streams the
-// weight tiles (128 outputs x 64 channels, 16 KB) through a TMA ring, warp 5 issues tcgen05.mma (128 x 128 x 16) into
-// one of two 128-column TMEM accumulators, and warps 0-3 drain the other one (tcgen05.ld, + bias, bf16, per-warp
-// transpose, coalesced stores) - full / empty mbarriers between the three roles, so the epilogue of output chunk c
-// overlaps the products of chunk c + 1.
+// activations in HBM).  Here a tile of 128 rows is fetched raw by TMA straight into the 128-byte-swizzled K-major
+// shared-memory tile the tensor core reads, normalised IN PLACE (two lanes per row keep their half row in registers:
+// one shared-memory read and one write per element, no shuffle chains) - the normalised activations never touch HBM -
+// and multiplied with the weights, which stream through a TMA ring of 16 KB stages (128 outputs x 64 channels);
+// tcgen05.mma 128 x 128 x 16 into 128-column TMEM accumulators; eight epilogue warps (two per TMEM lane quarter, one
+// 64-column half each) drain a finished accumulator (tcgen05.ld, + bias, bf16, swizzled staging buffer, TMA store)
+// while the MMA warp fills the next one.  Two kernels:
+//   C <= 256  ln_qkv_persist_kernel: one CTA per SM walks its tiles with TWO A tiles and four accumulators, so the x
+//             tile of tile t + 1 lands and is normalised while tile t is multiplied and drained; output staging in
+//             128-byte rows (one TMA store per chunk and warp).
+//   C <= 512  ln_qkv_kernel: one CTA per tile (the 128 KB A tile leaves no room for a second one), two accumulators,
+//             output staging in 32-byte rows.
+// Measured limit of both (profiles/r02_ncu_ln_qkv.md): every tile re-streams the whole weight matrix from L2 and the
+// shared memory left beside the A tiles holds four stages, i.e. 64 KB in flight against ~1.5 us of L2 latency.
 #include <cuda.h>
 #include <cuda_bf16.h>
 
@@ -50,8 +56,187 @@ __device__ __forceinline__ void add2(float& a0, float& a1, float x0, float x1) {
         : "+f"(a0), "+f"(a1) : "f"(x0), "f"(x1));
 }
 
-template <int NJ>     // 16-byte chunks of a row per lane: 1 for C <= 256, 2 for C <= 512
-__global__ void __launch_bounds__(kThreads, 2)
+// LayerNorm of warp `warp`'s 16 rows of the raw x tile in sA (SWIZZLE_128B half tiles of 64 channels), IN PLACE.
+// Two lanes per row: lane l owns row 16 warp + (l & 15), half tiles (l >> 4) KH .. + KH - 1 (KH = 2 for C <= 256, 4 for
+// C <= 512), i.e. up to 128 / 256 channels, which it keeps as raw bf16 pairs in registers (one smem read, one smem
+// write per element).  No shuffle chains: every lane runs long independent sums and meets its partner (lane ^ 16) twice
+// (sum, sum of centred squares).  bf16 halves enter the fp32 sums directly (FHADD), squares / scale / shift are packed
+// (FFMA2 / FMUL2); gamma / beta come from L1 as broadcast 16-byte loads.  Rows past n become zeros.
+template <int KH>
+__device__ __forceinline__ void ln_rows(uint8_t* sA, const LnQkvParams& p, int row0, int warp, int lane) {
+    const int KC = p.C / 64;
+    const int r = warp * 16 + (lane & 15), kk0 = (lane >> 4) * KH;
+    const uint32_t rbase = (uint32_t)((r >> 3) * 1024 + (r & 7) * 128), rx = (uint32_t)(r & 7);
+    uint4 raw[KH][8];
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+#pragma unroll
+    for (int k = 0; k < KH; ++k) {
+        const bool on = kk0 + k < KC;
+#pragma unroll
+        for (int cc = 0; cc < 8; ++cc) {
+            raw[k][cc] = make_uint4(0, 0, 0, 0);
+            if (on) raw[k][cc] = *reinterpret_cast<const uint4*>(sA + (kk0 + k) * kStage + rbase + (((uint32_t)cc ^ rx) << 4));
+            add_bf16x2(raw[k][cc].x, s0, s1, s0, s1);
+            add_bf16x2(raw[k][cc].y, s2, s3, s2, s3);
+            add_bf16x2(raw[k][cc].z, s0, s1, s0, s1);
+            add_bf16x2(raw[k][cc].w, s2, s3, s2, s3);
+        }
+    }
+    float sum = (s0 + s1) + (s2 + s3);
+    sum += __shfl_xor_sync(0xffffffffu, sum, 16);
+    const float inv_c = 1.f / (float)p.C;
+    const float nmean = -sum * inv_c;
+    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+#pragma unroll
+    for (int k = 0; k < KH; ++k) {
+        const float nm = kk0 + k < KC ? nmean : 0.f;          // half tiles past C hold zeros and stay zero
+#pragma unroll
+        for (int cc = 0; cc < 8; ++cc) {
+            const uint32_t w[4] = {raw[k][cc].x, raw[k][cc].y, raw[k][cc].z, raw[k][cc].w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                float a, b;
+                add_bf16x2(w[i], nm, nm, a, b);
+                if (i & 1) fma2v(q2, q3, a, b, a, b);
+                else fma2v(q0, q1, a, b, a, b);
+            }
+        }
+    }
+    float ss = (q0 + q1) + (q2 + q3);
+    ss += __shfl_xor_sync(0xffffffffu, ss, 16);
+    const bool rv = row0 + r < p.n;
+    const float rstd = rv ? 1.f / sqrtf(ss * inv_c + p.eps) : 0.f;
+#pragma unroll
+    for (int k = 0; k < KH; ++k) {
+        if (kk0 + k < KC) {
+#pragma unroll
+            for (int cc = 0; cc < 8; ++cc) {
+                const int ch = (kk0 + k) * 64 + cc * 8;
+                const float4 g0 = __ldg(reinterpret_cast<const float4*>(p.gamma + ch)), g1 = __ldg(reinterpret_cast<const float4*>(p.gamma + ch + 4));
+                float4 b0 = __ldg(reinterpret_cast<const float4*>(p.beta + ch)), b1 = __ldg(reinterpret_cast<const float4*>(p.beta + ch + 4));
+                if (!rv) { b0 = make_float4(0.f, 0.f, 0.f, 0.f); b1 = b0; }
+                const uint32_t w[4] = {raw[k][cc].x, raw[k][cc].y, raw[k][cc].z, raw[k][cc].w};
+                const float gg[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
+                float zz[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+                uint32_t o[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    float y0, y1;
+                    add_bf16x2(w[i], nmean, nmean, y0, y1);
+                    mul2(y0, y1, rstd);
+                    fma2v(zz[2 * i], zz[2 * i + 1], y0, y1, gg[2 * i], gg[2 * i + 1]);
+                    const __nv_bfloat162 yb = __floats2bfloat162_rn(zz[2 * i], zz[2 * i + 1]);
+                    o[i] = *reinterpret_cast<const uint32_t*>(&yb);
+                }
+                *reinterpret_cast<uint4*>(sA + (kk0 + k) * kStage + rbase + (((uint32_t)cc ^ rx) << 4)) = make_uint4(o[0], o[1], o[2], o[3]);
+            }
+        }
+    }
+}
+
+// epilogue state of one worker warp: warp w drains TMEM lanes 32 (w & 3) .. +31 (tile rows) of column half w >> 2 of every
+// accumulator: accumulator -> + bias -> bf16 -> 32-row x 16-column staging buffer (the layout TMA's 32-byte swizzle expects)
+// -> one TMA store per buffer (rows past n are clipped by the unit); the warp's two staging buffers alternate
+template <int W>       // W = 16: two 1 KB buffers per warp, 32-byte rows (SWIZZLE_32B maps), four stores per chunk;
+struct Epi {           // W = 64: one 4 KB buffer per warp, 128-byte rows (SWIZZLE_128B maps), one store per chunk
+    static constexpr int kBytes = W == 16 ? 2 * kOut : 4096;   // staging bytes per warp
+    float4 bb[8];          // bias of the next 32-column pass (prefetched one pass ahead)
+    uint8_t* stage;
+    uint32_t lane_off, my, sw;
+    int q4, hsel, lane, n_st;
+    __device__ __forceinline__ void init(const LnQkvParams& p, uint8_t* sT, int warp, int lane_) {
+        q4 = warp & 3; hsel = warp >> 2; lane = lane_; n_st = 0;
+        lane_off = (uint32_t)(q4 * 32) << 16;
+        stage = sT + warp * kBytes;
+        if (W == 16) { my = (uint32_t)lane * 32; sw = ((uint32_t)(lane >> 2) & 1u) << 4; }
+        else { my = (uint32_t)lane * 128; sw = (uint32_t)lane & 7u; }
+        if (p.bias) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) bb[i] = __ldg(reinterpret_cast<const float4*>(p.bias + 64 * hsel) + i);
+        }
+    }
+    // output chunk c (columns c * 128 ..) of the tile at row0 from the complete accumulator at TMEM column t_acc; arrives
+    // on `drained` after the last TMEM read
+    __device__ __forceinline__ void chunk(const LnQkvParams& p, uint32_t t_acc, uint64_t* drained, int c, int n_chunks, int row0,
+                                          const CUtensorMap* tmq, const CUtensorMap* tmk, const CUtensorMap* tmv) {
+        const int col0 = c * kNC + 64 * hsel;
+        const int t = col0 / p.R, off = col0 - t * p.R;
+        const CUtensorMap* tmo = t == 0 ? tmq : (t == 1 ? tmk : tmv);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll 1
+        for (int c0 = 0; c0 < 64; c0 += 32) {
+            float t32[32];
+            tmem_ld32(t_acc + lane_off + 64 * hsel + c0, t32);
+            if (c0 == 32) {                                 // last read of this accumulator half: hand it back to the MMA warp
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(drained);
+            }
+            if (p.bias) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    add2(t32[4 * i], t32[4 * i + 1], bb[i].x, bb[i].y);
+                    add2(t32[4 * i + 2], t32[4 * i + 3], bb[i].z, bb[i].w);
+                }
+                // the next pass's bias values travel while this pass is packed and stored
+                const int nxt = c0 == 0 ? col0 + 32 : ((c + 1) % n_chunks) * kNC + 64 * hsel;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) bb[i] = __ldg(reinterpret_cast<const float4*>(p.bias + nxt) + i);
+            }
+            if constexpr (W == 16) {
+    #pragma unroll
+                for (int g16 = 0; g16 < 2; ++g16, ++n_st) {
+                    uint8_t* buf = stage + (n_st & 1) * kOut;
+                    if (n_st >= 2) {                            // the store issued from this buffer two groups ago has read it
+                        if (lane == 0) tma_store_wait_read<1>();
+                        __syncwarp();
+                    }
+                    uint32_t o[8];
+    #pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const __nv_bfloat162 yb = __floats2bfloat162_rn(t32[16 * g16 + 2 * i], t32[16 * g16 + 2 * i + 1]);
+                        o[i] = *reinterpret_cast<const uint32_t*>(&yb);
+                    }
+                    *reinterpret_cast<uint4*>(buf + my + sw) = make_uint4(o[0], o[1], o[2], o[3]);
+                    *reinterpret_cast<uint4*>(buf + my + (sw ^ 16u)) = make_uint4(o[4], o[5], o[6], o[7]);
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    __syncwarp();
+                    if (lane == 0) {
+                        tma_store_2d(tmo, off + c0 + 16 * g16, row0 + 32 * q4, buf);
+                        tma_store_commit();
+                    }
+                }
+            } else {
+                if (c0 == 0 && n_st > 0) {                  // the previous chunk's store has read the buffer
+                    if (lane == 0) tma_store_wait_read<0>();
+                    __syncwarp();
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    uint32_t o[4];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const __nv_bfloat162 yb = __floats2bfloat162_rn(t32[8 * j + 2 * i], t32[8 * j + 2 * i + 1]);
+                        o[i] = *reinterpret_cast<const uint32_t*>(&yb);
+                    }
+                    *reinterpret_cast<uint4*>(stage + my + ((((uint32_t)(c0 >> 3) + j) ^ sw) << 4)) = make_uint4(o[0], o[1], o[2], o[3]);
+                }
+                if (c0 == 32) {
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    __syncwarp();
+                    if (lane == 0) {
+                        tma_store_2d(tmo, off, row0 + 32 * q4, stage);
+                        tma_store_commit();
+                    }
+                    ++n_st;
+                }
+            }
+        }
+    }
+};
+
+template <int NJ>     // 1: C <= 256 (two CTAs per SM), 2: C <= 512 (one CTA per SM)
+__global__ void __launch_bounds__(kThreads, 3 - NJ)
 ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmw,
               const __grid_constant__ CUtensorMap tmq, const __grid_constant__ CUtensorMap tmk,
               const __grid_constant__ CUtensorMap tmv, const LnQkvParams p) {
@@ -108,93 +293,9 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ C
             }
         }
     } else if (warp < kWorkWarps) {
-        // ===== LayerNorm of this warp's 16 rows, in place in the A tile (lane <-> 16-byte chunks lane [, lane + 32]).
-        // bf16 operands enter the fp32 sums directly (FHADD takes a register half: no unpack); squares, scale and shift
-        // run as packed fp32 pairs (FFMA2 / FMUL2).
-        const int nchunk = p.C / 8;
-        float g[NJ][8], b[NJ][8];
-        bool on[NJ];
-#pragma unroll
-        for (int j = 0; j < NJ; ++j) {
-            const int cc = lane + 32 * j;
-            on[j] = cc < nchunk;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                g[j][i] = on[j] ? __ldg(p.gamma + cc * 8 + i) : 0.f;
-                b[j][i] = on[j] ? __ldg(p.beta + cc * 8 + i) : 0.f;
-            }
-        }
-        const float inv_c = 1.f / (float)p.C;
+        // ===== LayerNorm of this warp's 16 rows, in place in the A tile
         mbar_wait(xfull, 0);
-        constexpr int RB = NJ == 1 ? 4 : 2;   // rows per batch (independent shuffle-reduction chains)
-        for (int rl = 0; rl < 16; rl += RB) {
-            uint4 raw[RB][NJ];
-            uint32_t addr[RB][NJ];
-            float s[RB];
-#pragma unroll
-            for (int u = 0; u < RB; ++u) {
-                float s0 = 0.f, s1 = 0.f;
-#pragma unroll
-                for (int j = 0; j < NJ; ++j) {
-                    const int r = warp * 16 + rl + u, cc = lane + 32 * j;
-                    addr[u][j] = (uint32_t)((cc >> 3) * kStage + (r >> 3) * 1024 + (r & 7) * 128 + (((cc & 7) ^ (r & 7)) << 4));
-                    raw[u][j] = make_uint4(0, 0, 0, 0);
-                    if (on[j]) raw[u][j] = *reinterpret_cast<const uint4*>(sA + addr[u][j]);
-                    add_bf16x2(raw[u][j].x, s0, s1, s0, s1);
-                    add_bf16x2(raw[u][j].y, s0, s1, s0, s1);
-                    add_bf16x2(raw[u][j].z, s0, s1, s0, s1);
-                    add_bf16x2(raw[u][j].w, s0, s1, s0, s1);
-                }
-                s[u] = s0 + s1;
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1)
-#pragma unroll
-                for (int u = 0; u < RB; ++u) s[u] += __shfl_xor_sync(0xffffffffu, s[u], o);
-            float v[RB][NJ][8], ss[RB];
-#pragma unroll
-            for (int u = 0; u < RB; ++u) {
-                const float nmean = -s[u] * inv_c;
-                float q0 = 0.f, q1 = 0.f;
-#pragma unroll
-                for (int j = 0; j < NJ; ++j) {
-                    const uint32_t w[4] = {raw[u][j].x, raw[u][j].y, raw[u][j].z, raw[u][j].w};
-                    const float nm = on[j] ? nmean : 0.f;     // lanes past the row's last chunk hold zeros and stay zero
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        add_bf16x2(w[i], nm, nm, v[u][j][2 * i], v[u][j][2 * i + 1]);
-                        fma2v(q0, q1, v[u][j][2 * i], v[u][j][2 * i + 1], v[u][j][2 * i], v[u][j][2 * i + 1]);
-                    }
-                }
-                ss[u] = q0 + q1;
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1)
-#pragma unroll
-                for (int u = 0; u < RB; ++u) ss[u] += __shfl_xor_sync(0xffffffffu, ss[u], o);
-#pragma unroll
-            for (int u = 0; u < RB; ++u) {
-                const int r = warp * 16 + rl + u;
-                const float rstd = row0 + r < p.n ? 1.f / sqrtf(ss[u] * inv_c + p.eps) : 0.f;
-                const bool rv = row0 + r < p.n;
-#pragma unroll
-                for (int j = 0; j < NJ; ++j) {
-                    if (on[j]) {
-                        uint32_t o[4];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            float y0 = v[u][j][2 * i], y1 = v[u][j][2 * i + 1];
-                            mul2(y0, y1, rstd);
-                            float z0 = rv ? b[j][2 * i] : 0.f, z1 = rv ? b[j][2 * i + 1] : 0.f;
-                            fma2v(z0, z1, y0, y1, g[j][2 * i], g[j][2 * i + 1]);
-                            const __nv_bfloat162 yb = __floats2bfloat162_rn(z0, z1);
-                            o[i] = *reinterpret_cast<const uint32_t*>(&yb);
-                        }
-                        *reinterpret_cast<uint4*>(sA + addr[u][j]) = make_uint4(o[0], o[1], o[2], o[3]);
-                    }
-                }
-            }
-        }
+        ln_rows<2 * NJ>(sA, p, row0, warp, lane);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();   // the A tile is complete and visible to the tensor core
@@ -232,75 +333,152 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ C
             }
         }
     } else if (warp < kWorkWarps) {
-        // ===== epilogue: warp w drains TMEM lanes 32 (w & 3) .. +31 (tile rows) of column half w >> 2 of every chunk:
-        // accumulator -> + bias -> bf16 -> 32-row x 16-column staging buffer (the layout TMA's 32-byte swizzle expects)
-        // -> one TMA store per buffer (rows past n are clipped by the unit); two buffers per warp alternate
-        const int q4 = warp & 3, hsel = warp >> 2;
-        const uint32_t t_lane = tmem + ((uint32_t)(q4 * 32) << 16);
-        uint8_t* stage = sT + warp * 2 * kOut;
-        const uint32_t my = (uint32_t)lane * 32, sw = ((uint32_t)(lane >> 2) & 1u) << 4;
-        int n_st = 0;
-        float4 bb[8];
-        if (p.bias) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) bb[i] = __ldg(reinterpret_cast<const float4*>(p.bias + 64 * hsel) + i);
-        }
+        // ===== epilogue (Epi)
+        Epi<16> ep;
+        ep.init(p, sT, warp, lane);
         for (int c = 0; c < n_chunks; ++c) {
-            const int bsel = c & 1;
-            const int col0 = c * kNC + 64 * hsel;
-            const int t = col0 / p.R, off = col0 - t * p.R;
-            const CUtensorMap* tmo = t == 0 ? &tmq : (t == 1 ? &tmk : &tmv);
-            mbar_wait(tfull + bsel, (uint32_t)((c >> 1) & 1));
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-#pragma unroll 1
-            for (int c0 = 0; c0 < 64; c0 += 32) {
-                float t32[32];
-                tmem_ld32(t_lane + bsel * kNC + 64 * hsel + c0, t32);
-                if (c0 == 32) {                                 // last read of this accumulator half: hand it back to the MMA warp
-                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(tempty + bsel);
-                }
-                if (p.bias) {
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        add2(t32[4 * i], t32[4 * i + 1], bb[i].x, bb[i].y);
-                        add2(t32[4 * i + 2], t32[4 * i + 3], bb[i].z, bb[i].w);
-                    }
-                    // the next pass's bias values travel while this pass is packed and stored
-                    const int nxt = c0 == 0 ? col0 + 32 : (c + 1 < n_chunks ? (c + 1) * kNC + 64 * hsel : col0);
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) bb[i] = __ldg(reinterpret_cast<const float4*>(p.bias + nxt) + i);
-                }
-#pragma unroll
-                for (int g16 = 0; g16 < 2; ++g16, ++n_st) {
-                    uint8_t* buf = stage + (n_st & 1) * kOut;
-                    if (n_st >= 2) {                            // the store issued from this buffer two groups ago has read it
-                        if (lane == 0) tma_store_wait_read<1>();
-                        __syncwarp();
-                    }
-                    uint32_t o[8];
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const __nv_bfloat162 yb = __floats2bfloat162_rn(t32[16 * g16 + 2 * i], t32[16 * g16 + 2 * i + 1]);
-                        o[i] = *reinterpret_cast<const uint32_t*>(&yb);
-                    }
-                    *reinterpret_cast<uint4*>(buf + my + sw) = make_uint4(o[0], o[1], o[2], o[3]);
-                    *reinterpret_cast<uint4*>(buf + my + (sw ^ 16u)) = make_uint4(o[4], o[5], o[6], o[7]);
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                    __syncwarp();
-                    if (lane == 0) {
-                        tma_store_2d(tmo, off + c0 + 16 * g16, row0 + 32 * q4, buf);
-                        tma_store_commit();
-                    }
-                }
-            }
+            mbar_wait(tfull + (c & 1), (uint32_t)((c >> 1) & 1));
+            ep.chunk(p, tmem + (c & 1) * kNC, tempty + (c & 1), c, n_chunks, row0, &tmq, &tmk, &tmv);
         }
         if (lane == 0) tma_store_wait<0>();
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     if (warp == 9) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(tmem) : "memory");
+}
+
+// ---- persistent variant for C <= 256: one CTA per SM walks tiles blockIdx.x, + gridDim.x, ... with TWO A tiles, so that
+// the raw x tile of tile t + 1 lands and is normalised while the tensor core works on tile t, four TMEM accumulators
+// (all 512 columns) so that the MMA warp runs ahead of the epilogue by up to four output chunks, and a weight ring of
+// all the shared memory that is left.  Roles: warps 0-7 LayerNorm(t + 1) then epilogue(t); warp 8 weight ring (TMA);
+// warp 9 MMA issue; warp 10 x tiles (TMA).  Barriers: xfull[b] (x tile landed in A[b]), aready[b] (A[b] normalised, 8
+// warp arrivals), afree[b] (tcgen05.commit after the last product of the tile in A[b]), full / empty (weight ring),
+// tfull / tempty (accumulators).
+constexpr int kPThreads = 352;
+constexpr int kAcc = 4;
+__global__ void __launch_bounds__(kPThreads, 1)
+ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmw,
+                      const __grid_constant__ CUtensorMap tmq, const __grid_constant__ CUtensorMap tmk,
+                      const __grid_constant__ CUtensorMap tmv, const LnQkvParams p) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = smem_raw + kBars + ((1024u - ((smem_u32(smem_raw) + kBars) & 1023u)) & 1023u);
+    const int KC = p.C / 64, NS = p.n_stages;
+    uint8_t* sA = smem;                                   // [2][KC] half tiles
+    uint8_t* sB = sA + 2 * KC * kStage;                   // [NS] weight stages
+    uint8_t* sT = sB + NS * kStage;                       // [kWorkWarps] staging buffers of 32 rows x 128 bytes
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
+    uint64_t* empty = full + 8;
+    uint64_t* tfull = empty + 8;                          // [kAcc]
+    uint64_t* tempty = tfull + kAcc;                      // [kAcc]
+    uint64_t* xfull = tempty + kAcc;                      // [2]
+    uint64_t* aready = xfull + 2;                         // [2]
+    uint64_t* afree = aready + 2;                         // [2]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(afree + 2);
+    static_assert((8 + 8 + 2 * kAcc + 6) * 8 + 4 <= kBars, "barrier block");
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    {
+        uint32_t dyn;
+        asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
+        if ((uint32_t)(sT + kWorkWarps * Epi<64>::kBytes - smem_raw) > dyn) __trap();
+    }
+    const int n_chunks = 3 * p.R / kNC;
+    const int tiles = (p.n + kRows - 1) / kRows;
+    const int nlt = ((int)blockIdx.x < tiles) ? (tiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;   // this CTA's tiles
+    auto tile_row0 = [&](int lt) { return ((int)blockIdx.x + lt * (int)gridDim.x) * kRows; };
+
+    if (tid == 0) {
+        for (int s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+        for (int b = 0; b < kAcc; ++b) { mbar_init(tfull + b, 1); mbar_init(tempty + b, kWorkWarps); }
+        for (int b = 0; b < 2; ++b) { mbar_init(xfull + b, 1); mbar_init(aready + b, kWorkWarps); mbar_init(afree + b, 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 9) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp == 10) {
+        // ===== x tiles: tile lt -> A[lt & 1] once the products of tile lt - 2 have left it
+        if (lane == 0) {
+            for (int lt = 0; lt < nlt; ++lt) {
+                const int b = lt & 1;
+                mbar_wait(afree + b, (uint32_t)((lt >> 1) & 1) ^ 1u);
+                mbar_expect_tx(xfull + b, KC * kStage);
+                for (int kk = 0; kk < KC; ++kk) tma_load_2d(sA + (b * KC + kk) * kStage, &tmx, kk * 64, tile_row0(lt), xfull + b);
+            }
+        }
+    } else if (warp == 8) {
+        // ===== weight ring: item i = (tile, chunk c, channel block kk) -> slot i % NS
+        if (lane == 0) {
+            const int per_tile = n_chunks * KC, items = nlt * per_tile;
+            for (int i = 0; i < items; ++i) {
+                const int s = i % NS, j = i % per_tile;
+                mbar_wait(empty + s, (uint32_t)((i / NS) & 1) ^ 1u);
+                mbar_expect_tx(full + s, kStage);
+                tma_load_2d(sB + s * kStage, &tmw, (j % KC) * 64, (j / KC) * kNC, full + s);
+            }
+        }
+    } else if (warp == 9) {
+        // ===== MMA issuer
+        if (lane == 0) {
+            constexpr uint32_t kIdesc = make_idesc(kRows, kNC, false);
+            int i = 0, g = 0;
+            for (int lt = 0; lt < nlt; ++lt) {
+                const int b = lt & 1;
+                mbar_wait(aready + b, (uint32_t)((lt >> 1) & 1));
+                for (int c = 0; c < n_chunks; ++c, ++g) {
+                    const int acc = g % kAcc;
+                    mbar_wait(tempty + acc, (uint32_t)((g / kAcc) & 1) ^ 1u);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    for (int kk = 0; kk < KC; ++kk, ++i) {
+                        const int s = i % NS;
+                        mbar_wait(full + s, (uint32_t)((i / NS) & 1));
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+                        for (int ks = 0; ks < 4; ++ks)
+                            umma(tmem + acc * kNC, make_desc_sw128(smem_u32(sA + (b * KC + kk) * kStage) + ks * 32, 1024),
+                                 make_desc_sw128(smem_u32(sB + s * kStage) + ks * 32, 1024), kIdesc, (kk | ks) > 0);
+                        umma_commit(empty + s);
+                    }
+                    umma_commit(tfull + acc);
+                }
+                umma_commit(afree + b);
+            }
+        }
+    } else if (warp < kWorkWarps) {
+        // ===== workers: LayerNorm of the NEXT tile, then the epilogue of the current one
+        Epi<64> ep;
+        ep.init(p, sT, warp, lane);
+        auto normalise = [&](int lt) {
+            const int b = lt & 1;
+            mbar_wait(xfull + b, (uint32_t)((lt >> 1) & 1));
+            ln_rows<2>(sA + b * KC * kStage, p, tile_row0(lt), warp, lane);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(aready + b);
+        };
+        if (nlt > 0) normalise(0);
+        int g = 0;
+        for (int lt = 0; lt < nlt; ++lt) {
+            for (int c = 0; c < n_chunks; ++c, ++g) {
+                // the next tile's LayerNorm goes after the first drained chunk: its x tile (issued when the products of
+                // tile lt - 1 left the buffer) has landed by then, and the MMA warp is still up to three chunks ahead
+                if (c == (n_chunks > 1 ? 1 : 0) && lt + 1 < nlt) normalise(lt + 1);
+                const int acc = g % kAcc;
+                mbar_wait(tfull + acc, (uint32_t)((g / kAcc) & 1));
+                ep.chunk(p, tmem + acc * kNC, tempty + acc, c, n_chunks, tile_row0(lt), &tmq, &tmk, &tmv);
+            }
+        }
+        if (lane == 0) tma_store_wait<0>();
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 9) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
 }
 
 }  // namespace
@@ -336,21 +514,48 @@ extern "C" gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, i
     p.x = (const __nv_bfloat16*)x; p.gamma = gamma; p.beta = beta; p.bias = bias;
     p.q = (__nv_bfloat16*)q; p.k = (__nv_bfloat16*)k; p.v = (__nv_bfloat16*)v;
     p.n = n; p.C = c_in; p.R = (int)R; p.eps = eps;
-    // weight ring: as many 16 KB stages as keep two CTAs per SM (113 KB each) when the A tile allows it, else one CTA
-    const size_t fixed = (size_t)(c_in / 64) * kStage + (size_t)kWorkWarps * 2 * kOut + 1024;   // 1024 = barriers + alignment pad
-    const size_t budget = fixed + 2 * kStage <= 113 * 1024 ? 113 * 1024 : 226 * 1024;
-    p.n_stages = (int)((budget - fixed) / kStage);
-    if (p.n_stages > 8) p.n_stages = 8;
-    const size_t smem = fixed + (size_t)p.n_stages * kStage;
-    auto kern = c_in <= 256 ? ln_qkv_kernel<1> : ln_qkv_kernel<2>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) {
-        cudaStream_t st = (cudaStream_t)stream;
-        prof_begin("ln_qkv", "gemm", st);
-        kern<<<(n + kRows - 1) / kRows, kThreads, smem, st>>>(tmx, tmw, tmq, tmk, tmv, p);
-        prof_end(st);
-        count_launch();
-        e = cudaGetLastError();
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    const int tiles = (n + kRows - 1) / kRows;
+    if (c_in <= 256) {
+        // persistent kernel: two A tiles + staging + barriers, the rest of the 226 KB is the weight ring
+        int dev = 0, sms = 0;
+        e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) { set_error("%s: CUDA error: %s", who, cudaGetErrorString(e)); return GNN_ECUDA; }
+        if (!tc::encode_row_tile_map(&tmq, q, n, (int)R, 64, 32) || !tc::encode_row_tile_map(&tmk, k, n, (int)R, 64, 32) ||
+            !tc::encode_row_tile_map(&tmv, v, n, (int)R, 64, 32)) {      // output boxes of 32 rows x 128 bytes, SWIZZLE_128B
+            set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who);
+            return GNN_ECUDA;
+        }
+        const size_t fixed = 2 * (size_t)(c_in / 64) * kStage + (size_t)kWorkWarps * 4096 + 1024;
+        p.n_stages = (int)((226 * 1024 - fixed) / kStage);
+        if (p.n_stages > 8) p.n_stages = 8;
+        const size_t smem = fixed + (size_t)p.n_stages * kStage;
+        e = cudaFuncSetAttribute(ln_qkv_persist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) {
+            prof_begin("ln_qkv", "gemm", st);
+            ln_qkv_persist_kernel<<<tiles < sms ? tiles : sms, kPThreads, smem, st>>>(tmx, tmw, tmq, tmk, tmv, p);
+            prof_end(st);
+            count_launch();
+            e = cudaGetLastError();
+        }
+    } else {
+        // weight ring: as many 16 KB stages as keep two CTAs per SM (113 KB each) when the A tile allows it, else one CTA
+        const size_t fixed = (size_t)(c_in / 64) * kStage + (size_t)kWorkWarps * 2 * kOut + 1024;   // 1024 = barriers + alignment pad
+        const size_t budget = fixed + 2 * kStage <= 113 * 1024 ? 113 * 1024 : 226 * 1024;
+        p.n_stages = (int)((budget - fixed) / kStage);
+        if (p.n_stages > 8) p.n_stages = 8;
+        const size_t smem = fixed + (size_t)p.n_stages * kStage;
+        auto kern = ln_qkv_kernel<2>;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) {
+            prof_begin("ln_qkv", "gemm", st);
+            kern<<<tiles, kThreads, smem, st>>>(tmx, tmw, tmq, tmk, tmv, p);
+            prof_end(st);
+            count_launch();
+            e = cudaGetLastError();
+        }
     }
     if (e != cudaSuccess) { set_error("%s: CUDA error: %s", who, cudaGetErrorString(e)); return GNN_ECUDA; }
     return GNN_OK;
