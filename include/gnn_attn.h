@@ -241,7 +241,7 @@ gnn_status_t gnn_gt_attn_bwd_block(const gnn_plan_t* plan, const int32_t* rowptr
  * source-side gradients computed over the WSB layout of the TRANSPOSED graph, so that no atomics are needed (the
  * paper accumulates dK / dV with atomicAdd; on an undirected graph both layouts are the same arrays).
  * The plan must have been built with GNN_BLOCKS_WSB (and build_transpose for the backward) from a CSR WITHOUT duplicate
- * entries (a bitmap stores each (dst, src) pair once: GNN_EUNSUPPORTED otherwise).  bf16 features, head_dim 64 or 128
+ * entries (a bitmap stores each (dst, src) pair once: GNN_EUNSUPPORTED otherwise).  bf16 features, head_dim 32, 64 or 128
  * (GNN_EUNSUPPORTED otherwise); feature / gradient pointers 32-byte aligned; no workspace; asynchronous on `stream`.
  *   forward : q, k, v [n,H,d] bf16 in; out [n,H,d] bf16, lse [n,H] fp32 out.
  *   backward: q, k, v, dout in; out = the forward output O (bf16, in: its row dot <O_i, dO_i> centres the bf16-staged

@@ -28,7 +28,8 @@
 // Operands: own tiles arrive by TMA (cp.async.bulk.tensor.2d, SWIZZLE_128B); gathered tiles are written by the threads
 // (8 lanes per 128-byte row slice, coalesced 16-byte loads, the same XOR swizzle); P / dS are staged as bf16 in the
 // canonical no-swizzle K-major layout; V_c / K_c / Q_c / dO_c double as MN-major B operands of the second products.
-// head_dim 64 or 128 (128 = two 64-channel half tiles per operand); bf16 features; outputs leave through a per-warp
+// head_dim 32, 64 or 128 (128 = two 64-channel half tiles per operand; 32 = one half tile whose upper 32 channels are
+// zeros, own rows placed by the threads instead of TMA); bf16 features; outputs leave through a per-warp
 // shared-memory transpose so global stores are coalesced 16-byte pieces.
 #include <cuda.h>
 #include <cuda_bf16.h>
@@ -54,6 +55,7 @@ struct WsbParams {
     const int32_t* cols;
     const uint8_t* bitmap;
     int n_win, n, H;
+    const __nv_bfloat16 *ox, *oy;    // own operands of the two products (what tmx / tmy map; read directly when head_dim = 32)
     const __nv_bfloat16* gx;         // gathered operand of the first product  (fwd / dst: K, src: Q)
     const __nv_bfloat16* gy;         // gathered operand of the second product (fwd / dst: V, src: dO)
     const __nv_bfloat16* o;          // dst: stored forward output; dout for the Delta~ estimate comes from gdo
@@ -70,7 +72,8 @@ struct WsbParams {
 };
 
 // one 128-row tile of `g` (rows s_col[0..128), -1 = zero row) -> NH half tiles at sT, 128-byte swizzled K-major
-template <int NH>
+// (NCH = valid 16-byte chunks of a row slice: 8, or 4 for head_dim 32, whose upper 32 channels of the tile are zeros)
+template <int NH, int NCH>
 __device__ __forceinline__ void gather_tile(uint8_t* sT, const __nv_bfloat16* __restrict__ g, const int* s_col, size_t rowe,
                                             int hoff, int tid) {
     const int c = tid & 7, rb = tid >> 3;
@@ -81,7 +84,7 @@ __device__ __forceinline__ void gather_tile(uint8_t* sT, const __nv_bfloat16* __
 #pragma unroll
         for (int hf = 0; hf < NH; ++hf) {
             v[i * NH + hf] = make_uint4(0, 0, 0, 0);
-            if (col >= 0) v[i * NH + hf] = __ldg(reinterpret_cast<const uint4*>(g + (size_t)col * rowe + hoff + hf * 64) + c);
+            if (col >= 0 && c < NCH) v[i * NH + hf] = __ldg(reinterpret_cast<const uint4*>(g + (size_t)col * rowe + hoff + hf * 64) + c);
         }
     }
 #pragma unroll
@@ -102,14 +105,16 @@ __device__ __forceinline__ void write_block(uint8_t* sW, int tid, int wl, const 
 }
 
 template <int MODE, int D>
-__global__ void __launch_bounds__(kTile, (MODE == kFwd && D == 64) ? 3 : (D == 64 ? 2 : 1))
+__global__ void __launch_bounds__(kTile, (MODE == kFwd && D <= 64) ? 3 : (D <= 64 ? 2 : 1))
 wsb_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmy, const WsbParams p) {
-    constexpr int NH = D / 64;
+    constexpr int NH = D >= 64 ? D / 64 : 1;      // half tiles per operand; head_dim 32 = one half tile, upper channels zero
+    constexpr int DP = NH * 64;                   // tile width in channels
+    constexpr int NCH = D >= 64 ? 8 : D / 8;      // valid 16-byte chunks per row slice
     constexpr bool BWD = MODE != kFwd;
     constexpr int kOwnBytes = (BWD ? 2 : 1) * NH * kHT;
     constexpr int kPadBytes = (!BWD && NH * kHT < kWBytes) ? kWBytes - NH * kHT : 0;   // fwd: P aliases K (+ pad)
-    constexpr int kTmemCols = BWD ? (D == 64 ? 256 : 512) : 128;
-    constexpr int kColAcc1 = 128, kColAcc2 = 128 + D;
+    constexpr int kTmemCols = BWD ? (DP == 64 ? 256 : 512) : 128;
+    constexpr int kColAcc1 = 128, kColAcc2 = 128 + DP;
     constexpr int SBO_W = (kTile / 8) * 128;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -168,7 +173,7 @@ wsb_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUte
     for (int h = 0; h < p.H; ++h) {
         const int hoff = h * D;
         // ---- own tiles of this head by TMA (rows past n arrive as zeros)
-        if (tid == 0) {
+        if (D >= 64 && tid == 0) {
             mbar_expect_tx(full, kOwnBytes);
 #pragma unroll
             for (int hf = 0; hf < NH; ++hf) {
@@ -194,6 +199,7 @@ wsb_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUte
                 if (rg < p.n) {
 #pragma unroll
                     for (int hf = 0; hf < NH; ++hf) {
+                        if (c8 >= NCH) continue;
                         const uint4 a = __ldg(reinterpret_cast<const uint4*>(p.o + (size_t)rg * rowe + hoff + hf * 64) + c8);
                         const uint4 b = __ldg(reinterpret_cast<const uint4*>(p.gdo + (size_t)rg * rowe + hoff + hf * 64) + c8);
                         fma_bf16x2(a.x, b.x, d0, d1); fma_bf16x2(a.y, b.y, d0, d1);
@@ -208,7 +214,17 @@ wsb_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUte
             __syncwarp();
             dtil = s_dt[tid];
         }
-        mbar_wait(full, (uint32_t)h & 1u);
+        if constexpr (D >= 64) {
+            mbar_wait(full, (uint32_t)h & 1u);
+        } else {
+            // head_dim 32: a 64-byte head slice is no TMA box of the 128-byte-swizzled tile; the threads place the own
+            // rows themselves, upper 32 channels zero (made visible to the tensor core by the fence of the first step)
+            s_col[tid] = rvalid ? row : -1;
+            __syncthreads();
+            gather_tile<NH, NCH>(sX, p.ox, s_col, rowe, hoff, tid);
+            if (BWD) gather_tile<NH, NCH>(sY, p.oy, s_col, rowe, hoff, tid);
+            __syncthreads();
+        }
 
         for (int s = 0; s < n_steps; ++s) {
             // ---- column of this thread's slot (window wl, position rr of the TCB pair) and this row's 16 mask bits
@@ -249,8 +265,8 @@ wsb_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUte
                 }
             }
             // ---- gathered tiles
-            gather_tile<NH>(sGx, p.gx, s_col, rowe, hoff, tid);
-            gather_tile<NH>(sGy, p.gy, s_col, rowe, hoff, tid);
+            gather_tile<NH, NCH>(sGx, p.gx, s_col, rowe, hoff, tid);
+            gather_tile<NH, NCH>(sGy, p.gy, s_col, rowe, hoff, tid);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncthreads();
@@ -464,7 +480,7 @@ wsb_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUte
 }
 
 template <int MODE, int D> size_t wsb_smem_bytes() {
-    constexpr int NH = D / 64;
+    constexpr int NH = D >= 64 ? D / 64 : 1;
     constexpr bool BWD = MODE != kFwd;
     const size_t own = (size_t)(BWD ? 2 : 1) * NH * kHT;
     const size_t pad = (!BWD && NH * kHT < kWBytes) ? kWBytes - NH * kHT : 0;
@@ -502,8 +518,8 @@ bool wsb_check(const gnn_plan* P, const int32_t* rowptr, const int32_t* colidx, 
                   P->wsb.n_dup);
         return false;
     }
-    if (dtype != GNN_BF16 || (head_dim != 64 && head_dim != 128) || heads < 1) {
-        set_error("%s: unsupported shape heads=%d head_dim=%d dtype=%d (bf16, head_dim 64 or 128)", who, heads, head_dim, dtype);
+    if (dtype != GNN_BF16 || (head_dim != 32 && head_dim != 64 && head_dim != 128) || heads < 1) {
+        set_error("%s: unsupported shape heads=%d head_dim=%d dtype=%d (bf16, head_dim 32, 64 or 128)", who, heads, head_dim, dtype);
         return false;
     }
     rc = GNN_OK;
@@ -527,7 +543,7 @@ extern "C" gnn_status_t gnn_gt_attn_fwd_wsb(const gnn_plan_t* P, const int32_t* 
         return GNN_EINVAL;
     }
     CUtensorMap tmq;
-    if (!tc::encode_row_tile_map(&tmq, q, n, heads * head_dim, 64, kTile)) {
+    if (!tc::encode_row_tile_map(&tmq, q, n, heads * head_dim, head_dim < 64 ? head_dim : 64, kTile)) {
         set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who);
         return GNN_ECUDA;
     }
@@ -535,10 +551,12 @@ extern "C" gnn_status_t gnn_gt_attn_fwd_wsb(const gnn_plan_t* P, const int32_t* 
     p.row_offset = P->wsb.row_offset; p.cols = P->wsb.cols; p.bitmap = P->wsb.bitmap;
     p.n_win = (n + 15) / 16; p.n = n; p.H = heads;
     p.gx = (const __nv_bfloat16*)k; p.gy = (const __nv_bfloat16*)v;
+    p.ox = (const __nv_bfloat16*)q; p.oy = nullptr;
     p.out = (__nv_bfloat16*)out; p.lse_out = lse;
     p.sscale = kLog2e / sqrtf((float)head_dim); p.inv_sqrt_d = 1.f / sqrtf((float)head_dim);
-    cudaError_t e = head_dim == 64 ? launch_wsb<kFwd, 64>(tmq, tmq, p, "gt_fwd_wsb", (cudaStream_t)stream)
-                                   : launch_wsb<kFwd, 128>(tmq, tmq, p, "gt_fwd_wsb", (cudaStream_t)stream);
+    cudaError_t e = head_dim == 64   ? launch_wsb<kFwd, 64>(tmq, tmq, p, "gt_fwd_wsb", (cudaStream_t)stream)
+                    : head_dim == 128 ? launch_wsb<kFwd, 128>(tmq, tmq, p, "gt_fwd_wsb", (cudaStream_t)stream)
+                                      : launch_wsb<kFwd, 32>(tmq, tmq, p, "gt_fwd_wsb", (cudaStream_t)stream);
     if (e != cudaSuccess) { set_error("%s: CUDA error: %s", who, cudaGetErrorString(e)); return GNN_ECUDA; }
     return GNN_OK;
 }
@@ -559,10 +577,10 @@ extern "C" gnn_status_t gnn_gt_attn_bwd_wsb(const gnn_plan_t* P, const int32_t* 
         set_error("%s: feature / gradient pointers must be 32-byte aligned", who);
         return GNN_EINVAL;
     }
-    const int R = heads * head_dim;
+    const int R = heads * head_dim, bc = head_dim < 64 ? head_dim : 64;
     CUtensorMap tmq, tmdo, tmk, tmv;
-    if (!tc::encode_row_tile_map(&tmq, q, n, R, 64, kTile) || !tc::encode_row_tile_map(&tmdo, dout, n, R, 64, kTile) ||
-        !tc::encode_row_tile_map(&tmk, k, n, R, 64, kTile) || !tc::encode_row_tile_map(&tmv, v, n, R, 64, kTile)) {
+    if (!tc::encode_row_tile_map(&tmq, q, n, R, bc, kTile) || !tc::encode_row_tile_map(&tmdo, dout, n, R, bc, kTile) ||
+        !tc::encode_row_tile_map(&tmk, k, n, R, bc, kTile) || !tc::encode_row_tile_map(&tmv, v, n, R, bc, kTile)) {
         set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who);
         return GNN_ECUDA;
     }
@@ -575,16 +593,20 @@ extern "C" gnn_status_t gnn_gt_attn_bwd_wsb(const gnn_plan_t* P, const int32_t* 
     p.row_offset = P->wsb.row_offset; p.cols = P->wsb.cols; p.bitmap = P->wsb.bitmap;
     p.gx = (const __nv_bfloat16*)k; p.gy = (const __nv_bfloat16*)v;
     p.o = (const __nv_bfloat16*)out; p.gdo = (const __nv_bfloat16*)dout;
+    p.ox = (const __nv_bfloat16*)q; p.oy = (const __nv_bfloat16*)dout;
     p.o1 = dq; p.delta_out = delta;
-    cudaError_t e = head_dim == 64 ? launch_wsb<kBwdDst, 64>(tmq, tmdo, p, "gt_bwd_wsb_dst", st)
-                                   : launch_wsb<kBwdDst, 128>(tmq, tmdo, p, "gt_bwd_wsb_dst", st);
+    cudaError_t e = head_dim == 64   ? launch_wsb<kBwdDst, 64>(tmq, tmdo, p, "gt_bwd_wsb_dst", st)
+                    : head_dim == 128 ? launch_wsb<kBwdDst, 128>(tmq, tmdo, p, "gt_bwd_wsb_dst", st)
+                                      : launch_wsb<kBwdDst, 32>(tmq, tmdo, p, "gt_bwd_wsb_dst", st);
     // src side over the WSB of CSR^T: dK, dV
     if (e == cudaSuccess) {
         p.row_offset = P->wsb_t.row_offset; p.cols = P->wsb_t.cols; p.bitmap = P->wsb_t.bitmap;
         p.gx = (const __nv_bfloat16*)q; p.gy = (const __nv_bfloat16*)dout;
+        p.ox = (const __nv_bfloat16*)k; p.oy = (const __nv_bfloat16*)v;
         p.delta_in = delta; p.o1 = dv; p.o2 = dk;
-        e = head_dim == 64 ? launch_wsb<kBwdSrc, 64>(tmk, tmv, p, "gt_bwd_wsb_src", st)
-                           : launch_wsb<kBwdSrc, 128>(tmk, tmv, p, "gt_bwd_wsb_src", st);
+        e = head_dim == 64   ? launch_wsb<kBwdSrc, 64>(tmk, tmv, p, "gt_bwd_wsb_src", st)
+            : head_dim == 128 ? launch_wsb<kBwdSrc, 128>(tmk, tmv, p, "gt_bwd_wsb_src", st)
+                              : launch_wsb<kBwdSrc, 32>(tmk, tmv, p, "gt_bwd_wsb_src", st);
     }
     if (e != cudaSuccess) { set_error("%s: CUDA error: %s", who, cudaGetErrorString(e)); return GNN_ECUDA; }
     return GNN_OK;

@@ -491,7 +491,7 @@ def test_wsb_layout_bit_exact():
     assert plan.wsb_info()["n_tcb"] == 0 and not plan.export(B.GNN_PLAN_WSB_ROW_OFFSET).any()
 
 
-@pytest.mark.parametrize("heads,d", [(1, 64), (8, 64), (3, 128)])
+@pytest.mark.parametrize("heads,d", [(1, 64), (8, 64), (3, 128), (8, 32), (1, 32)])
 def test_wsb_tensor_core_forward_backward(heads, d):
     """Row f2: GT attention on the general WSB layout, forward and tensor-core backward, against the
     fp64 oracle (the same functions as the CSR entry points): the locally dense config scaled (ragged last tile), a graph
@@ -539,7 +539,7 @@ def test_wsb_tensor_core_forward_backward(heads, d):
     with pytest.raises(G.GnnError, match="GNN_BLOCKS_WSB"):
         G.gnn_gt_attn_fwd_wsb(plan, q, q, q, torch.empty_like(q), torch.empty((c["n"], heads), device="cuda"))
     planw = und["plan"]
-    q3 = torch.zeros((c["n"], 2, 32), dtype=torch.bfloat16, device="cuda")
+    q3 = torch.zeros((c["n"], 2, 16), dtype=torch.bfloat16, device="cuda")
     with pytest.raises(G.GnnError, match="unsupported shape"):
         G.gnn_gt_attn_fwd_wsb(planw, q3, q3, q3, torch.empty_like(q3), torch.empty((c["n"], 2), device="cuda"))
 
