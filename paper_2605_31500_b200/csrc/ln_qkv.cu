@@ -13,13 +13,19 @@
 // tcgen05.mma 128 x 128 x 16 into 128-column TMEM accumulators; eight epilogue warps (two per TMEM lane quarter, one
 // 64-column half each) drain a finished accumulator (tcgen05.ld, + bias, bf16, swizzled staging buffer, TMA store)
 // while the MMA warp fills the next one.  Two kernels:
-//   C <= 256  ln_qkv_persist_kernel: one CTA per SM walks its tiles with TWO A tiles and four accumulators, so the x
-//             tile of tile t + 1 lands and is normalised while tile t is multiplied and drained; output staging in
-//             128-byte rows (one TMA store per chunk and warp).
+//   C <= 256  ln_qkv_persist_kernel: persistent CTAs (608 threads: 8 epilogue warps, weight-TMA / MMA / x-TMA warps, 8
+//             LayerNorm warps) with TWO A tiles, so the x tile of tile t + 1 lands and is normalised while tile t is
+//             multiplied and drained; output staging in 128-byte rows (one TMA store per chunk and warp).
+//             PAIR form (default when 3 H d is a multiple of 256): clusters of two CTAs on an SM pair; the rank-0 CTA issues
+//             tcgen05.mma.cta_group::2 256 x 256 x 16 - each CTA contributes its own 128-row A tile and 128 of the 256
+//             weight rows of a stage (TMA .cta_group::2 completing on rank 0's barrier), results land in each CTA's own
+//             TMEM (two 256-column accumulators); commits are multicast to both CTAs' barriers and the peer's warps
+//             report to rank 0's barriers through the cluster.  Half the operand bytes per flop of the single-CTA form
+//             (A and B are read from shared memory once per 256 outputs / 256 rows) - which is what the single-CTA form
+//             is bound by - and half the weight bytes per SM.
 //   C <= 512  ln_qkv_kernel: one CTA per tile (the 128 KB A tile leaves no room for a second one), two accumulators,
 //             output staging in 32-byte rows.
-// Measured limit of both (profiles/r02_ncu_ln_qkv.md): every tile re-streams the whole weight matrix from L2 and the
-// shared memory left beside the A tiles holds four stages, i.e. 64 KB in flight against ~1.5 us of L2 latency.
+// Measurements and what limits each form: profiles/r02_ncu_ln_qkv.md.
 #include <cuda.h>
 #include <cuda_bf16.h>
 
@@ -144,8 +150,9 @@ struct Epi {           // W = 64: one 4 KB buffer per warp, 128-byte rows (SWIZZ
     uint8_t* stage;
     uint32_t lane_off, my, sw;
     int q4, hsel, lane, n_st;
-    __device__ __forceinline__ void init(const LnQkvParams& p, uint8_t* sT, int warp, int lane_) {
-        q4 = warp & 3; hsel = warp >> 2; lane = lane_; n_st = 0;
+    bool to_leader;        // CTA pairs: "drained" is the barrier of the pair's rank-0 CTA (which issues the MMAs)
+    __device__ __forceinline__ void init(const LnQkvParams& p, uint8_t* sT, int warp, int lane_, bool to_leader_ = false) {
+        q4 = warp & 3; hsel = warp >> 2; lane = lane_; n_st = 0; to_leader = to_leader_;
         lane_off = (uint32_t)(q4 * 32) << 16;
         stage = sT + warp * kBytes;
         if (W == 16) { my = (uint32_t)lane * 32; sw = ((uint32_t)(lane >> 2) & 1u) << 4; }
@@ -158,7 +165,8 @@ struct Epi {           // W = 64: one 4 KB buffer per warp, 128-byte rows (SWIZZ
     // output chunk c (columns c * 128 ..) of the tile at row0 from the complete accumulator at TMEM column t_acc; arrives
     // on `drained` after the last TMEM read
     __device__ __forceinline__ void chunk(const LnQkvParams& p, uint32_t t_acc, uint64_t* drained, int c, int n_chunks, int row0,
-                                          const CUtensorMap* tmq, const CUtensorMap* tmk, const CUtensorMap* tmv) {
+                                          const CUtensorMap* tmq, const CUtensorMap* tmk, const CUtensorMap* tmv,
+                                          bool last = true) {
         const int col0 = c * kNC + 64 * hsel;
         const int t = col0 / p.R, off = col0 - t * p.R;
         const CUtensorMap* tmo = t == 0 ? tmq : (t == 1 ? tmk : tmv);
@@ -170,7 +178,10 @@ struct Epi {           // W = 64: one 4 KB buffer per warp, 128-byte rows (SWIZZ
             if (c0 == 32) {                                 // last read of this accumulator half: hand it back to the MMA warp
                 asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
                 __syncwarp();
-                if (lane == 0) mbar_arrive(drained);
+                if (lane == 0 && last) {
+                    if (to_leader) mbar_arrive_cluster_relaxed(drained, 0);
+                    else mbar_arrive(drained);
+                }
             }
             if (p.bias) {
 #pragma unroll
@@ -354,8 +365,11 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ C
 // warp 9 MMA issue; warp 10 x tiles (TMA).  Barriers: xfull[b] (x tile landed in A[b]), aready[b] (A[b] normalised, 8
 // warp arrivals), afree[b] (tcgen05.commit after the last product of the tile in A[b]), full / empty (weight ring),
 // tfull / tempty (accumulators).
-constexpr int kPThreads = 352;
+constexpr int kPThreads = 608;       // warps 0-7 epilogue, 8 weight TMA, 9 MMA, 10 x TMA, 11-18 LayerNorm
+constexpr int kLnWarp0 = 11;
 constexpr int kAcc = 4;
+template <bool PAIR>   // PAIR: clusters of two CTAs; one tcgen05.mma.cta_group::2 (M = 256) multiplies both CTAs' tiles against
+                       // a weight stage of which each CTA loads one half: half the weight bytes per SM, twice the stages
 __global__ void __launch_bounds__(kPThreads, 1)
 ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmw,
                       const __grid_constant__ CUtensorMap tmq, const __grid_constant__ CUtensorMap tmk,
@@ -364,8 +378,13 @@ ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_cons
     uint8_t* smem = smem_raw + kBars + ((1024u - ((smem_u32(smem_raw) + kBars) & 1023u)) & 1023u);
     const int KC = p.C / 64, NS = p.n_stages;
     uint8_t* sA = smem;                                   // [2][KC] half tiles
+    // PAIR: accumulators of 256 columns (MMA 256 x 256 x 16 over the pair): every A byte read from shared memory feeds 256
+    // outputs and every CTA loads 128 of a stage's 256 weight rows - half the operand bytes per flop of the single-CTA form
+    constexpr int NCc = PAIR ? 256 : kNC;                 // output columns per accumulator / weight stage
+    constexpr int NACC = 512 / NCc;                       // accumulators in the 512 TMEM columns
+    constexpr int kW = kStage;                            // bytes of this CTA's part of a weight stage (128 rows x 64 channels)
     uint8_t* sB = sA + 2 * KC * kStage;                   // [NS] weight stages
-    uint8_t* sT = sB + NS * kStage;                       // [kWorkWarps] staging buffers of 32 rows x 128 bytes
+    uint8_t* sT = sB + NS * kW;                           // [kWorkWarps] staging buffers of 32 rows x 128 bytes
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
     uint64_t* empty = full + 8;
     uint64_t* tfull = empty + 8;                          // [kAcc]
@@ -382,23 +401,35 @@ ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_cons
         asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
         if ((uint32_t)(sT + kWorkWarps * Epi<64>::kBytes - smem_raw) > dyn) __trap();
     }
-    const int n_chunks = 3 * p.R / kNC;
+    const int n_chunks = 3 * p.R / NCc;
     const int tiles = (p.n + kRows - 1) / kRows;
-    const int nlt = ((int)blockIdx.x < tiles) ? (tiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;   // this CTA's tiles
-    auto tile_row0 = [&](int lt) { return ((int)blockIdx.x + lt * (int)gridDim.x) * kRows; };
+    // walkers: single CTAs over the tiles, or CTA pairs over pairs of consecutive tiles (rank r takes tile 2 * pair + r; both
+    // CTAs of a pair run the same number of iterations - a tile past the end is skipped where it touches memory)
+    const uint32_t rank = PAIR ? cluster_ctarank() : 0u;
+    const int nwalk = PAIR ? (int)gridDim.x / 2 : (int)gridDim.x, me = PAIR ? (int)blockIdx.x / 2 : (int)blockIdx.x;
+    const int nunits = PAIR ? (tiles + 1) / 2 : tiles;
+    const int nlt = me < nunits ? (nunits - 1 - me) / nwalk + 1 : 0;
+    auto tile_row0 = [&](int lt) { return ((me + lt * nwalk) * (PAIR ? 2 : 1) + (int)rank) * kRows; };
 
     if (tid == 0) {
         for (int s = 0; s < NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
-        for (int b = 0; b < kAcc; ++b) { mbar_init(tfull + b, 1); mbar_init(tempty + b, kWorkWarps); }
-        for (int b = 0; b < 2; ++b) { mbar_init(xfull + b, 1); mbar_init(aready + b, kWorkWarps); mbar_init(afree + b, 1); }
+        constexpr int kArr = kWorkWarps * (PAIR ? 2 : 1);   // worker-warp arrivals: both CTAs of a pair report to rank 0
+        for (int b = 0; b < NACC; ++b) { mbar_init(tfull + b, 1); mbar_init(tempty + b, kArr); }
+        for (int b = 0; b < 2; ++b) { mbar_init(xfull + b, 1); mbar_init(aready + b, kArr); mbar_init(afree + b, 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 9) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        if (PAIR) {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (PAIR) cluster_sync_all();     // the peer's barriers exist before anything signals them
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = *tmem_slot;
 
@@ -407,6 +438,7 @@ ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_cons
         if (lane == 0) {
             for (int lt = 0; lt < nlt; ++lt) {
                 const int b = lt & 1;
+                if (tile_row0(lt) >= p.n) continue;          // (pairs) the odd tile past the end: nothing to load
                 mbar_wait(afree + b, (uint32_t)((lt >> 1) & 1) ^ 1u);
                 mbar_expect_tx(xfull + b, KC * kStage);
                 for (int kk = 0; kk < KC; ++kk) tma_load_2d(sA + (b * KC + kk) * kStage, &tmx, kk * 64, tile_row0(lt), xfull + b);
@@ -419,66 +451,91 @@ ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_cons
             for (int i = 0; i < items; ++i) {
                 const int s = i % NS, j = i % per_tile;
                 mbar_wait(empty + s, (uint32_t)((i / NS) & 1) ^ 1u);
-                mbar_expect_tx(full + s, kStage);
-                tma_load_2d(sB + s * kStage, &tmw, (j % KC) * 64, (j / KC) * kNC, full + s);
+                if (!PAIR) {
+                    mbar_expect_tx(full + s, kStage);
+                    tma_load_2d(sB + s * kW, &tmw, (j % KC) * 64, (j / KC) * NCc, full + s);
+                } else {
+                    // this CTA's 128 of the stage's 256 weight rows; both halves complete on rank 0's barrier
+                    if (rank == 0) mbar_expect_tx(full + s, 2 * kStage);
+                    tma_load_2d_pair(sB + s * kW, &tmw, (j % KC) * 64, (j / KC) * NCc + (int)rank * (NCc / 2), full + s);
+                }
             }
         }
     } else if (warp == 9) {
-        // ===== MMA issuer
-        if (lane == 0) {
-            constexpr uint32_t kIdesc = make_idesc(kRows, kNC, false);
+        // ===== MMA issuer (pairs: rank 0 only)
+        if (lane == 0 && rank == 0) {
+            constexpr uint32_t kIdesc = make_idesc(PAIR ? 2 * kRows : kRows, NCc, false);
+            auto commit = [&](uint64_t* bar) {
+                if (PAIR) umma2_commit_mc(bar, (uint16_t)3);
+                else umma_commit(bar);
+            };
             int i = 0, g = 0;
             for (int lt = 0; lt < nlt; ++lt) {
                 const int b = lt & 1;
                 mbar_wait(aready + b, (uint32_t)((lt >> 1) & 1));
                 for (int c = 0; c < n_chunks; ++c, ++g) {
-                    const int acc = g % kAcc;
-                    mbar_wait(tempty + acc, (uint32_t)((g / kAcc) & 1) ^ 1u);
+                    const int acc = g % NACC;
+                    mbar_wait(tempty + acc, (uint32_t)((g / NACC) & 1) ^ 1u);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     for (int kk = 0; kk < KC; ++kk, ++i) {
                         const int s = i % NS;
                         mbar_wait(full + s, (uint32_t)((i / NS) & 1));
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
-                        for (int ks = 0; ks < 4; ++ks)
-                            umma(tmem + acc * kNC, make_desc_sw128(smem_u32(sA + (b * KC + kk) * kStage) + ks * 32, 1024),
-                                 make_desc_sw128(smem_u32(sB + s * kStage) + ks * 32, 1024), kIdesc, (kk | ks) > 0);
-                        umma_commit(empty + s);
+                        for (int ks = 0; ks < 4; ++ks) {
+                            const uint64_t da = make_desc_sw128(smem_u32(sA + (b * KC + kk) * kStage) + ks * 32, 1024);
+                            const uint64_t db = make_desc_sw128(smem_u32(sB + s * kW) + ks * 32, 1024);
+                            if (PAIR) umma2(tmem + acc * NCc, da, db, kIdesc, (kk | ks) > 0);
+                            else umma(tmem + acc * NCc, da, db, kIdesc, (kk | ks) > 0);
+                        }
+                        commit(empty + s);
                     }
-                    umma_commit(tfull + acc);
+                    commit(tfull + acc);
                 }
-                umma_commit(afree + b);
+                commit(afree + b);
+            }
+        }
+    } else if (warp >= kLnWarp0) {
+        // ===== LayerNorm warps: tile lt in A[lt & 1] as soon as its x tile has landed (runs ahead of / under the epilogue)
+        for (int lt = 0; lt < nlt; ++lt) {
+            const int b = lt & 1;
+            if (tile_row0(lt) < p.n) {
+                mbar_wait(xfull + b, (uint32_t)((lt >> 1) & 1));
+                ln_rows<2>(sA + b * KC * kStage, p, tile_row0(lt), warp - kLnWarp0, lane);
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) {
+                if (PAIR) mbar_arrive_cluster(aready + b, 0);
+                else mbar_arrive(aready + b);
             }
         }
     } else if (warp < kWorkWarps) {
-        // ===== workers: LayerNorm of the NEXT tile, then the epilogue of the current one
+        // ===== epilogue warps
         Epi<64> ep;
-        ep.init(p, sT, warp, lane);
-        auto normalise = [&](int lt) {
-            const int b = lt & 1;
-            mbar_wait(xfull + b, (uint32_t)((lt >> 1) & 1));
-            ln_rows<2>(sA + b * KC * kStage, p, tile_row0(lt), warp, lane);
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) mbar_arrive(aready + b);
-        };
-        if (nlt > 0) normalise(0);
+        ep.init(p, sT, warp, lane, PAIR);
         int g = 0;
         for (int lt = 0; lt < nlt; ++lt) {
             for (int c = 0; c < n_chunks; ++c, ++g) {
-                // the next tile's LayerNorm goes after the first drained chunk: its x tile (issued when the products of
-                // tile lt - 1 left the buffer) has landed by then, and the MMA warp is still up to three chunks ahead
-                if (c == (n_chunks > 1 ? 1 : 0) && lt + 1 < nlt) normalise(lt + 1);
-                const int acc = g % kAcc;
-                mbar_wait(tfull + acc, (uint32_t)((g / kAcc) & 1));
-                ep.chunk(p, tmem + acc * kNC, tempty + acc, c, n_chunks, tile_row0(lt), &tmq, &tmk, &tmv);
+                const int acc = g % NACC;
+                mbar_wait(tfull + acc, (uint32_t)((g / NACC) & 1));
+                if (PAIR) {     // a 256-column accumulator leaves as two 128-column output chunks
+                    ep.chunk(p, tmem + acc * NCc, tempty + acc, 2 * c, 2 * n_chunks, tile_row0(lt), &tmq, &tmk, &tmv, false);
+                    ep.chunk(p, tmem + acc * NCc + kNC, tempty + acc, 2 * c + 1, 2 * n_chunks, tile_row0(lt), &tmq, &tmk, &tmv);
+                } else {
+                    ep.chunk(p, tmem + acc * NCc, tempty + acc, c, n_chunks, tile_row0(lt), &tmq, &tmk, &tmv);
+                }
             }
         }
         if (lane == 0) tma_store_wait<0>();
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 9) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+    if (PAIR) cluster_sync_all();     // no CTA leaves (or frees TMEM) while its peer may still signal it / multiply into it
+    if (warp == 9) {
+        if (PAIR) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+        else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+    }
 }
 
 }  // namespace
@@ -532,14 +589,39 @@ extern "C" gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, i
         p.n_stages = (int)((226 * 1024 - fixed) / kStage);
         if (p.n_stages > 8) p.n_stages = 8;
         const size_t smem = fixed + (size_t)p.n_stages * kStage;
-        e = cudaFuncSetAttribute(ln_qkv_persist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) {
-            prof_begin("ln_qkv", "gemm", st);
-            ln_qkv_persist_kernel<<<tiles < sms ? tiles : sms, kPThreads, smem, st>>>(tmx, tmw, tmq, tmk, tmv, p);
-            prof_end(st);
-            count_launch();
-            e = cudaGetLastError();
+        // CTA pairs (256 x 256 x 16 MMAs over two SMs) whenever the outputs split into 256-column accumulators; single CTAs
+        // otherwise, and as the fallback if the cluster launch is refused (e.g. a partitioned GPU without free SM pairs)
+        static const bool no_pair = [] { const char* v = getenv("GNN_LNQKV_NO_PAIR"); return v && atoi(v) != 0; }();
+        bool pair = !no_pair && (3 * R) % 256 == 0 && tiles > 1 && sms >= 2;
+        for (int attempt = 0; attempt < 2; ++attempt) {
+            CUtensorMap tmw_k = tmw;
+            if (pair && !tc::encode_row_tile_map(&tmw_k, w, (int)(3 * R), c_in, 64, 128)) {   // a CTA's 128 of a stage's 256 rows
+                set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who);
+                return GNN_ECUDA;
+            }
+            auto kern = pair ? ln_qkv_persist_kernel<true> : ln_qkv_persist_kernel<false>;
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e == cudaSuccess) {
+                const int units = pair ? (tiles + 1) / 2 : tiles, walkers = pair ? sms / 2 : sms;
+                cudaLaunchConfig_t cfg = {};
+                cfg.gridDim = dim3((units < walkers ? units : walkers) * (pair ? 2 : 1));
+                cfg.blockDim = dim3(kPThreads);
+                cfg.dynamicSmemBytes = smem;
+                cfg.stream = st;
+                cudaLaunchAttribute attr[1];
+                attr[0].id = cudaLaunchAttributeClusterDimension;
+                attr[0].val.clusterDim.x = pair ? 2 : 1; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+                cfg.attrs = attr; cfg.numAttrs = 1;
+                prof_begin("ln_qkv", "gemm", st);
+                e = cudaLaunchKernelEx(&cfg, kern, tmx, tmw_k, tmq, tmk, tmv, p);
+                prof_end(st);
+                if (e == cudaSuccess) e = cudaGetLastError();
+            }
+            if (e == cudaSuccess || !pair) break;
+            (void)cudaGetLastError();      // the pair launch was refused: clear the error and run the single-CTA form
+            pair = false;
         }
+        if (e == cudaSuccess) count_launch();
     } else {
         // weight ring: as many 16 KB stages as keep two CTAs per SM (113 KB each) when the A tile allows it, else one CTA
         const size_t fixed = (size_t)(c_in / 64) * kStage + (size_t)kWorkWarps * 2 * kOut + 1024;   // 1024 = barriers + alignment pad
