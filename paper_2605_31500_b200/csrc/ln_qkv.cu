@@ -174,7 +174,18 @@ struct Epi {           // W = 64: one 4 KB buffer per warp, 128-byte rows (SWIZZ
 #pragma unroll 1
         for (int c0 = 0; c0 < 64; c0 += 32) {
             float t32[32];
-            tmem_ld32(t_acc + lane_off + 64 * hsel + c0, t32);
+            if (W == 64 && c0 == 0 && n_st > 0) {
+                // the wait for the staging buffer (the previous chunk's TMA store reading it) hides under the TMEM read
+                uint32_t r32[32];
+                tmem_ld32_issue(t_acc + lane_off + 64 * hsel, r32);
+                if (lane == 0) tma_store_wait_read<0>();
+                __syncwarp();
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 32; ++i) t32[i] = __uint_as_float(r32[i]);
+            } else {
+                tmem_ld32(t_acc + lane_off + 64 * hsel + c0, t32);
+            }
             if (c0 == 32) {                                 // last read of this accumulator half: hand it back to the MMA warp
                 asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
                 __syncwarp();
@@ -218,10 +229,6 @@ struct Epi {           // W = 64: one 4 KB buffer per warp, 128-byte rows (SWIZZ
                     }
                 }
             } else {
-                if (c0 == 0 && n_st > 0) {                  // the previous chunk's store has read the buffer
-                    if (lane == 0) tma_store_wait_read<0>();
-                    __syncwarp();
-                }
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     uint32_t o[4];
