@@ -140,6 +140,74 @@ __device__ __forceinline__ void ln_rows(uint8_t* sA, const LnQkvParams& p, int r
     }
 }
 
+// The same for rows too wide to keep in registers (C > 256: up to 256 channels per lane): three sweeps over the lane's
+// half tiles - sum, centred squares, normalise + write - re-reading shared memory, 8 chunks (one half tile) live at a time.
+__device__ __forceinline__ void ln_rows_stream(uint8_t* sA, const LnQkvParams& p, int row0, int warp, int lane) {
+    const int KC = p.C / 64, KH = (KC + 1) / 2;
+    const int r = warp * 16 + (lane & 15), kk0 = (lane >> 4) * KH, kk1 = min(KC, kk0 + KH);
+    const uint32_t rbase = (uint32_t)((r >> 3) * 1024 + (r & 7) * 128), rx = (uint32_t)(r & 7);
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+#pragma unroll 1
+    for (int kk = kk0; kk < kk1; ++kk) {
+#pragma unroll
+        for (int cc = 0; cc < 8; ++cc) {
+            const uint4 w = *reinterpret_cast<const uint4*>(sA + kk * kStage + rbase + (((uint32_t)cc ^ rx) << 4));
+            add_bf16x2(w.x, s0, s1, s0, s1); add_bf16x2(w.y, s2, s3, s2, s3);
+            add_bf16x2(w.z, s0, s1, s0, s1); add_bf16x2(w.w, s2, s3, s2, s3);
+        }
+    }
+    float sum = (s0 + s1) + (s2 + s3);
+    sum += __shfl_xor_sync(0xffffffffu, sum, 16);
+    const float inv_c = 1.f / (float)p.C;
+    const float nmean = -sum * inv_c;
+    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+#pragma unroll 1
+    for (int kk = kk0; kk < kk1; ++kk) {
+#pragma unroll
+        for (int cc = 0; cc < 8; ++cc) {
+            const uint4 w4 = *reinterpret_cast<const uint4*>(sA + kk * kStage + rbase + (((uint32_t)cc ^ rx) << 4));
+            const uint32_t w[4] = {w4.x, w4.y, w4.z, w4.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                float a, b;
+                add_bf16x2(w[i], nmean, nmean, a, b);
+                if (i & 1) fma2v(q2, q3, a, b, a, b);
+                else fma2v(q0, q1, a, b, a, b);
+            }
+        }
+    }
+    float ss = (q0 + q1) + (q2 + q3);
+    ss += __shfl_xor_sync(0xffffffffu, ss, 16);
+    const bool rv = row0 + r < p.n;
+    const float rstd = rv ? 1.f / sqrtf(ss * inv_c + p.eps) : 0.f;
+#pragma unroll 1
+    for (int kk = kk0; kk < kk1; ++kk) {
+#pragma unroll
+        for (int cc = 0; cc < 8; ++cc) {
+            const int ch = kk * 64 + cc * 8;
+            uint8_t* at = sA + kk * kStage + rbase + (((uint32_t)cc ^ rx) << 4);
+            const uint4 w4 = *reinterpret_cast<const uint4*>(at);
+            const float4 g0 = __ldg(reinterpret_cast<const float4*>(p.gamma + ch)), g1 = __ldg(reinterpret_cast<const float4*>(p.gamma + ch + 4));
+            float4 b0 = __ldg(reinterpret_cast<const float4*>(p.beta + ch)), b1 = __ldg(reinterpret_cast<const float4*>(p.beta + ch + 4));
+            if (!rv) { b0 = make_float4(0.f, 0.f, 0.f, 0.f); b1 = b0; }
+            const uint32_t w[4] = {w4.x, w4.y, w4.z, w4.w};
+            const float gg[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
+            float zz[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+            uint32_t o[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                float y0, y1;
+                add_bf16x2(w[i], nmean, nmean, y0, y1);
+                mul2(y0, y1, rstd);
+                fma2v(zz[2 * i], zz[2 * i + 1], y0, y1, gg[2 * i], gg[2 * i + 1]);
+                const __nv_bfloat162 yb = __floats2bfloat162_rn(zz[2 * i], zz[2 * i + 1]);
+                o[i] = *reinterpret_cast<const uint32_t*>(&yb);
+            }
+            *reinterpret_cast<uint4*>(at) = make_uint4(o[0], o[1], o[2], o[3]);
+        }
+    }
+}
+
 // epilogue state of one worker warp: warp w drains TMEM lanes 32 (w & 3) .. +31 (tile rows) of column half w >> 2 of every
 // accumulator: accumulator -> + bias -> bf16 -> 32-row x 16-column staging buffer (the layout TMA's 32-byte swizzle expects)
 // -> one TMA store per buffer (rows past n are clipped by the unit); the warp's two staging buffers alternate
@@ -375,7 +443,8 @@ ln_qkv_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ C
 constexpr int kPThreads = 608;       // warps 0-7 epilogue, 8 weight TMA, 9 MMA, 10 x TMA, 11-18 LayerNorm
 constexpr int kLnWarp0 = 11;
 constexpr int kAcc = 4;
-template <bool PAIR>   // PAIR: clusters of two CTAs; one tcgen05.mma.cta_group::2 (M = 256) multiplies both CTAs' tiles against
+template <bool PAIR, int NBUF>   // NBUF: A tiles per CTA (2 for C <= 256; 1 for C <= 512: no room for a second);
+                                 // PAIR: clusters of two CTAs; one tcgen05.mma.cta_group::2 (M = 256) multiplies both CTAs' tiles against
                        // a weight stage of which each CTA loads one half: half the weight bytes per SM, twice the stages
 __global__ void __launch_bounds__(kPThreads, 1)
 ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUtensorMap tmw,
@@ -390,7 +459,7 @@ ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_cons
     constexpr int NCc = PAIR ? 256 : kNC;                 // output columns per accumulator / weight stage
     constexpr int NACC = 512 / NCc;                       // accumulators in the 512 TMEM columns
     constexpr int kW = kStage;                            // bytes of this CTA's part of a weight stage (128 rows x 64 channels)
-    uint8_t* sB = sA + 2 * KC * kStage;                   // [NS] weight stages
+    uint8_t* sB = sA + NBUF * KC * kStage;                // [NS] weight stages
     uint8_t* sT = sB + NS * kW;                           // [kWorkWarps] staging buffers of 32 rows x 128 bytes
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
     uint64_t* empty = full + 8;
@@ -444,9 +513,9 @@ ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_cons
         // ===== x tiles: tile lt -> A[lt & 1] once the products of tile lt - 2 have left it
         if (lane == 0) {
             for (int lt = 0; lt < nlt; ++lt) {
-                const int b = lt & 1;
+                const int b = lt % NBUF;
                 if (tile_row0(lt) >= p.n) continue;          // (pairs) the odd tile past the end: nothing to load
-                mbar_wait(afree + b, (uint32_t)((lt >> 1) & 1) ^ 1u);
+                mbar_wait(afree + b, (uint32_t)((lt / NBUF) & 1) ^ 1u);
                 mbar_expect_tx(xfull + b, KC * kStage);
                 for (int kk = 0; kk < KC; ++kk) tma_load_2d(sA + (b * KC + kk) * kStage, &tmx, kk * 64, tile_row0(lt), xfull + b);
             }
@@ -478,8 +547,8 @@ ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_cons
             };
             int i = 0, g = 0;
             for (int lt = 0; lt < nlt; ++lt) {
-                const int b = lt & 1;
-                mbar_wait(aready + b, (uint32_t)((lt >> 1) & 1));
+                const int b = lt % NBUF;
+                mbar_wait(aready + b, (uint32_t)((lt / NBUF) & 1));
                 for (int c = 0; c < n_chunks; ++c, ++g) {
                     const int acc = g % NACC;
                     mbar_wait(tempty + acc, (uint32_t)((g / NACC) & 1) ^ 1u);
@@ -505,10 +574,11 @@ ln_qkv_persist_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_cons
     } else if (warp >= kLnWarp0) {
         // ===== LayerNorm warps: tile lt in A[lt & 1] as soon as its x tile has landed (runs ahead of / under the epilogue)
         for (int lt = 0; lt < nlt; ++lt) {
-            const int b = lt & 1;
+            const int b = lt % NBUF;
             if (tile_row0(lt) < p.n) {
-                mbar_wait(xfull + b, (uint32_t)((lt >> 1) & 1));
-                ln_rows<2>(sA + b * KC * kStage, p, tile_row0(lt), warp - kLnWarp0, lane);
+                mbar_wait(xfull + b, (uint32_t)((lt / NBUF) & 1));
+                if (NBUF == 2) ln_rows<2>(sA + b * KC * kStage, p, tile_row0(lt), warp - kLnWarp0, lane);
+                else ln_rows_stream(sA + b * KC * kStage, p, tile_row0(lt), warp - kLnWarp0, lane);
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncwarp();
@@ -581,56 +651,59 @@ extern "C" gnn_status_t gnn_ln_qkv_fwd(int32_t n, int32_t c_in, int32_t heads, i
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e;
     const int tiles = (n + kRows - 1) / kRows;
-    if (c_in <= 256) {
-        // persistent kernel: two A tiles + staging + barriers, the rest of the 226 KB is the weight ring
-        int dev = 0, sms = 0;
-        e = cudaGetDevice(&dev);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) { set_error("%s: CUDA error: %s", who, cudaGetErrorString(e)); return GNN_ECUDA; }
-        if (!tc::encode_row_tile_map(&tmq, q, n, (int)R, 64, 32) || !tc::encode_row_tile_map(&tmk, k, n, (int)R, 64, 32) ||
-            !tc::encode_row_tile_map(&tmv, v, n, (int)R, 64, 32)) {      // output boxes of 32 rows x 128 bytes, SWIZZLE_128B
+    int dev = 0, sms = 0;
+    e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) { set_error("%s: CUDA error: %s", who, cudaGetErrorString(e)); return GNN_ECUDA; }
+    // Forms, in order of preference:
+    //   CTA pairs (256 x 256 x 16 MMAs over two SMs) whenever the outputs split into 256-column accumulators - persistent,
+    //     two A tiles for C <= 256, one for C <= 512;
+    //   single persistent CTAs for C <= 256 (also the fallback if the cluster launch is refused, e.g. a partitioned GPU
+    //     without free SM pairs);
+    //   one CTA per tile for 256 < C <= 512.
+    static const bool no_pair = [] { const char* v = getenv("GNN_LNQKV_NO_PAIR"); return v && atoi(v) != 0; }();
+    const bool wide = c_in > 256;
+    bool pair = !no_pair && (3 * R) % 256 == 0 && tiles > 1 && sms >= 2;
+    bool launched = false;
+    while (!wide || pair) {
+        const int nbuf = wide ? 1 : 2;
+        CUtensorMap oq, ok, ov, tmw_k = tmw;
+        if (!tc::encode_row_tile_map(&oq, q, n, (int)R, 64, 32) || !tc::encode_row_tile_map(&ok, k, n, (int)R, 64, 32) ||
+            !tc::encode_row_tile_map(&ov, v, n, (int)R, 64, 32) ||      // output boxes of 32 rows x 128 bytes, SWIZZLE_128B
+            (pair && !tc::encode_row_tile_map(&tmw_k, w, (int)(3 * R), c_in, 64, 128))) {   // a CTA's 128 of a stage's 256 rows
             set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who);
             return GNN_ECUDA;
         }
-        const size_t fixed = 2 * (size_t)(c_in / 64) * kStage + (size_t)kWorkWarps * 4096 + 1024;
+        const size_t fixed = (size_t)nbuf * (c_in / 64) * kStage + (size_t)kWorkWarps * 4096 + 1024;
         p.n_stages = (int)((226 * 1024 - fixed) / kStage);
         if (p.n_stages > 8) p.n_stages = 8;
         const size_t smem = fixed + (size_t)p.n_stages * kStage;
-        // CTA pairs (256 x 256 x 16 MMAs over two SMs) whenever the outputs split into 256-column accumulators; single CTAs
-        // otherwise, and as the fallback if the cluster launch is refused (e.g. a partitioned GPU without free SM pairs)
-        static const bool no_pair = [] { const char* v = getenv("GNN_LNQKV_NO_PAIR"); return v && atoi(v) != 0; }();
-        bool pair = !no_pair && (3 * R) % 256 == 0 && tiles > 1 && sms >= 2;
-        for (int attempt = 0; attempt < 2; ++attempt) {
-            CUtensorMap tmw_k = tmw;
-            if (pair && !tc::encode_row_tile_map(&tmw_k, w, (int)(3 * R), c_in, 64, 128)) {   // a CTA's 128 of a stage's 256 rows
-                set_error("%s: cuTensorMapEncodeTiled unavailable or failed", who);
-                return GNN_ECUDA;
-            }
-            auto kern = pair ? ln_qkv_persist_kernel<true> : ln_qkv_persist_kernel<false>;
-            e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e == cudaSuccess) {
-                const int units = pair ? (tiles + 1) / 2 : tiles, walkers = pair ? sms / 2 : sms;
-                cudaLaunchConfig_t cfg = {};
-                cfg.gridDim = dim3((units < walkers ? units : walkers) * (pair ? 2 : 1));
-                cfg.blockDim = dim3(kPThreads);
-                cfg.dynamicSmemBytes = smem;
-                cfg.stream = st;
-                cudaLaunchAttribute attr[1];
-                attr[0].id = cudaLaunchAttributeClusterDimension;
-                attr[0].val.clusterDim.x = pair ? 2 : 1; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-                cfg.attrs = attr; cfg.numAttrs = 1;
-                prof_begin("ln_qkv", "gemm", st);
-                e = cudaLaunchKernelEx(&cfg, kern, tmx, tmw_k, tmq, tmk, tmv, p);
-                prof_end(st);
-                if (e == cudaSuccess) e = cudaGetLastError();
-            }
-            if (e == cudaSuccess || !pair) break;
-            (void)cudaGetLastError();      // the pair launch was refused: clear the error and run the single-CTA form
-            pair = false;
+        auto kern = wide ? ln_qkv_persist_kernel<true, 1> : (pair ? ln_qkv_persist_kernel<true, 2> : ln_qkv_persist_kernel<false, 2>);
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) {
+            const int units = pair ? (tiles + 1) / 2 : tiles, walkers = pair ? sms / 2 : sms;
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((units < walkers ? units : walkers) * (pair ? 2 : 1));
+            cfg.blockDim = dim3(kPThreads);
+            cfg.dynamicSmemBytes = smem;
+            cfg.stream = st;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = pair ? 2 : 1; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            prof_begin("ln_qkv", "gemm", st);
+            e = cudaLaunchKernelEx(&cfg, kern, tmx, tmw_k, oq, ok, ov, p);
+            prof_end(st);
+            if (e == cudaSuccess) e = cudaGetLastError();
         }
-        if (e == cudaSuccess) count_launch();
-    } else {
-        // weight ring: as many 16 KB stages as keep two CTAs per SM (113 KB each) when the A tile allows it, else one CTA
+        if (e == cudaSuccess) { launched = true; count_launch(); break; }
+        if (!pair) break;                  // the single-CTA form failed: report it
+        (void)cudaGetLastError();          // the pair launch was refused: clear the error and take the next form
+        pair = false;
+        e = cudaSuccess;
+    }
+    if (!launched && e == cudaSuccess) {
+        // one CTA per tile (256 < C <= 512): weight ring = what the 226 KB leave beside the A tile
         const size_t fixed = (size_t)(c_in / 64) * kStage + (size_t)kWorkWarps * 2 * kOut + 1024;   // 1024 = barriers + alignment pad
         const size_t budget = fixed + 2 * kStage <= 113 * 1024 ? 113 * 1024 : 226 * 1024;
         p.n_stages = (int)((budget - fixed) / kStage);
