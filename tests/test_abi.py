@@ -50,3 +50,41 @@ def test_product_does_not_import_oracle():
         if f.endswith(".py"):
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(from|import)\s+paper_2605_31500_b200", src, flags=re.M), f
+
+
+def test_header_is_plain_c_and_links_from_c(tmp_path):
+    """The boundary is a C ABI: include/gnn_attn.h compiles as C99 (no C++ in the signatures), and a C program links
+    against the library and reaches the entry points that need no GPU."""
+    import shutil
+    import subprocess
+    from paper_2605_31500_b200 import build
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc")
+    lib = build.build()
+    src = tmp_path / "abi.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include <string.h>
+#include "gnn_attn.h"
+int main(void) {
+    const char* v = gnn_version();
+    if (!v || !strstr(v, "sm_100a")) return 1;
+    if (gnn_static_workspace_limit() != ((size_t)16 << 20)) return 2;
+    /* argument validation happens before any CUDA call: NULL plan / pointers are refused with a message */
+    size_t bytes = 0;
+    if (gnn_workspace_bytes(NULL, GNN_OP_GT_FWD, 4, 64, GNN_BF16, &bytes) == GNN_OK) return 3;
+    if (!gnn_last_error() || !gnn_last_error()[0]) return 4;
+    if (gnn_gt_attn_fwd_static(NULL, NULL, NULL, 0, NULL, NULL, NULL, 4, 64, GNN_BF16, NULL, NULL, NULL) == GNN_OK) return 5;
+    printf("%s\n", v);
+    return 0;
+}
+''')
+    exe = tmp_path / "abi"
+    inc = os.path.join(ROOT, "include")
+    r = subprocess.run([gcc, "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", inc, str(src), "-o", str(exe), lib,
+                        "-Wl,-rpath," + os.path.dirname(lib)], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    r = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert r.returncode == 0, (r.returncode, r.stdout, r.stderr)
+    assert "sm_100a" in r.stdout
