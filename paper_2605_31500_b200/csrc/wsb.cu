@@ -48,7 +48,6 @@ using namespace tc;
 constexpr int kTile = 128;      // rows per CTA = MMA M = TMEM lanes
 constexpr int kHT = 16384;      // bytes of a half tile: 128 rows x 64 channels bf16, 128-byte swizzled rows
 constexpr int kWBytes = 32768;  // bytes of the block-diagonal 128 x 128 bf16 weight tile (P / dS)
-constexpr int kSplitSteps = 4;  // src side: tiles with more steps (sources of out-degree > 64 possible) stage hi + lo weights
 enum { kFwd = 0, kBwdDst = 1, kBwdSrc = 2 };
 
 struct WsbParams {
@@ -422,13 +421,10 @@ wsb_kernel(const __grid_constant__ CUtensorMap tmx, const __grid_constant__ CUte
                 };
                 // Acc1 += P Z1 (dst: B = sum P K_c; src: dV = sum P^T dO_c); Acc2 += W2 Xc (dst: A = sum P (dP - Delta~) K_c;
                 // src: dK = sum dS^T Q_c)
-                // (the lo parts only where a source can have more than 16 kSplitSteps destinations: below that the single
-                // rounding of at most 64 weights per sum stays at ~1e-3 of the largest term; n_steps is uniform over the CTA)
-                const bool split = MODE == kBwdSrc && n_steps > kSplitSteps;
                 stage2(pk, MODE == kBwdSrc ? sGy : sGx, kColAcc1, s == 0);
-                if constexpr (MODE == kBwdSrc) { if (split) stage2(pkl, sGy, kColAcc1, false); }
+                if constexpr (MODE == kBwdSrc) stage2(pkl, sGy, kColAcc1, false);
                 stage2(pk2, sGx, kColAcc2, s == 0);
-                if constexpr (MODE == kBwdSrc) { if (split) stage2(pk2l, sGx, kColAcc2, false); }
+                if constexpr (MODE == kBwdSrc) stage2(pk2l, sGx, kColAcc2, false);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             }
         }
